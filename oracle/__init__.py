@@ -1,0 +1,190 @@
+"""ORACLE -- test infrastructure only (ctypes binding of ``tpc_oracle.cpp``).
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may
+import this package.  It shares no code with ``paper_2102_08862_b200/csrc`` and never imports the product
+package's CUDA binding.  See the header of ``tpc_oracle.cpp`` for what it follows and what pins it.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "tpc_oracle.cpp")
+_LIB = os.path.join(_HERE, "libtpcoracle.so")
+
+# -ffp-contract=off: no FMA contraction; no -ffast-math; x86-64 SSE2 scalar fp32 (no x87 excess precision)
+CXXFLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC"]
+
+
+class Geometry(C.Structure):
+    _fields_ = [("n_sectors", C.c_int32), ("n_rows", C.c_int32), ("x0_cm", C.c_float),
+                ("row_pitch_cm", C.c_float), ("pad_pitch_cm", C.c_float), ("tan_half_sector", C.c_float),
+                ("time_bin_cm", C.c_float), ("drift_len_cm", C.c_float), ("max_time_bin", C.c_float)]
+
+
+class Params(C.Structure):
+    _fields_ = [("win_slope", C.c_float), ("win_const", C.c_float), ("chi2_cut", C.c_float),
+                ("miss_limit", C.c_int32), ("min_hits", C.c_int32),
+                ("sigma_y_cm", C.c_float), ("sigma_z_cm", C.c_float),
+                ("slope_y_max", C.c_float), ("slope_z_max", C.c_float), ("seed_min_hits", C.c_int32),
+                ("sin_phi_max", C.c_float), ("inv_R_per_qpt", C.c_float),
+                ("c0_y2", C.c_float), ("c0_s2", C.c_float), ("c0_k2", C.c_float), ("c0_z2", C.c_float),
+                ("c0_t2", C.c_float), ("brute_force", C.c_int32)]
+
+
+def default_geometry(n_sectors: int = 36, max_time_bin: float = 487.0) -> Geometry:
+    """BASELINE.json L7: 152 rows at 85.0 + 1.07 r cm, 0.5 cm pads, +-10 deg sectors, 0.516 cm time bins."""
+    import math
+    return Geometry(n_sectors, 152, 85.0, 1.07, 0.5, math.tan(math.radians(10.0)), 0.516, 250.0, max_time_bin)
+
+
+def default_params(sigma_y: float = 0.08, sigma_z: float = 0.12) -> Params:
+    """BASELINE.json L7 cuts + the [proposed] readings of SURVEY.md §8(c) / DESIGN.md."""
+    return Params(win_slope=0.05, win_const=0.5, chi2_cut=9.0, miss_limit=10, min_hits=30,
+                  sigma_y_cm=sigma_y, sigma_z_cm=sigma_z, slope_y_max=1.0, slope_z_max=1.5,
+                  seed_min_hits=3, sin_phi_max=0.95, inv_R_per_qpt=1.0 / 666.7,
+                  c0_y2=1.0, c0_s2=0.1, c0_k2=100.0, c0_z2=1.0, c0_t2=0.1, brute_force=0)
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", *CXXFLAGS, "-o", _LIB, _SRC])
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        vp = C.c_void_p
+        L.orc_track.argtypes = [C.POINTER(Geometry), C.POINTER(Params), vp, vp, vp, C.c_int64, C.POINTER(vp)]
+        L.orc_track.restype = C.c_int
+        for nm in ("orc_n_tracklets", "orc_n_tracks", "orc_n_track_hits"):
+            getattr(L, nm).argtypes = [vp]
+            getattr(L, nm).restype = C.c_int64
+        L.orc_copy_links.argtypes = [vp] * 6
+        L.orc_copy_tracklets.argtypes = [vp] * 8
+        L.orc_copy_tracks.argtypes = [vp] * 10
+        L.orc_copy_stats.argtypes = [vp, vp]
+        L.orc_free.argtypes = [vp]
+        L.orc_transport.argtypes = [C.POINTER(Params), vp, vp, C.c_float]
+        L.orc_transport.restype = C.c_int
+        L.orc_update.argtypes = [vp, vp, C.c_float, C.c_float, C.c_float, C.c_float]
+        L.orc_tables.argtypes = [C.POINTER(Geometry), C.POINTER(Params), vp, vp, vp, vp]
+        for nm in ("orc_copy_links", "orc_copy_tracklets", "orc_copy_tracks", "orc_copy_stats", "orc_free",
+                   "orc_update", "orc_tables"):
+            getattr(L, nm).restype = None
+        _lib = L
+    return _lib
+
+
+STAT_NAMES = ("s_ingest", "s_finder", "s_cleaner_start", "s_constructor", "s_selector", "finder_candidates",
+              "finder_pairs", "transports", "searches", "search_candidates", "updates", "invalid_clusters",
+              "start_hits")
+
+PAR_NAMES = ("x", "y", "z_rel", "sin_phi", "dzds", "q_pt", "time_ref")
+
+
+@dataclass
+class Result:
+    n: int
+    up_raw: np.ndarray
+    down_raw: np.ndarray
+    link_up: np.ndarray        # cleaned, by original index, -1 = none
+    link_down: np.ndarray
+    is_start_hit: np.ndarray   # uint8[n]
+    tl_seed: np.ndarray        # tracklets: one per start hit, in ascending start-hit index
+    tl_n_hits: np.ndarray
+    tl_first_row: np.ndarray
+    tl_last_row: np.ndarray
+    tl_row_hit: np.ndarray     # int32[n_tracklets, n_rows]
+    tl_par: np.ndarray         # float32[n_tracklets, 7]
+    tl_cov: np.ndarray         # float32[n_tracklets, 9]
+    tr_seed: np.ndarray        # tracks
+    tr_sector: np.ndarray
+    tr_first_row: np.ndarray
+    tr_last_row: np.ndarray
+    tr_n_hits: np.ndarray
+    tr_hit_offset: np.ndarray
+    tr_par: np.ndarray
+    tr_cov: np.ndarray
+    tr_hit_index: np.ndarray   # original cluster indices, ascending row, per track contiguous
+    stats: dict
+
+    def track_hits(self, i: int) -> np.ndarray:
+        o = int(self.tr_hit_offset[i])
+        return self.tr_hit_index[o:o + int(self.tr_n_hits[i])]
+
+
+def track(geom: Geometry, params: Params, row, pad, time) -> Result:
+    """Run the whole path (C1..C6) on host fp32 arrays."""
+    L = lib()
+    row = np.ascontiguousarray(row, np.float32)
+    pad = np.ascontiguousarray(pad, np.float32)
+    time = np.ascontiguousarray(time, np.float32)
+    n = int(row.shape[0])
+    assert pad.shape[0] == n and time.shape[0] == n
+    h = C.c_void_p()
+    rc = L.orc_track(C.byref(geom), C.byref(params), row.ctypes.data, pad.ctypes.data, time.ctypes.data, n, C.byref(h))
+    if rc != 0:
+        raise ValueError("orc_track rejected its arguments")
+    try:
+        nr = geom.n_rows
+        i32 = lambda *s: np.empty(s, np.int32)
+        up_raw, down_raw, up, down = i32(n), i32(n), i32(n), i32(n)
+        st = np.empty(n, np.uint8)
+        L.orc_copy_links(h, up_raw.ctypes.data, down_raw.ctypes.data, up.ctypes.data, down.ctypes.data, st.ctypes.data)
+        nt = L.orc_n_tracklets(h)
+        ts, tn, tf, tl, trh = i32(nt), i32(nt), i32(nt), i32(nt), i32(nt, nr)
+        tp, tc = np.empty((nt, 7), np.float32), np.empty((nt, 9), np.float32)
+        L.orc_copy_tracklets(h, ts.ctypes.data, tn.ctypes.data, tf.ctypes.data, tl.ctypes.data, trh.ctypes.data,
+                             tp.ctypes.data, tc.ctypes.data)
+        nk, nh = L.orc_n_tracks(h), L.orc_n_track_hits(h)
+        ks, kc, kf, kl, kn = i32(nk), i32(nk), i32(nk), i32(nk), i32(nk)
+        ko = np.empty(nk, np.int64)
+        kp, kv = np.empty((nk, 7), np.float32), np.empty((nk, 9), np.float32)
+        kh = i32(nh)
+        L.orc_copy_tracks(h, ks.ctypes.data, kc.ctypes.data, kf.ctypes.data, kl.ctypes.data, kn.ctypes.data,
+                          ko.ctypes.data, kp.ctypes.data, kv.ctypes.data, kh.ctypes.data)
+        s16 = np.zeros(16, np.float64)
+        L.orc_copy_stats(h, s16.ctypes.data)
+        stats = {k: float(s16[i]) for i, k in enumerate(STAT_NAMES)}
+        return Result(n, up_raw, down_raw, up, down, st, ts, tn, tf, tl, trh, tp, tc,
+                      ks, kc, kf, kl, kn, ko, kp, kv, kh, stats)
+    finally:
+        L.orc_free(h)
+
+
+def transport(params: Params, state6, cov9, xn: float):
+    """One call of the oracle's transport (pins K1, K2).  Returns (ok, state6, cov9)."""
+    st = np.array(state6, np.float32)
+    cv = np.array(cov9, np.float32)
+    rc = lib().orc_transport(C.byref(params), st.ctypes.data, cv.ctypes.data, float(xn))
+    return rc == 0, st, cv
+
+
+def update(state6, cov9, ym: float, zm: float, ry: float, rz: float):
+    """One call of the oracle's Kalman update (pin K3)."""
+    st = np.array(state6, np.float32)
+    cv = np.array(cov9, np.float32)
+    lib().orc_update(st.ctypes.data, cv.ctypes.data, float(ym), float(zm), float(ry), float(rz))
+    return st, cv
+
+
+def tables(geom: Geometry, params: Params):
+    """Geometry tables and derived constants as the oracle computes them (pin G1)."""
+    nr = geom.n_rows
+    x = np.empty(nr, np.float32)
+    npads = np.empty(nr, np.int32)
+    cr = np.empty(nr, np.float32)
+    k = np.empty(8, np.float32)
+    lib().orc_tables(C.byref(geom), C.byref(params), x.ctypes.data, npads.ctypes.data, cr.ctypes.data, k.ctypes.data)
+    return x, npads, cr, dict(W1=k[0], Ay=k[1], Az=k[2], wy=k[3], wz=k[4], ry=k[5], rz=k[6])

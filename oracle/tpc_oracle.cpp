@@ -1,0 +1,530 @@
+// ORACLE -- TEST INFRASTRUCTURE ONLY.  Plain, slow, single-threaded C++ fp32 CPU implementation of
+// TPC sector tracking of a continuous-readout time frame: cellular-automaton seeding in native
+// (pad row, pad, time) coordinates followed by Kalman-filter track following.
+//
+// What it follows:
+//   * PAPER.md L23 (§1): "the track seeding operates using the time as coordinate instead of the
+//     spatial z coordinate"  -> z is only ever a difference of raw time values times the bin size.
+//   * PAPER.md L25 (§1): tracker derived from the Run 2 HLT TPC tracker, time frame processed as a whole.
+//   * BASELINE.json L5 (north_star): the five steps (ingest, neighbours finder, neighbours cleaner +
+//     start-hit finder, tracklet constructor, tracklet selector), fp32, lowest-index tie-breaking.
+//   * BASELINE.json L7: the cuts (windows 0.05*dx+0.5 cm, chi2 cut 9, miss limit 10, >= 30 unshared hits).
+//   * SURVEY.md §8(c) C1..C6 / DESIGN.md "Readings": every point on which those sources are silent.
+// The paper gives no algorithm listing, so this is a HEURISTIC followed step by step; there is no
+// closed-form result.  Every fp32 statement below is one rounded operation sequence evaluated left to
+// right as written; build with -O2 -ffp-contract=off (no FMA contraction, no fast-math).
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load
+// this.  It shares no code, header, table or constant generator with the CUDA path.
+//
+// Pins (tests/test_oracle_*.py): G1 geometry closed forms; N1 brute force == time-window search;
+// N2 noise-free straight track links; N3 reciprocity; K1 transport round trip / composition / exact
+// circle; K2 arc-length series vs asin; K3 KF == weighted least-squares line; K4 noise-free helix
+// end to end; S1 selector == sort-by-key first-come-first-served; E1 efficiency >= 95 % (pT > 0.2).
+// Parity unpinned (no external truth exists): absolute fitted values on noisy data.
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+extern "C" {
+
+struct orc_geometry {
+  int32_t n_sectors, n_rows;
+  float x0_cm, row_pitch_cm, pad_pitch_cm, tan_half_sector, time_bin_cm, drift_len_cm, max_time_bin;
+};
+
+struct orc_params {
+  float win_slope, win_const, chi2_cut;
+  int32_t miss_limit, min_hits;
+  float sigma_y_cm, sigma_z_cm, slope_y_max, slope_z_max;
+  int32_t seed_min_hits;
+  float sin_phi_max, inv_R_per_qpt;
+  float c0_y2, c0_s2, c0_k2, c0_z2, c0_t2;
+  int32_t brute_force;   // 1: neighbour / window searches scan whole rows (pin N1)
+};
+
+}  // extern "C"
+
+namespace {
+
+struct Derived {   // constants derived in double from the fp32 parameter values, rounded once
+  float W1, Ay, Az, wy, wz, ry, rz, Z, P, cB;
+  std::vector<float> xr, cr;      // row x, pad centre c_r = 0.5*(n_pads_r - 1)
+  std::vector<int32_t> npads;
+};
+
+Derived derive(const orc_geometry& g, const orc_params& p) {
+  Derived d;
+  const double pitch = (double)g.row_pitch_cm;
+  const double w1 = (double)p.win_slope * pitch + (double)p.win_const;
+  d.W1 = (float)w1;
+  d.Ay = (float)((double)p.slope_y_max * pitch + w1);
+  d.Az = (float)((double)p.slope_z_max * pitch + w1);
+  const double sy2 = (double)p.sigma_y_cm * (double)p.sigma_y_cm;
+  const double sz2 = (double)p.sigma_z_cm * (double)p.sigma_z_cm;
+  d.wy = (float)(1.0 / (6.0 * sy2));
+  d.wz = (float)(1.0 / (6.0 * sz2));
+  d.ry = (float)sy2;
+  d.rz = (float)sz2;
+  d.Z = g.time_bin_cm;
+  d.P = g.pad_pitch_cm;
+  d.cB = p.inv_R_per_qpt;
+  d.xr.resize(g.n_rows); d.cr.resize(g.n_rows); d.npads.resize(g.n_rows);
+  for (int r = 0; r < g.n_rows; ++r) {
+    const double x = (double)g.x0_cm + pitch * (double)r;
+    d.xr[r] = (float)x;
+    d.npads[r] = (int32_t)std::floor(2.0 * x * (double)g.tan_half_sector / (double)g.pad_pitch_cm);
+    d.cr[r] = (float)(0.5 * (double)(d.npads[r] - 1));
+  }
+  return d;
+}
+
+struct State {       // C5: (x; y, z, s = sin phi, t = dz/ds, k = q/pT), block covariance
+  float x, y, z, s, t, k;
+  float c0, c1, c2, c3, c4, c5;   // (yy, ys, ss, yk, sk, kk)
+  float d0, d1, d2;               // (zz, zt, tt)
+};
+
+// C5 transport: exact circle in the local x-y plane.  Returns false (state unchanged) on FAIL.
+bool transport(State& S, float xn, float cB, float sin_phi_max) {
+  const float dx = xn - S.x;
+  const float kc = cB * S.k;
+  const float sn = S.s + kc * dx;
+  if (!(std::fabs(sn) < sin_phi_max)) return false;
+  const float c = std::sqrt(1.0f - S.s * S.s);
+  const float cn = std::sqrt(1.0f - sn * sn);
+  const float ss = S.s + sn;
+  const float cc = c + cn;
+  const float icc = 1.0f / cc;
+  const float T = ss * icc;
+  const float q = 1.0f + T * T;
+  const float rq = std::sqrt(q);
+  const float u = kc * dx;
+  const float a = (u * u) * q;
+  const float dS = (dx * rq) * (1.0f + a * (0.041666668f + a * (0.0046875f + a * 0.00069754466f)));
+  const float g0 = (1.0f + T * (S.s / c)) * icc;
+  const float g1 = (1.0f + T * (sn / cn)) * icc;
+  const float fa = dx * (g0 + g1);
+  const float e = cB * dx;
+  const float fb = (dx * g1) * e;
+  S.y = S.y + dx * T;
+  S.z = S.z + S.t * dS;
+  S.s = sn;
+  S.x = xn;
+  const float h3 = S.c3 + fa * S.c4 + fb * S.c5;
+  const float h4 = S.c4 + e * S.c5;
+  const float h1 = S.c1 + fa * S.c2 + fb * S.c4;
+  S.c0 = S.c0 + fa * S.c1 + fb * S.c3 + fa * h1 + fb * h3;
+  S.c1 = h1 + e * h3;
+  S.c2 = S.c2 + e * S.c4 + e * h4;
+  S.c3 = h3;
+  S.c4 = h4;
+  const float n1 = S.d1 + dS * S.d2;
+  S.d0 = S.d0 + dS * S.d1 + dS * n1;
+  S.d1 = n1;
+  return true;
+}
+
+// C5 update with a measurement (ym, zm) of variances (ry, rz).
+void update(State& S, float ym, float zm, float ry, float rz) {
+  const float wy = 1.0f / (S.c0 + ry);
+  const float resy = ym - S.y;
+  const float k0 = S.c0 * wy, k1 = S.c1 * wy, k3 = S.c3 * wy;
+  S.y += k0 * resy;
+  S.s += k1 * resy;
+  S.k += k3 * resy;
+  S.c5 -= k3 * S.c3;
+  S.c4 -= k1 * S.c3;
+  S.c2 -= k1 * S.c1;
+  S.c3 -= k0 * S.c3;
+  S.c1 -= k0 * S.c1;
+  S.c0 -= k0 * S.c0;
+  const float wz = 1.0f / (S.d0 + rz);
+  const float resz = zm - S.z;
+  const float j0 = S.d0 * wz, j1 = S.d1 * wz;
+  S.z += j0 * resz;
+  S.t += j1 * resz;
+  S.d2 -= j1 * S.d1;
+  S.d1 -= j0 * S.d1;
+  S.d0 -= j0 * S.d0;
+}
+
+struct Tracklet {
+  int32_t seed;                 // original index of the start hit == tracklet id
+  int32_t n_hits, first_row, last_row;
+  std::vector<int32_t> row_hit; // [n_rows], original indices, -1 = none
+  State snap;                   // state after the last update (innermost hit)
+  float time_ref;
+};
+
+struct Track {
+  int32_t seed, sector, first_row, last_row, n_hits;
+  int64_t hit_offset;
+  State snap;
+  float time_ref;
+};
+
+}  // namespace
+
+struct orc_result {
+  int64_t n = 0;
+  int32_t n_rows = 0;
+  std::vector<int32_t> up_raw, down_raw, up, down;
+  std::vector<uint8_t> is_start;
+  std::vector<Tracklet> tracklets;
+  std::vector<Track> tracks;
+  std::vector<int32_t> track_hits;
+  double stats[16] = {0};
+  // [0..4] seconds: ingest, finder, cleaner+start, constructor, selector
+  // [5] candidates scanned in finder  [6] pairs tested  [7] transports  [8] searches
+  // [9] candidates scanned in searches [10] updates [11] invalid clusters [12] start hits
+};
+
+namespace {
+
+struct RowIndex {   // C1: hits grouped by (sector,row); sorted by (time, orig) as an acceleration only
+  std::vector<int64_t> start;     // [n_sr + 1]
+  std::vector<int32_t> idx;       // original indices
+  std::vector<float> t;           // time of idx[i], same order
+};
+
+inline double now() {
+  return std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count();
+}
+
+}  // namespace
+
+extern "C" {
+
+int orc_track(const orc_geometry* gp, const orc_params* pp, const float* row, const float* pad,
+              const float* time, int64_t n, orc_result** out) {
+  if (!gp || !pp || !out || n < 0 || n >= (int64_t)1 << 31 || (n > 0 && (!row || !pad || !time))) return -1;
+  const orc_geometry g = *gp;
+  const orc_params p = *pp;
+  if (g.n_rows < 3 || g.n_sectors < 1) return -1;
+  const Derived D = derive(g, p);
+  const int n_rows = g.n_rows;
+  const int64_t n_sr = (int64_t)g.n_sectors * n_rows;
+  orc_result* R = new orc_result();
+  R->n = n; R->n_rows = n_rows;
+
+  // ---------------- C1 ingest ----------------
+  double t0 = now();
+  std::vector<int32_t> sr(n, -1);     // sector*n_rows + row, -1 = outside the geometry (ignored)
+  std::vector<float> y(n, 0.0f);
+  RowIndex ri;
+  ri.start.assign(n_sr + 1, 0);
+  int64_t n_invalid = 0;
+  for (int64_t i = 0; i < n; ++i) {
+    const float rf = row[i];
+    bool ok = rf >= 0.0f && rf < (float)n_sr && rf == std::floor(rf);
+    int32_t isr = -1;
+    if (ok) {
+      isr = (int32_t)rf;
+      const int r = isr % n_rows;
+      ok = pad[i] >= -0.5f && pad[i] < (float)D.npads[r] - 0.5f && time[i] >= 0.0f && time[i] <= g.max_time_bin;
+      if (ok) y[i] = (pad[i] - D.cr[r]) * D.P;
+    }
+    if (!ok) { ++n_invalid; continue; }
+    sr[i] = isr;
+    ++ri.start[isr + 1];
+  }
+  for (int64_t b = 0; b < n_sr; ++b) ri.start[b + 1] += ri.start[b];
+  ri.idx.resize(ri.start[n_sr]);
+  {
+    std::vector<int64_t> fill(ri.start.begin(), ri.start.end() - 1);
+    for (int64_t i = 0; i < n; ++i) if (sr[i] >= 0) ri.idx[fill[sr[i]]++] = (int32_t)i;
+    for (int64_t b = 0; b < n_sr; ++b)
+      std::sort(ri.idx.begin() + ri.start[b], ri.idx.begin() + ri.start[b + 1],
+                [&](int32_t a, int32_t c) { return time[a] < time[c] || (time[a] == time[c] && a < c); });
+    ri.t.resize(ri.idx.size());
+    for (size_t k = 0; k < ri.idx.size(); ++k) ri.t[k] = time[ri.idx[k]];
+  }
+  R->stats[11] = (double)n_invalid;
+  // candidate range of bin b whose time lies in [tc - hw, tc + hw] (a superset is all that is needed)
+  auto range = [&](int64_t b, double tc, double hw, int64_t& lo, int64_t& hi) {
+    lo = ri.start[b]; hi = ri.start[b + 1];
+    if (p.brute_force) return;
+    const float* tb = ri.t.data();
+    lo = std::lower_bound(tb + lo, tb + hi, (float)(tc - hw - 0.05)) - tb;
+    hi = std::upper_bound(tb + lo, tb + hi, (float)(tc + hw + 0.05)) - tb;
+  };
+  double t1 = now();
+  R->stats[0] = t1 - t0;
+
+  // ---------------- C2 neighbours finder ----------------
+  R->up_raw.assign(n, -1); R->down_raw.assign(n, -1);
+  {
+    std::vector<int32_t> U, Dn;
+    double n_cand = 0, n_pairs = 0;
+    const double tw = (double)D.Az / (double)D.Z;
+    for (int64_t h = 0; h < n; ++h) {
+      if (sr[h] < 0) continue;
+      const int r = sr[h] % n_rows;
+      if (r < 1 || r > n_rows - 2) continue;
+      const float yh = y[h], th = time[h];
+      U.clear(); Dn.clear();
+      for (int side = 0; side < 2; ++side) {
+        const int64_t b = sr[h] + (side == 0 ? 1 : -1);
+        int64_t lo, hi;
+        range(b, (double)th, tw, lo, hi);
+        n_cand += (double)(hi - lo);
+        for (int64_t q = lo; q < hi; ++q) {
+          const int32_t c = ri.idx[q];
+          const float dy = y[c] - yh;
+          const float dz = (time[c] - th) * D.Z;
+          if (std::fabs(dy) < D.Ay && std::fabs(dz) < D.Az) (side == 0 ? U : Dn).push_back(c);
+        }
+      }
+      float best = 0.0f; int32_t bu = -1, bd = -1;
+      for (int32_t u : U) {
+        for (int32_t d : Dn) {
+          n_pairs += 1;
+          const float ay = y[u] - yh;
+          const float by = yh - y[d];
+          const float ey = ay - by;
+          const float az = (time[u] - th) * D.Z;
+          const float bz = (th - time[d]) * D.Z;
+          const float ez = az - bz;
+          if (!(std::fabs(ey) < D.W1 && std::fabs(ez) < D.W1)) continue;
+          const float chi2 = (ey * ey) * D.wy + (ez * ez) * D.wz;
+          if (!(chi2 < p.chi2_cut)) continue;
+          if (bu < 0 || chi2 < best || (chi2 == best && (u < bu || (u == bu && d < bd)))) {
+            best = chi2; bu = u; bd = d;
+          }
+        }
+      }
+      R->up_raw[h] = bu; R->down_raw[h] = bd;
+    }
+    R->stats[5] = n_cand; R->stats[6] = n_pairs;
+  }
+  double t2 = now();
+  R->stats[1] = t2 - t1;
+
+  // ---------------- C3 cleaner, C4 start hits ----------------
+  R->up.assign(n, -1); R->down.assign(n, -1); R->is_start.assign(n, 0);
+  for (int64_t h = 0; h < n; ++h) {
+    const int32_t u = R->up_raw[h], d = R->down_raw[h];
+    R->up[h] = (u >= 0 && R->down_raw[u] == (int32_t)h) ? u : -1;
+    R->down[h] = (d >= 0 && R->up_raw[d] == (int32_t)h) ? d : -1;
+  }
+  std::vector<int32_t> start_hits;
+  for (int64_t h = 0; h < n; ++h) {
+    if (sr[h] < 0 || R->down[h] >= 0) continue;
+    int len = 1; int32_t c = (int32_t)h;
+    while (len < p.seed_min_hits && R->up[c] >= 0) { c = R->up[c]; ++len; }
+    if (len >= p.seed_min_hits) { R->is_start[h] = 1; start_hits.push_back((int32_t)h); }
+  }
+  R->stats[12] = (double)start_hits.size();
+  double t3 = now();
+  R->stats[2] = t3 - t2;
+
+  // ---------------- C5 tracklet constructor ----------------
+  {
+    double n_tr = 0, n_se = 0, n_sc = 0, n_up = 0;
+    R->tracklets.reserve(start_hits.size());
+    for (int32_t h0 : start_hits) {
+      Tracklet T;
+      T.seed = h0; T.row_hit.assign(n_rows, -1); T.time_ref = time[h0];
+      const int64_t sec_base = (int64_t)(sr[h0] / n_rows) * n_rows;
+      const int r0 = sr[h0] % n_rows;
+      const float tstart = time[h0];
+      const int32_t h1 = R->up[h0];
+      const int r1 = sr[h1] % n_rows;
+      State S;
+      // 1. init from the first two chain hits
+      S.x = D.xr[r0]; S.y = y[h0]; S.z = 0.0f;
+      {
+        const float dxl = D.xr[r1] - D.xr[r0];
+        const float dy = y[h1] - y[h0];
+        const float dzl = (time[h1] - tstart) * D.Z;
+        const float L = std::sqrt(dxl * dxl + dy * dy);
+        S.s = dy / L; S.t = dzl / L; S.k = 0.0f;
+      }
+      S.c0 = D.ry; S.c1 = 0; S.c2 = p.c0_s2; S.c3 = 0; S.c4 = 0; S.c5 = p.c0_k2;
+      S.d0 = D.rz; S.d1 = 0; S.d2 = p.c0_t2;
+      T.row_hit[r0] = h0;
+      float x_last = S.x;
+      T.snap = S;
+      auto attach = [&](int32_t m, int r) {
+        update(S, y[m], (time[m] - tstart) * D.Z, D.ry, D.rz);
+        n_up += 1;
+        T.row_hit[r] = m; x_last = S.x; T.snap = S;
+      };
+      auto search = [&](int r) -> int32_t {
+        n_se += 1;
+        const float w = p.win_slope * std::fabs(D.xr[r] - x_last) + p.win_const;
+        int64_t lo, hi;
+        range(sec_base + r, (double)tstart + (double)S.z / (double)D.Z, (double)w / (double)D.Z, lo, hi);
+        n_sc += (double)(hi - lo);
+        int32_t bm = -1; float bdd = 0.0f;
+        for (int64_t q = lo; q < hi; ++q) {
+          const int32_t m = ri.idx[q];
+          const float ey = y[m] - S.y;
+          const float ez = (time[m] - tstart) * D.Z - S.z;
+          if (!(std::fabs(ey) < w && std::fabs(ez) < w)) continue;
+          const float dd = ey * ey + ez * ez;
+          if (bm < 0 || dd < bdd || (dd == bdd && m < bm)) { bm = m; bdd = dd; }
+        }
+        return bm;
+      };
+      // 2. chain phase (up), no gating
+      bool ok = true;
+      int r_last = r0;
+      for (int32_t c = h1; c >= 0; c = R->up[c]) {
+        const int r = sr[c] % n_rows;
+        n_tr += 1;
+        if (!transport(S, D.xr[r], D.cB, p.sin_phi_max)) { ok = false; break; }
+        attach(c, r);
+        r_last = r;
+      }
+      // 3. following (up)
+      if (ok) {
+        int misses = 0;
+        for (int r = r_last + 1; r < n_rows; ++r) {
+          n_tr += 1;
+          if (!transport(S, D.xr[r], D.cB, p.sin_phi_max)) break;
+          const int32_t m = search(r);
+          if (m >= 0) { attach(m, r); misses = 0; }
+          else if (++misses == p.miss_limit) break;
+        }
+      }
+      // 4. turn round: keep the state, reset the covariance
+      S.c0 = p.c0_y2; S.c1 = 0; S.c2 = p.c0_s2; S.c3 = 0; S.c4 = 0; S.c5 = p.c0_k2;
+      S.d0 = p.c0_z2; S.d1 = 0; S.d2 = p.c0_t2;
+      // 5. down pass
+      {
+        int r_top = n_rows - 1;
+        while (T.row_hit[r_top] < 0) --r_top;
+        int misses = 0;
+        for (int r = r_top; r >= 0; --r) {
+          n_tr += 1;
+          if (!transport(S, D.xr[r], D.cB, p.sin_phi_max)) break;
+          if (T.row_hit[r] >= 0) attach(T.row_hit[r], r);
+          else if (r < r0) {
+            const int32_t m = search(r);
+            if (m >= 0) { attach(m, r); misses = 0; }
+            else if (++misses == p.miss_limit) break;
+          }
+        }
+      }
+      // 6. result
+      T.n_hits = 0; T.first_row = -1; T.last_row = -1;
+      for (int r = 0; r < n_rows; ++r) if (T.row_hit[r] >= 0) { ++T.n_hits; if (T.first_row < 0) T.first_row = r; T.last_row = r; }
+      R->tracklets.push_back(std::move(T));
+    }
+    R->stats[7] = n_tr; R->stats[8] = n_se; R->stats[9] = n_sc; R->stats[10] = n_up;
+  }
+  double t4 = now();
+  R->stats[3] = t4 - t3;
+
+  // ---------------- C6 tracklet selector ----------------
+  {
+    std::vector<uint64_t> claim(n, 0);
+    auto key = [&](const Tracklet& T) { return ((uint64_t)(uint32_t)T.n_hits << 32) | (uint64_t)(0xFFFFFFFFu - (uint32_t)T.seed); };
+    for (const Tracklet& T : R->tracklets) {
+      if (T.n_hits < p.min_hits) continue;
+      const uint64_t k = key(T);
+      for (int r = 0; r < n_rows; ++r) if (T.row_hit[r] >= 0) claim[T.row_hit[r]] = std::max(claim[T.row_hit[r]], k);
+    }
+    for (const Tracklet& T : R->tracklets) {
+      if (T.n_hits < p.min_hits) continue;
+      const uint64_t k = key(T);
+      int owned = 0, first = -1, last = -1;
+      for (int r = 0; r < n_rows; ++r) if (T.row_hit[r] >= 0 && claim[T.row_hit[r]] == k) { ++owned; if (first < 0) first = r; last = r; }
+      if (owned < p.min_hits) continue;
+      Track K;
+      K.seed = T.seed; K.sector = sr[T.seed] / n_rows; K.first_row = first; K.last_row = last; K.n_hits = owned;
+      K.hit_offset = (int64_t)R->track_hits.size(); K.snap = T.snap; K.time_ref = T.time_ref;
+      for (int r = 0; r < n_rows; ++r) if (T.row_hit[r] >= 0 && claim[T.row_hit[r]] == k) R->track_hits.push_back(T.row_hit[r]);
+      R->tracks.push_back(K);
+    }
+  }
+  double t5 = now();
+  R->stats[4] = t5 - t4;
+  *out = R;
+  return 0;
+}
+
+int64_t orc_n_tracklets(const orc_result* r) { return (int64_t)r->tracklets.size(); }
+int64_t orc_n_tracks(const orc_result* r) { return (int64_t)r->tracks.size(); }
+int64_t orc_n_track_hits(const orc_result* r) { return (int64_t)r->track_hits.size(); }
+
+void orc_copy_links(const orc_result* r, int32_t* up_raw, int32_t* down_raw, int32_t* up, int32_t* down, uint8_t* is_start) {
+  const size_t n = (size_t)r->n;
+  if (up_raw) std::memcpy(up_raw, r->up_raw.data(), n * 4);
+  if (down_raw) std::memcpy(down_raw, r->down_raw.data(), n * 4);
+  if (up) std::memcpy(up, r->up.data(), n * 4);
+  if (down) std::memcpy(down, r->down.data(), n * 4);
+  if (is_start) std::memcpy(is_start, r->is_start.data(), n);
+}
+
+static void put_state(const State& S, float time_ref, float* par, float* cov) {
+  if (par) { par[0] = S.x; par[1] = S.y; par[2] = S.z; par[3] = S.s; par[4] = S.t; par[5] = S.k; par[6] = time_ref; }
+  if (cov) { cov[0] = S.c0; cov[1] = S.c1; cov[2] = S.c2; cov[3] = S.c3; cov[4] = S.c4; cov[5] = S.c5; cov[6] = S.d0; cov[7] = S.d1; cov[8] = S.d2; }
+}
+
+// par: [nt*7] = (x, y, z_rel, sin_phi, dzds, q_pt, time_ref); cov: [nt*9] = (c0..c5, d0..d2); row_hit: [nt*n_rows]
+void orc_copy_tracklets(const orc_result* r, int32_t* seed, int32_t* n_hits, int32_t* first_row, int32_t* last_row,
+                        int32_t* row_hit, float* par, float* cov) {
+  for (size_t i = 0; i < r->tracklets.size(); ++i) {
+    const Tracklet& T = r->tracklets[i];
+    if (seed) seed[i] = T.seed;
+    if (n_hits) n_hits[i] = T.n_hits;
+    if (first_row) first_row[i] = T.first_row;
+    if (last_row) last_row[i] = T.last_row;
+    if (row_hit) std::memcpy(row_hit + i * r->n_rows, T.row_hit.data(), (size_t)r->n_rows * 4);
+    put_state(T.snap, T.time_ref, par ? par + i * 7 : nullptr, cov ? cov + i * 9 : nullptr);
+  }
+}
+
+void orc_copy_tracks(const orc_result* r, int32_t* seed, int32_t* sector, int32_t* first_row, int32_t* last_row,
+                     int32_t* n_hits, int64_t* hit_offset, float* par, float* cov, int32_t* hit_index) {
+  for (size_t i = 0; i < r->tracks.size(); ++i) {
+    const Track& K = r->tracks[i];
+    if (seed) seed[i] = K.seed;
+    if (sector) sector[i] = K.sector;
+    if (first_row) first_row[i] = K.first_row;
+    if (last_row) last_row[i] = K.last_row;
+    if (n_hits) n_hits[i] = K.n_hits;
+    if (hit_offset) hit_offset[i] = K.hit_offset;
+    put_state(K.snap, K.time_ref, par ? par + i * 7 : nullptr, cov ? cov + i * 9 : nullptr);
+  }
+  if (hit_index) std::memcpy(hit_index, r->track_hits.data(), r->track_hits.size() * 4);
+}
+
+void orc_copy_stats(const orc_result* r, double* out16) { std::memcpy(out16, r->stats, sizeof(r->stats)); }
+void orc_free(orc_result* r) { delete r; }
+
+// ---- hooks for the pins (K1..K3, G1): the same functions the tracker uses, callable one at a time ----
+// state6 = (x, y, z, s, t, k); cov9 = (c0..c5, d0..d2).  Returns 0, or 1 on transport FAIL.
+int orc_transport(const orc_params* p, float* st, float* cv, float xn) {
+  State S{st[0], st[1], st[2], st[3], st[4], st[5], cv[0], cv[1], cv[2], cv[3], cv[4], cv[5], cv[6], cv[7], cv[8]};
+  const bool ok = transport(S, xn, p->inv_R_per_qpt, p->sin_phi_max);
+  put_state(S, 0.0f, nullptr, cv);
+  st[0] = S.x; st[1] = S.y; st[2] = S.z; st[3] = S.s; st[4] = S.t; st[5] = S.k;
+  return ok ? 0 : 1;
+}
+
+void orc_update(float* st, float* cv, float ym, float zm, float ry, float rz) {
+  State S{st[0], st[1], st[2], st[3], st[4], st[5], cv[0], cv[1], cv[2], cv[3], cv[4], cv[5], cv[6], cv[7], cv[8]};
+  update(S, ym, zm, ry, rz);
+  put_state(S, 0.0f, nullptr, cv);
+  st[0] = S.x; st[1] = S.y; st[2] = S.z; st[3] = S.s; st[4] = S.t; st[5] = S.k;
+}
+
+// x_r [n_rows], n_pads [n_rows], c_r [n_rows]; consts8 = (W1, Ay, Az, wy, wz, ry, rz, 0)
+void orc_tables(const orc_geometry* g, const orc_params* p, float* x_r, int32_t* n_pads, float* c_r, float* consts8) {
+  const Derived D = derive(*g, *p);
+  for (int r = 0; r < g->n_rows; ++r) {
+    if (x_r) x_r[r] = D.xr[r];
+    if (n_pads) n_pads[r] = D.npads[r];
+    if (c_r) c_r[r] = D.cr[r];
+  }
+  if (consts8) { consts8[0] = D.W1; consts8[1] = D.Ay; consts8[2] = D.Az; consts8[3] = D.wy; consts8[4] = D.wz; consts8[5] = D.ry; consts8[6] = D.rz; consts8[7] = 0; }
+}
+
+}  // extern "C"

@@ -1,0 +1,380 @@
+"""Pins of the oracle against what the paper's configuration and the mathematics fix (CPU only).
+
+The paper prints no worked numbers for this path (PAPER.md has no tables / equations), so each pin is a
+closed form, an invariant, a textbook special case or brute force on a tiny input -- SURVEY.md §8(c) table
+"What pins each part" (G1, N1-N3, K1-K4, S1, E1) and BASELINE.json L5 (a)-(d).
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from helpers import N_ROWS, PITCH, X0, ZBIN, clusters_from_xyz, concat, n_pads, row_x
+from paper_2102_08862_b200 import gen
+import truth_eval
+
+CB = 1.0 / 666.7
+
+
+def _geom(n_sectors=1, tmax=487.0):
+    return oracle.default_geometry(n_sectors, tmax)
+
+
+# ----------------------------------------------------------------------------- G1 geometry closed forms
+def test_G1_geometry_closed_forms():
+    """BASELINE.json L7: x_r = 85.0 + 1.07 r, pads = floor(2 x_r tan10 / 0.5), 0.516 cm time bins over 250 cm."""
+    x, npads, cr, k = oracle.tables(_geom(), oracle.default_params())
+    assert npads[0] == 59 and npads[151] == 173
+    assert int(npads.sum()) == 17698
+    assert abs(float(x[151]) - 246.57) < 1e-4
+    assert abs(250.0 / 0.516 - 484.496) < 1e-3
+    np.testing.assert_array_equal(npads, n_pads(np.arange(152)))
+    np.testing.assert_allclose(cr, 0.5 * (npads - 1))
+    # derived constants: W1 = 0.05*1.07+0.5, A = slope*1.07 + W1, w = 1/(6 sigma^2), r = sigma^2
+    assert abs(k["W1"] - 0.5535) < 1e-6 and abs(k["Ay"] - 1.6235) < 1e-6 and abs(k["Az"] - 2.1585) < 1e-6
+    assert abs(k["wy"] - 1 / (6 * 0.08 ** 2)) < 1e-4 and abs(k["wz"] - 1 / (6 * 0.12 ** 2)) < 1e-4
+    assert abs(k["ry"] - 0.0064) < 1e-9 and abs(k["rz"] - 0.0144) < 1e-9
+
+
+# ----------------------------------------------------------------------------- K1 / K2 transport
+def _state(x, y, z, s, t, k):
+    return [x, y, z, s, t, k], [0.01, 0, 0.01, 0, 0, 1.0, 0.01, 0, 0.01]
+
+
+@pytest.mark.parametrize("s0,k,dx", [(0.1, 2.0, 1.07), (-0.4, -4.0, 10.7), (0.6, 1.0, 50.0), (0.0, 5.0, 30.0),
+                                     (0.3, 0.0, 100.0), (-0.7, 3.3, 20.0)])
+def test_K1_transport_matches_exact_circle(s0, k, dx):
+    """y(x) of the fp32 transport equals the circle sin(phi)(x) = s0 + kappa (x - x0) integrated in double."""
+    p = oracle.default_params()
+    st, cv = _state(100.0, 3.0, 0.0, s0, 0.5, k)
+    ok, st1, _ = oracle.transport(p, st, cv, 100.0 + dx)
+    assert ok
+    kappa = float(np.float32(CB)) * k
+    s1 = s0 + kappa * dx
+    if kappa != 0.0:
+        y_exact = 3.0 + (math.sqrt(1 - s0 * s0) - math.sqrt(1 - s1 * s1)) / kappa
+        arc = (math.asin(s1) - math.asin(s0)) / kappa
+    else:
+        y_exact = 3.0 + dx * s0 / math.sqrt(1 - s0 * s0)
+        arc = dx / math.sqrt(1 - s0 * s0)
+    assert abs(float(st1[1]) - y_exact) < 1e-5 * max(1.0, abs(y_exact))
+    assert abs(float(st1[3]) - s1) < 2e-7
+    # K2: arc length (z advances by t * dS with t = 0.5): series vs asin form, < 1e-6 relative when kappa*chord <= 0.3
+    chord = math.hypot(dx, y_exact - 3.0)
+    assert abs(kappa) * chord <= 0.3
+    assert abs(float(st1[2]) / 0.5 - arc) < 2e-6 * abs(arc)
+
+
+def test_K2_arc_series_coefficients():
+    """arc/chord = (2/a) asin(a/2) = 1 + a^2/24 + 3a^4/640 + 5a^6/7168 + ...: relative error < 1e-6 for a <= 0.3."""
+    for a in np.linspace(1e-3, 0.3, 50):
+        q = a * a
+        series = 1 + q * (0.041666668 + q * (0.0046875 + q * 0.00069754466))
+        assert abs(series - (2 / a) * math.asin(a / 2)) < 1e-6
+
+
+def test_K1_transport_round_trip_and_composition():
+    p = oracle.default_params()
+    st, cv = _state(90.0, -2.0, 1.0, 0.25, -0.8, 3.0)
+    ok1, a, ca = oracle.transport(p, st, cv, 120.0)
+    ok2, b, _ = oracle.transport(p, a, ca, 90.0)
+    assert ok1 and ok2
+    np.testing.assert_allclose(b, np.array(st, np.float32), atol=3e-5, rtol=3e-6)
+    ok3, c, _ = oracle.transport(p, a, ca, 160.0)
+    ok4, d, _ = oracle.transport(p, st, cv, 160.0)
+    assert ok3 and ok4
+    np.testing.assert_allclose(c, d, atol=5e-5, rtol=5e-6)
+
+
+def test_K1_transport_fails_beyond_sin_phi_max_and_keeps_state():
+    p = oracle.default_params()
+    st, cv = _state(90.0, 0.0, 0.0, 0.9, 0.0, 10.0)     # s grows by cB*k*dx = 0.015/cm
+    ok, st1, cv1 = oracle.transport(p, st, cv, 100.0)
+    assert not ok
+    np.testing.assert_array_equal(st1, np.array(st, np.float32))
+    np.testing.assert_array_equal(cv1, np.array(cv, np.float32))
+
+
+def test_K1_covariance_transport_is_F_C_Ft():
+    """The staged covariance lines equal F C F^T with the Jacobian taken by finite differences in double."""
+    p = oracle.default_params()
+    rng = np.random.default_rng(5)
+    A = rng.normal(size=(3, 3)); CA = A @ A.T * 1e-3
+    B = rng.normal(size=(2, 2)); CBk = B @ B.T * 1e-3
+    cov = [CA[0, 0], CA[0, 1], CA[1, 1], CA[0, 2], CA[1, 2], CA[2, 2], CBk[0, 0], CBk[0, 1], CBk[1, 1]]
+    x0, y0, s0, k0, dx = 100.0, 1.0, 0.3, 2.5, 12.0
+    ok, _, cv1 = oracle.transport(p, [x0, y0, 0.0, s0, 0.4, k0], cov, x0 + dx)
+    assert ok
+
+    def prop(v):   # exact circle, double
+        y, s, k = v
+        kap = CB * k
+        s1 = s + kap * dx
+        return np.array([y + dx * (s + s1) / (math.sqrt(1 - s * s) + math.sqrt(1 - s1 * s1)), s1, k])
+
+    F = np.zeros((3, 3)); v0 = np.array([y0, s0, k0])
+    for j in range(3):
+        e = np.zeros(3); e[j] = 1e-6
+        F[:, j] = (prop(v0 + e) - prop(v0 - e)) / 2e-6
+    CA1 = F @ CA @ F.T
+    got = np.array([[cv1[0], cv1[1], cv1[3]], [cv1[1], cv1[2], cv1[4]], [cv1[3], cv1[4], cv1[5]]], np.float64)
+    np.testing.assert_allclose(got, CA1, rtol=2e-4, atol=1e-8)
+    s1 = s0 + CB * k0 * dx
+    dS = (math.asin(s1) - math.asin(s0)) / (CB * k0)
+    Fz = np.array([[1, dS], [0, 1]])
+    CB1 = Fz @ CBk @ Fz.T
+    np.testing.assert_allclose([cv1[6], cv1[7], cv1[8]], [CB1[0, 0], CB1[0, 1], CB1[1, 1]], rtol=2e-4, atol=1e-8)
+
+
+# ----------------------------------------------------------------------------- K3 filter == least squares
+def test_K3_filter_equals_weighted_least_squares_line():
+    """With the curvature frozen (k = 0, c3 = c4 = c5 = 0) the filter is the textbook weighted least-squares
+    straight-line fit with a Gaussian prior (normal equations (A^T A / r + P0^-1)^-1 A^T z / r): exactly linear
+    in the (z, t) block.  A prior of 100 keeps fp32 cancellation in c - k*c below the tolerance."""
+    p = oracle.default_params()
+    rng = np.random.default_rng(11)
+    xs = X0 + PITCH * np.arange(40)
+    zt, tt = 2.0, 0.7
+    zm = zt + tt * (xs - xs[0]) + rng.normal(0, 0.12, xs.size)
+    ym = 0.5 + 0.01 * (xs - xs[0]) + rng.normal(0, 0.01, xs.size)
+    P0 = 100.0
+    st = np.array([xs[0], 0.0, 0.0, 0.0, 0.0, 0.0], np.float32)
+    cv = np.array([P0, 0, P0, 0, 0, 0, P0, 0, P0], np.float32)
+    ry, rz = 0.01 ** 2, 0.12 ** 2
+    for i, x in enumerate(xs):
+        if i:
+            ok, st, cv = oracle.transport(p, st, cv, float(x))
+            assert ok
+        st, cv = oracle.update(st, cv, float(ym[i]), float(zm[i]), ry, rz)
+
+    def bayes_line(u, meas, r):
+        A = np.stack([np.ones_like(u), u], 1)
+        cov = np.linalg.inv(A.T @ A / r + np.eye(2) / P0)
+        return cov @ (A.T @ meas / r), cov
+
+    # z block: the path length per step is dx*sqrt(1+T^2) with T = tan(phi) ~ 0.01
+    T = 0.01
+    sl = (xs - xs[0]) * math.sqrt(1 + T * T)
+    (z_ls, t_ls), cov = bayes_line(sl, zm, rz)
+    a = np.array([1.0, sl[-1]])
+    assert abs(float(st[2]) - (z_ls + t_ls * sl[-1])) < 1e-4 and abs(float(st[4]) - t_ls) < 1e-5
+    assert abs(float(cv[6]) - a @ cov @ a) < 2e-3 * (a @ cov @ a)
+    assert abs(float(cv[8]) - cov[1, 1]) < 2e-3 * cov[1, 1]
+    # y block: a line in tan(phi); the filter's parameter is s = sin(phi) (linearisation error ~ T^2)
+    (y_ls, sl_ls), _ = bayes_line(xs - xs[0], ym, ry)
+    assert abs(float(st[1]) - (y_ls + sl_ls * (xs[-1] - xs[0]))) < 1e-4
+    assert abs(float(st[3]) - sl_ls / math.sqrt(1 + sl_ls ** 2)) < 1e-5
+
+
+# ----------------------------------------------------------------------------- N2 straight tracks
+def _straight_tracks(n_tracks=6, seed=3):
+    rng = np.random.default_rng(seed)
+    rows = np.arange(N_ROWS)
+    x = row_x(rows)
+    parts = []
+    for i in range(n_tracks):      # radial-ish lines that stay inside the +-10 degree wedge and the drift length
+        y = (-0.12 + 0.048 * i) * x + rng.uniform(-0.01, 0.01) * (x - X0)
+        z = 125.0 + rng.uniform(-0.7, 0.7) * (x - X0)
+        parts.append(clusters_from_xyz(rows, y, z))
+    return concat(parts), n_tracks
+
+
+def test_N2_noise_free_straight_tracks_link_to_true_neighbours():
+    (row, pad, time), nt = _straight_tracks()
+    r = oracle.track(_geom(), oracle.default_params(), row, pad, time)
+    idx = np.arange(row.size).reshape(nt, N_ROWS)
+    for t in range(nt):
+        # uncleaned: every interior hit links to the hits of its own track in rows r+1 and r-1
+        np.testing.assert_array_equal(r.up_raw[idx[t, 1:-1]], idx[t, 2:])
+        np.testing.assert_array_equal(r.down_raw[idx[t, 1:-1]], idx[t, :-2])
+        # edge rows are linkless, so after cleaning the chain is rows 1..150 and row 1 is the only start hit
+        assert r.link_up[idx[t, 150]] == -1 and r.link_down[idx[t, 1]] == -1
+        np.testing.assert_array_equal(r.link_up[idx[t, 1:150]], idx[t, 2:151])
+        assert r.is_start_hit[idx[t]].sum() == 1 and r.is_start_hit[idx[t, 1]] == 1
+    # BASELINE.json L5 (a): reconstructed exactly -- one track per line with all 152 hits
+    assert len(r.tr_seed) == nt
+    for i in range(nt):
+        t = int(np.where(idx[:, 1] == r.tr_seed[i])[0][0])
+        np.testing.assert_array_equal(r.track_hits(i), idx[t])
+        assert abs(float(r.tr_par[i, 5])) < 2e-2          # q/pT ~ 0 for a straight line
+
+
+# ----------------------------------------------------------------------------- N1 brute force
+def _small_frame(seed, n_tracks=40, **kw):
+    c = gen.preset(0, seed)
+    c.fixed_tracks = n_tracks
+    for k, v in kw.items():
+        setattr(c, k, v)
+    return gen.generate(c)
+
+
+def _numpy_all_pairs_links(row, pad, time, consts, npads_tab, chi2_cut):
+    """C2 by brute force over ALL hits of rows r+1 / r-1 in fp32 numpy (tiny inputs only)."""
+    f = np.float32
+    sr = row.astype(np.int64)
+    r = sr % N_ROWS
+    y = ((pad - (0.5 * (npads_tab[r] - 1)).astype(f)) * f(0.5)).astype(f)
+    n = row.size
+    up = np.full(n, -1, np.int32); dn = np.full(n, -1, np.int32)
+    Z = f(ZBIN)
+    for h in range(n):
+        if r[h] < 1 or r[h] > N_ROWS - 2:
+            continue
+        best = None
+        for u in np.where(sr == sr[h] + 1)[0]:
+            if not (abs(f(y[u] - y[h])) < consts["Ay"] and abs(f(f(time[u] - time[h]) * Z)) < consts["Az"]):
+                continue
+            for d in np.where(sr == sr[h] - 1)[0]:
+                if not (abs(f(y[d] - y[h])) < consts["Ay"] and abs(f(f(time[d] - time[h]) * Z)) < consts["Az"]):
+                    continue
+                ey = f(f(y[u] - y[h]) - f(y[h] - y[d]))
+                ez = f(f(f(time[u] - time[h]) * Z) - f(f(time[h] - time[d]) * Z))
+                if not (abs(ey) < consts["W1"] and abs(ez) < consts["W1"]):
+                    continue
+                chi2 = f(f(f(ey * ey) * consts["wy"]) + f(f(ez * ez) * consts["wz"]))
+                if not chi2 < chi2_cut:
+                    continue
+                key = (chi2, u, d)
+                if best is None or key < best:
+                    best = key
+        if best is not None:
+            up[h], dn[h] = best[1], best[2]
+    return up, dn
+
+
+def test_N1_brute_force_equals_window_search():
+    """BASELINE.json L5 (b): brute-force all-pairs neighbour search agrees with the windowed search."""
+    tf = _small_frame(7, n_tracks=12)
+    assert tf.n <= 2000
+    g, p = _geom(1, tf.max_time_bin), oracle.default_params()
+    fast = oracle.track(g, p, tf.row, tf.pad, tf.time)
+    p.brute_force = 1
+    brute = oracle.track(g, p, tf.row, tf.pad, tf.time)
+    for name in ("up_raw", "down_raw", "link_up", "link_down", "is_start_hit", "tl_row_hit", "tr_hit_index", "tr_par"):
+        np.testing.assert_array_equal(getattr(fast, name), getattr(brute, name), err_msg=name)
+    # and against an independent all-pairs evaluation in numpy fp32 (tie-breaks on original index)
+    _, npads_tab, _, consts = oracle.tables(g, p)
+    up, dn = _numpy_all_pairs_links(tf.row, tf.pad, tf.time, consts, npads_tab, np.float32(9.0))
+    np.testing.assert_array_equal(fast.up_raw, up)
+    np.testing.assert_array_equal(fast.down_raw, dn)
+    assert (up >= 0).sum() > 200
+
+
+def test_N1_ties_break_on_lowest_original_index():
+    """Two identical candidates in the upper row: the link goes to the lower original index, wherever it sits."""
+    rows = np.array([10, 11, 12, 12])
+    base = clusters_from_xyz(rows, [0.0, 0.1, 0.2, 0.2], [50.0, 50.5, 51.0, 51.0])
+    for perm in ([0, 1, 2, 3], [3, 2, 1, 0], [2, 0, 3, 1]):
+        row, pad, time = (a[perm] for a in base)
+        r = oracle.track(_geom(), oracle.default_params(), row, pad, time)
+        h = perm.index(1)
+        dup = sorted([perm.index(2), perm.index(3)])
+        assert r.up_raw[h] == dup[0] and r.down_raw[h] == perm.index(0)
+
+
+# ----------------------------------------------------------------------------- N3 / invariants
+@pytest.mark.parametrize("seed", [1, 2])
+def test_N3_invariants(seed):
+    """BASELINE.json L5 (c): links reciprocal after cleaning, each hit in at most one track, counts conserved."""
+    tf = _small_frame(seed, n_tracks=150)
+    r = oracle.track(_geom(1, tf.max_time_bin), oracle.default_params(), tf.row, tf.pad, tf.time)
+    h = np.where(r.link_up >= 0)[0]
+    np.testing.assert_array_equal(r.link_down[r.link_up[h]], h)
+    h = np.where(r.link_down >= 0)[0]
+    np.testing.assert_array_equal(r.link_up[r.link_down[h]], h)
+    # links join adjacent rows of the same sector
+    sr = tf.row.astype(np.int64)
+    h = np.where(r.link_up >= 0)[0]
+    np.testing.assert_array_equal(sr[r.link_up[h]], sr[h] + 1)
+    # start hits: no down link, chain of >= 3
+    s = np.where(r.is_start_hit)[0]
+    assert (r.link_down[s] < 0).all()
+    assert (r.link_up[s] >= 0).all() and (r.link_up[r.link_up[s]] >= 0).all()
+    np.testing.assert_array_equal(np.sort(s), np.sort(r.tl_seed))
+    # each hit in at most one final track; hit counts conserved
+    assert np.unique(r.tr_hit_index).size == r.tr_hit_index.size
+    assert int(r.tr_n_hits.sum()) == r.tr_hit_index.size
+    assert (r.tr_n_hits >= 30).all()
+    for i in range(len(r.tr_seed)):
+        hits = r.track_hits(i)
+        rows = sr[hits] % N_ROWS
+        assert (np.diff(rows) > 0).all()                       # ascending row, one hit per row
+        assert rows[0] == r.tr_first_row[i] and rows[-1] == r.tr_last_row[i]
+        t = int(np.where(r.tl_seed == r.tr_seed[i])[0][0])
+        assert set(hits.tolist()) <= set(r.tl_row_hit[t][r.tl_row_hit[t] >= 0].tolist())
+    # tracklet bookkeeping
+    np.testing.assert_array_equal((r.tl_row_hit >= 0).sum(1), r.tl_n_hits)
+
+
+# ----------------------------------------------------------------------------- S1 selector
+def test_S1_selector_equals_sorted_first_come_first_served():
+    tf = _small_frame(4, n_tracks=200)
+    p = oracle.default_params()
+    r = oracle.track(_geom(1, tf.max_time_bin), p, tf.row, tf.pad, tf.time)
+    cand = [i for i in range(len(r.tl_seed)) if r.tl_n_hits[i] >= p.min_hits]
+    cand.sort(key=lambda i: (-int(r.tl_n_hits[i]), int(r.tl_seed[i])))      # key (nHits, -id) descending
+    owner = {}
+    for i in cand:
+        for hidx in r.tl_row_hit[i][r.tl_row_hit[i] >= 0]:
+            owner.setdefault(int(hidx), i)
+    expect = {}
+    for i in cand:
+        own = [int(hidx) for hidx in r.tl_row_hit[i] if hidx >= 0 and owner[int(hidx)] == i]
+        if len(own) >= p.min_hits:
+            expect[int(r.tl_seed[i])] = own
+    assert len(expect) > 20
+    assert sorted(expect) == sorted(r.tr_seed.tolist())
+    for i in range(len(r.tr_seed)):
+        assert expect[int(r.tr_seed[i])] == r.track_hits(i).tolist()
+        t = int(np.where(r.tl_seed == r.tr_seed[i])[0][0])
+        np.testing.assert_array_equal(r.tr_par[i], r.tl_par[t])             # parameters unchanged, no refit
+
+
+# ----------------------------------------------------------------------------- K4 noise-free helices
+def test_K4_noise_free_helices_reconstructed_exactly():
+    """BASELINE.json L5 (a): noise-free helix tracks are reconstructed exactly."""
+    tf = _small_frame(9, n_tracks=12, sigma_y_cm=0.0, sigma_z_cm=0.0, dropout=0.0, noise_frac=0.0, pt_min=0.4)
+    p = oracle.default_params()
+    r = oracle.track(_geom(1, tf.max_time_bin), p, tf.row, tf.pad, tf.time)
+    seg = truth_eval.segment_ids(tf)
+    useg, cnt = np.unique(seg, return_counts=True)
+    long_segs = useg[cnt >= 40]
+    assert len(long_segs) >= 8
+    seg_of_track = {}
+    for i in range(len(r.tr_seed)):
+        s = np.unique(seg[r.track_hits(i)])
+        assert s.size == 1                                                   # pure
+        assert int(s[0]) not in seg_of_track                                 # no clones
+        seg_of_track[int(s[0])] = i
+    x_r = row_x(np.arange(N_ROWS))
+    for s in long_segs:
+        i = seg_of_track[int(s)]
+        hits = np.sort(np.where(seg == s)[0])
+        np.testing.assert_array_equal(np.sort(r.track_hits(i)), hits)        # exactly all its hits
+        tr = tf.tracks[int(s) // (64 * 16)]
+        qpt_true = tr["charge_sense"] / tr["pt"]
+        assert abs(float(r.tr_par[i, 5]) / qpt_true - 1.0) < 1e-3
+        # state at the innermost hit reproduces that hit and the true local direction
+        first = r.track_hits(i)[0]
+        row0 = int(tf.row[first]) % N_ROWS
+        y0 = (float(tf.pad[first]) - 0.5 * (n_pads(row0) - 1)) * 0.5
+        assert abs(float(r.tr_par[i, 1]) - y0) < 1e-4
+        sin_true = math.sin(tr["phi0"]) + tr["charge_sense"] * x_r[row0] / (666.7 * tr["pt"])
+        assert abs(float(r.tr_par[i, 3]) - sin_true) < 1e-4
+        z_rel_true = (float(tf.time[first]) - float(r.tr_par[i, 6])) * ZBIN
+        assert abs(float(r.tr_par[i, 2]) - z_rel_true) < 1e-4
+
+
+# ----------------------------------------------------------------------------- E1 efficiency
+@pytest.mark.parametrize("cid,seed", [(0, 1), (0, 2), (1, 1)])
+def test_E1_efficiency_at_least_95_percent(cid, seed):
+    """BASELINE.json L5 (d): efficiency >= 95 % against generator truth for pT > 0.2 GeV."""
+    cfg = gen.preset(cid, seed)
+    tf = gen.generate(cfg)
+    r = oracle.track(oracle.default_geometry(cfg.n_sectors, tf.max_time_bin),
+                     oracle.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm), tf.row, tf.pad, tf.time)
+    e = truth_eval.evaluate(tf, r.tr_hit_offset, r.tr_n_hits, r.tr_hit_index)
+    assert e["n_findable"] >= 50
+    assert e["efficiency"] >= 0.95, e
+    assert e["fake_rate"] <= 0.02 and e["clone_rate"] <= 0.02, e
