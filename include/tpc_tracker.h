@@ -1,0 +1,161 @@
+/* tpc_tracker.h -- C-ABI boundary of the B200-native TPC time-frame tracker.
+ *
+ * What it is: the step the paper names as "the most computing-intense workload of the synchronous
+ * reconstruction" (§1): TPC sector tracking of a whole continuous-readout time frame held in
+ * GPU memory -- cellular-automaton seeding in native (pad row, pad, time) coordinates ("the track seeding
+ * operates using the time as coordinate instead of the spatial z coordinate") followed by
+ * Kalman-filter track following, "derived from the Run 2 HLT TPC tracking", with "the
+ * reusage of memory for sequential steps of the tracking algorithm".
+ * The entry points and their argument lists are fixed by BASELINE.json L5 (north_star):
+ *   tpc_tracker_create(geometry, params), tpc_track_timeframe(clusters, n, stream, tracks_out),
+ *   tpc_tracker_destroy.  The exact operations (steps C1..C6) are defined in DESIGN.md §3.
+ *
+ * Conventions
+ *   - Plain C, no torch types.  Every pointer is marked DEVICE or HOST.
+ *   - Return value: 0 (TPC_OK) or a negative tpc_status_t.  tpc_strerror() names it.
+ *   - Ownership: the CALLER owns cluster arrays, output arrays and the scratch arena; the handle owns only
+ *     small geometry tables (a few KB of device memory) and CUDA events.  Inputs are never written.
+ *   - tpc_track_timeframe only enqueues work on `cuda_stream`: it never synchronises and never allocates.
+ *     One call in flight per handle; a handle is not thread-safe.
+ *   - All kernels are hand-written CUDA for sm_100a.  There is no CPU fallback: without a CUDA device
+ *     tpc_tracker_create fails with TPC_ECUDA.
+ */
+#ifndef TPC_TRACKER_H_
+#define TPC_TRACKER_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tpc_tracker tpc_tracker_t; /* opaque */
+
+typedef enum {
+  TPC_OK = 0,
+  TPC_EINVAL = -1, /* null pointer, bad geometry / params, n < 0, n > max_clusters, n >= 2^31           */
+  TPC_ENOMEM = -2, /* arena missing or smaller than tpc_tracker_arena_bytes()                            */
+  TPC_ECUDA = -3   /* a CUDA runtime call or kernel launch failed (also: no CUDA device)                 */
+} tpc_status_t;
+
+/* Bits of the device status word tpc_tracks_t::status (0 = everything fitted). */
+enum {
+  TPC_STATUS_TRACKLET_OVERFLOW = 1,  /* more start hits than max_tracklets: the excess was dropped       */
+  TPC_STATUS_TRACK_OVERFLOW = 2,     /* more tracks than max_tracks: *n_tracks holds the required count  */
+  TPC_STATUS_TRACK_HIT_OVERFLOW = 4, /* more track hits than max_track_hits                              */
+  TPC_STATUS_INVALID_CLUSTERS = 8    /* some clusters lay outside the geometry and were ignored          */
+};
+
+/* One parametric geometry serves all configs (BASELINE.json L7, L8).  Sector s of a 36-sector TPC is
+ * s < 18: A side, s >= 18: C side; every sector is tracked in its own local frame.                       */
+typedef struct {
+  int32_t n_sectors;     /* 1 or 36                                                                     */
+  int32_t n_rows;        /* 152 (3 <= n_rows <= 160)                                                    */
+  float x0_cm;           /* 85.0   x_r = (float)((double)x0_cm + (double)row_pitch_cm * r)              */
+  float row_pitch_cm;    /* 1.07                                                                        */
+  float pad_pitch_cm;    /* 0.5                                                                         */
+  float tan_half_sector; /* (float)tan(10 deg); pads_r = floor(2 x_r tan / pad_pitch) in double         */
+  float time_bin_cm;     /* 0.516 = 2.58 cm/us * 0.2 us                                                 */
+  float drift_len_cm;    /* 250 (informative)                                                           */
+  float max_time_bin;    /* upper bound of the time coordinate in a frame; sizes the grid               */
+} tpc_geometry_t;
+
+typedef struct {
+  float win_slope, win_const;     /* 0.05, 0.5 : window W(dx) = win_slope*|dx| + win_const [cm] (BASELINE L7) */
+  float chi2_cut;                 /* 9 : mid-point deviation chi2 of a hit triplet            (BASELINE L7) */
+  int32_t miss_limit, min_hits;   /* 10, 30                                                   (BASELINE L7) */
+  float sigma_y_cm, sigma_z_cm;   /* hit errors used by the tracker (reading A4)                  */
+  float slope_y_max, slope_z_max; /* 1.0, 1.5 : neighbour search area half size per cm of dx  (reading A1)  */
+  int32_t seed_min_hits;          /* 3 : reciprocal chain length that makes a start hit       (reading A7)  */
+  float sin_phi_max;              /* 0.95                                                     (reading A12) */
+  float inv_R_per_qpt;            /* (float)(1/666.7) : curvature [1/cm] per q/pT [1/GeV]     (BASELINE L7) */
+  float c0_y2, c0_s2, c0_k2, c0_z2, c0_t2; /* initial / reset covariance diagonal             (reading A8)  */
+  int32_t grid_time_bins;         /* width of one grid bin in time bins; 0 = default (4)                    */
+  int64_t max_clusters;           /* capacity: largest n of any tpc_track_timeframe call                    */
+  int64_t max_tracklets;          /* capacity of the tracklet store; 0 = max_clusters/10 + 4096             */
+  int64_t max_tracks;             /* host entry point only: staging capacity; 0 = max_clusters/64 + 4096    */
+  int64_t max_track_hits;         /* host entry point only: staging capacity; 0 = max_clusters              */
+  void* arena;                    /* DEVICE, caller-owned scratch (e.g. a torch uint8 tensor), 256-B aligned */
+  size_t arena_bytes;
+  int32_t host_staging;           /* 1: reserve arena space for tpc_track_timeframe_host                    */
+  int32_t profile;                /* 1: record a CUDA event after every step (tpc_tracker_step_ms)          */
+} tpc_params_t;
+
+/* fp32 SoA clusters, n entries each.  row[i] = sector*n_rows + pad_row as an integer-valued float (exact
+ * below 2^24); pad in pad units (pad p covers [p-0.5, p+0.5)); time in time bins; charge is never read.   */
+typedef struct {
+  const float* row;
+  const float* pad;
+  const float* time;
+  const float* charge; /* may be NULL */
+} tpc_clusters_t;
+
+/* Caller-allocated output buffers and their capacities.  DEVICE pointers for tpc_track_timeframe, HOST
+ * pointers for tpc_track_timeframe_host.  Track order is by ascending internal tracklet slot and is
+ * deterministic; `seed_hit` (original index of the start hit) is the unique key of a track.               */
+typedef struct {
+  int32_t max_tracks;
+  int64_t max_track_hits;
+  int32_t* n_tracks;     /* scalar: number of tracks found (may exceed max_tracks, see status)              */
+  int64_t* n_track_hits; /* scalar                                                                          */
+  int32_t* status;       /* scalar: TPC_STATUS_* bits                                                       */
+  int32_t *seed_hit, *sector, *first_row, *last_row, *n_hits; /* [max_tracks]                               */
+  int64_t* hit_offset;   /* [max_tracks] first entry of the track in hit_index                              */
+  float *x, *y, *z_rel, *time_ref, *sin_phi, *dzds, *q_pt;    /* [max_tracks] state at the innermost hit;
+                            z_rel [cm] is relative to time_ref [time bins] (reading A2)           */
+  float* cov9;           /* [max_tracks*9] (yy, ys, ss, yk, sk, kk | zz, zt, tt); may be NULL               */
+  int32_t* hit_index;    /* [max_track_hits] original cluster indices, ascending row, per track contiguous  */
+  /* parity taps, each may be NULL (device entry point only): */
+  int32_t *link_up, *link_down;   /* [n] indexed AND valued by original cluster index, -1 = none, after cleaning */
+  uint8_t* is_start_hit;          /* [n] by original index                                                  */
+  int32_t max_tracklets;          /* capacity of the four tracklet taps                                     */
+  int32_t* n_tracklets;           /* scalar: number of tracklets (= start hits) constructed                 */
+  int32_t* tracklet_seed;         /* [max_tracklets] original index of the start hit                        */
+  int32_t* tracklet_n_hits;       /* [max_tracklets]                                                        */
+  int32_t* tracklet_row_hit;      /* [max_tracklets*n_rows] original indices, -1 = none                     */
+  float* tracklet_par;            /* [max_tracklets*7] (x, y, z_rel, sin_phi, dzds, q_pt, time_ref)         */
+} tpc_tracks_t;
+
+/* Bytes of arena the tracker needs for params->max_clusters (the `max_clusters` argument, if > 0,
+ * overrides it).  Host-side arithmetic only; needs no device.  Returns 0 on invalid arguments.            */
+size_t tpc_tracker_arena_bytes(const tpc_geometry_t* geometry, const tpc_params_t* params, int64_t max_clusters);
+
+/* Validates, builds the per-row tables in double (rounded once to fp32), uploads them and plans the arena
+ * (lifetime-based reuse across steps).  Errors: TPC_EINVAL, TPC_ENOMEM, TPC_ECUDA.          */
+int tpc_tracker_create(const tpc_geometry_t* geometry, const tpc_params_t* params, tpc_tracker_t** out);
+
+/* Tracks one time frame: steps C1 ingest -> C2 neighbours finder -> C3/C4 cleaner + start hits ->
+ * C5 tracklet constructor -> C6 selector, all enqueued on `cuda_stream` (a cudaStream_t; NULL = default).
+ * `clusters` holds DEVICE pointers.  Asynchronous.  Device-detected overflow sets *status.                  */
+int tpc_track_timeframe(tpc_tracker_t* tracker, const tpc_clusters_t* clusters, int64_t n, void* cuda_stream,
+                        tpc_tracks_t* tracks_out);
+
+/* Same, with HOST buffers (pinned for full speed): copies row/pad/time host->device into arena staging,
+ * tracks, copies the scalars and exactly the produced tracks / hits back, and synchronises the stream
+ * before returning.  Needs params->host_staging = 1 at create time.  Taps are ignored.                     */
+int tpc_track_timeframe_host(tpc_tracker_t* tracker, const tpc_clusters_t* host_clusters, int64_t n,
+                             void* cuda_stream, tpc_tracks_t* host_tracks_out);
+
+/* With params->profile = 1: milliseconds of each step of the last completed call (synchronises on the
+ * handle's last event).  ms_out[0..n_steps) in the order of tpc_tracker_step_name().  Returns the number of
+ * steps, or a negative status.                                                                              */
+int tpc_tracker_step_ms(tpc_tracker_t* tracker, float* ms_out, int32_t capacity);
+const char* tpc_tracker_step_name(int32_t step);
+
+/* Number of kernel launches the last tpc_track_timeframe call enqueued (memsets not counted).              */
+int64_t tpc_tracker_last_launches(const tpc_tracker_t* tracker);
+
+/* Arena plan: for allocation i writes name, offset, bytes, first and last step of its lifetime.
+ * Returns the number of allocations; i out of range returns -1.                                            */
+int tpc_tracker_arena_plan(const tpc_tracker_t* tracker, int32_t i, const char** name, size_t* offset,
+                           size_t* bytes, int32_t* first_step, int32_t* last_step);
+
+int tpc_tracker_destroy(tpc_tracker_t* tracker);
+
+const char* tpc_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPC_TRACKER_H_ */

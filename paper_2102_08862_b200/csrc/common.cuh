@@ -1,0 +1,40 @@
+// Device-side definitions shared by the tracker's kernels (sm_100a).  See DESIGN.md §4 (data layout).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace tpc {
+
+constexpr int kRowStride = 160;          // padded row count of one tracklet's row->hit table (5 x 32 lanes)
+constexpr uint32_t kInvalidRank = 0xFFFFFFFFu;
+
+// Constants of one tracker handle, passed by value to every kernel.  All fp32 decision constants are derived
+// on the host in double from the fp32 parameter values and rounded once ("Notation").
+struct Consts {
+  // geometry
+  int n_rows, n_sr, n_tb, n_bins;        // rows per sector, sector-rows, time bins per sector-row, n_sr*n_tb
+  float max_time, inv_bin_w;             // validity bound of the time coordinate; 1 / grid bin width
+  float Z, inv_Z, P;                     // time-bin size [cm], its inverse (grid lookups only), pad pitch
+  // neighbours finder (C2)
+  float W1, Ay, Az, wy, wz, chi2_cut, finder_tw;   // finder_tw: half width of the lookup in time bins (+margin)
+  // tracklet constructor (C5)
+  float ry, rz, cB, sin_phi_max, win_slope, win_const;
+  float c0_y2, c0_s2, c0_k2, c0_z2, c0_t2;
+  int miss_limit, min_hits, seed_min_hits;
+  // per-row tables in device memory owned by the handle
+  const float* xr;                       // [n_rows] x of the pad row
+  const float* cr;                       // [n_rows] pad centre 0.5*(n_pads-1)
+  const int* npads;                      // [n_rows]
+};
+
+// Grid bin of a time value: monotone non-decreasing in t, so a lookup over [bin(t_lo), bin(t_hi)] is a
+// superset of the hits with time in [t_lo, t_hi].  The grid only accelerates; every decision is re-made by
+// the exact fp32 predicate on the candidates.
+__device__ __forceinline__ int time_bin(float t, const Consts& c) {
+  int b = (int)floorf(t * c.inv_bin_w);
+  return min(max(b, 0), c.n_tb - 1);
+}
+
+__device__ __forceinline__ unsigned lane_id() { return threadIdx.x & 31u; }
+
+}  // namespace tpc

@@ -1,0 +1,433 @@
+// C-ABI boundary and host orchestration of the B200-native TPC time-frame tracker (include/tpc_tracker.h).
+// Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo --fmad=false -shared -Xcompiler -fPIC
+// (--fmad=false: the decision arithmetic must round like the definition, BASELINE.json L5.)
+#include "../../include/tpc_tracker.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "arena.h"
+#include "common.cuh"
+#include "finder.cuh"
+#include "ingest.cuh"
+#include "links.cuh"
+#include "scan.cuh"
+#include "selector.cuh"
+#include "tracklet.cuh"
+
+using namespace tpc;
+
+namespace {
+
+enum Step {
+  S_INGEST_COUNT = 0, S_GRID_SCAN, S_INGEST_SCATTER, S_BIN_SORT, S_FINDER, S_CLEAN_START, S_COMPACT,
+  S_CONSTRUCT, S_CLAIM, S_COUNT, S_SELECT_SCAN, S_EMIT, N_STEPS
+};
+const char* const kStepNames[N_STEPS] = {
+    "ingest_count", "grid_scan", "ingest_scatter", "bin_sort", "neighbours_finder", "cleaner_start_hits",
+    "start_hit_compaction", "tracklet_constructor", "selector_claim", "selector_count", "selector_scan",
+    "selector_emit"};
+
+struct Ids {   // arena allocation ids
+  int stage_in = -1, stage_out = -1;
+  int bin_start, rank, yt, orig, hsr, link_up, link_down, link_up_clean, start_flag, cta_count, start_hits,
+      counters, scan_a, scan_b, row_hit, tl_n_hits, tl_first, tl_last, tl_seed, tl_par, tl_cov, claim, owned,
+      flag, track_idx, hit_off;
+};
+
+struct Capacities {
+  int64_t max_clusters, max_tracklets, max_tracks, max_track_hits;
+  int n_tb, n_bins, n_link_ctas;
+};
+
+bool valid_geometry(const tpc_geometry_t* g) {
+  return g && g->n_sectors >= 1 && g->n_rows >= 3 && g->n_rows <= kRowStride &&
+         (int64_t)g->n_sectors * g->n_rows <= 65535 && g->row_pitch_cm > 0 && g->pad_pitch_cm > 0 &&
+         g->tan_half_sector > 0 && g->time_bin_cm > 0 && g->max_time_bin >= 0 && std::isfinite(g->max_time_bin);
+}
+
+bool valid_params(const tpc_params_t* p) {
+  return p && p->miss_limit >= 1 && p->min_hits >= 1 && p->seed_min_hits >= 2 && p->sigma_y_cm > 0 &&
+         p->sigma_z_cm > 0 && p->sin_phi_max > 0 && p->sin_phi_max < 1 && p->grid_time_bins >= 0 &&
+         p->max_clusters >= 0 && p->max_clusters < ((int64_t)1 << 31) && p->max_tracklets >= 0 &&
+         p->max_tracklets < ((int64_t)1 << 31) / kRowStride * 32 && p->max_tracks >= 0 && p->max_track_hits >= 0 &&
+         p->win_const > 0 && p->win_slope >= 0 && p->chi2_cut > 0;
+}
+
+bool capacities(const tpc_geometry_t* g, const tpc_params_t* p, int64_t max_clusters, Capacities& c) {
+  c.max_clusters = max_clusters > 0 ? max_clusters : p->max_clusters;
+  if (c.max_clusters < 1) c.max_clusters = 1;
+  if (c.max_clusters >= ((int64_t)1 << 31)) return false;
+  c.max_tracklets = p->max_tracklets > 0 ? p->max_tracklets : c.max_clusters / 10 + 4096;
+  c.max_tracks = p->max_tracks > 0 ? p->max_tracks : c.max_clusters / 64 + 4096;
+  c.max_track_hits = p->max_track_hits > 0 ? p->max_track_hits : c.max_clusters;
+  const int w = p->grid_time_bins > 0 ? p->grid_time_bins : 4;
+  const double ntb = std::floor((double)g->max_time_bin / (double)w) + 1.0;
+  const double nb = ntb * (double)g->n_sectors * (double)g->n_rows;
+  if (nb >= 2147483000.0) return false;
+  c.n_tb = (int)ntb;
+  c.n_bins = (int)nb;
+  c.n_link_ctas = (int)((c.max_clusters + kLinkThreads - 1) / kLinkThreads);
+  return true;
+}
+
+void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids& id) {
+  const size_t N = (size_t)c.max_clusters, T = (size_t)c.max_tracklets, B = (size_t)c.n_bins + 1;
+  if (p->host_staging) {
+    id.stage_in = plan.add("host_staging_in(row,pad,time)", 3 * 4 * N, S_INGEST_COUNT, S_INGEST_SCATTER);
+    const size_t K = (size_t)c.max_tracks;
+    id.stage_out = plan.add("host_staging_out(tracks)", 256 + K * (5 * 4 + 8 + 7 * 4 + 9 * 4) + 4 * (size_t)c.max_track_hits + 64,
+                            S_EMIT, S_EMIT);
+  }
+  const size_t scan_len = std::max(std::max(scan_tiles(B), scan_tiles((size_t)c.n_link_ctas + 1)), scan_tiles(T)) + 2;
+  id.counters = plan.add("counters", 256, S_INGEST_COUNT, S_EMIT);
+  id.scan_a = plan.add("scan_tile_sums_a", 4 * scan_len, S_INGEST_COUNT, S_EMIT);
+  id.scan_b = plan.add("scan_tile_sums_b", 4 * scan_len, S_INGEST_COUNT, S_EMIT);
+  id.bin_start = plan.add("grid_bin_start", 4 * B, S_INGEST_COUNT, S_CONSTRUCT);
+  id.rank = plan.add("ingest_rank", 4 * N, S_INGEST_COUNT, S_INGEST_SCATTER);
+  id.yt = plan.add("hits_y_time(float2)", 8 * N, S_INGEST_SCATTER, S_CONSTRUCT);
+  id.orig = plan.add("hits_orig_index", 4 * N, S_INGEST_SCATTER, S_EMIT);
+  id.hsr = plan.add("hits_sector_row(u16)", 2 * N, S_INGEST_SCATTER, S_EMIT);
+  id.link_up = plan.add("link_up_raw", 4 * N, S_FINDER, S_CLEAN_START);
+  id.link_down = plan.add("link_down_raw", 4 * N, S_FINDER, S_CLEAN_START);
+  id.link_up_clean = plan.add("link_up_clean", 4 * N, S_CLEAN_START, S_CONSTRUCT);
+  id.start_flag = plan.add("start_flag(u8)", N, S_CLEAN_START, S_COMPACT);
+  id.cta_count = plan.add("start_cta_count", 4 * ((size_t)c.n_link_ctas + 2), S_CLEAN_START, S_COMPACT);
+  id.start_hits = plan.add("start_hits", 4 * T, S_COMPACT, S_EMIT);
+  id.row_hit = plan.add("tracklet_row_hit", 4 * (size_t)kRowStride * T, S_CONSTRUCT, S_EMIT);
+  id.tl_n_hits = plan.add("tracklet_n_hits", 4 * T, S_CONSTRUCT, S_EMIT);
+  id.tl_first = plan.add("tracklet_first_row", 4 * T, S_CONSTRUCT, S_EMIT);
+  id.tl_last = plan.add("tracklet_last_row", 4 * T, S_CONSTRUCT, S_EMIT);
+  id.tl_seed = plan.add("tracklet_seed_orig", 4 * T, S_CONSTRUCT, S_EMIT);
+  id.tl_par = plan.add("tracklet_par", 7 * 4 * T, S_CONSTRUCT, S_EMIT);
+  id.tl_cov = plan.add("tracklet_cov", 9 * 4 * T, S_CONSTRUCT, S_EMIT);
+  id.claim = plan.add("selector_claim(u64)", 8 * N, S_CLAIM, S_EMIT);
+  id.owned = plan.add("selector_owned", 4 * T, S_COUNT, S_EMIT);
+  id.flag = plan.add("selector_flag", 4 * T, S_COUNT, S_EMIT);
+  id.track_idx = plan.add("selector_track_idx", 4 * T, S_SELECT_SCAN, S_EMIT);
+  id.hit_off = plan.add("selector_hit_off", 4 * T, S_SELECT_SCAN, S_EMIT);
+  plan.plan();
+}
+
+}  // namespace
+
+struct tpc_tracker {
+  tpc_geometry_t geom;
+  tpc_params_t params;
+  Capacities cap;
+  ArenaPlan plan;
+  Ids id;
+  Consts consts;
+  void* tables = nullptr;          // device: xr | cr | npads
+  cudaEvent_t ev[N_STEPS + 1] = {};
+  bool profile = false, have_times = false;
+  int64_t last_launches = 0;
+};
+
+extern "C" {
+
+const char* tpc_strerror(int code) {
+  switch (code) {
+    case TPC_OK: return "ok";
+    case TPC_EINVAL: return "invalid argument";
+    case TPC_ENOMEM: return "scratch arena missing or too small";
+    case TPC_ECUDA: return "CUDA error (no device, launch or runtime failure)";
+    default: return "unknown status";
+  }
+}
+
+const char* tpc_tracker_step_name(int32_t step) { return step >= 0 && step < N_STEPS ? kStepNames[step] : nullptr; }
+
+size_t tpc_tracker_arena_bytes(const tpc_geometry_t* g, const tpc_params_t* p, int64_t max_clusters) {
+  if (!valid_geometry(g) || !valid_params(p)) return 0;
+  Capacities c;
+  if (!capacities(g, p, max_clusters, c)) return 0;
+  ArenaPlan plan;
+  Ids id;
+  build_plan(p, c, plan, id);
+  return plan.peak_bytes();
+}
+
+int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_tracker_t** out) {
+  if (!out) return TPC_EINVAL;
+  *out = nullptr;
+  if (!valid_geometry(g) || !valid_params(p)) return TPC_EINVAL;
+  tpc_tracker* t = new (std::nothrow) tpc_tracker();
+  if (!t) return TPC_ENOMEM;
+  t->geom = *g;
+  t->params = *p;
+  if (!capacities(g, p, 0, t->cap)) { delete t; return TPC_EINVAL; }
+  build_plan(p, t->cap, t->plan, t->id);
+  if (!p->arena || p->arena_bytes < t->plan.peak_bytes() || (reinterpret_cast<uintptr_t>(p->arena) & 255)) { delete t; return TPC_ENOMEM; }
+
+  // per-row tables in double, rounded once
+  const int nr = g->n_rows;
+  std::vector<float> xr(nr), cr(nr);
+  std::vector<int> npads(nr);
+  const double pitch = (double)g->row_pitch_cm;
+  for (int r = 0; r < nr; ++r) {
+    const double x = (double)g->x0_cm + pitch * (double)r;
+    xr[r] = (float)x;
+    npads[r] = (int)std::floor(2.0 * x * (double)g->tan_half_sector / (double)g->pad_pitch_cm);
+    if (npads[r] < 1) { delete t; return TPC_EINVAL; }
+    cr[r] = (float)(0.5 * (double)(npads[r] - 1));
+  }
+  int n_dev = 0;
+  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) { cudaGetLastError(); delete t; return TPC_ECUDA; }
+  const size_t tab_bytes = (size_t)nr * 12;
+  if (cudaMalloc(&t->tables, tab_bytes) != cudaSuccess) { cudaGetLastError(); delete t; return TPC_ECUDA; }
+  char* tb = static_cast<char*>(t->tables);
+  if (cudaMemcpy(tb, xr.data(), (size_t)nr * 4, cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemcpy(tb + (size_t)nr * 4, cr.data(), (size_t)nr * 4, cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemcpy(tb + (size_t)nr * 8, npads.data(), (size_t)nr * 4, cudaMemcpyHostToDevice) != cudaSuccess) {
+    cudaGetLastError(); cudaFree(t->tables); delete t; return TPC_ECUDA;
+  }
+
+  Consts& c = t->consts;
+  const int w = p->grid_time_bins > 0 ? p->grid_time_bins : 4;
+  c.n_rows = nr; c.n_sr = g->n_sectors * nr; c.n_tb = t->cap.n_tb; c.n_bins = t->cap.n_bins;
+  c.max_time = g->max_time_bin; c.inv_bin_w = (float)(1.0 / (double)w);
+  c.Z = g->time_bin_cm; c.inv_Z = (float)(1.0 / (double)g->time_bin_cm); c.P = g->pad_pitch_cm;
+  const double w1 = (double)p->win_slope * pitch + (double)p->win_const;
+  c.W1 = (float)w1;
+  c.Ay = (float)((double)p->slope_y_max * pitch + w1);
+  c.Az = (float)((double)p->slope_z_max * pitch + w1);
+  const double sy2 = (double)p->sigma_y_cm * (double)p->sigma_y_cm, sz2 = (double)p->sigma_z_cm * (double)p->sigma_z_cm;
+  c.wy = (float)(1.0 / (6.0 * sy2)); c.wz = (float)(1.0 / (6.0 * sz2));
+  c.ry = (float)sy2; c.rz = (float)sz2;
+  c.chi2_cut = p->chi2_cut;
+  c.finder_tw = (float)((double)c.Az / (double)g->time_bin_cm + 0.02);
+  c.cB = p->inv_R_per_qpt; c.sin_phi_max = p->sin_phi_max; c.win_slope = p->win_slope; c.win_const = p->win_const;
+  c.c0_y2 = p->c0_y2; c.c0_s2 = p->c0_s2; c.c0_k2 = p->c0_k2; c.c0_z2 = p->c0_z2; c.c0_t2 = p->c0_t2;
+  c.miss_limit = p->miss_limit; c.min_hits = p->min_hits; c.seed_min_hits = p->seed_min_hits;
+  c.xr = reinterpret_cast<const float*>(tb);
+  c.cr = reinterpret_cast<const float*>(tb + (size_t)nr * 4);
+  c.npads = reinterpret_cast<const int*>(tb + (size_t)nr * 8);
+
+  t->profile = p->profile != 0;
+  for (int i = 0; i <= N_STEPS; ++i)
+    if (cudaEventCreate(&t->ev[i]) != cudaSuccess) { cudaGetLastError(); tpc_tracker_destroy(t); return TPC_ECUDA; }
+  *out = t;
+  return TPC_OK;
+}
+
+int tpc_tracker_destroy(tpc_tracker_t* t) {
+  if (!t) return TPC_EINVAL;
+  for (int i = 0; i <= N_STEPS; ++i) if (t->ev[i]) cudaEventDestroy(t->ev[i]);
+  if (t->tables) cudaFree(t->tables);
+  delete t;
+  return TPC_OK;
+}
+
+int tpc_tracker_arena_plan(const tpc_tracker_t* t, int32_t i, const char** name, size_t* offset, size_t* bytes,
+                           int32_t* first_step, int32_t* last_step) {
+  if (!t) return -1;
+  const auto& a = t->plan.allocs();
+  if (i < 0 || i >= (int)a.size()) return -1;
+  if (name) *name = a[i].name.c_str();
+  if (offset) *offset = a[i].offset;
+  if (bytes) *bytes = a[i].bytes;
+  if (first_step) *first_step = a[i].first_step;
+  if (last_step) *last_step = a[i].last_step;
+  return (int)a.size();
+}
+
+int64_t tpc_tracker_last_launches(const tpc_tracker_t* t) { return t ? t->last_launches : -1; }
+
+int tpc_tracker_step_ms(tpc_tracker_t* t, float* ms_out, int32_t capacity) {
+  if (!t || !ms_out) return TPC_EINVAL;
+  if (!t->profile || !t->have_times) return TPC_EINVAL;
+  if (cudaEventSynchronize(t->ev[N_STEPS]) != cudaSuccess) { cudaGetLastError(); return TPC_ECUDA; }
+  for (int i = 0; i < N_STEPS && i < capacity; ++i)
+    if (cudaEventElapsedTime(&ms_out[i], t->ev[i], t->ev[i + 1]) != cudaSuccess) { cudaGetLastError(); return TPC_ECUDA; }
+  return N_STEPS;
+}
+
+int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, void* cuda_stream, tpc_tracks_t* o) {
+  if (!t || !cl || !o || n < 0 || n > t->cap.max_clusters) return TPC_EINVAL;
+  if (n > 0 && (!cl->row || !cl->pad || !cl->time)) return TPC_EINVAL;
+  if (!o->n_tracks || !o->n_track_hits || !o->status || o->max_tracks < 0 || o->max_track_hits < 0) return TPC_EINVAL;
+  if (o->max_tracks > 0 && (!o->seed_hit || !o->sector || !o->first_row || !o->last_row || !o->n_hits || !o->hit_offset ||
+                            !o->x || !o->y || !o->z_rel || !o->time_ref || !o->sin_phi || !o->dzds || !o->q_pt)) return TPC_EINVAL;
+  if (o->max_track_hits > 0 && !o->hit_index) return TPC_EINVAL;
+  const bool link_taps = o->link_up || o->link_down || o->is_start_hit;
+  if (link_taps && !(o->link_up && o->link_down && o->is_start_hit)) return TPC_EINVAL;
+  const bool tl_taps = o->tracklet_seed || o->tracklet_n_hits || o->tracklet_row_hit || o->tracklet_par || o->n_tracklets;
+  if (tl_taps && o->max_tracklets < 0) return TPC_EINVAL;
+
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const Consts& c = t->consts;
+  const ArenaPlan& P = t->plan;
+  const Ids& id = t->id;
+  void* A = t->params.arena;
+  const int T = (int)t->cap.max_tracklets;
+  int64_t launches = 0;
+  auto mark = [&](int step) { if (t->profile) cudaEventRecord(t->ev[step], st); };
+
+  uint32_t* bin_start = P.ptr<uint32_t>(A, id.bin_start);
+  uint32_t* rank = P.ptr<uint32_t>(A, id.rank);
+  float2* yt = P.ptr<float2>(A, id.yt);
+  uint32_t* orig = P.ptr<uint32_t>(A, id.orig);
+  uint16_t* hsr = P.ptr<uint16_t>(A, id.hsr);
+  int* link_up = P.ptr<int>(A, id.link_up);
+  int* link_down = P.ptr<int>(A, id.link_down);
+  int* link_up_clean = P.ptr<int>(A, id.link_up_clean);
+  uint8_t* start_flag = P.ptr<uint8_t>(A, id.start_flag);
+  uint32_t* cta_count = P.ptr<uint32_t>(A, id.cta_count);
+  uint32_t* start_hits = P.ptr<uint32_t>(A, id.start_hits);
+  int32_t* counters = P.ptr<int32_t>(A, id.counters);          // [0] tracklets, [1] start hits, [2] invalid clusters
+  uint32_t* n_invalid = reinterpret_cast<uint32_t*>(counters + 2);
+  uint32_t* scan_a = P.ptr<uint32_t>(A, id.scan_a);
+  uint32_t* scan_b = P.ptr<uint32_t>(A, id.scan_b);
+  unsigned long long* claim = P.ptr<unsigned long long>(A, id.claim);
+  uint32_t* owned = P.ptr<uint32_t>(A, id.owned);
+  uint32_t* flag = P.ptr<uint32_t>(A, id.flag);
+  uint32_t* track_idx = P.ptr<uint32_t>(A, id.track_idx);
+  uint32_t* hit_off = P.ptr<uint32_t>(A, id.hit_off);
+  TrackletStore tl;
+  tl.row_hit = P.ptr<int>(A, id.row_hit);
+  tl.n_hits = P.ptr<int>(A, id.tl_n_hits);
+  tl.first_row = P.ptr<int>(A, id.tl_first);
+  tl.last_row = P.ptr<int>(A, id.tl_last);
+  tl.seed_orig = P.ptr<uint32_t>(A, id.tl_seed);
+  tl.par = P.ptr<float>(A, id.tl_par);
+  tl.cov = P.ptr<float>(A, id.tl_cov);
+  tl.cap = (size_t)T;
+
+  const int stream_ctas = (int)std::min<int64_t>(std::max<int64_t>((n + 255) / 256, 1), 148 * 32);
+  const int hit_ctas = (int)std::max<int64_t>((n + 255) / 256, 1);
+  const int link_ctas = (int)std::max<int64_t>((n + kLinkThreads - 1) / kLinkThreads, 1);
+
+  // ---- C1 ingest ----
+  mark(S_INGEST_COUNT);
+  cudaMemsetAsync(bin_start, 0, 4 * ((size_t)c.n_bins + 1), st);
+  cudaMemsetAsync(counters, 0, 256, st);
+  if (link_taps && n > 0) {
+    cudaMemsetAsync(o->link_up, 0xFF, 4 * (size_t)n, st);
+    cudaMemsetAsync(o->link_down, 0xFF, 4 * (size_t)n, st);
+    cudaMemsetAsync(o->is_start_hit, 0, (size_t)n, st);
+  }
+  k_ingest_count<<<stream_ctas, 256, 0, st>>>(cl->row, cl->pad, cl->time, n, bin_start, rank, n_invalid, c); ++launches;
+  mark(S_GRID_SCAN);
+  launches += exclusive_scan_u32(bin_start, bin_start, (size_t)c.n_bins + 1, scan_a, st);
+  mark(S_INGEST_SCATTER);
+  k_ingest_scatter<<<stream_ctas, 256, 0, st>>>(cl->row, cl->pad, cl->time, n, rank, bin_start, yt, orig, hsr, c); ++launches;
+  mark(S_BIN_SORT);
+  k_bin_sort<<<(c.n_bins + 255) / 256, 256, 0, st>>>(bin_start, yt, orig, c.n_bins); ++launches;
+
+  // ---- C2 neighbours finder ----
+  mark(S_FINDER);
+  k_neighbours_finder<<<hit_ctas, 256, 0, st>>>(yt, orig, hsr, bin_start, link_up, link_down, c); ++launches;
+
+  // ---- C3 cleaner + C4 start hits ----
+  mark(S_CLEAN_START);
+  k_clean_links_find_starts<<<link_ctas, kLinkThreads, 0, st>>>(link_up, link_down, bin_start, link_up_clean, start_flag, cta_count,
+                                                                orig, link_taps ? o->link_up : nullptr, o->link_down,
+                                                                o->is_start_hit, c); ++launches;
+  mark(S_COMPACT);
+  launches += exclusive_scan_u32(cta_count, cta_count, (size_t)link_ctas + 1, scan_a, st);
+  k_compact_start_hits<<<link_ctas, kLinkThreads, 0, st>>>(start_flag, cta_count, bin_start, start_hits, (uint32_t)T, link_ctas,
+                                                           counters, c); ++launches;
+
+  // ---- C5 tracklet constructor ----
+  mark(S_CONSTRUCT);
+  const int64_t tl_bound = std::min<int64_t>(T, n / std::max(2, c.seed_min_hits) + 1);   // start hits own disjoint chains
+  k_tracklet_constructor<<<(int)((tl_bound + kTrackletThreads - 1) / kTrackletThreads), kTrackletThreads, 0, st>>>(
+      yt, orig, hsr, bin_start, link_up_clean, start_hits, counters, tl, c); ++launches;
+  const int warp_ctas = (int)((tl_bound * 32 + kSelectorThreads - 1) / kSelectorThreads);
+  if (tl_taps) {
+    k_export_tracklets<<<warp_ctas, kSelectorThreads, 0, st>>>(tl, counters, orig, o->n_tracklets, o->tracklet_seed, o->tracklet_n_hits,
+                                                               o->tracklet_row_hit, o->tracklet_par, o->max_tracklets, c); ++launches;
+  }
+
+  // ---- C6 tracklet selector ----
+  mark(S_CLAIM);
+  if (n > 0) cudaMemsetAsync(claim, 0, 8 * (size_t)n, st);
+  k_selector_claim<<<warp_ctas, kSelectorThreads, 0, st>>>(tl, counters, claim, c); ++launches;
+  mark(S_COUNT);
+  const int cap_warp_ctas = (int)(((int64_t)T * 32 + kSelectorThreads - 1) / kSelectorThreads);
+  k_selector_count<<<cap_warp_ctas, kSelectorThreads, 0, st>>>(tl, counters, claim, owned, flag, T, c); ++launches;
+  mark(S_SELECT_SCAN);
+  launches += exclusive_scan_u32(flag, track_idx, (size_t)T, scan_a, st);
+  launches += exclusive_scan_u32(owned, hit_off, (size_t)T, scan_b, st);
+  mark(S_EMIT);
+  TrackOutputs to;
+  to.max_tracks = o->max_tracks; to.max_track_hits = o->max_track_hits;
+  to.n_tracks = o->n_tracks; to.n_track_hits = o->n_track_hits; to.status = o->status;
+  to.seed_hit = o->seed_hit; to.sector = o->sector; to.first_row = o->first_row; to.last_row = o->last_row; to.n_hits = o->n_hits;
+  to.hit_offset = o->hit_offset; to.x = o->x; to.y = o->y; to.z_rel = o->z_rel; to.time_ref = o->time_ref;
+  to.sin_phi = o->sin_phi; to.dzds = o->dzds; to.q_pt = o->q_pt; to.cov9 = o->cov9; to.hit_index = o->hit_index;
+  const int n_scan_tiles = (int)scan_tiles((size_t)T);
+  k_selector_emit<<<std::max(warp_ctas, 1), kSelectorThreads, 0, st>>>(tl, counters, claim, flag, track_idx, hit_off, scan_a + n_scan_tiles,
+                                                                       scan_b + n_scan_tiles, orig, hsr, start_hits, n_invalid, to, c); ++launches;
+  mark(N_STEPS);
+  t->have_times = t->profile;
+  t->last_launches = launches;
+  if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;
+  return TPC_OK;
+}
+
+int tpc_track_timeframe_host(tpc_tracker_t* t, const tpc_clusters_t* hc, int64_t n, void* cuda_stream, tpc_tracks_t* ho) {
+  if (!t || !hc || !ho || n < 0 || n > t->cap.max_clusters) return TPC_EINVAL;
+  if (t->id.stage_in < 0) return TPC_EINVAL;
+  if (n > 0 && (!hc->row || !hc->pad || !hc->time)) return TPC_EINVAL;
+  if (!ho->n_tracks || !ho->n_track_hits || !ho->status) return TPC_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  void* A = t->params.arena;
+  const size_t N = (size_t)t->cap.max_clusters;
+  float* d_in = t->plan.ptr<float>(A, t->id.stage_in);
+  const int64_t K = std::min<int64_t>(t->cap.max_tracks, ho->max_tracks);
+  const int64_t H = std::min<int64_t>(t->cap.max_track_hits, ho->max_track_hits);
+  // carve the output staging block
+  char* p = t->plan.ptr<char>(A, t->id.stage_out);
+  auto take = [&](size_t bytes) { char* q = p; p += (bytes + 15) / 16 * 16; return q; };
+  tpc_tracks_t d;
+  std::memset(&d, 0, sizeof(d));
+  d.max_tracks = (int32_t)K; d.max_track_hits = H;
+  d.n_track_hits = reinterpret_cast<int64_t*>(take(8));
+  d.n_tracks = reinterpret_cast<int32_t*>(take(4));
+  d.status = reinterpret_cast<int32_t*>(take(4));
+  d.hit_offset = reinterpret_cast<int64_t*>(take(8 * (size_t)K));
+  int32_t** i32s[] = {&d.seed_hit, &d.sector, &d.first_row, &d.last_row, &d.n_hits};
+  for (auto pp : i32s) *pp = reinterpret_cast<int32_t*>(take(4 * (size_t)K));
+  float** f32s[] = {&d.x, &d.y, &d.z_rel, &d.time_ref, &d.sin_phi, &d.dzds, &d.q_pt};
+  for (auto pp : f32s) *pp = reinterpret_cast<float*>(take(4 * (size_t)K));
+  d.cov9 = ho->cov9 ? reinterpret_cast<float*>(take(36 * (size_t)K)) : nullptr;
+  d.hit_index = reinterpret_cast<int32_t*>(take(4 * (size_t)H));
+
+  tpc_clusters_t dc;
+  dc.row = d_in; dc.pad = d_in + N; dc.time = d_in + 2 * N; dc.charge = nullptr;
+  if (n > 0) {
+    if (cudaMemcpyAsync(d_in, hc->row, 4 * (size_t)n, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(d_in + N, hc->pad, 4 * (size_t)n, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(d_in + 2 * N, hc->time, 4 * (size_t)n, cudaMemcpyHostToDevice, st) != cudaSuccess) {
+      cudaGetLastError(); return TPC_ECUDA;
+    }
+  }
+  const int rc = tpc_track_timeframe(t, &dc, n, cuda_stream, &d);
+  if (rc != TPC_OK) return rc;
+  struct { int64_t nh; int32_t nt; int32_t status; } head;
+  if (cudaMemcpyAsync(&head.nh, d.n_track_hits, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+      cudaMemcpyAsync(&head.nt, d.n_tracks, 4, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+      cudaMemcpyAsync(&head.status, d.status, 4, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+      cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return TPC_ECUDA; }
+  *ho->n_tracks = head.nt; *ho->n_track_hits = head.nh; *ho->status = head.status;
+  const size_t k = (size_t)std::min<int64_t>(head.nt, K), h = (size_t)std::min<int64_t>(head.nh, H);
+  bool ok = true;
+  auto back = [&](void* dst, const void* src, size_t bytes) {
+    if (dst && bytes) ok = ok && cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  };
+  back(ho->hit_offset, d.hit_offset, 8 * k);
+  back(ho->seed_hit, d.seed_hit, 4 * k); back(ho->sector, d.sector, 4 * k); back(ho->first_row, d.first_row, 4 * k);
+  back(ho->last_row, d.last_row, 4 * k); back(ho->n_hits, d.n_hits, 4 * k);
+  back(ho->x, d.x, 4 * k); back(ho->y, d.y, 4 * k); back(ho->z_rel, d.z_rel, 4 * k); back(ho->time_ref, d.time_ref, 4 * k);
+  back(ho->sin_phi, d.sin_phi, 4 * k); back(ho->dzds, d.dzds, 4 * k); back(ho->q_pt, d.q_pt, 4 * k);
+  if (d.cov9) back(ho->cov9, d.cov9, 36 * k);
+  back(ho->hit_index, d.hit_index, 4 * h);
+  if (!ok || cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return TPC_ECUDA; }
+  return TPC_OK;
+}
+
+}  // extern "C"

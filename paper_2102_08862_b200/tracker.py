@@ -1,0 +1,281 @@
+"""Thin Python binding of the C-ABI in ``include/tpc_tracker.h`` (same names; argument marshalling only).
+
+PyTorch is used for device memory and streams, nothing else: every step of the path runs in the CUDA kernels of
+``csrc/``.  There is no CPU fallback -- a missing library or a missing GPU raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import math
+import os
+from dataclasses import dataclass
+
+from . import build as _build
+
+TPC_OK, TPC_EINVAL, TPC_ENOMEM, TPC_ECUDA = 0, -1, -2, -3
+STATUS_TRACKLET_OVERFLOW, STATUS_TRACK_OVERFLOW, STATUS_TRACK_HIT_OVERFLOW, STATUS_INVALID_CLUSTERS = 1, 2, 4, 8
+
+EXPORTS = ("tpc_tracker_arena_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
+           "tpc_tracker_step_ms", "tpc_tracker_step_name", "tpc_tracker_last_launches", "tpc_tracker_arena_plan",
+           "tpc_tracker_destroy", "tpc_strerror")
+
+
+class Geometry(C.Structure):
+    """``tpc_geometry_t``"""
+    _fields_ = [("n_sectors", C.c_int32), ("n_rows", C.c_int32), ("x0_cm", C.c_float), ("row_pitch_cm", C.c_float),
+                ("pad_pitch_cm", C.c_float), ("tan_half_sector", C.c_float), ("time_bin_cm", C.c_float),
+                ("drift_len_cm", C.c_float), ("max_time_bin", C.c_float)]
+
+
+class Params(C.Structure):
+    """``tpc_params_t``"""
+    _fields_ = [("win_slope", C.c_float), ("win_const", C.c_float), ("chi2_cut", C.c_float),
+                ("miss_limit", C.c_int32), ("min_hits", C.c_int32), ("sigma_y_cm", C.c_float), ("sigma_z_cm", C.c_float),
+                ("slope_y_max", C.c_float), ("slope_z_max", C.c_float), ("seed_min_hits", C.c_int32),
+                ("sin_phi_max", C.c_float), ("inv_R_per_qpt", C.c_float),
+                ("c0_y2", C.c_float), ("c0_s2", C.c_float), ("c0_k2", C.c_float), ("c0_z2", C.c_float), ("c0_t2", C.c_float),
+                ("grid_time_bins", C.c_int32), ("max_clusters", C.c_int64), ("max_tracklets", C.c_int64),
+                ("max_tracks", C.c_int64), ("max_track_hits", C.c_int64), ("arena", C.c_void_p), ("arena_bytes", C.c_size_t),
+                ("host_staging", C.c_int32), ("profile", C.c_int32)]
+
+
+class Clusters(C.Structure):
+    """``tpc_clusters_t``"""
+    _fields_ = [("row", C.c_void_p), ("pad", C.c_void_p), ("time", C.c_void_p), ("charge", C.c_void_p)]
+
+
+class Tracks(C.Structure):
+    """``tpc_tracks_t``"""
+    _fields_ = [("max_tracks", C.c_int32), ("max_track_hits", C.c_int64),
+                ("n_tracks", C.c_void_p), ("n_track_hits", C.c_void_p), ("status", C.c_void_p),
+                ("seed_hit", C.c_void_p), ("sector", C.c_void_p), ("first_row", C.c_void_p), ("last_row", C.c_void_p),
+                ("n_hits", C.c_void_p), ("hit_offset", C.c_void_p),
+                ("x", C.c_void_p), ("y", C.c_void_p), ("z_rel", C.c_void_p), ("time_ref", C.c_void_p),
+                ("sin_phi", C.c_void_p), ("dzds", C.c_void_p), ("q_pt", C.c_void_p), ("cov9", C.c_void_p),
+                ("hit_index", C.c_void_p), ("link_up", C.c_void_p), ("link_down", C.c_void_p), ("is_start_hit", C.c_void_p),
+                ("max_tracklets", C.c_int32), ("n_tracklets", C.c_void_p), ("tracklet_seed", C.c_void_p),
+                ("tracklet_n_hits", C.c_void_p), ("tracklet_row_hit", C.c_void_p), ("tracklet_par", C.c_void_p)]
+
+
+def default_geometry(n_sectors: int = 36, max_time_bin: float = 487.0) -> Geometry:
+    """BASELINE.json L7: 152 rows at 85.0 + 1.07 r cm, 0.5 cm pads, +-10 degree sectors, 0.516 cm time bins."""
+    return Geometry(n_sectors, 152, 85.0, 1.07, 0.5, math.tan(math.radians(10.0)), 0.516, 250.0, max_time_bin)
+
+
+def default_params(sigma_y: float = 0.08, sigma_z: float = 0.12, max_clusters: int = 0) -> Params:
+    """BASELINE.json L7 cuts and the readings of DESIGN.md §3."""
+    return Params(win_slope=0.05, win_const=0.5, chi2_cut=9.0, miss_limit=10, min_hits=30,
+                  sigma_y_cm=sigma_y, sigma_z_cm=sigma_z, slope_y_max=1.0, slope_z_max=1.5, seed_min_hits=3,
+                  sin_phi_max=0.95, inv_R_per_qpt=1.0 / 666.7, c0_y2=1.0, c0_s2=0.1, c0_k2=100.0, c0_z2=1.0, c0_t2=0.1,
+                  grid_time_bins=0, max_clusters=max_clusters, max_tracklets=0, max_tracks=0, max_track_hits=0,
+                  arena=None, arena_bytes=0, host_staging=0, profile=0)
+
+
+_lib = None
+
+
+def load_library(build_if_missing: bool = True):
+    """Loads ``csrc/libtpctracker.so`` (building it in-tree if missing or stale).  Raises if that fails."""
+    global _lib
+    if _lib is None:
+        path = _build.build_cuda() if build_if_missing else _build.LIB
+        if not os.path.exists(path):
+            raise RuntimeError(f"CUDA library {path} is missing; run __graft_entry__.build()")
+        L = C.CDLL(path)
+        vp = C.c_void_p
+        L.tpc_tracker_arena_bytes.argtypes = [C.POINTER(Geometry), C.POINTER(Params), C.c_int64]
+        L.tpc_tracker_arena_bytes.restype = C.c_size_t
+        L.tpc_tracker_create.argtypes = [C.POINTER(Geometry), C.POINTER(Params), C.POINTER(vp)]
+        L.tpc_track_timeframe.argtypes = [vp, C.POINTER(Clusters), C.c_int64, vp, C.POINTER(Tracks)]
+        L.tpc_track_timeframe_host.argtypes = [vp, C.POINTER(Clusters), C.c_int64, vp, C.POINTER(Tracks)]
+        L.tpc_tracker_step_ms.argtypes = [vp, C.POINTER(C.c_float), C.c_int32]
+        L.tpc_tracker_step_name.argtypes = [C.c_int32]
+        L.tpc_tracker_step_name.restype = C.c_char_p
+        L.tpc_tracker_last_launches.argtypes = [vp]
+        L.tpc_tracker_last_launches.restype = C.c_int64
+        L.tpc_tracker_arena_plan.argtypes = [vp, C.c_int32, C.POINTER(C.c_char_p), C.POINTER(C.c_size_t),
+                                             C.POINTER(C.c_size_t), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+        L.tpc_tracker_destroy.argtypes = [vp]
+        L.tpc_strerror.argtypes = [C.c_int]
+        L.tpc_strerror.restype = C.c_char_p
+        for nm in ("tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host", "tpc_tracker_step_ms",
+                   "tpc_tracker_arena_plan", "tpc_tracker_destroy"):
+            getattr(L, nm).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+class TpcError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {load_library().tpc_strerror(code).decode()} ({code})")
+
+
+def tpc_tracker_arena_bytes(geometry: Geometry, params: Params, max_clusters: int = 0) -> int:
+    return int(load_library().tpc_tracker_arena_bytes(C.byref(geometry), C.byref(params), int(max_clusters)))
+
+
+@dataclass
+class TrackResult:
+    """Device (or pinned host) tensors written by one call; ``n_tracks`` etc. are 0-dim-like 1-element tensors."""
+    n_tracks: object
+    n_track_hits: object
+    status: object
+    seed_hit: object
+    sector: object
+    first_row: object
+    last_row: object
+    n_hits: object
+    hit_offset: object
+    x: object
+    y: object
+    z_rel: object
+    time_ref: object
+    sin_phi: object
+    dzds: object
+    q_pt: object
+    cov9: object
+    hit_index: object
+    link_up: object = None
+    link_down: object = None
+    is_start_hit: object = None
+    n_tracklets: object = None
+    tracklet_seed: object = None
+    tracklet_n_hits: object = None
+    tracklet_row_hit: object = None
+    tracklet_par: object = None
+
+
+class Tracker:
+    """``tpc_tracker_create`` / ``tpc_track_timeframe`` / ``tpc_tracker_destroy`` with torch-owned buffers."""
+
+    def __init__(self, geometry: Geometry, params: Params, device: str = "cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the tracker has no CPU fallback")
+        self._torch = torch
+        self.lib = load_library()
+        self.device = torch.device(device)
+        self.geometry = geometry
+        self.params = Params.from_buffer_copy(params)
+        need = self.lib.tpc_tracker_arena_bytes(C.byref(geometry), C.byref(self.params), 0)
+        if need == 0:
+            raise TpcError(TPC_EINVAL, "tpc_tracker_arena_bytes")
+        with torch.cuda.device(self.device):
+            self.arena = torch.empty(int(need) + 256, dtype=torch.uint8, device=self.device)
+            base = (self.arena.data_ptr() + 255) // 256 * 256
+            self.params.arena = base
+            self.params.arena_bytes = int(need)
+            self.handle = C.c_void_p()
+            rc = self.lib.tpc_tracker_create(C.byref(geometry), C.byref(self.params), C.byref(self.handle))
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_tracker_create")
+        self.arena_bytes = int(need)
+
+    # -- buffers ---------------------------------------------------------------------------------------------
+    def _alloc_outputs(self, n: int, max_tracks: int, max_track_hits: int, taps: bool, max_tracklets: int, host: bool):
+        torch = self._torch
+        kw = dict(device="cpu", pin_memory=True) if host else dict(device=self.device)
+        e = lambda shape, dt: torch.empty(shape, dtype=dt, **kw)
+        K, H = max_tracks, max_track_hits
+        r = TrackResult(
+            n_tracks=e(1, torch.int32), n_track_hits=e(1, torch.int64), status=e(1, torch.int32),
+            seed_hit=e(K, torch.int32), sector=e(K, torch.int32), first_row=e(K, torch.int32), last_row=e(K, torch.int32),
+            n_hits=e(K, torch.int32), hit_offset=e(K, torch.int64),
+            x=e(K, torch.float32), y=e(K, torch.float32), z_rel=e(K, torch.float32), time_ref=e(K, torch.float32),
+            sin_phi=e(K, torch.float32), dzds=e(K, torch.float32), q_pt=e(K, torch.float32), cov9=e((K, 9), torch.float32),
+            hit_index=e(H, torch.int32))
+        if taps:
+            nr = self.geometry.n_rows
+            r.link_up, r.link_down, r.is_start_hit = e(n, torch.int32), e(n, torch.int32), e(n, torch.uint8)
+            r.n_tracklets = e(1, torch.int32)
+            r.tracklet_seed, r.tracklet_n_hits = e(max_tracklets, torch.int32), e(max_tracklets, torch.int32)
+            r.tracklet_row_hit = e((max_tracklets, nr), torch.int32)
+            r.tracklet_par = e((max_tracklets, 7), torch.float32)
+        return r
+
+    @staticmethod
+    def _tracks_struct(r: TrackResult, max_tracks: int, max_track_hits: int, max_tracklets: int) -> Tracks:
+        p = lambda t: (t.data_ptr() if t is not None else None)
+        return Tracks(max_tracks, max_track_hits, p(r.n_tracks), p(r.n_track_hits), p(r.status), p(r.seed_hit), p(r.sector),
+                      p(r.first_row), p(r.last_row), p(r.n_hits), p(r.hit_offset), p(r.x), p(r.y), p(r.z_rel), p(r.time_ref),
+                      p(r.sin_phi), p(r.dzds), p(r.q_pt), p(r.cov9), p(r.hit_index), p(r.link_up), p(r.link_down),
+                      p(r.is_start_hit), max_tracklets, p(r.n_tracklets), p(r.tracklet_seed), p(r.tracklet_n_hits),
+                      p(r.tracklet_row_hit), p(r.tracklet_par))
+
+    def default_capacities(self, n: int):
+        return max(n // 64 + 4096, 1), max(n, 1)
+
+    def alloc_outputs(self, n: int, taps: bool = False, host: bool = False, max_tracks: int = 0, max_track_hits: int = 0):
+        K, H = self.default_capacities(n)
+        K, H = (max_tracks or K), (max_track_hits or H)
+        T = int(self.params.max_tracklets or (self.params.max_clusters // 10 + 4096)) if taps else 0
+        out = self._alloc_outputs(n, K, H, taps, T, host)
+        return out, self._tracks_struct(out, K, H, T)
+
+    # -- the C-ABI calls -------------------------------------------------------------------------------------
+    def tpc_track_timeframe(self, row, pad, time, n: int | None = None, outputs=None, taps: bool = False, stream=None):
+        """Device tensors in, device tensors out; asynchronous on ``stream`` (default: torch's current stream)."""
+        torch = self._torch
+        n = int(row.shape[0]) if n is None else int(n)
+        for t in (row, pad, time):
+            if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.shape[0] >= n):
+                raise ValueError("clusters must be contiguous float32 CUDA tensors of length >= n")
+        if outputs is None:
+            outputs = self.alloc_outputs(n, taps=taps)
+        out, st = outputs
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        cl = Clusters(row.data_ptr(), pad.data_ptr(), time.data_ptr(), None)
+        rc = self.lib.tpc_track_timeframe(self.handle, C.byref(cl), n, C.c_void_p(s.cuda_stream), C.byref(st))
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_track_timeframe")
+        return out
+
+    def tpc_track_timeframe_host(self, row, pad, time, n: int | None = None, outputs=None, stream=None):
+        """Host (pinned) tensors in and out; H2D + tracking + D2H inside the call; synchronous."""
+        torch = self._torch
+        n = int(row.shape[0]) if n is None else int(n)
+        for t in (row, pad, time):
+            if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
+                raise ValueError("clusters must be contiguous float32 host tensors")
+        if outputs is None:
+            outputs = self.alloc_outputs(n, host=True, max_tracks=int(self.params.max_tracks or 0),
+                                         max_track_hits=int(self.params.max_track_hits or 0))
+        out, st = outputs
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        cl = Clusters(row.data_ptr(), pad.data_ptr(), time.data_ptr(), None)
+        rc = self.lib.tpc_track_timeframe_host(self.handle, C.byref(cl), n, C.c_void_p(s.cuda_stream), C.byref(st))
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_track_timeframe_host")
+        return out
+
+    def step_ms(self) -> dict:
+        buf = (C.c_float * 32)()
+        k = self.lib.tpc_tracker_step_ms(self.handle, buf, 32)
+        if k < 0:
+            raise TpcError(k, "tpc_tracker_step_ms")
+        return {self.lib.tpc_tracker_step_name(i).decode(): float(buf[i]) for i in range(k)}
+
+    def last_launches(self) -> int:
+        return int(self.lib.tpc_tracker_last_launches(self.handle))
+
+    def arena_plan(self) -> list:
+        out, i = [], 0
+        name, off, nb, a, b = C.c_char_p(), C.c_size_t(), C.c_size_t(), C.c_int32(), C.c_int32()
+        while self.lib.tpc_tracker_arena_plan(self.handle, i, C.byref(name), C.byref(off), C.byref(nb), C.byref(a), C.byref(b)) > 0:
+            out.append(dict(name=name.value.decode(), offset=off.value, bytes=nb.value, first_step=a.value, last_step=b.value))
+            i += 1
+        return out
+
+    def tpc_tracker_destroy(self):
+        if getattr(self, "handle", None) is not None and self.handle:
+            self.lib.tpc_tracker_destroy(self.handle)
+            self.handle = None
+
+    close = tpc_tracker_destroy
+
+    def __del__(self):
+        try:
+            self.tpc_tracker_destroy()
+        except Exception:
+            pass

@@ -1,0 +1,206 @@
+"""Parity of the CUDA path (through the C-ABI) with the oracle, element by element on the same seeded inputs.
+
+Bit-exact: cleaned neighbour links, start hits, tracklet row->hit tables, track hit lists.  Fits: y, z within
+1e-3 cm, q/pT within 1e-4 relative (BASELINE.json L5).  Run on the B200 box: ``pytest -m gpu``.
+"""
+import numpy as np
+import pytest
+
+from helpers import N_ROWS, clusters_from_xyz, concat, row_x
+from paper_2102_08862_b200 import gen
+import parity_util as PU
+
+pytestmark = pytest.mark.gpu
+
+
+def _frame(cid, seed, frame_us=None, **kw):
+    c = gen.preset(cid, seed, frame_us)
+    for k, v in kw.items():
+        setattr(c, k, v)
+    return c, gen.generate(c)
+
+
+def _both(tf, cfg, time=None, tmax=None, **overrides):
+    time = tf.time if time is None else time
+    tmax = tf.max_time_bin if tmax is None else tmax
+    g = PU.run_gpu(tf.row, tf.pad, time, cfg.n_sectors, tmax, cfg.sigma_y_cm, cfg.sigma_z_cm, **overrides)
+    o = PU.run_oracle(tf.row, tf.pad, time, cfg.n_sectors, tmax, cfg.sigma_y_cm, cfg.sigma_z_cm, **overrides)
+    return g, o
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_config0_single_sector(seed):
+    cfg, tf = _frame(0, seed)
+    g, o = _both(tf, cfg)
+    rep = PU.compare(g, o)
+    assert rep["n_tracks"] > 50 and rep["n_links"] > 1000
+    assert rep["track_par_bit_identical"] and rep["tracklet_par_bit_identical"]
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_config1_full_tpc(seed):
+    cfg, tf = _frame(1, seed)
+    g, o = _both(tf, cfg)
+    rep = PU.compare(g, o)
+    assert rep["n_tracks"] > 5000
+    assert rep["track_par_bit_identical"] and rep["tracklet_par_bit_identical"] and rep["track_cov_bit_identical"]
+
+
+@pytest.mark.parametrize("cid,seed", [(2, 1), (3, 2), (4, 1), (4, 3)])
+def test_continuous_readout_short_frames(cid, seed):
+    """configs[2..4] with the frame cut to 150 us (7-8 overlapping collisions): same generator, oracle-sized."""
+    cfg, tf = _frame(cid, seed, frame_us=150.0)
+    g, o = _both(tf, cfg)
+    rep = PU.compare(g, o)
+    assert rep["n_tracks"] > 1000
+
+
+def test_time_coordinate_at_the_end_of_a_10ms_frame():
+    """fp32 time values near 5e4 bins (ulp 2^-8 bin): all z arithmetic is on differences of raw time values."""
+    cfg, tf = _frame(3, 5, frame_us=100.0)
+    time = (tf.time.astype(np.float64) + 49000.0).astype(np.float32)
+    g, o = _both(tf, cfg, time=time, tmax=tf.max_time_bin + 49000.0)
+    rep = PU.compare(g, o)
+    assert rep["n_tracks"] > 500
+
+
+@pytest.mark.parametrize("grid_time_bins", [1, 3, 16])
+def test_grid_bin_width_does_not_change_results(grid_time_bins):
+    """The grid only accelerates (BASELINE.json L5 (b)): any bin width gives the oracle's links and tracks."""
+    cfg, tf = _frame(0, 4)
+    g = PU.run_gpu(tf.row, tf.pad, tf.time, 1, tf.max_time_bin, grid_time_bins=grid_time_bins)
+    o = PU.run_oracle(tf.row, tf.pad, tf.time, 1, tf.max_time_bin)
+    PU.compare(g, o)
+
+
+def test_other_cuts():
+    cfg, tf = _frame(0, 6)
+    g, o = _both(tf, cfg, seed_min_hits=5, miss_limit=4, min_hits=20, chi2_cut=4.0)
+    PU.compare(g, o)
+
+
+def test_empty_and_tiny_inputs():
+    e = np.zeros(0, np.float32)
+    g = PU.run_gpu(e, e, e, 36, 487.0)
+    assert int(g["n_tracks"][0]) == 0 and int(g["n_track_hits"][0]) == 0 and int(g["status"][0]) == 0
+    assert int(g["n_tracklets"][0]) == 0
+    one = clusters_from_xyz([5], [0.3], [100.0])
+    g = PU.run_gpu(*one, 1, 487.0)
+    o = PU.run_oracle(*one, 1, 487.0)
+    PU.compare(g, o)
+    assert int(g["n_tracks"][0]) == 0
+
+
+def test_invalid_clusters_are_ignored_and_flagged():
+    cfg, tf = _frame(0, 2)
+    row, pad, time = tf.row.copy(), tf.pad.copy(), tf.time.copy()
+    row[::97] = 152.0            # beyond the single sector
+    row[5::101] += 0.5           # not an integer
+    pad[3::89] = 400.0
+    pad[7::83] = -0.75
+    time[11::79] = -1.0
+    time[13::73] = tf.max_time_bin + 10.0
+    g = PU.run_gpu(row, pad, time, 1, tf.max_time_bin)
+    o = PU.run_oracle(row, pad, time, 1, tf.max_time_bin)
+    PU.compare(g, o)
+    assert int(g["status"][0]) & 8
+    assert o.stats["invalid_clusters"] > 500
+
+
+def test_duplicate_hits_tie_break_on_original_index():
+    """Exact duplicates of whole tracks: every chi2 / distance tie must go to the lowest original index."""
+    rows = np.arange(N_ROWS)
+    x = row_x(rows)
+    parts = []
+    for i in range(4):
+        y = (-0.1 + 0.06 * i) * x
+        z = 100.0 + 0.3 * i * (x - 85.0)
+        p = clusters_from_xyz(rows, y, z)
+        parts += [p, p]                                   # each track twice
+    row, pad, time = concat(parts)
+    rng = np.random.default_rng(3)
+    perm = rng.permutation(row.size)
+    row, pad, time = row[perm], pad[perm], time[perm]
+    g = PU.run_gpu(row, pad, time, 1, 487.0)
+    o = PU.run_oracle(row, pad, time, 1, 487.0)
+    rep = PU.compare(g, o)
+    assert rep["n_tracks"] >= 4
+
+
+def test_runs_are_deterministic_including_output_order():
+    cfg, tf = _frame(1, 7)
+    a = PU.run_gpu(tf.row, tf.pad, tf.time, 36, tf.max_time_bin)
+    b = PU.run_gpu(tf.row, tf.pad, tf.time, 36, tf.max_time_bin)
+    k, h = int(a["n_tracks"][0]), int(a["n_track_hits"][0])
+    assert k == int(b["n_tracks"][0])
+    for name in ("seed_hit", "n_hits", "hit_offset", "q_pt", "y"):
+        np.testing.assert_array_equal(a[name][:k], b[name][:k])
+    np.testing.assert_array_equal(a["hit_index"][:h], b["hit_index"][:h])
+    nt = int(a["n_tracklets"][0])
+    np.testing.assert_array_equal(a["tracklet_seed"][:nt], b["tracklet_seed"][:nt])
+
+
+def test_capacity_overflow_sets_status_and_keeps_a_valid_prefix():
+    import torch
+    from paper_2102_08862_b200 import tracker as T
+    cfg, tf = _frame(0, 1)
+    full = PU.run_gpu(tf.row, tf.pad, tf.time, 1, tf.max_time_bin)
+    k = int(full["n_tracks"][0])
+    g = T.default_geometry(1, tf.max_time_bin)
+    p = T.default_params(max_clusters=tf.n)
+    trk = T.Tracker(g, p)
+    d = [torch.from_numpy(a).cuda() for a in (tf.row, tf.pad, tf.time)]
+    outs = trk.alloc_outputs(tf.n, max_tracks=10, max_track_hits=500)
+    out = trk.tpc_track_timeframe(*d, outputs=outs)
+    torch.cuda.synchronize()
+    assert int(out.status[0]) & 2 and int(out.status[0]) & 4
+    assert int(out.n_tracks[0]) == k
+    np.testing.assert_array_equal(out.seed_hit.cpu().numpy(), full["seed_hit"][:10])
+    trk.close()
+    p = T.default_params(max_clusters=tf.n)
+    p.max_tracklets = 100
+    trk = T.Tracker(g, p)
+    out = trk.tpc_track_timeframe(*d)
+    torch.cuda.synchronize()
+    assert int(out.status[0]) & 1
+    trk.close()
+
+
+def test_host_entry_point_matches_device_entry_point():
+    import torch
+    from paper_2102_08862_b200 import tracker as T
+    cfg, tf = _frame(1, 2)
+    ref = PU.run_gpu(tf.row, tf.pad, tf.time, 36, tf.max_time_bin, taps=False)
+    g = T.default_geometry(36, tf.max_time_bin)
+    p = T.default_params(max_clusters=tf.n)
+    p.host_staging = 1
+    trk = T.Tracker(g, p)
+    h = [torch.from_numpy(a).pin_memory() for a in (tf.row, tf.pad, tf.time)]
+    out = trk.tpc_track_timeframe_host(*h)
+    k, nh = int(out.n_tracks[0]), int(out.n_track_hits[0])
+    assert k == int(ref["n_tracks"][0]) and nh == int(ref["n_track_hits"][0])
+    for name in ("seed_hit", "sector", "first_row", "last_row", "n_hits", "hit_offset", "x", "y", "z_rel", "time_ref",
+                 "sin_phi", "dzds", "q_pt", "cov9"):
+        np.testing.assert_array_equal(getattr(out, name).numpy()[:k], ref[name][:k], err_msg=name)
+    np.testing.assert_array_equal(out.hit_index.numpy()[:nh], ref["hit_index"][:nh])
+    trk.close()
+
+
+def test_arena_plan_reuses_memory_across_steps():
+    from paper_2102_08862_b200 import tracker as T
+    g = T.default_geometry(36, 2000.0)
+    trk = T.Tracker(g, T.default_params(max_clusters=1_000_000))
+    plan = trk.arena_plan()
+    by = {a["name"]: a for a in plan}
+    total = sum(a["bytes"] for a in plan)
+    assert trk.arena_bytes < total
+    # no two arrays alive in the same step overlap in memory
+    for i, a in enumerate(plan):
+        for b in plan[i + 1:]:
+            if a["first_step"] <= b["last_step"] and b["first_step"] <= a["last_step"]:
+                assert a["offset"] + a["bytes"] <= b["offset"] or b["offset"] + b["bytes"] <= a["offset"], (a, b)
+    # the selector's claim array lives in memory that earlier steps used
+    c = by["selector_claim(u64)"]
+    assert any(a["last_step"] < c["first_step"] and a["offset"] < c["offset"] + c["bytes"] and c["offset"] < a["offset"] + a["bytes"]
+               for a in plan)
+    trk.close()
