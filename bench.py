@@ -1,0 +1,312 @@
+#!/usr/bin/env python
+"""bench.py -- TPC time-frame tracking throughput on B200 (metric of BASELINE.json: clusters tracked per second,
+ms per 10 ms time frame, HBM GB/s vs peak).
+
+A "step" is one pass of the whole hot path (C1 ingest -> C2 finder -> C3/C4 cleaner + start hits -> C5 tracklet
+constructor -> C6 selector) over one synthetic continuous-readout time frame (configs[3] of BASELINE.json: 10 ms at
+50 kHz, ~500 collisions).  `value` is measured with the clusters resident in HBM; `e2e` goes through the C-ABI host
+entry point with pinned HOST buffers (H2D of the clusters and D2H of the tracks inside the timed region).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--frame-us F] [--impl reference]
+
+N > 1 (torchrun, one rank per GPU): every rank tracks its own time frame (the paper's farm runs independent time
+frames per GPU) -> weak scaling, no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+CONFIG_NAMES = {0: "configs[0] single sector, 300 tracks", 1: "configs[1] full TPC, one 4000-track collision",
+                2: "configs[2] 2 ms continuous readout at 50 kHz", 3: "configs[3] 10 ms continuous readout at 50 kHz",
+                4: "configs[4] 10 ms high-occupancy stress frame"}
+
+# Algorithmic HBM bytes per cluster of each step -- what the method must move, not what it moves.
+ALGO_BYTES_PER_CLUSTER = {
+    "ingest_count": 12 + 4 + 4, "grid_scan": 0, "ingest_scatter": 12 + 4 + 4 + 14, "bin_sort": 0,
+    "neighbours_finder": 10 + 8 + 8, "cleaner_start_hits": 8 + 4 + 1, "start_hit_compaction": 1,
+}
+
+
+def _peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with nvidia-smi during the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.samples, self._stop, self._th = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.samples.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        self._th = threading.Thread(target=self._run, daemon=True)
+        self._th.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._th.join(timeout=6)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for s in self.samples:
+            try:
+                sm.append(float(s[0])); mx.append(float(s[1]))
+                for nm, v in zip(names, s[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                continue
+        sm.sort()
+        return {"sm_mhz": (sm[len(sm) // 2] if sm else None), "sm_max_mhz": (max(mx) if mx else None),
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _tracker_params(T, cfg, n, host_staging, profile):
+    p = T.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm, max_clusters=n)
+    p.host_staging, p.profile = int(host_staging), int(profile)
+    return p
+
+
+def _cpu_oracle_run(cid, seed, frame_us):
+    """Times the oracle, as it stands, on one host core over a bounded sample of the workload."""
+    import oracle
+    from paper_2102_08862_b200 import gen
+    cfg = gen.preset(cid, seed, frame_us if cid >= 2 else None)
+    tf = gen.generate(cfg, want_truth=False)
+    g = oracle.default_geometry(cfg.n_sectors, tf.max_time_bin)
+    p = oracle.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm)
+    t0 = time.perf_counter()
+    r = oracle.track(g, p, tf.row, tf.pad, tf.time)
+    dt = time.perf_counter() - t0
+    return tf.n, dt, len(r.tr_seed)
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the box's host cores, same metric; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cid = args.config
+    sample_us = args.ref_frame_us
+    total_n, total_t = 0, 0.0
+    for i in range(args.warmup + args.steps):
+        n, dt, _ = _cpu_oracle_run(cid, 1000 + i, sample_us)
+        if i >= args.warmup:
+            total_n += n; total_t += dt
+    value = total_n / total_t
+    sample = (f"{CONFIG_NAMES[cid]} generator with the frame cut to {sample_us:g} us per step"
+              if cid >= 2 else CONFIG_NAMES[cid])
+    line = {"impl": "reference", "metric": "tpc_clusters_tracked_per_s", "value": value, "unit": "clusters/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_t / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": CONFIG_NAMES[cid], "sample": sample, "clusters_per_step": total_n // args.steps},
+            "cpu_baseline": {"value": value, "unit": "clusters/s", "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "clusters/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (default 3: the 10 ms frame)")
+    ap.add_argument("--frame-us", type=float, default=None, help="override the frame length (smoke runs only)")
+    ap.add_argument("--seed", type=int, default=1)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-frame-us", type=float, default=60.0, help="frame length of one reference-arm step")
+    ap.add_argument("--cpu-sample-us", type=float, default=150.0, help="frame length of the cpu_baseline sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2102_08862_b200 import gen, tracker as T
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the tracker has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    # ---- synthetic time frame (one per rank; seeded) ----
+    cid = args.config
+    cfg = gen.preset(cid, args.seed + rank, args.frame_us if cid >= 2 else None)
+    cfg.n_threads = max(1, (os.cpu_count() or 8) // max(world, 1))
+    t_gen = time.perf_counter()
+    tf = gen.generate(cfg, want_truth=False)
+    t_gen = time.perf_counter() - t_gen
+    n = tf.n
+    host = [torch.from_numpy(a).pin_memory() for a in (tf.row, tf.pad, tf.time)]
+    devc = [h.to(dev, non_blocking=True) for h in host]
+    torch.cuda.synchronize()
+
+    g = T.default_geometry(cfg.n_sectors, tf.max_time_bin)
+    trk = T.Tracker(g, _tracker_params(T, cfg, n, host_staging=False, profile=True), device=str(dev))
+    outs = trk.alloc_outputs(n)
+    stream = torch.cuda.Stream(device=dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing ----
+    with torch.cuda.stream(stream):
+        for _ in range(args.warmup):
+            trk.tpc_track_timeframe(*devc, n=n, outputs=outs, stream=stream)
+    barrier()
+    step_acc = {}
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clocks:
+        barrier()
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            for _ in range(args.steps):
+                trk.tpc_track_timeframe(*devc, n=n, outputs=outs, stream=stream)
+            e1.record(stream)
+        barrier()
+    total_ms = e0.elapsed_time(e1)
+    launches = trk.last_launches() * args.steps
+    # per-kernel durations: CUDA events recorded by the library on the same stream (params.profile = 1),
+    # averaged over a few extra steps
+    n_prof = min(args.steps, 5)
+    for _ in range(n_prof):
+        with torch.cuda.stream(stream):
+            trk.tpc_track_timeframe(*devc, n=n, outputs=outs, stream=stream)
+        stream.synchronize()
+        for k, v in trk.step_ms().items():
+            step_acc[k] = step_acc.get(k, 0.0) + v / n_prof
+    n_tracks = int(outs[0].n_tracks[0])
+    n_track_hits = int(outs[0].n_track_hits[0])
+    status = int(outs[0].status[0])
+    arena_gb = trk.arena_bytes / 1e9
+    trk.close()
+    del trk, outs
+
+    t = torch.tensor([total_ms, float(n)], dtype=torch.float64, device=dev)
+    if world > 1:
+        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        total_ms_max, n_all = float(tmax[0]), float(tsum[1])
+    else:
+        total_ms_max, n_all = total_ms, float(n)
+    ms_per_step = total_ms_max / args.steps
+    value = n_all / (ms_per_step * 1e-3)
+
+    # ---- end to end through the C-ABI host entry point (pinned host buffers) ----
+    e2e = None
+    if not args.no_e2e:
+        trk = T.Tracker(g, _tracker_params(T, cfg, n, host_staging=True, profile=False), device=str(dev))
+        houts = trk.alloc_outputs(n, host=True)
+        for _ in range(2):
+            trk.tpc_track_timeframe_host(*host, n=n, outputs=houts, stream=stream)
+        barrier()
+        k_e2e = max(3, args.steps // 2)
+        e0.record(stream)
+        for _ in range(k_e2e):
+            trk.tpc_track_timeframe_host(*host, n=n, outputs=houts, stream=stream)
+        e1.record(stream)
+        barrier()
+        ms = e0.elapsed_time(e1) / k_e2e
+        t2 = torch.tensor([ms], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t2, op=dist.ReduceOp.MAX)
+        k = int(houts[0].n_tracks[0]); h = int(houts[0].n_track_hits[0])
+        d2h = 16 + k * (8 + 5 * 4 + 7 * 4 + 36) + 4 * h
+        e2e = {"value": n_all / (float(t2[0]) * 1e-3), "unit": "clusters/s", "ms_per_step": float(t2[0]),
+               "h2d_bytes_per_step": 12 * n, "d2h_bytes_per_step": d2h, "steps": k_e2e}
+        trk.close()
+        del trk, houts
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel ----
+    peak, peak_src = _peaks()
+    dom = max(step_acc, key=step_acc.get)
+    hbm_rows = {}
+    for k, bpc in ALGO_BYTES_PER_CLUSTER.items():
+        if bpc and step_acc.get(k, 0) > 0:
+            hbm_rows[k] = {"ms": round(step_acc[k], 4), "algo_gbs": round(bpc * n / (step_acc[k] * 1e-3) / 1e9, 1)}
+    # tracklet-level steps: algorithmic bytes depend on the tracklet count
+    roof = {"kernel": dom, "ms": step_acc[dom], "share_of_step": step_acc[dom] / sum(step_acc.values())}
+    if dom in ALGO_BYTES_PER_CLUSTER and ALGO_BYTES_PER_CLUSTER[dom]:
+        a = ALGO_BYTES_PER_CLUSTER[dom] * n / (step_acc[dom] * 1e-3) / 1e9
+        roof.update({"bound": "hbm", "achieved": a, "peak": peak, "unit": "GB/s", "frac": a / peak, "traffic": None,
+                     "peak_source": peak_src})
+    else:
+        roof.update({"bound": "hbm", "achieved": None, "peak": peak, "unit": "GB/s", "frac": None, "traffic": None,
+                     "peak_source": peak_src})
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        cn, cdt, _ = _cpu_oracle_run(cid, args.seed, args.cpu_sample_us)
+        sample = (f"{CONFIG_NAMES[cid]} generator, seed {args.seed}, frame cut to {args.cpu_sample_us:g} us ({cn} clusters)"
+                  if cid >= 2 else f"{CONFIG_NAMES[cid]} ({cn} clusters)")
+        cpu = {"value": cn / cdt, "unit": "clusters/s", "cores": 1, "kind": "oracle", "sample": sample, "seconds": cdt}
+
+    line = {"metric": "tpc_clusters_tracked_per_s", "value": value, "unit": "clusters/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": CONFIG_NAMES[cid] + (f" (frame cut to {args.frame_us:g} us)" if args.frame_us else ""),
+                       "n_clusters_rank0": n, "n_clusters_all_ranks": int(n_all), "n_collisions": tf.n_collisions,
+                       "n_tracks": n_tracks, "n_track_hits": n_track_hits, "status": status, "seed": args.seed,
+                       "parallelism": f"{world} independent time frame(s), one per GPU", "arena_gb": round(arena_gb, 2),
+                       "l2": "inputs and scratch are larger than L2 (no flush needed)" if n * 12 > 2.5e8 else
+                             "working set may fit L2 (small config)", "gen_seconds": round(t_gen, 1)},
+            "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches,
+            "step_ms": {k: round(v, 4) for k, v in step_acc.items()}, "hbm_steps": hbm_rows,
+            "roofline": roof, "cpu_baseline": cpu}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
