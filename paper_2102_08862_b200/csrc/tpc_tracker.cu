@@ -33,7 +33,7 @@ const char* const kStepNames[N_STEPS] = {
 struct Ids {   // arena allocation ids
   int stage_in = -1, stage_out = -1;
   int bin_start, rank, yt, orig, hsr, link_up, link_down, link_up_clean, start_flag, cta_count, start_hits,
-      counters, scan_a, scan_b, row_hit, tl_n_hits, tl_first, tl_last, tl_seed, tl_par, tl_cov, claim, owned,
+      counters, scan_a, scan_b, seeds_a, seeds_b, row_hit, tl_n_hits, tl_first, tl_last, tl_seed, tl_par, tl_cov, claim, owned,
       flag, track_idx, hit_off;
 };
 
@@ -63,7 +63,7 @@ bool capacities(const tpc_geometry_t* g, const tpc_params_t* p, int64_t max_clus
   c.max_tracklets = p->max_tracklets > 0 ? p->max_tracklets : c.max_clusters / 10 + 4096;
   c.max_tracks = p->max_tracks > 0 ? p->max_tracks : c.max_clusters / 64 + 4096;
   c.max_track_hits = p->max_track_hits > 0 ? p->max_track_hits : c.max_clusters;
-  const int w = p->grid_time_bins > 0 ? p->grid_time_bins : 4;
+  const int w = p->grid_time_bins > 0 ? p->grid_time_bins : 2;
   const double ntb = std::floor((double)g->max_time_bin / (double)w) + 1.0;
   const double nb = ntb * (double)g->n_sectors * (double)g->n_rows;
   if (nb >= 2147483000.0) return false;
@@ -96,6 +96,8 @@ void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids
   id.start_flag = plan.add("start_flag(u8)", N, S_CLEAN_START, S_COMPACT);
   id.cta_count = plan.add("start_cta_count", 4 * ((size_t)c.n_link_ctas + 2), S_CLEAN_START, S_COMPACT);
   id.start_hits = plan.add("start_hits", 4 * T, S_COMPACT, S_EMIT);
+  id.seeds_a = plan.add("tracklet_seeds_a(int4)", 16 * T, S_CONSTRUCT, S_CONSTRUCT);
+  id.seeds_b = plan.add("tracklet_seeds_b(float4)", 16 * T, S_CONSTRUCT, S_CONSTRUCT);
   id.row_hit = plan.add("tracklet_row_hit", 4 * (size_t)kRowStride * T, S_CONSTRUCT, S_EMIT);
   id.tl_n_hits = plan.add("tracklet_n_hits", 4 * T, S_CONSTRUCT, S_EMIT);
   id.tl_first = plan.add("tracklet_first_row", 4 * T, S_CONSTRUCT, S_EMIT);
@@ -124,6 +126,7 @@ struct tpc_tracker {
   cudaEvent_t ev[N_STEPS + 1] = {};
   bool profile = false, have_times = false;
   int64_t last_launches = 0;
+  int constructor_ctas = 148;      // persistent grid: SMs x resident CTAs per SM
 };
 
 extern "C" {
@@ -186,7 +189,7 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
   }
 
   Consts& c = t->consts;
-  const int w = p->grid_time_bins > 0 ? p->grid_time_bins : 4;
+  const int w = p->grid_time_bins > 0 ? p->grid_time_bins : 2;
   c.n_rows = nr; c.n_sr = g->n_sectors * nr; c.n_tb = t->cap.n_tb; c.n_bins = t->cap.n_bins;
   c.max_time = g->max_time_bin; c.inv_bin_w = (float)(1.0 / (double)w);
   c.Z = g->time_bin_cm; c.inv_Z = (float)(1.0 / (double)g->time_bin_cm); c.P = g->pad_pitch_cm;
@@ -207,6 +210,15 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
   c.npads = reinterpret_cast<const int*>(tb + (size_t)nr * 8);
 
   t->profile = p->profile != 0;
+  {
+    int dev = 0, sms = 148, per_sm = 1;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_tracklet_constructor, kTrackletThreads, 0) != cudaSuccess || per_sm < 1) {
+      cudaGetLastError(); per_sm = 1;
+    }
+    t->constructor_ctas = sms * per_sm;
+  }
   for (int i = 0; i <= N_STEPS; ++i)
     if (cudaEventCreate(&t->ev[i]) != cudaSuccess) { cudaGetLastError(); tpc_tracker_destroy(t); return TPC_ECUDA; }
   *out = t;
@@ -277,8 +289,12 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   uint8_t* start_flag = P.ptr<uint8_t>(A, id.start_flag);
   uint32_t* cta_count = P.ptr<uint32_t>(A, id.cta_count);
   uint32_t* start_hits = P.ptr<uint32_t>(A, id.start_hits);
-  int32_t* counters = P.ptr<int32_t>(A, id.counters);          // [0] tracklets, [1] start hits, [2] invalid clusters
+  int32_t* counters = P.ptr<int32_t>(A, id.counters);          // [0] tracklets, [1] start hits, [2] invalid clusters, [3] work queue
   uint32_t* n_invalid = reinterpret_cast<uint32_t*>(counters + 2);
+  uint32_t* work_counter = reinterpret_cast<uint32_t*>(counters + 3);
+  TrackletSeeds seeds;
+  seeds.a = P.ptr<int4>(A, id.seeds_a);
+  seeds.b = P.ptr<float4>(A, id.seeds_b);
   uint32_t* scan_a = P.ptr<uint32_t>(A, id.scan_a);
   uint32_t* scan_b = P.ptr<uint32_t>(A, id.scan_b);
   unsigned long long* claim = P.ptr<unsigned long long>(A, id.claim);
@@ -334,8 +350,9 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   // ---- C5 tracklet constructor ----
   mark(S_CONSTRUCT);
   const int64_t tl_bound = std::min<int64_t>(T, n / std::max(2, c.seed_min_hits) + 1);   // start hits own disjoint chains
-  k_tracklet_constructor<<<(int)((tl_bound + kTrackletThreads - 1) / kTrackletThreads), kTrackletThreads, 0, st>>>(
-      yt, orig, hsr, bin_start, link_up_clean, start_hits, counters, tl, c); ++launches;
+  k_tracklet_init<<<(int)((tl_bound + 255) / 256), 256, 0, st>>>(yt, hsr, link_up_clean, start_hits, counters, seeds, c); ++launches;
+  k_tracklet_constructor<<<(int)std::min<int64_t>(t->constructor_ctas, (tl_bound + kTrackletThreads - 1) / kTrackletThreads),
+                           kTrackletThreads, 0, st>>>(yt, orig, bin_start, link_up_clean, seeds, counters, work_counter, tl, c); ++launches;
   const int warp_ctas = (int)((tl_bound * 32 + kSelectorThreads - 1) / kSelectorThreads);
   if (tl_taps) {
     k_export_tracklets<<<warp_ctas, kSelectorThreads, 0, st>>>(tl, counters, orig, o->n_tracklets, o->tracklet_seed, o->tracklet_n_hits,

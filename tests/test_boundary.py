@@ -35,7 +35,7 @@ def test_arena_bytes_is_host_arithmetic_and_reuses_memory():
     assert need > 0
     T_cap = n // 10 + 4096
     # sum of all arrays if nothing were reused vs the planned peak
-    n_bins = (50485 // 4 + 1) * 36 * 152
+    n_bins = (50485 // 2 + 1) * 36 * 152
     no_reuse = (4 * (n_bins + 1) + 4 * n + 8 * n + 4 * n + 2 * n + 3 * 4 * n + n + 8 * n
                 + T_cap * (4 * 160 + 4 * 4 + 28 + 36 + 4 * 5))
     assert need < 0.85 * no_reuse

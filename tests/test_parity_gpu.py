@@ -107,8 +107,10 @@ def test_invalid_clusters_are_ignored_and_flagged():
     assert o.stats["invalid_clusters"] > 500
 
 
-def test_duplicate_hits_tie_break_on_original_index():
-    """Exact duplicates of whole tracks: every chi2 / distance tie must go to the lowest original index."""
+@pytest.mark.parametrize("copies", [2, 6])
+def test_duplicate_hits_tie_break_on_original_index(copies):
+    """Exact duplicates of whole tracks: every chi2 / distance tie must go to the lowest original index
+    (6 copies also overflow the finder's 4 candidate slots per row -> generic path)."""
     rows = np.arange(N_ROWS)
     x = row_x(rows)
     parts = []
@@ -116,7 +118,7 @@ def test_duplicate_hits_tie_break_on_original_index():
         y = (-0.1 + 0.06 * i) * x
         z = 100.0 + 0.3 * i * (x - 85.0)
         p = clusters_from_xyz(rows, y, z)
-        parts += [p, p]                                   # each track twice
+        parts += [p] * copies                             # each track several times
     row, pad, time = concat(parts)
     rng = np.random.default_rng(3)
     perm = rng.permutation(row.size)
