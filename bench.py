@@ -31,7 +31,7 @@ CONFIG_NAMES = {0: "configs[0] single sector, 300 tracks", 1: "configs[1] full T
 
 # Algorithmic HBM bytes per cluster of each step -- what the method must move, not what it moves.
 ALGO_BYTES_PER_CLUSTER = {
-    "ingest_count": 12 + 4 + 4, "grid_scan": 0, "ingest_scatter": 12 + 4 + 4 + 14, "bin_sort": 0,
+    "ingest_radix_sort": 4 * (4 + 16 + 16), "grid_build": 4 + 4 + 2,
     "neighbours_finder": 10 + 8 + 8, "cleaner_start_hits": 8 + 4 + 1, "start_hit_compaction": 1,
 }
 

@@ -1,82 +1,188 @@
-// C1 cluster ingest (BASELINE.json L5 item 1; PAPER.md L23 native coordinates): sorts the frame's clusters
-// into per-(sector,row) grids of time bins -- a one-digit radix (counting) sort on the key
-// (sector*n_rows + row, time_bin) with a prefix scan of the bin histogram -- and converts pad -> local y.
+// C1 cluster ingest (BASELINE.json L5 item 1: "sorts clusters into per-(sector, row) grids of (pad, time) bins by
+// radix sort and prefix scan"; PAPER.md L23 native coordinates).
 //
-//   k_ingest_count  : validity, key, rank[i] = atomicAdd(binCount[key], 1)             (12 B read, 4 B write)
-//   exclusive scan  : binStart = scan(binCount)                                        (scan.cuh)
-//   k_ingest_scatter: pos = binStart[key] + rank[i]; yt[pos] = (y, time); orig[pos] = i; hsr[pos] = sector-row
-//   k_bin_sort      : orders each bin by original index so the sorted layout is run-to-run deterministic
-//                     (atomic ranks are not); results never depend on it -- every tie-break is on `orig`.
+// key(i) = (sector*n_rows + row) * n_tb + time_bin(time)   (= grid bin index; n_bins for clusters outside the
+// geometry, which therefore sort to the end).  A stable least-significant-digit radix sort on the key orders the
+// frame by (sector-row, time bin) and, inside a bin, by original index -- the layout is deterministic.
+// One pass = k_radix_histogram (digit counts per 2048-element tile) -> exclusive prefix scan over
+// (digit, tile) -> k_radix_scatter (stable in-tile ranking by warp match, local reorder in shared memory, then
+// every digit's run is written contiguously: coalesced writes instead of 4..8-byte random scatters).
+// The first pass reads the raw fp32 SoA input and converts pad -> local y on the fly; the last pass writes the
+// final hit arrays.  k_grid_build then derives the grid's bin offsets from the sorted keys (no atomics).
+//
+// Algorithmic HBM bytes per cluster: passes * (4 + 16 + 16) + grid build ~ 8.
 #pragma once
 #include "common.cuh"
 
 namespace tpc {
 
+constexpr int kRadixThreads = 256;
+constexpr int kRadixItems = 8;
+constexpr int kRadixTile = kRadixThreads * kRadixItems;   // 2048
+constexpr int kRadixMaxBits = 8;
+constexpr int kRadixBuckets = 1 << kRadixMaxBits;
+constexpr size_t kRadixScatterSmem = (size_t)kRadixTile * 16 + (size_t)(kRadixThreads / 32 + 2) * kRadixBuckets * 4;
+
 // A cluster is inside the geometry iff row is an integer in [0, n_sr), pad in [-0.5, n_pads-0.5) and
 // time in [0, max_time]; evaluated in fp32 on the raw values (DESIGN.md §3 C1).
-__device__ __forceinline__ bool cluster_key(float rf, float pad, float time, const Consts& c, int& sr, int& bin) {
+__device__ __forceinline__ uint32_t cluster_key(float rf, float pad, float time, const Consts& c) {
   bool ok = rf >= 0.0f && rf < (float)c.n_sr && rf == floorf(rf);
-  if (!ok) return false;
-  sr = (int)rf;
+  if (!ok) return (uint32_t)c.n_bins;
+  const int sr = (int)rf;
   const int r = sr % c.n_rows;
   ok = pad >= -0.5f && pad < (float)__ldg(c.npads + r) - 0.5f && time >= 0.0f && time <= c.max_time;
-  if (!ok) return false;
-  bin = sr * c.n_tb + time_bin(time, c);
-  return true;
+  if (!ok) return (uint32_t)c.n_bins;
+  return (uint32_t)(sr * c.n_tb + time_bin(time, c));
 }
 
-__global__ void __launch_bounds__(256) k_ingest_count(const float* __restrict__ row, const float* __restrict__ pad,
-                                                      const float* __restrict__ time, int64_t n,
-                                                      uint32_t* __restrict__ bin_count, uint32_t* __restrict__ rank,
-                                                      uint32_t* __restrict__ n_invalid, const __grid_constant__ Consts c) {
-  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  uint32_t bad = 0;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-    int sr, bin;
-    if (cluster_key(row[i], pad[i], time[i], c, sr, bin)) {
-      rank[i] = atomicAdd(bin_count + bin, 1u);
-    } else {
-      rank[i] = kInvalidRank;
-      ++bad;
+struct RadixSrc {        // input of a pass: either the raw clusters (first pass) or a sorted-so-far set
+  const float* row; const float* pad; const float* time;        // first pass
+  const uint32_t* keys; const uint32_t* orig; const float2* yt; // later passes
+};
+struct RadixDst { uint32_t* keys; uint32_t* orig; float2* yt; };
+
+// Digit histogram of one tile: hist[digit * n_tiles + tile].
+template <bool kFirst>
+__global__ void __launch_bounds__(kRadixThreads) k_radix_histogram(RadixSrc src, int64_t n, int shift, uint32_t mask,
+                                                                   uint32_t* __restrict__ hist, int n_tiles,
+                                                                   const __grid_constant__ Consts c) {
+  __shared__ uint32_t cnt[kRadixBuckets];
+  for (int i = threadIdx.x; i < kRadixBuckets; i += kRadixThreads) cnt[i] = 0;
+  __syncthreads();
+  const int64_t base = (int64_t)blockIdx.x * kRadixTile;
+#pragma unroll 4
+  for (int k = 0; k < kRadixItems; ++k) {
+    const int64_t i = base + (int64_t)k * kRadixThreads + threadIdx.x;
+    if (i < n) {
+      const uint32_t key = kFirst ? cluster_key(src.row[i], src.pad[i], src.time[i], c) : src.keys[i];
+      atomicAdd(&cnt[(key >> shift) & mask], 1u);
     }
   }
-  bad = __reduce_add_sync(0xffffffffu, bad);
-  if (bad && lane_id() == 0) atomicAdd(n_invalid, bad);
+  __syncthreads();
+  for (int d = threadIdx.x; d <= (int)mask; d += kRadixThreads) hist[(size_t)d * n_tiles + blockIdx.x] = cnt[d];
 }
 
-__global__ void __launch_bounds__(256) k_ingest_scatter(const float* __restrict__ row, const float* __restrict__ pad,
-                                                        const float* __restrict__ time, int64_t n,
-                                                        const uint32_t* __restrict__ rank, const uint32_t* __restrict__ bin_start,
-                                                        float2* __restrict__ yt, uint32_t* __restrict__ orig,
-                                                        uint16_t* __restrict__ hsr, const __grid_constant__ Consts c) {
-  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-    const uint32_t rk = rank[i];
-    if (rk == kInvalidRank) continue;
-    const float p = pad[i], t = time[i];
-    int sr, bin;
-    cluster_key(row[i], p, t, c, sr, bin);
-    const uint32_t pos = __ldg(bin_start + bin) + rk;
-    const float y = (p - __ldg(c.cr + sr % c.n_rows)) * c.P;     // y(h) = (pad - c_r) * P
-    yt[pos] = make_float2(y, t);
-    orig[pos] = (uint32_t)i;
-    hsr[pos] = (uint16_t)sr;
+// Stable scatter of one tile.  `offsets` = exclusive scan of hist (same layout): global position of the first
+// element of (digit, tile).
+template <bool kFirst>
+__global__ void __launch_bounds__(kRadixThreads, 3) k_radix_scatter(RadixSrc src, RadixDst dst, int64_t n, int shift, uint32_t mask,
+                                                                 const uint32_t* __restrict__ offsets, int n_tiles,
+                                                                 uint32_t* __restrict__ n_invalid,
+                                                                 const __grid_constant__ Consts c) {
+  constexpr int kWarps = kRadixThreads / 32;
+  constexpr int kWarpItems = kRadixTile / kWarps;                 // 256 consecutive elements per warp
+  extern __shared__ __align__(16) unsigned char radix_smem[];     // kRadixScatterSmem bytes (dynamic: > 48 KB)
+  float2* s_yt = reinterpret_cast<float2*>(radix_smem);                                   // [kRadixTile]
+  uint32_t* s_keys = reinterpret_cast<uint32_t*>(s_yt + kRadixTile);                      // [kRadixTile]
+  uint32_t* s_orig = s_keys + kRadixTile;                                                 // [kRadixTile]
+  uint32_t (*warp_cnt)[kRadixBuckets] = reinterpret_cast<uint32_t (*)[kRadixBuckets]>(s_orig + kRadixTile);  // per-warp digit counts
+  uint32_t* digit_start = &warp_cnt[kWarps][0];                   // first local position of each digit in the tile
+  uint32_t* gbase = digit_start + kRadixBuckets;                  // global position of the tile's first element of a digit
+  const int w = threadIdx.x >> 5;
+  const unsigned lane = lane_id();
+  const int n_dig = (int)mask + 1;
+  for (int i = threadIdx.x; i < kWarps * kRadixBuckets; i += kRadixThreads) (&warp_cnt[0][0])[i] = 0;
+  __syncthreads();
+
+  // 1. load (warp w owns elements [w*256, w*256+256) of the tile, lane-strided -> coalesced)
+  const int64_t tile_base = (int64_t)blockIdx.x * kRadixTile;
+  const int64_t wbase = tile_base + (int64_t)w * kWarpItems;
+  uint32_t key[kRadixItems], og[kRadixItems], rank[kRadixItems];
+  float2 yt[kRadixItems];
+  uint32_t bad = 0;
+#pragma unroll
+  for (int k = 0; k < kRadixItems; ++k) {
+    const int64_t i = wbase + k * 32 + lane;
+    key[k] = 0xFFFFFFFFu; og[k] = 0; yt[k] = make_float2(0.0f, 0.0f);
+    if (i < n) {
+      if (kFirst) {
+        const float rf = src.row[i], p = src.pad[i], t = src.time[i];
+        key[k] = cluster_key(rf, p, t, c);
+        og[k] = (uint32_t)i;
+        float y = 0.0f;
+        if (key[k] != (uint32_t)c.n_bins) y = (p - __ldg(c.cr + ((int)rf) % c.n_rows)) * c.P;   // y(h) = (pad - c_r) * P
+        else ++bad;
+        yt[k] = make_float2(y, t);
+      } else {
+        key[k] = src.keys[i]; og[k] = src.orig[i]; yt[k] = src.yt[i];
+      }
+    }
+  }
+  if (kFirst) {
+    bad = __reduce_add_sync(0xffffffffu, bad);
+    if (bad && lane == 0) atomicAdd(n_invalid, bad);
+  }
+
+  // 2. stable rank inside the warp: elements are visited in index order (k-major, lane-minor)
+#pragma unroll
+  for (int k = 0; k < kRadixItems; ++k) {
+    const bool valid = wbase + k * 32 + lane < n;
+    const uint32_t d = valid ? (key[k] >> shift) & mask : mask + 1u;      // padding never matches a digit
+    const unsigned peers = __match_any_sync(0xffffffffu, d);
+    const int leader = __ffs(peers) - 1;
+    uint32_t before = 0;
+    if (valid && (int)lane == leader) { before = warp_cnt[w][d]; warp_cnt[w][d] = before + __popc(peers); }
+    before = __shfl_sync(0xffffffffu, before, leader);
+    rank[k] = before + __popc(peers & ((1u << lane) - 1u));
+    __syncwarp();
+  }
+  __syncthreads();
+
+  // 3. per digit: exclusive offsets over the warps, tile totals, then an exclusive scan over the digits
+  uint32_t tile_total = 0;
+  if ((int)threadIdx.x < n_dig) {
+    uint32_t run = 0;
+#pragma unroll
+    for (int ww = 0; ww < kWarps; ++ww) { const uint32_t t = warp_cnt[ww][threadIdx.x]; warp_cnt[ww][threadIdx.x] = run; run += t; }
+    tile_total = run;
+    gbase[threadIdx.x] = offsets[(size_t)threadIdx.x * n_tiles + blockIdx.x];
+  }
+  {
+    // block exclusive scan of tile_total over threads 0..255 (n_dig <= 256)
+    __shared__ uint32_t wsum[kWarps];
+    uint32_t inc = tile_total;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o); if ((int)lane >= o) inc += t; }
+    if (lane == 31) wsum[w] = inc;
+    __syncthreads();
+    uint32_t pre = 0;
+    for (int ww = 0; ww < w; ++ww) pre += wsum[ww];
+    if ((int)threadIdx.x < n_dig) digit_start[threadIdx.x] = pre + inc - tile_total;
+  }
+  __syncthreads();
+
+  // 4. local reorder into shared memory
+#pragma unroll
+  for (int k = 0; k < kRadixItems; ++k) {
+    if (wbase + k * 32 + lane < n) {
+      const uint32_t d = (key[k] >> shift) & mask;
+      const uint32_t pos = digit_start[d] + warp_cnt[w][d] + rank[k];
+      s_keys[pos] = key[k]; s_orig[pos] = og[k]; s_yt[pos] = yt[k];
+    }
+  }
+  __syncthreads();
+
+  // 5. write every digit's run contiguously
+  const int n_here = (int)min((int64_t)kRadixTile, n - tile_base);
+  for (int p = threadIdx.x; p < n_here; p += kRadixThreads) {
+    const uint32_t kk = s_keys[p];
+    const uint32_t d = (kk >> shift) & mask;
+    const uint32_t g = gbase[d] + ((uint32_t)p - digit_start[d]);
+    dst.keys[g] = kk; dst.orig[g] = s_orig[p]; dst.yt[g] = s_yt[p];
   }
 }
 
-// One thread per grid bin: insertion sort of the bin's entries by original index (bins hold a few hits).
-__global__ void __launch_bounds__(256) k_bin_sort(const uint32_t* __restrict__ bin_start, float2* __restrict__ yt,
-                                                  uint32_t* __restrict__ orig, int n_bins) {
-  const int b = blockIdx.x * blockDim.x + threadIdx.x;
-  if (b >= n_bins) return;
-  const uint32_t lo = bin_start[b], hi = bin_start[b + 1];
-  for (uint32_t i = lo + 1; i < hi; ++i) {
-    const uint32_t o = orig[i];
-    const float2 v = yt[i];
-    uint32_t j = i;
-    while (j > lo && orig[j - 1] > o) { orig[j] = orig[j - 1]; yt[j] = yt[j - 1]; --j; }
-    if (j != i) { orig[j] = o; yt[j] = v; }
-  }
+// Grid bin offsets from the sorted keys: bin_start[b] = first position whose key >= b, for b in [0, n_bins].
+// Thread i (0 <= i <= n) fills the bins in (key[i-1], key[i]]; also writes the hit's sector-row (u16).
+__global__ void __launch_bounds__(256) k_grid_build(const uint32_t* __restrict__ keys, int64_t n, uint32_t* __restrict__ bin_start,
+                                                    uint16_t* __restrict__ hsr, const __grid_constant__ Consts c) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i > n) return;
+  const uint32_t nb = (uint32_t)c.n_bins;
+  const int64_t kprev = i == 0 ? -1 : (int64_t)min(keys[i - 1], nb);
+  const uint32_t kcur = i == n ? nb : min(keys[i], nb);
+  if (i < n && kcur < nb) hsr[i] = (uint16_t)(kcur / (uint32_t)c.n_tb);
+  for (int64_t b = kprev + 1; b <= (int64_t)kcur; ++b) bin_start[b] = (uint32_t)i;
 }
 
 }  // namespace tpc

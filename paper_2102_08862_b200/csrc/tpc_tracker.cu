@@ -22,17 +22,15 @@ using namespace tpc;
 namespace {
 
 enum Step {
-  S_INGEST_COUNT = 0, S_GRID_SCAN, S_INGEST_SCATTER, S_BIN_SORT, S_FINDER, S_CLEAN_START, S_COMPACT,
-  S_CONSTRUCT, S_CLAIM, S_COUNT, S_SELECT_SCAN, S_EMIT, N_STEPS
+  S_SORT = 0, S_GRID, S_FINDER, S_CLEAN_START, S_COMPACT, S_CONSTRUCT, S_CLAIM, S_COUNT, S_SELECT_SCAN, S_EMIT, N_STEPS
 };
 const char* const kStepNames[N_STEPS] = {
-    "ingest_count", "grid_scan", "ingest_scatter", "bin_sort", "neighbours_finder", "cleaner_start_hits",
-    "start_hit_compaction", "tracklet_constructor", "selector_claim", "selector_count", "selector_scan",
-    "selector_emit"};
+    "ingest_radix_sort", "grid_build", "neighbours_finder", "cleaner_start_hits", "start_hit_compaction",
+    "tracklet_constructor", "selector_claim", "selector_count", "selector_scan", "selector_emit"};
 
 struct Ids {   // arena allocation ids
   int stage_in = -1, stage_out = -1;
-  int bin_start, rank, yt, orig, hsr, link_up, link_down, link_up_clean, start_flag, cta_count, start_hits,
+  int bin_start, sort_keys, tmp_keys, tmp_orig, tmp_yt, sort_hist, yt, orig, hsr, link_up, link_down, link_up_clean, start_flag, cta_count, start_hits,
       counters, scan_a, scan_b, seeds_a, seeds_b, row_hit, tl_n_hits, tl_first, tl_last, tl_seed, tl_par, tl_cov, claim, owned,
       flag, track_idx, hit_off;
 };
@@ -40,6 +38,7 @@ struct Ids {   // arena allocation ids
 struct Capacities {
   int64_t max_clusters, max_tracklets, max_tracks, max_track_hits;
   int n_tb, n_bins, n_link_ctas;
+  int sort_passes, sort_digit_bits, sort_tiles;
 };
 
 bool valid_geometry(const tpc_geometry_t* g) {
@@ -70,26 +69,36 @@ bool capacities(const tpc_geometry_t* g, const tpc_params_t* p, int64_t max_clus
   c.n_tb = (int)ntb;
   c.n_bins = (int)nb;
   c.n_link_ctas = (int)((c.max_clusters + kLinkThreads - 1) / kLinkThreads);
+  int bits = 1;
+  while (((int64_t)1 << bits) <= (int64_t)c.n_bins) ++bits;          // the sentinel key n_bins must be representable
+  c.sort_passes = (bits + kRadixMaxBits - 1) / kRadixMaxBits;
+  c.sort_digit_bits = (bits + c.sort_passes - 1) / c.sort_passes;
+  c.sort_tiles = (int)((c.max_clusters + kRadixTile - 1) / kRadixTile);
   return true;
 }
 
 void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids& id) {
   const size_t N = (size_t)c.max_clusters, T = (size_t)c.max_tracklets, B = (size_t)c.n_bins + 1;
   if (p->host_staging) {
-    id.stage_in = plan.add("host_staging_in(row,pad,time)", 3 * 4 * N, S_INGEST_COUNT, S_INGEST_SCATTER);
+    id.stage_in = plan.add("host_staging_in(row,pad,time)", 3 * 4 * N, S_SORT, S_SORT);
     const size_t K = (size_t)c.max_tracks;
     id.stage_out = plan.add("host_staging_out(tracks)", 256 + K * (5 * 4 + 8 + 7 * 4 + 9 * 4) + 4 * (size_t)c.max_track_hits + 64,
                             S_EMIT, S_EMIT);
   }
-  const size_t scan_len = std::max(std::max(scan_tiles(B), scan_tiles((size_t)c.n_link_ctas + 1)), scan_tiles(T)) + 2;
-  id.counters = plan.add("counters", 256, S_INGEST_COUNT, S_EMIT);
-  id.scan_a = plan.add("scan_tile_sums_a", 4 * scan_len, S_INGEST_COUNT, S_EMIT);
-  id.scan_b = plan.add("scan_tile_sums_b", 4 * scan_len, S_INGEST_COUNT, S_EMIT);
-  id.bin_start = plan.add("grid_bin_start", 4 * B, S_INGEST_COUNT, S_CONSTRUCT);
-  id.rank = plan.add("ingest_rank", 4 * N, S_INGEST_COUNT, S_INGEST_SCATTER);
-  id.yt = plan.add("hits_y_time(float2)", 8 * N, S_INGEST_SCATTER, S_CONSTRUCT);
-  id.orig = plan.add("hits_orig_index", 4 * N, S_INGEST_SCATTER, S_EMIT);
-  id.hsr = plan.add("hits_sector_row(u16)", 2 * N, S_INGEST_SCATTER, S_EMIT);
+  const size_t hist_len = (size_t)kRadixBuckets * (size_t)c.sort_tiles + 1;
+  const size_t scan_len = std::max(std::max(scan_tiles(hist_len), scan_tiles((size_t)c.n_link_ctas + 1)), scan_tiles(T)) + 2;
+  id.counters = plan.add("counters", 256, S_SORT, S_EMIT);
+  id.scan_a = plan.add("scan_tile_sums_a", 4 * scan_len, S_SORT, S_EMIT);
+  id.scan_b = plan.add("scan_tile_sums_b", 4 * scan_len, S_SORT, S_EMIT);
+  id.bin_start = plan.add("grid_bin_start", 4 * B, S_GRID, S_CONSTRUCT);
+  id.sort_keys = plan.add("sort_keys", 4 * N, S_SORT, S_GRID);
+  id.tmp_keys = plan.add("sort_tmp_keys", 4 * N, S_SORT, S_SORT);
+  id.tmp_orig = plan.add("sort_tmp_orig", 4 * N, S_SORT, S_SORT);
+  id.tmp_yt = plan.add("sort_tmp_y_time", 8 * N, S_SORT, S_SORT);
+  id.sort_hist = plan.add("sort_tile_histograms", 4 * hist_len, S_SORT, S_SORT);
+  id.yt = plan.add("hits_y_time(float2)", 8 * N, S_SORT, S_CONSTRUCT);
+  id.orig = plan.add("hits_orig_index", 4 * N, S_SORT, S_EMIT);
+  id.hsr = plan.add("hits_sector_row(u16)", 2 * N, S_GRID, S_EMIT);
   id.link_up = plan.add("link_up_raw", 4 * N, S_FINDER, S_CLEAN_START);
   id.link_down = plan.add("link_down_raw", 4 * N, S_FINDER, S_CLEAN_START);
   id.link_up_clean = plan.add("link_up_clean", 4 * N, S_CLEAN_START, S_CONSTRUCT);
@@ -210,6 +219,10 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
   c.npads = reinterpret_cast<const int*>(tb + (size_t)nr * 8);
 
   t->profile = p->profile != 0;
+  if (cudaFuncSetAttribute(k_radix_scatter<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRadixScatterSmem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_radix_scatter<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRadixScatterSmem) != cudaSuccess) {
+    cudaGetLastError(); tpc_tracker_destroy(t); return TPC_ECUDA;
+  }
   {
     int dev = 0, sms = 148, per_sm = 1;
     cudaGetDevice(&dev);
@@ -279,7 +292,8 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   auto mark = [&](int step) { if (t->profile) cudaEventRecord(t->ev[step], st); };
 
   uint32_t* bin_start = P.ptr<uint32_t>(A, id.bin_start);
-  uint32_t* rank = P.ptr<uint32_t>(A, id.rank);
+  uint32_t* sort_keys = P.ptr<uint32_t>(A, id.sort_keys);
+  uint32_t* sort_hist = P.ptr<uint32_t>(A, id.sort_hist);
   float2* yt = P.ptr<float2>(A, id.yt);
   uint32_t* orig = P.ptr<uint32_t>(A, id.orig);
   uint16_t* hsr = P.ptr<uint16_t>(A, id.hsr);
@@ -312,26 +326,39 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   tl.cov = P.ptr<float>(A, id.tl_cov);
   tl.cap = (size_t)T;
 
-  const int stream_ctas = (int)std::min<int64_t>(std::max<int64_t>((n + 255) / 256, 1), 148 * 32);
   const int hit_ctas = (int)std::max<int64_t>((n + 255) / 256, 1);
   const int link_ctas = (int)std::max<int64_t>((n + kLinkThreads - 1) / kLinkThreads, 1);
 
-  // ---- C1 ingest ----
-  mark(S_INGEST_COUNT);
-  cudaMemsetAsync(bin_start, 0, 4 * ((size_t)c.n_bins + 1), st);
+  // ---- C1 ingest: stable LSD radix sort on the grid bin index, then the bin offsets ----
+  mark(S_SORT);
   cudaMemsetAsync(counters, 0, 256, st);
   if (link_taps && n > 0) {
     cudaMemsetAsync(o->link_up, 0xFF, 4 * (size_t)n, st);
     cudaMemsetAsync(o->link_down, 0xFF, 4 * (size_t)n, st);
     cudaMemsetAsync(o->is_start_hit, 0, (size_t)n, st);
   }
-  k_ingest_count<<<stream_ctas, 256, 0, st>>>(cl->row, cl->pad, cl->time, n, bin_start, rank, n_invalid, c); ++launches;
-  mark(S_GRID_SCAN);
-  launches += exclusive_scan_u32(bin_start, bin_start, (size_t)c.n_bins + 1, scan_a, st);
-  mark(S_INGEST_SCATTER);
-  k_ingest_scatter<<<stream_ctas, 256, 0, st>>>(cl->row, cl->pad, cl->time, n, rank, bin_start, yt, orig, hsr, c); ++launches;
-  mark(S_BIN_SORT);
-  k_bin_sort<<<(c.n_bins + 255) / 256, 256, 0, st>>>(bin_start, yt, orig, c.n_bins); ++launches;
+  if (n > 0) {
+    const int n_tiles = (int)((n + kRadixTile - 1) / kRadixTile);
+    const int passes = t->cap.sort_passes, dbits = t->cap.sort_digit_bits;
+    const uint32_t mask = (1u << dbits) - 1u;
+    RadixDst fin{sort_keys, orig, yt};
+    RadixDst tmp{P.ptr<uint32_t>(A, id.tmp_keys), P.ptr<uint32_t>(A, id.tmp_orig), P.ptr<float2>(A, id.tmp_yt)};
+    RadixSrc src{cl->row, cl->pad, cl->time, nullptr, nullptr, nullptr};
+    for (int p = 0; p < passes; ++p) {
+      const RadixDst dst = ((passes - 1 - p) % 2 == 0) ? fin : tmp;
+      const size_t hist_n = (size_t)(mask + 1) * n_tiles;
+      if (p == 0) k_radix_histogram<true><<<n_tiles, kRadixThreads, 0, st>>>(src, n, p * dbits, mask, sort_hist, n_tiles, c);
+      else k_radix_histogram<false><<<n_tiles, kRadixThreads, 0, st>>>(src, n, p * dbits, mask, sort_hist, n_tiles, c);
+      ++launches;
+      launches += exclusive_scan_u32(sort_hist, sort_hist, hist_n, scan_a, st);
+      if (p == 0) k_radix_scatter<true><<<n_tiles, kRadixThreads, kRadixScatterSmem, st>>>(src, dst, n, p * dbits, mask, sort_hist, n_tiles, n_invalid, c);
+      else k_radix_scatter<false><<<n_tiles, kRadixThreads, kRadixScatterSmem, st>>>(src, dst, n, p * dbits, mask, sort_hist, n_tiles, n_invalid, c);
+      ++launches;
+      src = RadixSrc{nullptr, nullptr, nullptr, dst.keys, dst.orig, dst.yt};
+    }
+  }
+  mark(S_GRID);
+  k_grid_build<<<(int)((n + 1 + 255) / 256), 256, 0, st>>>(sort_keys, n, bin_start, hsr, c); ++launches;
 
   // ---- C2 neighbours finder ----
   mark(S_FINDER);

@@ -24,7 +24,7 @@ def test_library_exports_every_declared_symbol():
     for nm in names:
         assert getattr(lib, nm) is not None
     assert lib.tpc_strerror(0) == b"ok" and b"arena" in lib.tpc_strerror(-2)
-    assert lib.tpc_tracker_step_name(0) == b"ingest_count" and lib.tpc_tracker_step_name(99) is None
+    assert lib.tpc_tracker_step_name(0) == b"ingest_radix_sort" and lib.tpc_tracker_step_name(99) is None
 
 
 def test_arena_bytes_is_host_arithmetic_and_reuses_memory():
@@ -36,8 +36,8 @@ def test_arena_bytes_is_host_arithmetic_and_reuses_memory():
     T_cap = n // 10 + 4096
     # sum of all arrays if nothing were reused vs the planned peak
     n_bins = (50485 // 2 + 1) * 36 * 152
-    no_reuse = (4 * (n_bins + 1) + 4 * n + 8 * n + 4 * n + 2 * n + 3 * 4 * n + n + 8 * n
-                + T_cap * (4 * 160 + 4 * 4 + 28 + 36 + 4 * 5))
+    no_reuse = (4 * (n_bins + 1) + 16 * n + 16 * n + 2 * n + 3 * 4 * n + n + 8 * n
+                + T_cap * (4 * 160 + 4 * 4 + 28 + 36 + 4 * 5 + 32))
     assert need < 0.85 * no_reuse
     # the floor: what is alive at the same time in the selector (tracklet store + claim + orig + hsr)
     assert need > T_cap * 4 * 160 + 8 * n + 4 * n + 2 * n
