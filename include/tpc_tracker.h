@@ -146,6 +146,12 @@ const char* tpc_tracker_step_name(int32_t step);
 /* Number of kernel launches the last tpc_track_timeframe call enqueued (memsets not counted).              */
 int64_t tpc_tracker_last_launches(const tpc_tracker_t* tracker);
 
+/* Work counters of the last completed call, read back from the device (synchronises `cuda_stream`):
+ * out[0] tracklets constructed, [1] start hits found, [2] invalid clusters, [3] row steps (transports) of the
+ * tracklet constructor, [4] Kalman updates, [5] candidates scanned by its window searches.  These are the units of
+ * the constructor's roofline.  Returns the number of counters (6) or a negative status.      */
+int tpc_tracker_work_counters(tpc_tracker_t* tracker, void* cuda_stream, int64_t* out, int32_t capacity);
+
 /* Arena plan: for allocation i writes name, offset, bytes, first and last step of its lifetime.
  * Returns the number of allocations; i out of range returns -1.                                            */
 int tpc_tracker_arena_plan(const tpc_tracker_t* tracker, int32_t i, const char** name, size_t* offset,

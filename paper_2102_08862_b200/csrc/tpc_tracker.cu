@@ -261,6 +261,19 @@ int tpc_tracker_arena_plan(const tpc_tracker_t* t, int32_t i, const char** name,
 
 int64_t tpc_tracker_last_launches(const tpc_tracker_t* t) { return t ? t->last_launches : -1; }
 
+int tpc_tracker_work_counters(tpc_tracker_t* t, void* cuda_stream, int64_t* out, int32_t capacity) {
+  if (!t || !out || capacity < 0) return TPC_EINVAL;
+  struct { int32_t i32[8]; unsigned long long u64[28]; } h;     // the 256-byte counter block
+  static_assert(sizeof(h) == 256, "counter block");
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (cudaMemcpyAsync(&h, t->plan.ptr<char>(t->params.arena, t->id.counters), 256, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+      cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return TPC_ECUDA; }
+  const int64_t v[7] = {h.i32[kCntTracklets], h.i32[kCntStartHits], (int64_t)(uint32_t)h.i32[kCntInvalid],
+                        (int64_t)h.u64[kCnt64RowSteps - 4], (int64_t)h.u64[kCnt64Updates - 4], (int64_t)h.u64[kCnt64Candidates - 4], 0};
+  for (int i = 0; i < 6 && i < capacity; ++i) out[i] = v[i];
+  return 6;
+}
+
 int tpc_tracker_step_ms(tpc_tracker_t* t, float* ms_out, int32_t capacity) {
   if (!t || !ms_out) return TPC_EINVAL;
   if (!t->profile || !t->have_times) return TPC_EINVAL;
@@ -303,9 +316,8 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   uint8_t* start_flag = P.ptr<uint8_t>(A, id.start_flag);
   uint32_t* cta_count = P.ptr<uint32_t>(A, id.cta_count);
   uint32_t* start_hits = P.ptr<uint32_t>(A, id.start_hits);
-  int32_t* counters = P.ptr<int32_t>(A, id.counters);          // [0] tracklets, [1] start hits, [2] invalid clusters, [3] work queue
-  uint32_t* n_invalid = reinterpret_cast<uint32_t*>(counters + 2);
-  uint32_t* work_counter = reinterpret_cast<uint32_t*>(counters + 3);
+  int32_t* counters = P.ptr<int32_t>(A, id.counters);          // layout: kCnt* in tracklet.cuh
+  uint32_t* n_invalid = reinterpret_cast<uint32_t*>(counters + kCntInvalid);
   TrackletSeeds seeds;
   seeds.a = P.ptr<int4>(A, id.seeds_a);
   seeds.b = P.ptr<float4>(A, id.seeds_b);
@@ -377,9 +389,9 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   // ---- C5 tracklet constructor ----
   mark(S_CONSTRUCT);
   const int64_t tl_bound = std::min<int64_t>(T, n / std::max(2, c.seed_min_hits) + 1);   // start hits own disjoint chains
-  k_tracklet_init<<<(int)((tl_bound + 255) / 256), 256, 0, st>>>(yt, hsr, link_up_clean, start_hits, counters, seeds, c); ++launches;
+  k_tracklet_init<<<(int)((tl_bound + 255) / 256), 256, 0, st>>>(yt, hsr, link_up_clean, start_hits, counters, seeds, tl.row_hit, c); ++launches;
   k_tracklet_constructor<<<(int)std::min<int64_t>(t->constructor_ctas, (tl_bound + kTrackletThreads - 1) / kTrackletThreads),
-                           kTrackletThreads, 0, st>>>(yt, orig, bin_start, link_up_clean, seeds, counters, work_counter, tl, c); ++launches;
+                           kTrackletThreads, 0, st>>>(yt, orig, bin_start, seeds, counters, tl, c); ++launches;
   const int warp_ctas = (int)((tl_bound * 32 + kSelectorThreads - 1) / kSelectorThreads);
   if (tl_taps) {
     k_export_tracklets<<<warp_ctas, kSelectorThreads, 0, st>>>(tl, counters, orig, o->n_tracklets, o->tracklet_seed, o->tracklet_n_hits,

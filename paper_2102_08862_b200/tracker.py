@@ -16,7 +16,8 @@ TPC_OK, TPC_EINVAL, TPC_ENOMEM, TPC_ECUDA = 0, -1, -2, -3
 STATUS_TRACKLET_OVERFLOW, STATUS_TRACK_OVERFLOW, STATUS_TRACK_HIT_OVERFLOW, STATUS_INVALID_CLUSTERS = 1, 2, 4, 8
 
 EXPORTS = ("tpc_tracker_arena_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
-           "tpc_tracker_step_ms", "tpc_tracker_step_name", "tpc_tracker_last_launches", "tpc_tracker_arena_plan",
+           "tpc_tracker_step_ms", "tpc_tracker_step_name", "tpc_tracker_last_launches", "tpc_tracker_work_counters",
+           "tpc_tracker_arena_plan",
            "tpc_tracker_destroy", "tpc_strerror")
 
 
@@ -93,13 +94,14 @@ def load_library(build_if_missing: bool = True):
         L.tpc_tracker_step_name.restype = C.c_char_p
         L.tpc_tracker_last_launches.argtypes = [vp]
         L.tpc_tracker_last_launches.restype = C.c_int64
+        L.tpc_tracker_work_counters.argtypes = [vp, vp, C.POINTER(C.c_int64), C.c_int32]
         L.tpc_tracker_arena_plan.argtypes = [vp, C.c_int32, C.POINTER(C.c_char_p), C.POINTER(C.c_size_t),
                                              C.POINTER(C.c_size_t), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
         L.tpc_tracker_destroy.argtypes = [vp]
         L.tpc_strerror.argtypes = [C.c_int]
         L.tpc_strerror.restype = C.c_char_p
         for nm in ("tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host", "tpc_tracker_step_ms",
-                   "tpc_tracker_arena_plan", "tpc_tracker_destroy"):
+                   "tpc_tracker_work_counters", "tpc_tracker_arena_plan", "tpc_tracker_destroy"):
             getattr(L, nm).restype = C.c_int
         _lib = L
     return _lib
@@ -258,6 +260,15 @@ class Tracker:
 
     def last_launches(self) -> int:
         return int(self.lib.tpc_tracker_last_launches(self.handle))
+
+    def work_counters(self, stream=None) -> dict:
+        s = stream if stream is not None else self._torch.cuda.current_stream(self.device)
+        buf = (C.c_int64 * 8)()
+        k = self.lib.tpc_tracker_work_counters(self.handle, C.c_void_p(s.cuda_stream), buf, 8)
+        if k < 0:
+            raise TpcError(k, "tpc_tracker_work_counters")
+        names = ("tracklets", "start_hits", "invalid_clusters", "row_steps", "updates", "candidates")
+        return {nm: int(buf[i]) for i, nm in enumerate(names)}
 
     def arena_plan(self) -> list:
         out, i = [], 0
