@@ -90,9 +90,10 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def _tracker_params(T, cfg, n, host_staging, profile, grid_time_bins=0):
+def _tracker_params(T, cfg, n, host_staging, profile, grid=(0, 0, 0)):
     p = T.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm, max_clusters=n)
-    p.host_staging, p.profile, p.grid_time_bins = int(host_staging), int(profile), int(grid_time_bins)
+    p.host_staging, p.profile, p.grid_time_bins, p.grid_pad_bins = int(host_staging), int(profile), int(grid[0]), int(grid[1])
+    p.slice_time_bins = int(grid[2])
     return p
 
 
@@ -148,6 +149,8 @@ def main():
     ap.add_argument("--ref-frame-us", type=float, default=60.0, help="frame length of one reference-arm step")
     ap.add_argument("--cpu-sample-us", type=float, default=150.0, help="frame length of the cpu_baseline sample")
     ap.add_argument("--grid-time-bins", type=int, default=0, help="grid bin width in time bins (0 = library default)")
+    ap.add_argument("--slice-time-bins", type=int, default=0, help="processing-order time slice (0 = library default)")
+    ap.add_argument("--grid-pad-bins", type=int, default=0, help="grid bins across a pad row (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -184,7 +187,7 @@ def main():
     torch.cuda.synchronize()
 
     g = T.default_geometry(cfg.n_sectors, tf.max_time_bin)
-    trk = T.Tracker(g, _tracker_params(T, cfg, n, False, True, args.grid_time_bins), device=str(dev))
+    trk = T.Tracker(g, _tracker_params(T, cfg, n, False, True, (args.grid_time_bins, args.grid_pad_bins, args.slice_time_bins)), device=str(dev))
     outs = trk.alloc_outputs(n)
     stream = torch.cuda.Stream(device=dev)
 
@@ -240,7 +243,7 @@ def main():
     # ---- end to end through the C-ABI host entry point (pinned host buffers) ----
     e2e = None
     if not args.no_e2e:
-        trk = T.Tracker(g, _tracker_params(T, cfg, n, True, False, args.grid_time_bins), device=str(dev))
+        trk = T.Tracker(g, _tracker_params(T, cfg, n, True, False, (args.grid_time_bins, args.grid_pad_bins, args.slice_time_bins)), device=str(dev))
         houts = trk.alloc_outputs(n, host=True)
         for _ in range(2):
             trk.tpc_track_timeframe_host(*host, n=n, outputs=houts, stream=stream)

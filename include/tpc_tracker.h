@@ -71,7 +71,13 @@ typedef struct {
   float sin_phi_max;              /* 0.95                                                     (reading A12) */
   float inv_R_per_qpt;            /* (float)(1/666.7) : curvature [1/cm] per q/pT [1/GeV]     (BASELINE L7) */
   float c0_y2, c0_s2, c0_k2, c0_z2, c0_t2; /* initial / reset covariance diagonal             (reading A8)  */
-  int32_t grid_time_bins;         /* width of one grid bin in time bins; 0 = default (2)                    */
+  int32_t grid_time_bins;         /* width of one grid bin in time bins; 0 = default (4)                    */
+  int32_t grid_pad_bins;          /* grid bins across a pad row; 0 = default (8); lowered automatically so that
+                                     no lookup window spans more than two of them.  The grid only accelerates:
+                                     results do not depend on either value.                                  */
+  int32_t slice_time_bins;        /* tracklets are constructed in (sector, time slice, row) order for cache
+                                     locality; width of a slice in time bins; 0 = default (256)              */
+  int32_t reserved0;
   int64_t max_clusters;           /* capacity: largest n of any tpc_track_timeframe call                    */
   int64_t max_tracklets;          /* capacity of the tracklet store; 0 = max_clusters/10 + 4096             */
   int64_t max_tracks;             /* host entry point only: staging capacity; 0 = max_clusters/64 + 4096    */

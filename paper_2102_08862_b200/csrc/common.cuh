@@ -12,11 +12,12 @@ constexpr uint32_t kInvalidRank = 0xFFFFFFFFu;
 // on the host in double from the fp32 parameter values and rounded once ("Notation").
 struct Consts {
   // geometry
-  int n_rows, n_sr, n_tb, n_bins;        // rows per sector, sector-rows, time bins per sector-row, n_sr*n_tb
-  float max_time, inv_bin_w;             // validity bound of the time coordinate; 1 / grid bin width
+  int n_rows, n_sr, n_tb, n_pb, n_bins;  // rows per sector, sector-rows, time bins and pad bins per sector-row, n_sr*n_pb*n_tb
+  float max_time, inv_bin_w;             // validity bound of the time coordinate; 1 / grid bin width (time)
   float Z, inv_Z, P;                     // time-bin size [cm], its inverse (grid lookups only), pad pitch
   // neighbours finder (C2)
-  float W1, Ay, Az, wy, wz, chi2_cut, finder_tw;   // finder_tw: half width of the lookup in time bins (+margin)
+  float W1, Ay, Az, wy, wz, chi2_cut;
+  float finder_tw, finder_yw;            // half widths of the grid lookup: time bins / cm, each with a safety margin
   // tracklet constructor (C5)
   float ry, rz, cB, sin_phi_max, win_slope, win_const;
   float c0_y2, c0_s2, c0_k2, c0_z2, c0_t2;
@@ -25,6 +26,8 @@ struct Consts {
   const float* xr;                       // [n_rows] x of the pad row
   const float* cr;                       // [n_rows] pad centre 0.5*(n_pads-1)
   const int* npads;                      // [n_rows]
+  const float* yoff;                     // [n_rows] half width of the row in cm: pad bin = floor((y + yoff) * pscale)
+  const float* pscale;                   // [n_rows] n_pb / (row width in cm)
 };
 
 // Grid bin of a time value: monotone non-decreasing in t, so a lookup over [bin(t_lo), bin(t_hi)] is a
@@ -33,6 +36,12 @@ struct Consts {
 __device__ __forceinline__ int time_bin(float t, const Consts& c) {
   int b = (int)floorf(t * c.inv_bin_w);
   return min(max(b, 0), c.n_tb - 1);
+}
+
+// Grid pad bin of a local y in a row (yoff, pscale of that row): monotone non-decreasing in y for the same reason.
+__device__ __forceinline__ int pad_bin(float y, float yoff, float pscale, const Consts& c) {
+  int b = (int)floorf((y + yoff) * pscale);
+  return min(max(b, 0), c.n_pb - 1);
 }
 
 __device__ __forceinline__ unsigned lane_id() { return threadIdx.x & 31u; }

@@ -38,9 +38,18 @@ __device__ __forceinline__ bool in_search_area(const float2 me, const float2 cq,
   return fabsf(dy) < c.Ay && fabsf(dz) < c.Az;
 }
 
-// SIMT shape: ONE flat loop scans the candidates of both neighbour rows and keeps those inside the search area
-// in register slots (<= 4 per row; more is rare and takes the generic nested loop), then a short pair loop.
-// The nested "for u: for d" form ran at 4.5 of 32 lanes (profiles/r01a_ncu_full_baseline.md).
+// Candidate span of one (sector-row, pad bin): the hits of the time bins [tb_lo, tb_hi].
+struct Span { uint32_t lo, n; };
+__device__ __forceinline__ Span grid_span(const uint32_t* __restrict__ bin_start, int sr, int pb, int tb_lo, int tb_hi, const Consts& c) {
+  const uint32_t* bs = bin_start + ((size_t)sr * c.n_pb + pb) * c.n_tb;
+  const uint32_t lo = __ldg(bs + tb_lo);
+  return Span{lo, __ldg(bs + tb_hi + 1) - lo};
+}
+
+// SIMT shape: ONE flat loop scans the candidates of both neighbour rows (each row: the spans of one or two pad
+// bins -- the create-time check guarantees that the search area is narrower than a pad bin) and keeps those inside
+// the search area in register slots (<= 4 per row; more is rare and takes the generic nested loop), then a short
+// pair loop.  The nested "for u: for d" form ran at 4.5 of 32 lanes (profiles/r01a_ncu_full_baseline.md).
 __global__ void __launch_bounds__(256) k_neighbours_finder(const float2* __restrict__ yt, const uint32_t* __restrict__ orig,
                                                            const uint16_t* __restrict__ hsr, const uint32_t* __restrict__ bin_start,
                                                            int* __restrict__ link_up, int* __restrict__ link_down,
@@ -54,11 +63,20 @@ __global__ void __launch_bounds__(256) k_neighbours_finder(const float2* __restr
   if (r >= 1 && r <= c.n_rows - 2) {
     const float2 me = yt[h];
     const int tb_lo = time_bin(me.y - c.finder_tw, c), tb_hi = time_bin(me.y + c.finder_tw, c);
-    const uint32_t* bs_u = bin_start + (size_t)(sr + 1) * c.n_tb;
-    const uint32_t* bs_d = bin_start + (size_t)(sr - 1) * c.n_tb;
-    const uint32_t u_lo = __ldg(bs_u + tb_lo), u_hi = __ldg(bs_u + tb_hi + 1);
-    const uint32_t d_lo = __ldg(bs_d + tb_lo), d_hi = __ldg(bs_d + tb_hi + 1);
-    const uint32_t n_u = u_hi - u_lo, n_all = n_u + (d_hi - d_lo);
+    const float yo_u = __ldg(c.yoff + r + 1), ps_u = __ldg(c.pscale + r + 1);
+    const float yo_d = __ldg(c.yoff + r - 1), ps_d = __ldg(c.pscale + r - 1);
+    const int pu0 = pad_bin(me.x - c.finder_yw, yo_u, ps_u, c), pu1 = pad_bin(me.x + c.finder_yw, yo_u, ps_u, c);
+    const int pd0 = pad_bin(me.x - c.finder_yw, yo_d, ps_d, c), pd1 = pad_bin(me.x + c.finder_yw, yo_d, ps_d, c);
+    // spans: u0, u1 (row r+1), d0, d1 (row r-1); the second span of a row is empty unless the area straddles two pad bins
+    const Span u0 = grid_span(bin_start, sr + 1, pu0, tb_lo, tb_hi, c);
+    const Span d0 = grid_span(bin_start, sr - 1, pd0, tb_lo, tb_hi, c);
+    Span u1{0u, 0u}, d1{0u, 0u};
+    if (pu1 != pu0) u1 = grid_span(bin_start, sr + 1, pu1, tb_lo, tb_hi, c);
+    if (pd1 != pd0) d1 = grid_span(bin_start, sr - 1, pd1, tb_lo, tb_hi, c);
+    const uint32_t e0 = u0.n, e1 = e0 + u1.n, e2 = e1 + d0.n, n_all = e2 + d1.n;   // n_u = e1
+    auto index_of = [&](uint32_t i) -> uint32_t {
+      return i < e0 ? u0.lo + i : i < e1 ? u1.lo + (i - e0) : i < e2 ? d0.lo + (i - e1) : d1.lo + (i - e2);
+    };
     uint32_t us0 = 0, us1 = 0, us2 = 0, us3 = 0, ds0 = 0, ds1 = 0, ds2 = 0, ds3 = 0;
     int nu = 0, nd = 0;
     for (uint32_t ib = 0; ib < n_all; ib += 4) {     // batches of 4 independent loads
@@ -66,8 +84,7 @@ __global__ void __launch_bounds__(256) k_neighbours_finder(const float2* __restr
       uint32_t qq[4];
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
-        const uint32_t i = min(ib + k, n_all - 1);
-        qq[k] = i < n_u ? u_lo + i : d_lo + (i - n_u);
+        qq[k] = index_of(min(ib + k, n_all - 1));
         cq[k] = yt[qq[k]];
       }
 #pragma unroll
@@ -75,7 +92,7 @@ __global__ void __launch_bounds__(256) k_neighbours_finder(const float2* __restr
         const uint32_t i = ib + k;
         if (!(i < n_all && in_search_area(me, cq[k], c))) continue;
         const uint32_t q = qq[k];
-        if (i < n_u) {
+        if (i < e1) {
           if (nu == 0) us0 = q; else if (nu == 1) us1 = q; else if (nu == 2) us2 = q; else if (nu == 3) us3 = q;
           ++nu;
         } else {
@@ -94,11 +111,13 @@ __global__ void __launch_bounds__(256) k_neighbours_finder(const float2* __restr
           finder_try_pair(me, cu, yt[qd], qu, qd, orig, c, best, bu, bd);
         }
       }
-    } else {   // crowded area: generic nested loops over the spans, same pair order
-      for (uint32_t qu = u_lo; qu < u_hi; ++qu) {
+    } else {   // crowded area: generic nested loops over the spans (ties are decided on the original index)
+      for (uint32_t iu = 0; iu < e1; ++iu) {
+        const uint32_t qu = index_of(iu);
         const float2 cu = yt[qu];
         if (!in_search_area(me, cu, c)) continue;
-        for (uint32_t qd = d_lo; qd < d_hi; ++qd) {
+        for (uint32_t id = e1; id < n_all; ++id) {
+          const uint32_t qd = index_of(id);
           const float2 cd = yt[qd];
           if (!in_search_area(me, cd, c)) continue;
           finder_try_pair(me, cu, cd, qu, qd, orig, c, best, bu, bd);

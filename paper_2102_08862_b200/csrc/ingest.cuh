@@ -1,8 +1,8 @@
 // C1 cluster ingest (BASELINE.json L5 item 1: "sorts clusters into per-(sector, row) grids of (pad, time) bins by
 // radix sort and prefix scan"; PAPER.md L23 native coordinates).
 //
-// key(i) = (sector*n_rows + row) * n_tb + time_bin(time)   (= grid bin index; n_bins for clusters outside the
-// geometry, which therefore sort to the end).  A stable least-significant-digit radix sort on the key orders the
+// key(i) = ((sector*n_rows + row) * n_pb + pad_bin(y)) * n_tb + time_bin(time)   (= grid bin index; n_bins for
+// clusters outside the geometry, which therefore sort to the end).  A stable least-significant-digit radix sort on the key orders the
 // frame by (sector-row, time bin) and, inside a bin, by original index -- the layout is deterministic.
 // One pass = k_radix_histogram (digit counts per 2048-element tile) -> exclusive prefix scan over
 // (digit, tile) -> k_radix_scatter (stable in-tile ranking by warp match, local reorder in shared memory, then
@@ -25,14 +25,17 @@ constexpr size_t kRadixScatterSmem = (size_t)kRadixTile * 16 + (size_t)(kRadixTh
 
 // A cluster is inside the geometry iff row is an integer in [0, n_sr), pad in [-0.5, n_pads-0.5) and
 // time in [0, max_time]; evaluated in fp32 on the raw values (DESIGN.md §3 C1).
-__device__ __forceinline__ uint32_t cluster_key(float rf, float pad, float time, const Consts& c) {
+// Also returns the local y of a valid cluster.
+__device__ __forceinline__ uint32_t cluster_key(float rf, float pad, float time, const Consts& c, float& y) {
+  y = 0.0f;
   bool ok = rf >= 0.0f && rf < (float)c.n_sr && rf == floorf(rf);
   if (!ok) return (uint32_t)c.n_bins;
   const int sr = (int)rf;
   const int r = sr % c.n_rows;
   ok = pad >= -0.5f && pad < (float)__ldg(c.npads + r) - 0.5f && time >= 0.0f && time <= c.max_time;
   if (!ok) return (uint32_t)c.n_bins;
-  return (uint32_t)(sr * c.n_tb + time_bin(time, c));
+  y = (pad - __ldg(c.cr + r)) * c.P;                                   // y(h) = (pad - c_r) * P
+  return (uint32_t)((sr * c.n_pb + pad_bin(y, __ldg(c.yoff + r), __ldg(c.pscale + r), c)) * c.n_tb + time_bin(time, c));
 }
 
 struct RadixSrc {        // input of a pass: either the raw clusters (first pass) or a sorted-so-far set
@@ -54,7 +57,8 @@ __global__ void __launch_bounds__(kRadixThreads) k_radix_histogram(RadixSrc src,
   for (int k = 0; k < kRadixItems; ++k) {
     const int64_t i = base + (int64_t)k * kRadixThreads + threadIdx.x;
     if (i < n) {
-      const uint32_t key = kFirst ? cluster_key(src.row[i], src.pad[i], src.time[i], c) : src.keys[i];
+      float y;
+      const uint32_t key = kFirst ? cluster_key(src.row[i], src.pad[i], src.time[i], c, y) : src.keys[i];
       atomicAdd(&cnt[(key >> shift) & mask], 1u);
     }
   }
@@ -97,11 +101,10 @@ __global__ void __launch_bounds__(kRadixThreads, 3) k_radix_scatter(RadixSrc src
     if (i < n) {
       if (kFirst) {
         const float rf = src.row[i], p = src.pad[i], t = src.time[i];
-        key[k] = cluster_key(rf, p, t, c);
+        float y;
+        key[k] = cluster_key(rf, p, t, c, y);
         og[k] = (uint32_t)i;
-        float y = 0.0f;
-        if (key[k] != (uint32_t)c.n_bins) y = (p - __ldg(c.cr + ((int)rf) % c.n_rows)) * c.P;   // y(h) = (pad - c_r) * P
-        else ++bad;
+        if (key[k] == (uint32_t)c.n_bins) ++bad;
         yt[k] = make_float2(y, t);
       } else {
         key[k] = src.keys[i]; og[k] = src.orig[i]; yt[k] = src.yt[i];
@@ -181,7 +184,7 @@ __global__ void __launch_bounds__(256) k_grid_build(const uint32_t* __restrict__
   const uint32_t nb = (uint32_t)c.n_bins;
   const int64_t kprev = i == 0 ? -1 : (int64_t)min(keys[i - 1], nb);
   const uint32_t kcur = i == n ? nb : min(keys[i], nb);
-  if (i < n && kcur < nb) hsr[i] = (uint16_t)(kcur / (uint32_t)c.n_tb);
+  if (i < n && kcur < nb) hsr[i] = (uint16_t)(kcur / (uint32_t)(c.n_tb * c.n_pb));
   for (int64_t b = kprev + 1; b <= (int64_t)kcur; ++b) bin_start[b] = (uint32_t)i;
 }
 

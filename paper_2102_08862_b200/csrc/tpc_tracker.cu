@@ -30,16 +30,21 @@ const char* const kStepNames[N_STEPS] = {
 
 struct Ids {   // arena allocation ids
   int stage_in = -1, stage_out = -1;
-  int bin_start, sort_keys, tmp_keys, tmp_orig, tmp_yt, sort_hist, yt, orig, hsr, link_up, link_down, link_up_clean, start_flag, cta_count, start_hits,
+  int bin_start, sort_keys, tmp_keys, tmp_orig, tmp_yt, sort_hist, yt, orig, hsr, link_up, link_down, link_up_clean, start_flag, cell_count, start_hits,
       counters, scan_a, scan_b, seeds_a, seeds_b, row_hit, tl_n_hits, tl_first, tl_last, tl_seed, tl_par, tl_cov, claim, owned,
       flag, track_idx, hit_off;
 };
 
 struct Capacities {
   int64_t max_clusters, max_tracklets, max_tracks, max_track_hits;
-  int n_tb, n_bins, n_link_ctas;
+  int n_tb, n_pb, grid_w, n_bins, n_link_ctas;
+  int n_slices, slice_bins;     // start-hit processing order: time slices of slice_bins grid time bins
+  int64_t n_cells;
   int sort_passes, sort_digit_bits, sort_tiles;
 };
+
+constexpr int kDefaultGridTimeBins = 4, kDefaultGridPadBins = 8, kDefaultSliceTimeBins = 256;
+constexpr double kGridMarginCm = 0.01;   // superset margin of the pad-bin lookups (fp32 rounding of a difference is << this)
 
 bool valid_geometry(const tpc_geometry_t* g) {
   return g && g->n_sectors >= 1 && g->n_rows >= 3 && g->n_rows <= kRowStride &&
@@ -49,7 +54,7 @@ bool valid_geometry(const tpc_geometry_t* g) {
 
 bool valid_params(const tpc_params_t* p) {
   return p && p->miss_limit >= 1 && p->min_hits >= 1 && p->seed_min_hits >= 2 && p->sigma_y_cm > 0 &&
-         p->sigma_z_cm > 0 && p->sin_phi_max > 0 && p->sin_phi_max < 1 && p->grid_time_bins >= 0 &&
+         p->sigma_z_cm > 0 && p->sin_phi_max > 0 && p->sin_phi_max < 1 && p->grid_time_bins >= 0 && p->slice_time_bins >= 0 && p->grid_pad_bins >= 0 && p->grid_pad_bins <= 64 &&
          p->max_clusters >= 0 && p->max_clusters < ((int64_t)1 << 31) && p->max_tracklets >= 0 &&
          p->max_tracklets < ((int64_t)1 << 31) / kRowStride * 32 && p->max_tracks >= 0 && p->max_track_hits >= 0 &&
          p->win_const > 0 && p->win_slope >= 0 && p->chi2_cut > 0;
@@ -62,13 +67,30 @@ bool capacities(const tpc_geometry_t* g, const tpc_params_t* p, int64_t max_clus
   c.max_tracklets = p->max_tracklets > 0 ? p->max_tracklets : c.max_clusters / 10 + 4096;
   c.max_tracks = p->max_tracks > 0 ? p->max_tracks : c.max_clusters / 64 + 4096;
   c.max_track_hits = p->max_track_hits > 0 ? p->max_track_hits : c.max_clusters;
-  const int w = p->grid_time_bins > 0 ? p->grid_time_bins : 2;
-  const double ntb = std::floor((double)g->max_time_bin / (double)w) + 1.0;
-  const double nb = ntb * (double)g->n_sectors * (double)g->n_rows;
+  c.grid_w = p->grid_time_bins > 0 ? p->grid_time_bins : kDefaultGridTimeBins;
+  // Pad bins per row: as requested, but a lookup window must never span more than two of them.  Widest windows:
+  // the finder's search area A_y and the follower's window after miss_limit missed rows, each with its margin.
+  {
+    const double pitch = (double)g->row_pitch_cm;
+    const double w1 = (double)p->win_slope * pitch + (double)p->win_const;
+    const double ay = (double)p->slope_y_max * pitch + w1 + kGridMarginCm;
+    const double wf = (double)p->win_slope * pitch * (double)(p->miss_limit + 1) + (double)p->win_const + kGridMarginCm;
+    const double narrowest = std::floor(2.0 * (double)g->x0_cm * (double)g->tan_half_sector / (double)g->pad_pitch_cm) * (double)g->pad_pitch_cm;
+    int npb = p->grid_pad_bins > 0 ? p->grid_pad_bins : kDefaultGridPadBins;
+    while (npb > 1 && 2.0 * std::max(ay, wf) * 1.01 > narrowest / (double)npb) --npb;
+    c.n_pb = npb;
+  }
+  const double ntb = std::floor((double)g->max_time_bin / (double)c.grid_w) + 1.0;
+  const double nb = ntb * (double)c.n_pb * (double)g->n_sectors * (double)g->n_rows;
   if (nb >= 2147483000.0) return false;
   c.n_tb = (int)ntb;
   c.n_bins = (int)nb;
   c.n_link_ctas = (int)((c.max_clusters + kLinkThreads - 1) / kLinkThreads);
+  const int slice_tb = p->slice_time_bins > 0 ? p->slice_time_bins : kDefaultSliceTimeBins;
+  c.slice_bins = std::max(1, slice_tb / c.grid_w);
+  c.n_slices = (c.n_tb + c.slice_bins - 1) / c.slice_bins;
+  c.n_cells = (int64_t)g->n_sectors * g->n_rows * c.n_pb * c.n_slices;
+  if (c.n_cells >= 2147483000) return false;
   int bits = 1;
   while (((int64_t)1 << bits) <= (int64_t)c.n_bins) ++bits;          // the sentinel key n_bins must be representable
   c.sort_passes = (bits + kRadixMaxBits - 1) / kRadixMaxBits;
@@ -86,7 +108,7 @@ void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids
                             S_EMIT, S_EMIT);
   }
   const size_t hist_len = (size_t)kRadixBuckets * (size_t)c.sort_tiles + 1;
-  const size_t scan_len = std::max(std::max(scan_tiles(hist_len), scan_tiles((size_t)c.n_link_ctas + 1)), scan_tiles(T)) + 2;
+  const size_t scan_len = std::max(std::max(scan_tiles(hist_len), scan_tiles((size_t)c.n_cells + 1)), scan_tiles(T)) + 2;
   id.counters = plan.add("counters", 256, S_SORT, S_EMIT);
   id.scan_a = plan.add("scan_tile_sums_a", 4 * scan_len, S_SORT, S_EMIT);
   id.scan_b = plan.add("scan_tile_sums_b", 4 * scan_len, S_SORT, S_EMIT);
@@ -103,7 +125,7 @@ void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids
   id.link_down = plan.add("link_down_raw", 4 * N, S_FINDER, S_CLEAN_START);
   id.link_up_clean = plan.add("link_up_clean", 4 * N, S_CLEAN_START, S_CONSTRUCT);
   id.start_flag = plan.add("start_flag(u8)", N, S_CLEAN_START, S_COMPACT);
-  id.cta_count = plan.add("start_cta_count", 4 * ((size_t)c.n_link_ctas + 2), S_CLEAN_START, S_COMPACT);
+  id.cell_count = plan.add("start_cell_count", 4 * ((size_t)c.n_cells + 2), S_COMPACT, S_COMPACT);
   id.start_hits = plan.add("start_hits", 4 * T, S_COMPACT, S_EMIT);
   id.seeds_a = plan.add("tracklet_seeds_a(int4)", 16 * T, S_CONSTRUCT, S_CONSTRUCT);
   id.seeds_b = plan.add("tracklet_seeds_b(float4)", 16 * T, S_CONSTRUCT, S_CONSTRUCT);
@@ -176,7 +198,7 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
 
   // per-row tables in double, rounded once
   const int nr = g->n_rows;
-  std::vector<float> xr(nr), cr(nr);
+  std::vector<float> xr(nr), cr(nr), yoff(nr), pscale(nr);
   std::vector<int> npads(nr);
   const double pitch = (double)g->row_pitch_cm;
   for (int r = 0; r < nr; ++r) {
@@ -185,21 +207,26 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
     npads[r] = (int)std::floor(2.0 * x * (double)g->tan_half_sector / (double)g->pad_pitch_cm);
     if (npads[r] < 1) { delete t; return TPC_EINVAL; }
     cr[r] = (float)(0.5 * (double)(npads[r] - 1));
+    const double width = (double)npads[r] * (double)g->pad_pitch_cm;       // y spans [-width/2, +width/2)
+    yoff[r] = (float)(0.5 * width);
+    pscale[r] = (float)((double)t->cap.n_pb / width);
   }
   int n_dev = 0;
   if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) { cudaGetLastError(); delete t; return TPC_ECUDA; }
-  const size_t tab_bytes = (size_t)nr * 12;
+  const size_t tab_bytes = (size_t)nr * 20;
   if (cudaMalloc(&t->tables, tab_bytes) != cudaSuccess) { cudaGetLastError(); delete t; return TPC_ECUDA; }
   char* tb = static_cast<char*>(t->tables);
   if (cudaMemcpy(tb, xr.data(), (size_t)nr * 4, cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaMemcpy(tb + (size_t)nr * 4, cr.data(), (size_t)nr * 4, cudaMemcpyHostToDevice) != cudaSuccess ||
-      cudaMemcpy(tb + (size_t)nr * 8, npads.data(), (size_t)nr * 4, cudaMemcpyHostToDevice) != cudaSuccess) {
+      cudaMemcpy(tb + (size_t)nr * 8, npads.data(), (size_t)nr * 4, cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemcpy(tb + (size_t)nr * 12, yoff.data(), (size_t)nr * 4, cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemcpy(tb + (size_t)nr * 16, pscale.data(), (size_t)nr * 4, cudaMemcpyHostToDevice) != cudaSuccess) {
     cudaGetLastError(); cudaFree(t->tables); delete t; return TPC_ECUDA;
   }
 
   Consts& c = t->consts;
-  const int w = p->grid_time_bins > 0 ? p->grid_time_bins : 2;
-  c.n_rows = nr; c.n_sr = g->n_sectors * nr; c.n_tb = t->cap.n_tb; c.n_bins = t->cap.n_bins;
+  const int w = t->cap.grid_w;
+  c.n_rows = nr; c.n_sr = g->n_sectors * nr; c.n_tb = t->cap.n_tb; c.n_pb = t->cap.n_pb; c.n_bins = t->cap.n_bins;
   c.max_time = g->max_time_bin; c.inv_bin_w = (float)(1.0 / (double)w);
   c.Z = g->time_bin_cm; c.inv_Z = (float)(1.0 / (double)g->time_bin_cm); c.P = g->pad_pitch_cm;
   const double w1 = (double)p->win_slope * pitch + (double)p->win_const;
@@ -211,12 +238,15 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
   c.ry = (float)sy2; c.rz = (float)sz2;
   c.chi2_cut = p->chi2_cut;
   c.finder_tw = (float)((double)c.Az / (double)g->time_bin_cm + 0.02);
+  c.finder_yw = (float)((double)c.Ay + kGridMarginCm);
   c.cB = p->inv_R_per_qpt; c.sin_phi_max = p->sin_phi_max; c.win_slope = p->win_slope; c.win_const = p->win_const;
   c.c0_y2 = p->c0_y2; c.c0_s2 = p->c0_s2; c.c0_k2 = p->c0_k2; c.c0_z2 = p->c0_z2; c.c0_t2 = p->c0_t2;
   c.miss_limit = p->miss_limit; c.min_hits = p->min_hits; c.seed_min_hits = p->seed_min_hits;
   c.xr = reinterpret_cast<const float*>(tb);
   c.cr = reinterpret_cast<const float*>(tb + (size_t)nr * 4);
   c.npads = reinterpret_cast<const int*>(tb + (size_t)nr * 8);
+  c.yoff = reinterpret_cast<const float*>(tb + (size_t)nr * 12);
+  c.pscale = reinterpret_cast<const float*>(tb + (size_t)nr * 16);
 
   t->profile = p->profile != 0;
   if (cudaFuncSetAttribute(k_radix_scatter<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRadixScatterSmem) != cudaSuccess ||
@@ -314,7 +344,7 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   int* link_down = P.ptr<int>(A, id.link_down);
   int* link_up_clean = P.ptr<int>(A, id.link_up_clean);
   uint8_t* start_flag = P.ptr<uint8_t>(A, id.start_flag);
-  uint32_t* cta_count = P.ptr<uint32_t>(A, id.cta_count);
+  uint32_t* cell_count = P.ptr<uint32_t>(A, id.cell_count);
   uint32_t* start_hits = P.ptr<uint32_t>(A, id.start_hits);
   int32_t* counters = P.ptr<int32_t>(A, id.counters);          // layout: kCnt* in tracklet.cuh
   uint32_t* n_invalid = reinterpret_cast<uint32_t*>(counters + kCntInvalid);
@@ -378,13 +408,19 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
 
   // ---- C3 cleaner + C4 start hits ----
   mark(S_CLEAN_START);
-  k_clean_links_find_starts<<<link_ctas, kLinkThreads, 0, st>>>(link_up, link_down, bin_start, link_up_clean, start_flag, cta_count,
+  k_clean_links_find_starts<<<link_ctas, kLinkThreads, 0, st>>>(link_up, link_down, bin_start, link_up_clean, start_flag,
                                                                 orig, link_taps ? o->link_up : nullptr, o->link_down,
                                                                 o->is_start_hit, c); ++launches;
   mark(S_COMPACT);
-  launches += exclusive_scan_u32(cta_count, cta_count, (size_t)link_ctas + 1, scan_a, st);
-  k_compact_start_hits<<<link_ctas, kLinkThreads, 0, st>>>(start_flag, cta_count, bin_start, start_hits, (uint32_t)T, link_ctas,
-                                                           counters, c); ++launches;
+  {
+    const StartCells sc{t->cap.n_slices, t->cap.slice_bins, (uint32_t)t->cap.n_cells};
+    const int cell_ctas = (int)((t->cap.n_cells + kLinkThreads - 1) / kLinkThreads);
+    const size_t n_cells = (size_t)t->cap.n_cells;
+    k_start_cell_count<<<cell_ctas, kLinkThreads, 0, st>>>(start_flag, bin_start, sc, cell_count, c); ++launches;
+    launches += exclusive_scan_u32(cell_count, cell_count, n_cells, scan_a, st);
+    k_start_cell_write<<<cell_ctas, kLinkThreads, 0, st>>>(start_flag, bin_start, sc, cell_count, scan_a + scan_tiles(n_cells), start_hits,
+                                                           (uint32_t)T, counters, c); ++launches;
+  }
 
   // ---- C5 tracklet constructor ----
   mark(S_CONSTRUCT);

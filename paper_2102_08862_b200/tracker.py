@@ -35,7 +35,8 @@ class Params(C.Structure):
                 ("slope_y_max", C.c_float), ("slope_z_max", C.c_float), ("seed_min_hits", C.c_int32),
                 ("sin_phi_max", C.c_float), ("inv_R_per_qpt", C.c_float),
                 ("c0_y2", C.c_float), ("c0_s2", C.c_float), ("c0_k2", C.c_float), ("c0_z2", C.c_float), ("c0_t2", C.c_float),
-                ("grid_time_bins", C.c_int32), ("max_clusters", C.c_int64), ("max_tracklets", C.c_int64),
+                ("grid_time_bins", C.c_int32), ("grid_pad_bins", C.c_int32), ("slice_time_bins", C.c_int32), ("reserved0", C.c_int32),
+                ("max_clusters", C.c_int64), ("max_tracklets", C.c_int64),
                 ("max_tracks", C.c_int64), ("max_track_hits", C.c_int64), ("arena", C.c_void_p), ("arena_bytes", C.c_size_t),
                 ("host_staging", C.c_int32), ("profile", C.c_int32)]
 
@@ -68,7 +69,7 @@ def default_params(sigma_y: float = 0.08, sigma_z: float = 0.12, max_clusters: i
     return Params(win_slope=0.05, win_const=0.5, chi2_cut=9.0, miss_limit=10, min_hits=30,
                   sigma_y_cm=sigma_y, sigma_z_cm=sigma_z, slope_y_max=1.0, slope_z_max=1.5, seed_min_hits=3,
                   sin_phi_max=0.95, inv_R_per_qpt=1.0 / 666.7, c0_y2=1.0, c0_s2=0.1, c0_k2=100.0, c0_z2=1.0, c0_t2=0.1,
-                  grid_time_bins=0, max_clusters=max_clusters, max_tracklets=0, max_tracks=0, max_track_hits=0,
+                  grid_time_bins=0, grid_pad_bins=0, slice_time_bins=0, reserved0=0, max_clusters=max_clusters, max_tracklets=0, max_tracks=0, max_track_hits=0,
                   arena=None, arena_bytes=0, host_staging=0, profile=0)
 
 

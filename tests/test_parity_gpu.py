@@ -64,11 +64,11 @@ def test_time_coordinate_at_the_end_of_a_10ms_frame():
     assert rep["n_tracks"] > 500
 
 
-@pytest.mark.parametrize("grid_time_bins", [1, 3, 16])
-def test_grid_bin_width_does_not_change_results(grid_time_bins):
-    """The grid only accelerates (BASELINE.json L5 (b)): any bin width gives the oracle's links and tracks."""
+@pytest.mark.parametrize("grid_time_bins,grid_pad_bins", [(1, 1), (3, 2), (16, 8), (2, 5), (4, 64)])
+def test_grid_bin_width_does_not_change_results(grid_time_bins, grid_pad_bins):
+    """The grid only accelerates (BASELINE.json L5 (b)): any bin shape gives the oracle's links and tracks."""
     cfg, tf = _frame(0, 4)
-    g = PU.run_gpu(tf.row, tf.pad, tf.time, 1, tf.max_time_bin, grid_time_bins=grid_time_bins)
+    g = PU.run_gpu(tf.row, tf.pad, tf.time, 1, tf.max_time_bin, grid_time_bins=grid_time_bins, grid_pad_bins=grid_pad_bins)
     o = PU.run_oracle(tf.row, tf.pad, tf.time, 1, tf.max_time_bin)
     PU.compare(g, o)
 
