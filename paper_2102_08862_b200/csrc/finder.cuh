@@ -46,14 +46,21 @@ __device__ __forceinline__ Span grid_span(const uint32_t* __restrict__ bin_start
   return Span{lo, __ldg(bs + tb_hi + 1) - lo};
 }
 
-// SIMT shape: ONE flat loop scans the candidates of both neighbour rows (each row: the spans of one or two pad
-// bins -- the create-time check guarantees that the search area is narrower than a pad bin) and keeps those inside
-// the search area in register slots (<= 4 per row; more is rare and takes the generic nested loop), then a short
-// pair loop.  The nested "for u: for d" form ran at 4.5 of 32 lanes (profiles/r01a_ncu_full_baseline.md).
-__global__ void __launch_bounds__(256) k_neighbours_finder(const float2* __restrict__ yt, const uint32_t* __restrict__ orig,
-                                                           const uint16_t* __restrict__ hsr, const uint32_t* __restrict__ bin_start,
-                                                           int* __restrict__ link_up, int* __restrict__ link_down,
-                                                           const __grid_constant__ Consts c) {
+constexpr int kFinderThreads = 256;
+constexpr int kFinderSlots = 4;       // candidates kept per neighbour row in shared memory; more -> generic path
+
+// SIMT shape: (1) ONE flat loop scans the candidates of both neighbour rows (each row: the spans of one or two pad
+// bins -- the create-time check guarantees that the search area is narrower than a pad bin) and appends those inside
+// the search area to two small per-thread lists in shared memory ([slot][thread]: conflict-free); (2) ONE flat loop
+// over the nu x nd pairs.  Both trip counts are the maximum over the warp of a small number, and the bodies are
+// branch-free apart from the rare exact-tie case.  The nested "for u: for d" form over the raw spans ran at 4.5 of
+// 32 lanes (profiles/r01a_ncu_full_baseline.md).
+__global__ void __launch_bounds__(kFinderThreads) k_neighbours_finder(const float2* __restrict__ yt, const uint32_t* __restrict__ orig,
+                                                                      const uint16_t* __restrict__ hsr, const uint32_t* __restrict__ bin_start,
+                                                                      int* __restrict__ link_up, int* __restrict__ link_down,
+                                                                      const __grid_constant__ Consts c) {
+  __shared__ float2 s_val[2 * kFinderSlots][kFinderThreads];      // rows 0..3: up candidates, 4..7: down candidates
+  __shared__ uint32_t s_idx[2 * kFinderSlots][kFinderThreads];
   const uint32_t n_valid = __ldg(bin_start + c.n_bins);
   const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
   if (h >= n_valid) return;
@@ -73,45 +80,42 @@ __global__ void __launch_bounds__(256) k_neighbours_finder(const float2* __restr
     Span u1{0u, 0u}, d1{0u, 0u};
     if (pu1 != pu0) u1 = grid_span(bin_start, sr + 1, pu1, tb_lo, tb_hi, c);
     if (pd1 != pd0) d1 = grid_span(bin_start, sr - 1, pd1, tb_lo, tb_hi, c);
-    const uint32_t e0 = u0.n, e1 = e0 + u1.n, e2 = e1 + d0.n, n_all = e2 + d1.n;   // n_u = e1
-    auto index_of = [&](uint32_t i) -> uint32_t {
-      return i < e0 ? u0.lo + i : i < e1 ? u1.lo + (i - e0) : i < e2 ? d0.lo + (i - e1) : d1.lo + (i - e2);
-    };
-    uint32_t us0 = 0, us1 = 0, us2 = 0, us3 = 0, ds0 = 0, ds1 = 0, ds2 = 0, ds3 = 0;
+    const uint32_t e0 = u0.n, e1 = e0 + u1.n, e2 = e1 + d0.n, n_all = e2 + d1.n;   // up candidates: i < e1
+    // flat index i -> sorted-hit index: base of the span that holds i, minus the span's first i
+    const uint32_t b0 = u0.lo, b1 = u1.lo - e0, b2 = d0.lo - e1, b3 = d1.lo - e2;
     int nu = 0, nd = 0;
-    for (uint32_t ib = 0; ib < n_all; ib += 4) {     // batches of 4 independent loads
-      float2 cq[4];
-      uint32_t qq[4];
+    for (uint32_t ib = 0; ib < n_all; ib += 2) {     // two independent loads per trip
+      uint32_t qq[2];
+      float2 cq[2];
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        qq[k] = index_of(min(ib + k, n_all - 1));
+      for (int k = 0; k < 2; ++k) {
+        const uint32_t i = min(ib + k, n_all - 1);
+        qq[k] = (i < e1 ? (i < e0 ? b0 : b1) : (i < e2 ? b2 : b3)) + i;
         cq[k] = yt[qq[k]];
       }
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
+      for (int k = 0; k < 2; ++k) {
         const uint32_t i = ib + k;
-        if (!(i < n_all && in_search_area(me, cq[k], c))) continue;
-        const uint32_t q = qq[k];
-        if (i < e1) {
-          if (nu == 0) us0 = q; else if (nu == 1) us1 = q; else if (nu == 2) us2 = q; else if (nu == 3) us3 = q;
-          ++nu;
-        } else {
-          if (nd == 0) ds0 = q; else if (nd == 1) ds1 = q; else if (nd == 2) ds2 = q; else if (nd == 3) ds3 = q;
-          ++nd;
+        if (i < n_all && in_search_area(me, cq[k], c)) {
+          const bool up = i < e1;
+          const int slot = up ? nu : kFinderSlots + nd;
+          if ((up ? nu : nd) < kFinderSlots) { s_val[slot][threadIdx.x] = cq[k]; s_idx[slot][threadIdx.x] = qq[k]; }
+          nu += up ? 1 : 0;
+          nd += up ? 0 : 1;
         }
       }
     }
     float best = 0.0f;
-    if (nu <= 4 && nd <= 4) {
-      for (int a = 0; a < nu; ++a) {
-        const uint32_t qu = a == 0 ? us0 : a == 1 ? us1 : a == 2 ? us2 : us3;
-        const float2 cu = yt[qu];
-        for (int b = 0; b < nd; ++b) {
-          const uint32_t qd = b == 0 ? ds0 : b == 1 ? ds1 : b == 2 ? ds2 : ds3;
-          finder_try_pair(me, cu, yt[qd], qu, qd, orig, c, best, bu, bd);
-        }
+    if (nu <= kFinderSlots && nd <= kFinderSlots) {
+      const int n_pairs = nu * nd;
+      int a = 0, b = 0;
+      for (int p = 0; p < n_pairs; ++p) {            // pair (a, b), a-major like the definition's loops
+        finder_try_pair(me, s_val[a][threadIdx.x], s_val[kFinderSlots + b][threadIdx.x], s_idx[a][threadIdx.x],
+                        s_idx[kFinderSlots + b][threadIdx.x], orig, c, best, bu, bd);
+        if (++b == nd) { b = 0; ++a; }
       }
     } else {   // crowded area: generic nested loops over the spans (ties are decided on the original index)
+      auto index_of = [&](uint32_t i) -> uint32_t { return (i < e1 ? (i < e0 ? b0 : b1) : (i < e2 ? b2 : b3)) + i; };
       for (uint32_t iu = 0; iu < e1; ++iu) {
         const uint32_t qu = index_of(iu);
         const float2 cu = yt[qu];

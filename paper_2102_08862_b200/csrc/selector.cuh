@@ -13,13 +13,13 @@ namespace tpc {
 
 constexpr int kSelectorThreads = 256;   // 8 tracklets per CTA
 
-__device__ __forceinline__ unsigned long long tracklet_key(int n_hits, uint32_t seed_orig) {
-  return ((unsigned long long)(uint32_t)n_hits << 32) | (unsigned long long)(0xFFFFFFFFu - seed_orig);
-}
-
+// One warp per tracklet; the five row words are loaded back to back, then the atomics are fired (no return value).
+// (Claiming from inside the constructor when a tracklet retires was measured: it stalls the whole warp on the row
+// reads and costs 10 ms against 6 ms for this kernel.)
 __global__ void __launch_bounds__(kSelectorThreads) k_selector_claim(TrackletStore tl, const int32_t* __restrict__ counters,
                                                                      unsigned long long* __restrict__ claim,
                                                                      const __grid_constant__ Consts c) {
+  constexpr int kWords = kRowStride / 32;
   const int j = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (j >= counters[0]) return;
   const int nh = tl.n_hits[j];
@@ -27,19 +27,29 @@ __global__ void __launch_bounds__(kSelectorThreads) k_selector_claim(TrackletSto
   const unsigned long long key = tracklet_key(nh, tl.seed_orig[j]);
   const int first = tl.first_row[j], last = tl.last_row[j];
   const int* rows = tl.row_hit + (size_t)j * kRowStride;
-  for (int r = (first & ~31) + (int)lane_id(); r <= last; r += 32) {
-    if (r < first) continue;
-    const int m = rows[r];
-    if (m >= 0) atomicMax(claim + m, key);
+  int m[kWords];
+#pragma unroll
+  for (int i = 0; i < kWords; ++i) {
+    const int r = i * 32 + (int)lane_id();
+    m[i] = (r >= first && r <= last) ? rows[r] : -1;
   }
+#pragma unroll
+  for (int i = 0; i < kWords; ++i)
+    if (m[i] >= 0) atomicMax(claim + m[i], key);
 }
 
-// owned[j] = number of hits tracklet j still owns if that reaches min_hits, else 0; flag[j] = owned[j] > 0.
+
+// owned[j] = number of hits tracklet j still owns if that reaches min_hits, else 0; flag[j] = owned[j] > 0;
+// own_mask[j][i] = ballot of the owned rows 32 i .. 32 i + 31 (so that emit needs no second claim gather).
 // Entries j >= n_tracklets are written as 0 so the scans can run over the whole capacity.
+// One warp per tracklet; the five row words and then the five claim gathers are issued back to back (memory-level
+// parallelism: the kernel is bound by the latency of the random 8-byte claim reads).
 __global__ void __launch_bounds__(kSelectorThreads) k_selector_count(TrackletStore tl, const int32_t* __restrict__ counters,
                                                                      const unsigned long long* __restrict__ claim,
                                                                      uint32_t* __restrict__ owned, uint32_t* __restrict__ flag,
-                                                                     int max_tracklets, const __grid_constant__ Consts c) {
+                                                                     uint32_t* __restrict__ own_mask, int max_tracklets,
+                                                                     const __grid_constant__ Consts c) {
+  constexpr int kWords = kRowStride / 32;
   const int j = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (j >= max_tracklets) return;
   int n_owned = 0;
@@ -49,14 +59,23 @@ __global__ void __launch_bounds__(kSelectorThreads) k_selector_count(TrackletSto
       const unsigned long long key = tracklet_key(nh, tl.seed_orig[j]);
       const int first = tl.first_row[j], last = tl.last_row[j];
       const int* rows = tl.row_hit + (size_t)j * kRowStride;
-      for (int r = (first & ~31) + (int)lane_id(); r - (int)lane_id() <= last; r += 32) {
-        bool mine = false;
-        if (r >= first && r <= last) {
-          const int m = rows[r];
-          mine = m >= 0 && claim[m] == key;
-        }
-        n_owned += __popc(__ballot_sync(0xffffffffu, mine));
+      int m[kWords];
+#pragma unroll
+      for (int i = 0; i < kWords; ++i) {
+        const int r = i * 32 + (int)lane_id();
+        m[i] = (r >= first && r <= last) ? rows[r] : -1;
       }
+      unsigned long long cl[kWords];
+#pragma unroll
+      for (int i = 0; i < kWords; ++i) cl[i] = m[i] >= 0 ? claim[m[i]] : 0ull;
+      uint32_t my_word = 0;
+#pragma unroll
+      for (int i = 0; i < kWords; ++i) {
+        const unsigned b = __ballot_sync(0xffffffffu, m[i] >= 0 && cl[i] == key);
+        n_owned += __popc(b);
+        if ((int)lane_id() == i) my_word = b;
+      }
+      if (n_owned >= c.min_hits && lane_id() < kWords) own_mask[(size_t)j * kWords + lane_id()] = my_word;
     }
   }
   if (lane_id() == 0) {
@@ -76,11 +95,12 @@ struct TrackOutputs {   // device pointers of tpc_tracks_t (include/tpc_tracker.
 
 // track_idx / hit_off are the exclusive scans of flag / owned; their totals sit behind the last tile offset.
 __global__ void __launch_bounds__(kSelectorThreads) k_selector_emit(
-    TrackletStore tl, const int32_t* __restrict__ counters, const unsigned long long* __restrict__ claim,
+    TrackletStore tl, const int32_t* __restrict__ counters, const uint32_t* __restrict__ own_mask,
     const uint32_t* __restrict__ flag_in, const uint32_t* __restrict__ track_idx, const uint32_t* __restrict__ hit_off,
     const uint32_t* __restrict__ track_total, const uint32_t* __restrict__ hit_total,
     const uint32_t* __restrict__ orig, const uint16_t* __restrict__ hsr, const uint32_t* __restrict__ start_hits,
     const uint32_t* __restrict__ n_invalid, TrackOutputs o, const __grid_constant__ Consts c) {
+  constexpr int kWords = kRowStride / 32;
   const int j = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (j == 0 && lane_id() == 0) {
     const uint32_t nt = *track_total, nh = *hit_total;
@@ -94,32 +114,24 @@ __global__ void __launch_bounds__(kSelectorThreads) k_selector_emit(
     *o.status = st;
   }
   if (j >= counters[0]) return;
-  // flag is re-derived from the scanned arrays' neighbours being unavailable for the last element -> use flag_in
   if (flag_in[j] == 0) return;
   const uint32_t ti = track_idx[j];
   const uint32_t off = hit_off[j];
   if ((int64_t)ti >= (int64_t)o.max_tracks) return;
-  const int nh = tl.n_hits[j];
-  const unsigned long long key = tracklet_key(nh, tl.seed_orig[j]);
-  const int first = tl.first_row[j], last = tl.last_row[j];
   const int* rows = tl.row_hit + (size_t)j * kRowStride;
+  const uint32_t my_word = lane_id() < kWords ? own_mask[(size_t)j * kWords + lane_id()] : 0u;
   int n_owned = 0, own_first = -1, own_last = -1;
-  for (int r = (first & ~31) + (int)lane_id(); r - (int)lane_id() <= last; r += 32) {
-    int m = -1;
-    bool mine = false;
-    if (r >= first && r <= last) {
-      m = rows[r];
-      mine = m >= 0 && claim[m] == key;
-    }
-    const unsigned b = __ballot_sync(0xffffffffu, mine);
-    if (mine) {
+#pragma unroll
+  for (int i = 0; i < kWords; ++i) {
+    const unsigned b = __shfl_sync(0xffffffffu, my_word, i);
+    if (b >> lane_id() & 1u) {
+      const int m = rows[i * 32 + (int)lane_id()];
       const int64_t pos = (int64_t)off + n_owned + __popc(b & ((1u << lane_id()) - 1u));
       if (pos < o.max_track_hits) o.hit_index[pos] = (int32_t)orig[m];
     }
     if (b) {
-      const int base = r - (int)lane_id();
-      if (own_first < 0) own_first = base + __ffs(b) - 1;
-      own_last = base + 31 - __clz(b);
+      if (own_first < 0) own_first = i * 32 + __ffs(b) - 1;
+      own_last = i * 32 + 31 - __clz(b);
     }
     n_owned += __popc(b);
   }

@@ -31,7 +31,7 @@ const char* const kStepNames[N_STEPS] = {
 struct Ids {   // arena allocation ids
   int stage_in = -1, stage_out = -1;
   int bin_start, sort_keys, tmp_keys, tmp_orig, tmp_yt, sort_hist, yt, orig, hsr, link_up, link_down, link_up_clean, start_flag, cell_count, start_hits,
-      counters, scan_a, scan_b, seeds_a, seeds_b, row_hit, tl_n_hits, tl_first, tl_last, tl_seed, tl_par, tl_cov, claim, owned,
+      counters, scan_a, scan_b, seeds_a, seeds_b, row_hit, tl_n_hits, tl_first, tl_last, tl_seed, tl_par, tl_cov, claim, owned, own_mask,
       flag, track_idx, hit_off;
 };
 
@@ -136,7 +136,8 @@ void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids
   id.tl_seed = plan.add("tracklet_seed_orig", 4 * T, S_CONSTRUCT, S_EMIT);
   id.tl_par = plan.add("tracklet_par", 7 * 4 * T, S_CONSTRUCT, S_EMIT);
   id.tl_cov = plan.add("tracklet_cov", 9 * 4 * T, S_CONSTRUCT, S_EMIT);
-  id.claim = plan.add("selector_claim(u64)", 8 * N, S_CLAIM, S_EMIT);
+  id.claim = plan.add("selector_claim(u64)", 8 * N, S_CLAIM, S_COUNT);
+  id.own_mask = plan.add("selector_own_mask", 4 * (size_t)(kRowStride / 32) * T, S_COUNT, S_EMIT);
   id.owned = plan.add("selector_owned", 4 * T, S_COUNT, S_EMIT);
   id.flag = plan.add("selector_flag", 4 * T, S_COUNT, S_EMIT);
   id.track_idx = plan.add("selector_track_idx", 4 * T, S_SELECT_SCAN, S_EMIT);
@@ -355,6 +356,7 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   uint32_t* scan_b = P.ptr<uint32_t>(A, id.scan_b);
   unsigned long long* claim = P.ptr<unsigned long long>(A, id.claim);
   uint32_t* owned = P.ptr<uint32_t>(A, id.owned);
+  uint32_t* own_mask = P.ptr<uint32_t>(A, id.own_mask);
   uint32_t* flag = P.ptr<uint32_t>(A, id.flag);
   uint32_t* track_idx = P.ptr<uint32_t>(A, id.track_idx);
   uint32_t* hit_off = P.ptr<uint32_t>(A, id.hit_off);
@@ -404,7 +406,7 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
 
   // ---- C2 neighbours finder ----
   mark(S_FINDER);
-  k_neighbours_finder<<<hit_ctas, 256, 0, st>>>(yt, orig, hsr, bin_start, link_up, link_down, c); ++launches;
+  k_neighbours_finder<<<hit_ctas, kFinderThreads, 0, st>>>(yt, orig, hsr, bin_start, link_up, link_down, c); ++launches;
 
   // ---- C3 cleaner + C4 start hits ----
   mark(S_CLEAN_START);
@@ -440,7 +442,7 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   k_selector_claim<<<warp_ctas, kSelectorThreads, 0, st>>>(tl, counters, claim, c); ++launches;
   mark(S_COUNT);
   const int cap_warp_ctas = (int)(((int64_t)T * 32 + kSelectorThreads - 1) / kSelectorThreads);
-  k_selector_count<<<cap_warp_ctas, kSelectorThreads, 0, st>>>(tl, counters, claim, owned, flag, T, c); ++launches;
+  k_selector_count<<<cap_warp_ctas, kSelectorThreads, 0, st>>>(tl, counters, claim, owned, flag, own_mask, T, c); ++launches;
   mark(S_SELECT_SCAN);
   launches += exclusive_scan_u32(flag, track_idx, (size_t)T, scan_a, st);
   launches += exclusive_scan_u32(owned, hit_off, (size_t)T, scan_b, st);
@@ -452,7 +454,7 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   to.hit_offset = o->hit_offset; to.x = o->x; to.y = o->y; to.z_rel = o->z_rel; to.time_ref = o->time_ref;
   to.sin_phi = o->sin_phi; to.dzds = o->dzds; to.q_pt = o->q_pt; to.cov9 = o->cov9; to.hit_index = o->hit_index;
   const int n_scan_tiles = (int)scan_tiles((size_t)T);
-  k_selector_emit<<<std::max(warp_ctas, 1), kSelectorThreads, 0, st>>>(tl, counters, claim, flag, track_idx, hit_off, scan_a + n_scan_tiles,
+  k_selector_emit<<<std::max(warp_ctas, 1), kSelectorThreads, 0, st>>>(tl, counters, own_mask, flag, track_idx, hit_off, scan_a + n_scan_tiles,
                                                                        scan_b + n_scan_tiles, orig, hsr, start_hits, n_invalid, to, c); ++launches;
   mark(N_STEPS);
   t->have_times = t->profile;
