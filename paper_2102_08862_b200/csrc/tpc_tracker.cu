@@ -5,6 +5,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -261,6 +262,7 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_tracklet_constructor, kTrackletThreads, 0) != cudaSuccess || per_sm < 1) {
       cudaGetLastError(); per_sm = 1;
     }
+    if (const char* e = getenv("TPC_CTOR_CTAS_PER_SM")) per_sm = std::max(1, std::min(per_sm, atoi(e)));   // experiments only
     t->constructor_ctas = sms * per_sm;
   }
   for (int i = 0; i <= N_STEPS; ++i)
