@@ -34,6 +34,11 @@ ALGO_BYTES_PER_CLUSTER = {
     "ingest_radix_sort": 4 * (4 + 16 + 16), "grid_build": 4 + 4 + 2,
     "neighbours_finder": 10 + 8 + 8, "cleaner_start_hits": 8 + 4 + 1, "start_hit_compaction": 1,
 }
+# Tracklet constructor: bound by plain fp32 ALU issue.  Algorithmic lane-instructions of one row step
+# (= one transport [+ search] [+ update]) counted from the statement lists of DESIGN.md §3 with IEEE division and
+# square root ~ 8 instructions each: transport 123, update 52 x 0.85 of steps, search 12 per candidate.
+ALGO_LANE_INST_TRANSPORT, ALGO_LANE_INST_UPDATE, ALGO_LANE_INST_PER_CANDIDATE = 123, 52, 12
+SM_COUNT, SMSP_PER_SM, LANES = 148, 4, 32      # B300_MICROARCH.md: 4 schedulers per SM, <= 1 warp instruction per cycle each
 
 
 def _peaks():
@@ -223,6 +228,7 @@ def main():
         stream.synchronize()
         for k, v in trk.step_ms().items():
             step_acc[k] = step_acc.get(k, 0.0) + v / n_prof
+    work = trk.work_counters(stream)
     n_tracks = int(outs[0].n_tracks[0])
     n_track_hits = int(outs[0].n_track_hits[0])
     status = int(outs[0].status[0])
@@ -283,6 +289,16 @@ def main():
         a = ALGO_BYTES_PER_CLUSTER[dom] * n / (step_acc[dom] * 1e-3) / 1e9
         roof.update({"bound": "hbm", "achieved": a, "peak": peak, "unit": "GB/s", "frac": a / peak, "traffic": None,
                      "peak_source": peak_src})
+    elif dom == "tracklet_constructor":
+        clk = clocks.summary()
+        mhz = clk["sm_mhz"] or clk["sm_max_mhz"] or 1965.0
+        alu_peak = SM_COUNT * SMSP_PER_SM * LANES * mhz * 1e6 / 1e12          # T lane-instructions / s at the clock under load
+        inst = (ALGO_LANE_INST_TRANSPORT * work["row_steps"] + ALGO_LANE_INST_UPDATE * work["updates"] +
+                ALGO_LANE_INST_PER_CANDIDATE * work["candidates"])
+        a = inst / (step_acc[dom] * 1e-3) / 1e12
+        roof.update({"bound": "alu", "achieved": a, "peak": alu_peak, "unit": "T lane-inst/s", "frac": a / alu_peak,
+                     "traffic": None, "peak_source": f"148 SMs x 4 schedulers x 32 lanes x {mhz:.0f} MHz (SM clock under load)",
+                     "units": {k: work[k] for k in ("tracklets", "row_steps", "updates", "candidates")}})
     else:
         roof.update({"bound": "hbm", "achieved": None, "peak": peak, "unit": "GB/s", "frac": None, "traffic": None,
                      "peak_source": peak_src})
