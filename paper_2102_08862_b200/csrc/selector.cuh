@@ -22,10 +22,11 @@ __global__ void __launch_bounds__(kSelectorThreads) k_selector_claim(TrackletSto
   constexpr int kWords = kRowStride / 32;
   const int j = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (j >= counters[0]) return;
-  const int nh = tl.n_hits[j];
+  const int4 meta = tl.meta[j];                      // n_hits, first_row, last_row, seed_orig
+  const int nh = meta.x;
   if (nh < c.min_hits) return;
-  const unsigned long long key = tracklet_key(nh, tl.seed_orig[j]);
-  const int first = tl.first_row[j], last = tl.last_row[j];
+  const unsigned long long key = tracklet_key(nh, (uint32_t)meta.w);
+  const int first = meta.y, last = meta.z;
   const int* rows = tl.row_hit + (size_t)j * kRowStride;
   int m[kWords];
 #pragma unroll
@@ -54,10 +55,11 @@ __global__ void __launch_bounds__(kSelectorThreads) k_selector_count(TrackletSto
   if (j >= max_tracklets) return;
   int n_owned = 0;
   if (j < counters[0]) {
-    const int nh = tl.n_hits[j];
+    const int4 meta = tl.meta[j];
+    const int nh = meta.x;
     if (nh >= c.min_hits) {
-      const unsigned long long key = tracklet_key(nh, tl.seed_orig[j]);
-      const int first = tl.first_row[j], last = tl.last_row[j];
+      const unsigned long long key = tracklet_key(nh, (uint32_t)meta.w);
+      const int first = meta.y, last = meta.z;
       const int* rows = tl.row_hit + (size_t)j * kRowStride;
       int m[kWords];
 #pragma unroll
@@ -136,17 +138,20 @@ __global__ void __launch_bounds__(kSelectorThreads) k_selector_emit(
     n_owned += __popc(b);
   }
   if (lane_id() == 0) {
-    const size_t cap = tl.cap;
-    o.seed_hit[ti] = (int32_t)tl.seed_orig[j];
+    const float4* rec = tl.rec + 4 * (size_t)j;
+    const float4 q0 = rec[0], q1 = rec[1], q2 = rec[2], q3 = rec[3];
+    o.seed_hit[ti] = tl.meta[j].w;
     o.sector[ti] = (int32_t)(hsr[start_hits[j]] / c.n_rows);
     o.first_row[ti] = own_first;
     o.last_row[ti] = own_last;
     o.n_hits[ti] = n_owned;
     o.hit_offset[ti] = (int64_t)off;
-    o.x[ti] = tl.par[0 * cap + j]; o.y[ti] = tl.par[1 * cap + j]; o.z_rel[ti] = tl.par[2 * cap + j];
-    o.sin_phi[ti] = tl.par[3 * cap + j]; o.dzds[ti] = tl.par[4 * cap + j]; o.q_pt[ti] = tl.par[5 * cap + j];
-    o.time_ref[ti] = tl.par[6 * cap + j];
-    if (o.cov9) for (int i = 0; i < 9; ++i) o.cov9[(size_t)ti * 9 + i] = tl.cov[i * cap + j];
+    o.x[ti] = q0.x; o.y[ti] = q0.y; o.z_rel[ti] = q0.z; o.sin_phi[ti] = q0.w; o.dzds[ti] = q1.x; o.q_pt[ti] = q1.y;
+    o.time_ref[ti] = q3.w;
+    if (o.cov9) {
+      float* cv = o.cov9 + (size_t)ti * 9;
+      cv[0] = q1.z; cv[1] = q1.w; cv[2] = q2.x; cv[3] = q2.y; cv[4] = q2.z; cv[5] = q2.w; cv[6] = q3.x; cv[7] = q3.y; cv[8] = q3.z;
+    }
   }
 }
 
@@ -158,7 +163,8 @@ __global__ void __launch_bounds__(kSelectorThreads) k_export_tracklets(
   const int j = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (j == 0 && lane_id() == 0 && tap_n) *tap_n = counters[0];
   if (j >= counters[0] || j >= tap_capacity) return;
-  const int first = tl.first_row[j], last = tl.last_row[j];
+  const int4 meta = tl.meta[j];
+  const int first = meta.y, last = meta.z;
   const int* rows = tl.row_hit + (size_t)j * kRowStride;
   if (tap_row_hit)
     for (int r = lane_id(); r < c.n_rows; r += 32) {
@@ -167,10 +173,13 @@ __global__ void __launch_bounds__(kSelectorThreads) k_export_tracklets(
       tap_row_hit[(size_t)j * c.n_rows + r] = v;
     }
   if (lane_id() == 0) {
-    if (tap_seed) tap_seed[j] = (int32_t)tl.seed_orig[j];
-    if (tap_n_hits) tap_n_hits[j] = tl.n_hits[j];
+    if (tap_seed) tap_seed[j] = meta.w;
+    if (tap_n_hits) tap_n_hits[j] = meta.x;
   }
-  if (tap_par && lane_id() < 7) tap_par[(size_t)j * 7 + lane_id()] = tl.par[lane_id() * tl.cap + j];
+  if (tap_par && lane_id() < 7) {                     // x, y, z_rel, sin_phi, dzds, q_pt, time_ref
+    const float* rec = reinterpret_cast<const float*>(tl.rec + 4 * (size_t)j);
+    tap_par[(size_t)j * 7 + lane_id()] = rec[lane_id() < 6 ? lane_id() : 15];
+  }
 }
 
 }  // namespace tpc

@@ -32,7 +32,7 @@ const char* const kStepNames[N_STEPS] = {
 struct Ids {   // arena allocation ids
   int stage_in = -1, stage_out = -1;
   int bin_start, sort_keys, tmp_keys, tmp_orig, tmp_yt, sort_hist, yt, orig, hsr, link_up, link_down, link_up_clean, start_flag, cell_count, start_hits,
-      counters, scan_a, scan_b, seeds_a, seeds_b, row_hit, tl_n_hits, tl_first, tl_last, tl_seed, tl_par, tl_cov, claim, owned, own_mask,
+      counters, scan_a, scan_b, seeds_a, seeds_b, row_hit, tl_meta, tl_rec, tl_cur, claim, owned, own_mask,
       flag, track_idx, hit_off;
 };
 
@@ -131,12 +131,9 @@ void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids
   id.seeds_a = plan.add("tracklet_seeds_a(int4)", 16 * T, S_CONSTRUCT, S_CONSTRUCT);
   id.seeds_b = plan.add("tracklet_seeds_b(float4)", 16 * T, S_CONSTRUCT, S_CONSTRUCT);
   id.row_hit = plan.add("tracklet_row_hit", 4 * (size_t)kRowStride * T, S_CONSTRUCT, S_EMIT);
-  id.tl_n_hits = plan.add("tracklet_n_hits", 4 * T, S_CONSTRUCT, S_EMIT);
-  id.tl_first = plan.add("tracklet_first_row", 4 * T, S_CONSTRUCT, S_EMIT);
-  id.tl_last = plan.add("tracklet_last_row", 4 * T, S_CONSTRUCT, S_EMIT);
-  id.tl_seed = plan.add("tracklet_seed_orig", 4 * T, S_CONSTRUCT, S_EMIT);
-  id.tl_par = plan.add("tracklet_par", 7 * 4 * T, S_CONSTRUCT, S_EMIT);
-  id.tl_cov = plan.add("tracklet_cov", 9 * 4 * T, S_CONSTRUCT, S_EMIT);
+  id.tl_meta = plan.add("tracklet_meta(int4)", 16 * T, S_CONSTRUCT, S_EMIT);
+  id.tl_rec = plan.add("tracklet_record(4 x float4)", 64 * T, S_CONSTRUCT, S_EMIT);
+  id.tl_cur = plan.add("tracklet_handover(2 x float4)", 32 * T, S_CONSTRUCT, S_CONSTRUCT);
   id.claim = plan.add("selector_claim(u64)", 8 * N, S_CLAIM, S_COUNT);
   id.own_mask = plan.add("selector_own_mask", 4 * (size_t)(kRowStride / 32) * T, S_COUNT, S_EMIT);
   id.owned = plan.add("selector_owned", 4 * T, S_COUNT, S_EMIT);
@@ -159,7 +156,7 @@ struct tpc_tracker {
   cudaEvent_t ev[N_STEPS + 1] = {};
   bool profile = false, have_times = false;
   int64_t last_launches = 0;
-  int constructor_ctas = 148;      // persistent grid: SMs x resident CTAs per SM
+  int ctas_fit_up = 148, ctas_follow_up = 148, ctas_fit_down = 148, ctas_follow_down = 148;   // persistent grids: SMs x resident CTAs per SM
 };
 
 extern "C" {
@@ -256,14 +253,20 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
     cudaGetLastError(); tpc_tracker_destroy(t); return TPC_ECUDA;
   }
   {
-    int dev = 0, sms = 148, per_sm = 1;
+    int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_tracklet_constructor, kTrackletThreads, 0) != cudaSuccess || per_sm < 1) {
-      cudaGetLastError(); per_sm = 1;
-    }
-    if (const char* e = getenv("TPC_CTOR_CTAS_PER_SM")) per_sm = std::max(1, std::min(per_sm, atoi(e)));   // experiments only
-    t->constructor_ctas = sms * per_sm;
+    auto resident = [&](auto kernel) {
+      int per_sm = 1;
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kTrackletThreads, 0) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError(); per_sm = 1;
+      }
+      return sms * per_sm;
+    };
+    t->ctas_fit_up = resident(k_tracklet_fit<false>);
+    t->ctas_follow_up = resident(k_tracklet_follow<false>);
+    t->ctas_fit_down = resident(k_tracklet_fit<true>);
+    t->ctas_follow_down = resident(k_tracklet_follow<true>);
   }
   for (int i = 0; i <= N_STEPS; ++i)
     if (cudaEventCreate(&t->ev[i]) != cudaSuccess) { cudaGetLastError(); tpc_tracker_destroy(t); return TPC_ECUDA; }
@@ -364,12 +367,9 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   uint32_t* hit_off = P.ptr<uint32_t>(A, id.hit_off);
   TrackletStore tl;
   tl.row_hit = P.ptr<int>(A, id.row_hit);
-  tl.n_hits = P.ptr<int>(A, id.tl_n_hits);
-  tl.first_row = P.ptr<int>(A, id.tl_first);
-  tl.last_row = P.ptr<int>(A, id.tl_last);
-  tl.seed_orig = P.ptr<uint32_t>(A, id.tl_seed);
-  tl.par = P.ptr<float>(A, id.tl_par);
-  tl.cov = P.ptr<float>(A, id.tl_cov);
+  tl.meta = P.ptr<int4>(A, id.tl_meta);
+  tl.rec = P.ptr<float4>(A, id.tl_rec);
+  tl.cur = P.ptr<float4>(A, id.tl_cur);
   tl.cap = (size_t)T;
 
   const int hit_ctas = (int)std::max<int64_t>((n + 255) / 256, 1);
@@ -430,8 +430,14 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   mark(S_CONSTRUCT);
   const int64_t tl_bound = std::min<int64_t>(T, n / std::max(2, c.seed_min_hits) + 1);   // start hits own disjoint chains
   k_tracklet_init<<<(int)((tl_bound + 255) / 256), 256, 0, st>>>(yt, hsr, link_up_clean, start_hits, counters, seeds, tl.row_hit, c); ++launches;
-  k_tracklet_constructor<<<(int)std::min<int64_t>(t->constructor_ctas, (tl_bound + kTrackletThreads - 1) / kTrackletThreads),
-                           kTrackletThreads, 0, st>>>(yt, orig, bin_start, seeds, counters, tl, c); ++launches;
+  {
+    const int need = (int)((tl_bound + kTrackletThreads - 1) / kTrackletThreads);
+    k_tracklet_fit<false><<<std::min(t->ctas_fit_up, need), kTrackletThreads, 0, st>>>(yt, orig, seeds, counters, tl, c);
+    k_tracklet_follow<false><<<std::min(t->ctas_follow_up, need), kTrackletThreads, 0, st>>>(yt, orig, bin_start, seeds, counters, tl, c);
+    k_tracklet_fit<true><<<std::min(t->ctas_fit_down, need), kTrackletThreads, 0, st>>>(yt, orig, seeds, counters, tl, c);
+    k_tracklet_follow<true><<<std::min(t->ctas_follow_down, need), kTrackletThreads, 0, st>>>(yt, orig, bin_start, seeds, counters, tl, c);
+    launches += 4;
+  }
   const int warp_ctas = (int)((tl_bound * 32 + kSelectorThreads - 1) / kSelectorThreads);
   if (tl_taps) {
     k_export_tracklets<<<warp_ctas, kSelectorThreads, 0, st>>>(tl, counters, orig, o->n_tracklets, o->tracklet_seed, o->tracklet_n_hits,
