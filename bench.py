@@ -38,6 +38,8 @@ ALGO_BYTES_PER_CLUSTER = {
 # (= one transport [+ search] [+ update]) counted from the statement lists of DESIGN.md §3 with IEEE division and
 # square root ~ 8 instructions each: transport 123, update 52 x 0.85 of steps, search 12 per candidate.
 ALGO_LANE_INST_TRANSPORT, ALGO_LANE_INST_UPDATE, ALGO_LANE_INST_PER_CANDIDATE = 123, 52, 12
+TRACKLET_PHASES = {"tracklet_fit_up": "fit_up", "tracklet_follow_up": "follow_up", "tracklet_fit_down": "fit_down",
+                   "tracklet_follow_down": "follow_down"}     # step name -> work-counter group
 SM_COUNT, SMSP_PER_SM, LANES = 148, 4, 32      # B300_MICROARCH.md: 4 schedulers per SM, <= 1 warp instruction per cycle each
 
 
@@ -276,32 +278,41 @@ def main():
             dist.destroy_process_group()
         return 0
 
-    # ---- roofline of the dominant kernel ----
+    # ---- per-kernel rooflines; `roofline` = the dominant kernel's ----
     peak, peak_src = _peaks()
+    clk = clocks.summary()
+    mhz = clk["sm_mhz"] or clk["sm_max_mhz"] or 1965.0
+    alu_peak = SM_COUNT * SMSP_PER_SM * LANES * mhz * 1e6 / 1e12          # T lane-instructions / s at the clock under load
+    alu_src = f"148 SMs x 4 schedulers x 32 lanes x {mhz:.0f} MHz (SM clock under load)"
+    total_step_ms = sum(step_acc.values())
+    kernels = {}
+    for k, ms in step_acc.items():
+        row = {"ms": round(ms, 4), "share_of_step": round(ms / total_step_ms, 4)}
+        if ALGO_BYTES_PER_CLUSTER.get(k) and ms > 0:
+            a = ALGO_BYTES_PER_CLUSTER[k] * n / (ms * 1e-3) / 1e9
+            row.update({"bound": "hbm", "achieved": round(a, 1), "peak": peak, "unit": "GB/s", "frac": round(a / peak, 4)})
+        elif k in TRACKLET_PHASES and ms > 0:
+            w = work[TRACKLET_PHASES[k]]
+            inst = (ALGO_LANE_INST_TRANSPORT * w["row_steps"] + ALGO_LANE_INST_UPDATE * w["updates"] +
+                    (ALGO_LANE_INST_PER_CANDIDATE * w["candidates"] if "follow" in k else 0))
+            a = inst / (ms * 1e-3) / 1e12
+            row.update({"bound": "alu", "achieved": round(a, 3), "peak": round(alu_peak, 3), "unit": "T lane-inst/s",
+                        "frac": round(a / alu_peak, 4), "units": w})
+        kernels[k] = row
     dom = max(step_acc, key=step_acc.get)
-    hbm_rows = {}
-    for k, bpc in ALGO_BYTES_PER_CLUSTER.items():
-        if bpc and step_acc.get(k, 0) > 0:
-            hbm_rows[k] = {"ms": round(step_acc[k], 4), "algo_gbs": round(bpc * n / (step_acc[k] * 1e-3) / 1e9, 1)}
-    # tracklet-level steps: algorithmic bytes depend on the tracklet count
-    roof = {"kernel": dom, "ms": step_acc[dom], "share_of_step": step_acc[dom] / sum(step_acc.values())}
-    if dom in ALGO_BYTES_PER_CLUSTER and ALGO_BYTES_PER_CLUSTER[dom]:
-        a = ALGO_BYTES_PER_CLUSTER[dom] * n / (step_acc[dom] * 1e-3) / 1e9
-        roof.update({"bound": "hbm", "achieved": a, "peak": peak, "unit": "GB/s", "frac": a / peak, "traffic": None,
-                     "peak_source": peak_src})
-    elif dom == "tracklet_constructor":
-        clk = clocks.summary()
-        mhz = clk["sm_mhz"] or clk["sm_max_mhz"] or 1965.0
-        alu_peak = SM_COUNT * SMSP_PER_SM * LANES * mhz * 1e6 / 1e12          # T lane-instructions / s at the clock under load
-        inst = (ALGO_LANE_INST_TRANSPORT * work["row_steps"] + ALGO_LANE_INST_UPDATE * work["updates"] +
-                ALGO_LANE_INST_PER_CANDIDATE * work["candidates"])
-        a = inst / (step_acc[dom] * 1e-3) / 1e12
-        roof.update({"bound": "alu", "achieved": a, "peak": alu_peak, "unit": "T lane-inst/s", "frac": a / alu_peak,
-                     "traffic": None, "peak_source": f"148 SMs x 4 schedulers x 32 lanes x {mhz:.0f} MHz (SM clock under load)",
-                     "units": {k: work[k] for k in ("tracklets", "row_steps", "updates", "candidates")}})
-    else:
-        roof.update({"bound": "hbm", "achieved": None, "peak": peak, "unit": "GB/s", "frac": None, "traffic": None,
-                     "peak_source": peak_src})
+    roof = {"kernel": dom, "ms": step_acc[dom], "share_of_step": step_acc[dom] / total_step_ms, "traffic": None}
+    roof.update({k: v for k, v in kernels[dom].items() if k not in ("ms", "share_of_step")})
+    roof["peak_source"] = alu_src if roof.get("bound") == "alu" else peak_src
+    if "bound" not in roof:
+        roof.update({"bound": "hbm", "achieved": None, "peak": peak, "unit": "GB/s", "frac": None})
+    # the whole constructor (seed + four phase kernels) against the same ALU peak
+    c_ms = sum(step_acc.get(k, 0.0) for k in ("tracklet_init", *TRACKLET_PHASES))
+    c_inst = (ALGO_LANE_INST_TRANSPORT * work["row_steps"] + ALGO_LANE_INST_UPDATE * work["updates"] +
+              ALGO_LANE_INST_PER_CANDIDATE * (work["follow_up"]["candidates"] + work["follow_down"]["candidates"]))
+    constructor = {"ms": round(c_ms, 4), "share_of_step": round(c_ms / total_step_ms, 4), "bound": "alu",
+                   "achieved": round(c_inst / (c_ms * 1e-3) / 1e12, 3) if c_ms > 0 else None, "peak": round(alu_peak, 3),
+                   "unit": "T lane-inst/s", "frac": round(c_inst / (c_ms * 1e-3) / 1e12 / alu_peak, 4) if c_ms > 0 else None,
+                   "units": {k: work[k] for k in ("tracklets", "row_steps", "updates", "candidates")}}
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -320,8 +331,8 @@ def main():
                        "l2": "inputs and scratch are larger than L2 (no flush needed)" if n * 12 > 2.5e8 else
                              "working set may fit L2 (small config)", "gen_seconds": round(t_gen, 1)},
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches,
-            "step_ms": {k: round(v, 4) for k, v in step_acc.items()}, "hbm_steps": hbm_rows,
-            "roofline": roof, "cpu_baseline": cpu}
+            "step_ms": {k: round(v, 4) for k, v in step_acc.items()}, "kernels": kernels,
+            "tracklet_constructor": constructor, "roofline": roof, "cpu_baseline": cpu}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -154,14 +154,23 @@ int64_t tpc_tracker_last_launches(const tpc_tracker_t* tracker);
 
 /* Work counters of the last completed call, read back from the device (synchronises `cuda_stream`):
  * out[0] tracklets constructed, [1] start hits found, [2] invalid clusters, [3] row steps (transports) of the
- * tracklet constructor, [4] Kalman updates, [5] candidates scanned by its window searches.  These are the units of
- * the constructor's roofline.  Returns the number of counters (6) or a negative status.      */
+ * tracklet constructor, [4] Kalman updates, [5] candidates scanned by its window searches (each the sum over the
+ * four phase kernels), then [6 + 3 p + k] the same three counts (k = 0 row steps, 1 updates, 2 candidates) of phase
+ * p = 0 chain fit, 1 follow up, 2 refit down, 3 follow down.  These are the units of the constructor's roofline
+ * (DESIGN.md §6).  Returns the number of counters (18) or a negative status.                                 */
 int tpc_tracker_work_counters(tpc_tracker_t* tracker, void* cuda_stream, int64_t* out, int32_t capacity);
 
 /* Arena plan: for allocation i writes name, offset, bytes, first and last step of its lifetime.
  * Returns the number of allocations; i out of range returns -1.                                            */
 int tpc_tracker_arena_plan(const tpc_tracker_t* tracker, int32_t i, const char** name, size_t* offset,
                            size_t* bytes, int32_t* first_step, int32_t* last_step);
+
+/* Self test of the constructor's arithmetic (synchronises `cuda_stream`; allocates 16 bytes for its duration): the
+ * range-restricted square root and reciprocal sequences used by the Kalman transport / update are compared with the
+ * IEEE-754 correctly rounded sqrtf(x) and 1.0f / x over EVERY fp32 bit pattern of their ranges.  mismatches_out
+ * (HOST, 2 entries) receives the number of differing bit patterns for sqrt and for the reciprocal (both must be 0:
+ * the decision arithmetic has to round like the definition, BASELINE.json L5).                              */
+int tpc_selftest_fast_math(void* cuda_stream, uint64_t* mismatches_out);
 
 int tpc_tracker_destroy(tpc_tracker_t* tracker);
 

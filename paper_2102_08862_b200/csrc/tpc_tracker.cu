@@ -23,11 +23,13 @@ using namespace tpc;
 namespace {
 
 enum Step {
-  S_SORT = 0, S_GRID, S_FINDER, S_CLEAN_START, S_COMPACT, S_CONSTRUCT, S_CLAIM, S_COUNT, S_SELECT_SCAN, S_EMIT, N_STEPS
+  S_SORT = 0, S_GRID, S_FINDER, S_CLEAN_START, S_COMPACT,
+  S_TL_INIT, S_FIT_UP, S_FOLLOW_UP, S_FIT_DOWN, S_FOLLOW_DOWN,      // C5 tracklet constructor: seed + its four phase kernels
+  S_CLAIM, S_COUNT, S_SELECT_SCAN, S_EMIT, N_STEPS
 };
 const char* const kStepNames[N_STEPS] = {
     "ingest_radix_sort", "grid_build", "neighbours_finder", "cleaner_start_hits", "start_hit_compaction",
-    "tracklet_constructor", "selector_claim", "selector_count", "selector_scan", "selector_emit"};
+    "tracklet_init", "tracklet_fit_up", "tracklet_follow_up", "tracklet_fit_down", "tracklet_follow_down", "selector_claim", "selector_count", "selector_scan", "selector_emit"};
 
 struct Ids {   // arena allocation ids
   int stage_in = -1, stage_out = -1;
@@ -113,27 +115,27 @@ void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids
   id.counters = plan.add("counters", 256, S_SORT, S_EMIT);
   id.scan_a = plan.add("scan_tile_sums_a", 4 * scan_len, S_SORT, S_EMIT);
   id.scan_b = plan.add("scan_tile_sums_b", 4 * scan_len, S_SORT, S_EMIT);
-  id.bin_start = plan.add("grid_bin_start", 4 * B, S_GRID, S_CONSTRUCT);
+  id.bin_start = plan.add("grid_bin_start", 4 * B, S_GRID, S_FOLLOW_DOWN);
   id.sort_keys = plan.add("sort_keys", 4 * N, S_SORT, S_GRID);
   id.tmp_keys = plan.add("sort_tmp_keys", 4 * N, S_SORT, S_SORT);
   id.tmp_orig = plan.add("sort_tmp_orig", 4 * N, S_SORT, S_SORT);
   id.tmp_yt = plan.add("sort_tmp_y_time", 8 * N, S_SORT, S_SORT);
   id.sort_hist = plan.add("sort_tile_histograms", 4 * hist_len, S_SORT, S_SORT);
-  id.yt = plan.add("hits_y_time(float2)", 8 * N, S_SORT, S_CONSTRUCT);
+  id.yt = plan.add("hits_y_time(float2)", 8 * N, S_SORT, S_FOLLOW_DOWN);
   id.orig = plan.add("hits_orig_index", 4 * N, S_SORT, S_EMIT);
   id.hsr = plan.add("hits_sector_row(u16)", 2 * N, S_GRID, S_EMIT);
   id.link_up = plan.add("link_up_raw", 4 * N, S_FINDER, S_CLEAN_START);
   id.link_down = plan.add("link_down_raw", 4 * N, S_FINDER, S_CLEAN_START);
-  id.link_up_clean = plan.add("link_up_clean", 4 * N, S_CLEAN_START, S_CONSTRUCT);
+  id.link_up_clean = plan.add("link_up_clean", 4 * N, S_CLEAN_START, S_TL_INIT);
   id.start_flag = plan.add("start_flag(u8)", N, S_CLEAN_START, S_COMPACT);
   id.cell_count = plan.add("start_cell_count", 4 * ((size_t)c.n_cells + 2), S_COMPACT, S_COMPACT);
   id.start_hits = plan.add("start_hits", 4 * T, S_COMPACT, S_EMIT);
-  id.seeds_a = plan.add("tracklet_seeds_a(int4)", 16 * T, S_CONSTRUCT, S_CONSTRUCT);
-  id.seeds_b = plan.add("tracklet_seeds_b(float4)", 16 * T, S_CONSTRUCT, S_CONSTRUCT);
-  id.row_hit = plan.add("tracklet_row_hit", 4 * (size_t)kRowStride * T, S_CONSTRUCT, S_EMIT);
-  id.tl_meta = plan.add("tracklet_meta(int4)", 16 * T, S_CONSTRUCT, S_EMIT);
-  id.tl_rec = plan.add("tracklet_record(4 x float4)", 64 * T, S_CONSTRUCT, S_EMIT);
-  id.tl_cur = plan.add("tracklet_handover(2 x float4)", 32 * T, S_CONSTRUCT, S_CONSTRUCT);
+  id.seeds_a = plan.add("tracklet_seeds_a(int4)", 16 * T, S_TL_INIT, S_FOLLOW_DOWN);
+  id.seeds_b = plan.add("tracklet_seeds_b(float4)", 16 * T, S_TL_INIT, S_FOLLOW_DOWN);
+  id.row_hit = plan.add("tracklet_row_hit", 4 * (size_t)kRowStride * T, S_TL_INIT, S_EMIT);
+  id.tl_meta = plan.add("tracklet_meta(int4)", 16 * T, S_FIT_UP, S_EMIT);
+  id.tl_rec = plan.add("tracklet_record(4 x float4)", 64 * T, S_FIT_UP, S_EMIT);
+  id.tl_cur = plan.add("tracklet_handover(2 x float4)", 32 * T, S_FOLLOW_UP, S_FIT_DOWN);
   id.claim = plan.add("selector_claim(u64)", 8 * N, S_CLAIM, S_COUNT);
   id.own_mask = plan.add("selector_own_mask", 4 * (size_t)(kRowStride / 32) * T, S_COUNT, S_EMIT);
   id.owned = plan.add("selector_owned", 4 * T, S_COUNT, S_EMIT);
@@ -158,6 +160,25 @@ struct tpc_tracker {
   int64_t last_launches = 0;
   int ctas_fit_up = 148, ctas_follow_up = 148, ctas_fit_down = 148, ctas_follow_down = 148;   // persistent grids: SMs x resident CTAs per SM
 };
+
+// Exhaustive check of sqrt_rn_normal / rcp_rn_normal (tracklet.cuh) against sqrtf() / (1.0f / x) over every fp32 bit
+// pattern of their stated ranges; counts the mismatching patterns (expected: 0, 0).
+__global__ void __launch_bounds__(256) k_selftest_fast_math(unsigned long long* __restrict__ mismatches) {
+  unsigned long long bad_sqrt = 0, bad_rcp = 0;
+  const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+  for (uint64_t b = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; b < (1ull << 32); b += stride) {
+    const uint32_t bits = (uint32_t)b;
+    const float x = __uint_as_float(bits);
+    if (bits >= 0x0d000000u && bits <= 0x7f7fffffu)                       // [2^-101, FLT_MAX]
+      if (__float_as_uint(sqrt_rn_normal(x)) != __float_as_uint(sqrtf(x))) ++bad_sqrt;
+    const uint32_t e = (bits >> 23) & 0xffu;
+    if (e >= 1u && e <= 252u)                                             // |x| in [2^-126, 2^126)
+      if (__float_as_uint(rcp_rn_normal(x)) != __float_as_uint(1.0f / x)) ++bad_rcp;
+  }
+  bad_sqrt = __reduce_add_sync(0xffffffffu, (unsigned)bad_sqrt);
+  bad_rcp = __reduce_add_sync(0xffffffffu, (unsigned)bad_rcp);
+  if (lane_id() == 0) { if (bad_sqrt) atomicAdd(mismatches, bad_sqrt); if (bad_rcp) atomicAdd(mismatches + 1, bad_rcp); }
+}
 
 extern "C" {
 
@@ -304,10 +325,14 @@ int tpc_tracker_work_counters(tpc_tracker_t* t, void* cuda_stream, int64_t* out,
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (cudaMemcpyAsync(&h, t->plan.ptr<char>(t->params.arena, t->id.counters), 256, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
       cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return TPC_ECUDA; }
-  const int64_t v[7] = {h.i32[kCntTracklets], h.i32[kCntStartHits], (int64_t)(uint32_t)h.i32[kCntInvalid],
-                        (int64_t)h.u64[kCnt64RowSteps - 4], (int64_t)h.u64[kCnt64Updates - 4], (int64_t)h.u64[kCnt64Candidates - 4], 0};
-  for (int i = 0; i < 6 && i < capacity; ++i) out[i] = v[i];
-  return 6;
+  int64_t v[18] = {h.i32[kCntTracklets], h.i32[kCntStartHits], (int64_t)(uint32_t)h.i32[kCntInvalid], 0, 0, 0};
+  for (int ph = 0; ph < 4; ++ph)
+    for (int k = 0; k < 3; ++k) {
+      v[6 + 3 * ph + k] = (int64_t)h.u64[kCnt64Phase0 - 4 + 3 * ph + k];
+      v[3 + k] += v[6 + 3 * ph + k];
+    }
+  for (int i = 0; i < 18 && i < capacity; ++i) out[i] = v[i];
+  return 18;
 }
 
 int tpc_tracker_step_ms(tpc_tracker_t* t, float* ms_out, int32_t capacity) {
@@ -427,14 +452,18 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   }
 
   // ---- C5 tracklet constructor ----
-  mark(S_CONSTRUCT);
+  mark(S_TL_INIT);
   const int64_t tl_bound = std::min<int64_t>(T, n / std::max(2, c.seed_min_hits) + 1);   // start hits own disjoint chains
   k_tracklet_init<<<(int)((tl_bound + 255) / 256), 256, 0, st>>>(yt, hsr, link_up_clean, start_hits, counters, seeds, tl.row_hit, c); ++launches;
   {
     const int need = (int)((tl_bound + kTrackletThreads - 1) / kTrackletThreads);
+    mark(S_FIT_UP);
     k_tracklet_fit<false><<<std::min(t->ctas_fit_up, need), kTrackletThreads, 0, st>>>(yt, orig, seeds, counters, tl, c);
+    mark(S_FOLLOW_UP);
     k_tracklet_follow<false><<<std::min(t->ctas_follow_up, need), kTrackletThreads, 0, st>>>(yt, orig, bin_start, seeds, counters, tl, c);
+    mark(S_FIT_DOWN);
     k_tracklet_fit<true><<<std::min(t->ctas_fit_down, need), kTrackletThreads, 0, st>>>(yt, orig, seeds, counters, tl, c);
+    mark(S_FOLLOW_DOWN);
     k_tracklet_follow<true><<<std::min(t->ctas_follow_down, need), kTrackletThreads, 0, st>>>(yt, orig, bin_start, seeds, counters, tl, c);
     launches += 4;
   }
@@ -468,6 +497,21 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   t->have_times = t->profile;
   t->last_launches = launches;
   if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;
+  return TPC_OK;
+}
+
+int tpc_selftest_fast_math(void* cuda_stream, uint64_t* mismatches_out) {
+  if (!mismatches_out) return TPC_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  unsigned long long* d = nullptr;
+  if (cudaMalloc(&d, 16) != cudaSuccess) { cudaGetLastError(); return TPC_ECUDA; }
+  unsigned long long h[2] = {0, 0};
+  bool ok = cudaMemsetAsync(d, 0, 16, st) == cudaSuccess;
+  if (ok) { k_selftest_fast_math<<<148 * 16, 256, 0, st>>>(d); ok = cudaGetLastError() == cudaSuccess; }
+  ok = ok && cudaMemcpyAsync(h, d, 16, cudaMemcpyDeviceToHost, st) == cudaSuccess && cudaStreamSynchronize(st) == cudaSuccess;
+  cudaFree(d);
+  if (!ok) { cudaGetLastError(); return TPC_ECUDA; }
+  mismatches_out[0] = h[0]; mismatches_out[1] = h[1];
   return TPC_OK;
 }
 

@@ -17,7 +17,7 @@ STATUS_TRACKLET_OVERFLOW, STATUS_TRACK_OVERFLOW, STATUS_TRACK_HIT_OVERFLOW, STAT
 
 EXPORTS = ("tpc_tracker_arena_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
            "tpc_tracker_step_ms", "tpc_tracker_step_name", "tpc_tracker_last_launches", "tpc_tracker_work_counters",
-           "tpc_tracker_arena_plan",
+           "tpc_tracker_arena_plan", "tpc_selftest_fast_math",
            "tpc_tracker_destroy", "tpc_strerror")
 
 
@@ -99,6 +99,8 @@ def load_library(build_if_missing: bool = True):
         L.tpc_tracker_arena_plan.argtypes = [vp, C.c_int32, C.POINTER(C.c_char_p), C.POINTER(C.c_size_t),
                                              C.POINTER(C.c_size_t), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
         L.tpc_tracker_destroy.argtypes = [vp]
+        L.tpc_selftest_fast_math.argtypes = [vp, C.POINTER(C.c_uint64)]
+        L.tpc_selftest_fast_math.restype = C.c_int
         L.tpc_strerror.argtypes = [C.c_int]
         L.tpc_strerror.restype = C.c_char_p
         for nm in ("tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host", "tpc_tracker_step_ms",
@@ -112,6 +114,20 @@ class TpcError(RuntimeError):
     def __init__(self, code: int, where: str):
         self.code = code
         super().__init__(f"{where}: {load_library().tpc_strerror(code).decode()} ({code})")
+
+
+def tpc_selftest_fast_math(stream=None) -> tuple:
+    """(sqrt mismatches, reciprocal mismatches) of the constructor's range-restricted sqrt / reciprocal against the
+    IEEE results over every fp32 bit pattern of their ranges (include/tpc_tracker.h); both must be 0."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("tpc_selftest_fast_math needs a CUDA device")
+    s = stream if stream is not None else torch.cuda.current_stream()
+    out = (C.c_uint64 * 2)()
+    rc = load_library().tpc_selftest_fast_math(C.c_void_p(s.cuda_stream), out)
+    if rc != TPC_OK:
+        raise TpcError(rc, "tpc_selftest_fast_math")
+    return int(out[0]), int(out[1])
 
 
 def tpc_tracker_arena_bytes(geometry: Geometry, params: Params, max_clusters: int = 0) -> int:
@@ -264,12 +280,15 @@ class Tracker:
 
     def work_counters(self, stream=None) -> dict:
         s = stream if stream is not None else self._torch.cuda.current_stream(self.device)
-        buf = (C.c_int64 * 8)()
-        k = self.lib.tpc_tracker_work_counters(self.handle, C.c_void_p(s.cuda_stream), buf, 8)
+        buf = (C.c_int64 * 18)()
+        k = self.lib.tpc_tracker_work_counters(self.handle, C.c_void_p(s.cuda_stream), buf, 18)
         if k < 0:
             raise TpcError(k, "tpc_tracker_work_counters")
         names = ("tracklets", "start_hits", "invalid_clusters", "row_steps", "updates", "candidates")
-        return {nm: int(buf[i]) for i, nm in enumerate(names)}
+        out = {nm: int(buf[i]) for i, nm in enumerate(names)}
+        for p, ph in enumerate(("fit_up", "follow_up", "fit_down", "follow_down")):
+            out[ph] = {nm: int(buf[6 + 3 * p + i]) for i, nm in enumerate(("row_steps", "updates", "candidates"))}
+        return out
 
     def arena_plan(self) -> list:
         out, i = [], 0

@@ -206,3 +206,11 @@ def test_arena_plan_reuses_memory_across_steps():
     assert any(a["last_step"] < c["first_step"] and a["offset"] < c["offset"] + c["bytes"] and c["offset"] < a["offset"] + a["bytes"]
                for a in plan)
     trk.close()
+
+
+def test_fast_sqrt_rcp_are_ieee_exact_exhaustively():
+    """The constructor replaces sqrtf() and 1.0f / x by range-restricted refinement sequences (csrc/tracklet.cuh); they
+    must be bit-identical to the IEEE results the oracle computes, for EVERY fp32 operand of their ranges."""
+    from paper_2102_08862_b200 import tracker as T
+    bad_sqrt, bad_rcp = T.tpc_selftest_fast_math()
+    assert (bad_sqrt, bad_rcp) == (0, 0)
