@@ -14,6 +14,7 @@ struct Consts {
   // geometry
   int n_rows, n_sr, n_tb, n_pb, n_bins;  // rows per sector, sector-rows, time bins and pad bins per sector-row, n_sr*n_pb*n_tb
   float max_time, inv_bin_w;             // validity bound of the time coordinate; 1 / grid bin width (time)
+  float inv_n_rows;                      // (float)(1 / n_rows), for row = sector_row mod n_rows without a division
   float Z, inv_Z, P;                     // time-bin size [cm], its inverse (grid lookups only), pad pitch
   // neighbours finder (C2)
   float W1, Ay, Az, wy, wz, chi2_cut;

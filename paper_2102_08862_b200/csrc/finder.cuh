@@ -48,91 +48,41 @@ __device__ __forceinline__ Span grid_span(const uint32_t* __restrict__ bin_start
 
 constexpr int kFinderThreads = 256;
 constexpr int kFinderSlots = 4;       // candidates kept per neighbour row in shared memory; more -> generic path
-constexpr int kFinderBuckets = 64;    // work classes of the in-CTA balancing (candidate count, clamped)
 
-// SIMT shape.  The candidate count of a hit has a heavy tail (dense collisions, loopers), and a warp that runs
-// "one hit per thread" in index order pays for its heaviest lane: the straight version ran at 12 of 32 lanes
-// (profiles/r01c_ncu_full.md).  So a CTA of 256 consecutive hits first looks up every hit's candidate spans (thread t
-// <-> hit t, coalesced), then sorts its 256 hits by candidate count (counting sort in shared memory) and hands hit
-// perm[t] to thread t: the lanes of a warp now carry about the same number of candidates.  The result of a hit does
-// not depend on which thread computes it.  Per hit: (1) ONE flat loop scans the candidates of both neighbour rows
-// (each row: the spans of one or two pad bins -- the create-time check guarantees that the search area is narrower
-// than a pad bin) and appends those inside the search area to two small per-thread lists in shared memory
-// ([slot][thread]: conflict-free); (2) ONE flat loop over the nu x nd pairs.  Both bodies are branch-free apart from
-// the rare exact-tie case.
+// SIMT shape: (1) ONE flat loop scans the candidates of both neighbour rows (each row: the spans of one or two pad
+// bins -- the create-time check guarantees that the search area is narrower than a pad bin) and appends those inside
+// the search area to two small per-thread lists in shared memory ([slot][thread]: conflict-free); (2) ONE flat loop
+// over the nu x nd pairs.  Both trip counts are the maximum over the warp of a small number, and the bodies are
+// branch-free apart from the rare exact-tie case.  The nested "for u: for d" form over the raw spans ran at 4.5 of
+// 32 lanes (profiles/r01a_ncu_full_baseline.md).
 __global__ void __launch_bounds__(kFinderThreads) k_neighbours_finder(const float2* __restrict__ yt, const uint32_t* __restrict__ orig,
                                                                       const uint16_t* __restrict__ hsr, const uint32_t* __restrict__ bin_start,
                                                                       int* __restrict__ link_up, int* __restrict__ link_down,
                                                                       const __grid_constant__ Consts c) {
   __shared__ float2 s_val[2 * kFinderSlots][kFinderThreads];      // rows 0..3: up candidates, 4..7: down candidates
   __shared__ uint32_t s_idx[2 * kFinderSlots][kFinderThreads];
-  __shared__ uint32_t s_span[8][kFinderThreads];                  // per hit: e0, e1, e2, n_all, b0, b1, b2, b3
-  __shared__ float2 s_me[kFinderThreads];
-  __shared__ uint32_t s_bucket[kFinderBuckets];
-  __shared__ uint16_t s_perm[kFinderThreads];
   const uint32_t n_valid = __ldg(bin_start + c.n_bins);
-  const int tx = threadIdx.x;
-  const uint32_t h_base = blockIdx.x * blockDim.x;
-  if (h_base >= n_valid) return;
-  if (tx < kFinderBuckets) s_bucket[tx] = 0;
-  __syncthreads();
-
-  // ---- A. thread t <-> hit h_base + t: candidate spans of rows r+1 and r-1 ----
-  uint32_t my_class = 0;
-  {
-    const uint32_t h = h_base + tx;
-    uint32_t e0 = 0, e1 = 0, e2 = 0, n_all = 0, b0 = 0, b1 = 0, b2 = 0, b3 = 0;
-    float2 me = make_float2(0.0f, 0.0f);
-    if (h < n_valid) {
-      const int sr = hsr[h];
-      const int r = sr % c.n_rows;
-      if (r >= 1 && r <= c.n_rows - 2) {
-        me = yt[h];
-        const int tb_lo = time_bin(me.y - c.finder_tw, c), tb_hi = time_bin(me.y + c.finder_tw, c);
-        const float yo_u = __ldg(c.yoff + r + 1), ps_u = __ldg(c.pscale + r + 1);
-        const float yo_d = __ldg(c.yoff + r - 1), ps_d = __ldg(c.pscale + r - 1);
-        const int pu0 = pad_bin(me.x - c.finder_yw, yo_u, ps_u, c), pu1 = pad_bin(me.x + c.finder_yw, yo_u, ps_u, c);
-        const int pd0 = pad_bin(me.x - c.finder_yw, yo_d, ps_d, c), pd1 = pad_bin(me.x + c.finder_yw, yo_d, ps_d, c);
-        // spans: u0, u1 (row r+1), d0, d1 (row r-1); the second span of a row is empty unless the area straddles two pad bins
-        const Span u0 = grid_span(bin_start, sr + 1, pu0, tb_lo, tb_hi, c);
-        const Span d0 = grid_span(bin_start, sr - 1, pd0, tb_lo, tb_hi, c);
-        Span u1{0u, 0u}, d1{0u, 0u};
-        if (pu1 != pu0) u1 = grid_span(bin_start, sr + 1, pu1, tb_lo, tb_hi, c);
-        if (pd1 != pd0) d1 = grid_span(bin_start, sr - 1, pd1, tb_lo, tb_hi, c);
-        e0 = u0.n; e1 = e0 + u1.n; e2 = e1 + d0.n; n_all = e2 + d1.n;      // up candidates: i < e1
-        // flat index i -> sorted-hit index: base of the span that holds i, minus the span's first i
-        b0 = u0.lo; b1 = u1.lo - e0; b2 = d0.lo - e1; b3 = d1.lo - e2;
-      }
-    }
-    s_span[0][tx] = e0; s_span[1][tx] = e1; s_span[2][tx] = e2; s_span[3][tx] = n_all;
-    s_span[4][tx] = b0; s_span[5][tx] = b1; s_span[6][tx] = b2; s_span[7][tx] = b3;
-    s_me[tx] = me;
-    my_class = min(n_all, (uint32_t)kFinderBuckets - 1u);
-    atomicAdd(&s_bucket[my_class], 1u);
-  }
-  __syncthreads();
-  // ---- counting sort of the CTA's hits by candidate count (heaviest first) ----
-  if (tx < 32) {
-    const uint32_t c0 = s_bucket[kFinderBuckets - 1 - 2 * tx], c1 = s_bucket[kFinderBuckets - 2 - 2 * tx];
-    uint32_t inc = c0 + c1;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o); if (tx >= o) inc += v; }
-    s_bucket[kFinderBuckets - 1 - 2 * tx] = inc - c0 - c1;
-    s_bucket[kFinderBuckets - 2 - 2 * tx] = inc - c1;
-  }
-  __syncthreads();
-  s_perm[atomicAdd(&s_bucket[my_class], 1u)] = (uint16_t)tx;
-  __syncthreads();
-
-  // ---- B. thread t <-> hit h_base + perm[t] ----
-  const int src = s_perm[tx];
-  const uint32_t h = h_base + src;
+  const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
   if (h >= n_valid) return;
-  const uint32_t e0 = s_span[0][src], e1 = s_span[1][src], e2 = s_span[2][src], n_all = s_span[3][src];
-  const uint32_t b0 = s_span[4][src], b1 = s_span[5][src], b2 = s_span[6][src], b3 = s_span[7][src];
-  const float2 me = s_me[src];
+  const int sr = hsr[h];
+  const int r = sr % c.n_rows;
   int bu = -1, bd = -1;
-  if (n_all > 0) {
+  if (r >= 1 && r <= c.n_rows - 2) {
+    const float2 me = yt[h];
+    const int tb_lo = time_bin(me.y - c.finder_tw, c), tb_hi = time_bin(me.y + c.finder_tw, c);
+    const float yo_u = __ldg(c.yoff + r + 1), ps_u = __ldg(c.pscale + r + 1);
+    const float yo_d = __ldg(c.yoff + r - 1), ps_d = __ldg(c.pscale + r - 1);
+    const int pu0 = pad_bin(me.x - c.finder_yw, yo_u, ps_u, c), pu1 = pad_bin(me.x + c.finder_yw, yo_u, ps_u, c);
+    const int pd0 = pad_bin(me.x - c.finder_yw, yo_d, ps_d, c), pd1 = pad_bin(me.x + c.finder_yw, yo_d, ps_d, c);
+    // spans: u0, u1 (row r+1), d0, d1 (row r-1); the second span of a row is empty unless the area straddles two pad bins
+    const Span u0 = grid_span(bin_start, sr + 1, pu0, tb_lo, tb_hi, c);
+    const Span d0 = grid_span(bin_start, sr - 1, pd0, tb_lo, tb_hi, c);
+    Span u1{0u, 0u}, d1{0u, 0u};
+    if (pu1 != pu0) u1 = grid_span(bin_start, sr + 1, pu1, tb_lo, tb_hi, c);
+    if (pd1 != pd0) d1 = grid_span(bin_start, sr - 1, pd1, tb_lo, tb_hi, c);
+    const uint32_t e0 = u0.n, e1 = e0 + u1.n, e2 = e1 + d0.n, n_all = e2 + d1.n;   // up candidates: i < e1
+    // flat index i -> sorted-hit index: base of the span that holds i, minus the span's first i
+    const uint32_t b0 = u0.lo, b1 = u1.lo - e0, b2 = d0.lo - e1, b3 = d1.lo - e2;
     int nu = 0, nd = 0;
     for (uint32_t ib = 0; ib < n_all; ib += 2) {     // two independent loads per trip
       uint32_t qq[2];
@@ -149,7 +99,7 @@ __global__ void __launch_bounds__(kFinderThreads) k_neighbours_finder(const floa
         if (i < n_all && in_search_area(me, cq[k], c)) {
           const bool up = i < e1;
           const int slot = up ? nu : kFinderSlots + nd;
-          if ((up ? nu : nd) < kFinderSlots) { s_val[slot][tx] = cq[k]; s_idx[slot][tx] = qq[k]; }
+          if ((up ? nu : nd) < kFinderSlots) { s_val[slot][threadIdx.x] = cq[k]; s_idx[slot][threadIdx.x] = qq[k]; }
           nu += up ? 1 : 0;
           nd += up ? 0 : 1;
         }
@@ -160,8 +110,8 @@ __global__ void __launch_bounds__(kFinderThreads) k_neighbours_finder(const floa
       const int n_pairs = nu * nd;
       int a = 0, b = 0;
       for (int p = 0; p < n_pairs; ++p) {            // pair (a, b), a-major like the definition's loops
-        finder_try_pair(me, s_val[a][tx], s_val[kFinderSlots + b][tx], s_idx[a][tx],
-                        s_idx[kFinderSlots + b][tx], orig, c, best, bu, bd);
+        finder_try_pair(me, s_val[a][threadIdx.x], s_val[kFinderSlots + b][threadIdx.x], s_idx[a][threadIdx.x],
+                        s_idx[kFinderSlots + b][threadIdx.x], orig, c, best, bu, bd);
         if (++b == nd) { b = 0; ++a; }
       }
     } else {   // crowded area: generic nested loops over the spans (ties are decided on the original index)

@@ -27,15 +27,15 @@ constexpr size_t kRadixScatterSmem = (size_t)kRadixTile * 16 + (size_t)(kRadixTh
 // time in [0, max_time]; evaluated in fp32 on the raw values (DESIGN.md §3 C1).
 // Also returns the local y of a valid cluster.
 __device__ __forceinline__ uint32_t cluster_key(float rf, float pad, float time, const Consts& c, float& y) {
-  y = 0.0f;
-  bool ok = rf >= 0.0f && rf < (float)c.n_sr && rf == floorf(rf);
-  if (!ok) return (uint32_t)c.n_bins;
-  const int sr = (int)rf;
-  const int r = sr % c.n_rows;
-  ok = pad >= -0.5f && pad < (float)__ldg(c.npads + r) - 0.5f && time >= 0.0f && time <= c.max_time;
-  if (!ok) return (uint32_t)c.n_bins;
-  y = (pad - __ldg(c.cr + r)) * c.P;                                   // y(h) = (pad - c_r) * P
-  return (uint32_t)((sr * c.n_pb + pad_bin(y, __ldg(c.yoff + r), __ldg(c.pscale + r), c)) * c.n_tb + time_bin(time, c));
+  const bool ok_row = rf >= 0.0f && rf < (float)c.n_sr && rf == floorf(rf);
+  const int sr = ok_row ? (int)rf : 0;
+  // r = sr mod n_rows without an integer division: sr < 2^16 and n_rows <= 160, so (sr + 0.5) / n_rows is at least
+  // 0.003 away from an integer while the fp32 product is off by < 1e-4
+  const int r = sr - (int)(((float)sr + 0.5f) * c.inv_n_rows) * c.n_rows;
+  const bool ok = ok_row && pad >= -0.5f && pad < (float)__ldg(c.npads + r) - 0.5f && time >= 0.0f && time <= c.max_time;
+  y = ok ? (pad - __ldg(c.cr + r)) * c.P : 0.0f;                       // y(h) = (pad - c_r) * P
+  const uint32_t key = (uint32_t)((sr * c.n_pb + pad_bin(y, __ldg(c.yoff + r), __ldg(c.pscale + r), c)) * c.n_tb + time_bin(time, c));
+  return ok ? key : (uint32_t)c.n_bins;
 }
 
 struct RadixSrc {        // input of a pass: either the raw clusters (first pass) or a sorted-so-far set
@@ -53,13 +53,25 @@ __global__ void __launch_bounds__(kRadixThreads) k_radix_histogram(RadixSrc src,
   for (int i = threadIdx.x; i < kRadixBuckets; i += kRadixThreads) cnt[i] = 0;
   __syncthreads();
   const int64_t base = (int64_t)blockIdx.x * kRadixTile;
-#pragma unroll 4
-  for (int k = 0; k < kRadixItems; ++k) {
-    const int64_t i = base + (int64_t)k * kRadixThreads + threadIdx.x;
-    if (i < n) {
+  if (kFirst) {                                     // all loads of the tile first, then the key arithmetic
+    float rf[kRadixItems], pd[kRadixItems], tm[kRadixItems];
+#pragma unroll
+    for (int k = 0; k < kRadixItems; ++k) {
+      const int64_t i = base + (int64_t)k * kRadixThreads + threadIdx.x;
+      const bool in = i < n;
+      rf[k] = in ? src.row[i] : -1.0f; pd[k] = in ? src.pad[i] : 0.0f; tm[k] = in ? src.time[i] : 0.0f;
+    }
+#pragma unroll
+    for (int k = 0; k < kRadixItems; ++k) {
       float y;
-      const uint32_t key = kFirst ? cluster_key(src.row[i], src.pad[i], src.time[i], c, y) : src.keys[i];
-      atomicAdd(&cnt[(key >> shift) & mask], 1u);
+      const uint32_t key = cluster_key(rf[k], pd[k], tm[k], c, y);
+      if (base + (int64_t)k * kRadixThreads + threadIdx.x < n) atomicAdd(&cnt[(key >> shift) & mask], 1u);
+    }
+  } else {
+#pragma unroll
+    for (int k = 0; k < kRadixItems; ++k) {
+      const int64_t i = base + (int64_t)k * kRadixThreads + threadIdx.x;
+      if (i < n) atomicAdd(&cnt[(src.keys[i] >> shift) & mask], 1u);
     }
   }
   __syncthreads();
@@ -68,8 +80,11 @@ __global__ void __launch_bounds__(kRadixThreads) k_radix_histogram(RadixSrc src,
 
 // Stable scatter of one tile.  `offsets` = exclusive scan of hist (same layout): global position of the first
 // element of (digit, tile).
+#ifndef TPC_SCATTER_CTAS
+#define TPC_SCATTER_CTAS 4
+#endif
 template <bool kFirst>
-__global__ void __launch_bounds__(kRadixThreads, 3) k_radix_scatter(RadixSrc src, RadixDst dst, int64_t n, int shift, uint32_t mask,
+__global__ void __launch_bounds__(kRadixThreads, TPC_SCATTER_CTAS) k_radix_scatter(RadixSrc src, RadixDst dst, int64_t n, int shift, uint32_t mask,
                                                                  const uint32_t* __restrict__ offsets, int n_tiles,
                                                                  uint32_t* __restrict__ n_invalid,
                                                                  const __grid_constant__ Consts c) {
@@ -93,40 +108,53 @@ __global__ void __launch_bounds__(kRadixThreads, 3) k_radix_scatter(RadixSrc src
   const int64_t wbase = tile_base + (int64_t)w * kWarpItems;
   uint32_t key[kRadixItems], og[kRadixItems], rank[kRadixItems];
   float2 yt[kRadixItems];
-  uint32_t bad = 0;
-#pragma unroll
-  for (int k = 0; k < kRadixItems; ++k) {
-    const int64_t i = wbase + k * 32 + lane;
-    key[k] = 0xFFFFFFFFu; og[k] = 0; yt[k] = make_float2(0.0f, 0.0f);
-    if (i < n) {
-      if (kFirst) {
-        const float rf = src.row[i], p = src.pad[i], t = src.time[i];
-        float y;
-        key[k] = cluster_key(rf, p, t, c, y);
-        og[k] = (uint32_t)i;
-        if (key[k] == (uint32_t)c.n_bins) ++bad;
-        yt[k] = make_float2(y, t);
-      } else {
-        key[k] = src.keys[i]; og[k] = src.orig[i]; yt[k] = src.yt[i];
-      }
-    }
-  }
+  const int n_mine = (int)min((int64_t)kWarpItems, max(n - wbase, (int64_t)0));   // elements of this warp's slice that exist
   if (kFirst) {
+    float rf[kRadixItems];
+#pragma unroll
+    for (int k = 0; k < kRadixItems; ++k) {           // all loads first, then the key arithmetic
+      const bool in = k * 32 + (int)lane < n_mine;
+      const int64_t i = wbase + k * 32 + lane;
+      rf[k] = in ? src.row[i] : -1.0f; yt[k].x = in ? src.pad[i] : 0.0f; yt[k].y = in ? src.time[i] : 0.0f;
+      og[k] = (uint32_t)i;
+    }
+    uint32_t bad = 0;
+#pragma unroll
+    for (int k = 0; k < kRadixItems; ++k) {
+      float y;
+      key[k] = cluster_key(rf[k], yt[k].x, yt[k].y, c, y);
+      yt[k].x = y;
+      if (k * 32 + (int)lane < n_mine && key[k] == (uint32_t)c.n_bins) ++bad;
+    }
     bad = __reduce_add_sync(0xffffffffu, bad);
     if (bad && lane == 0) atomicAdd(n_invalid, bad);
+  } else {
+#pragma unroll
+    for (int k = 0; k < kRadixItems; ++k) {
+      const bool in = k * 32 + (int)lane < n_mine;
+      const int64_t i = wbase + k * 32 + lane;
+      key[k] = in ? src.keys[i] : 0xFFFFFFFFu; og[k] = in ? src.orig[i] : 0u; yt[k] = in ? src.yt[i] : make_float2(0.0f, 0.0f);
+    }
   }
 
-  // 2. stable rank inside the warp: elements are visited in index order (k-major, lane-minor)
+  // 2. stable rank inside the warp: elements are visited in index order (k-major, lane-minor).  The eight warp
+  // matches are independent and issued back to back; only the counter updates form a chain.
+  unsigned peers[kRadixItems];
 #pragma unroll
   for (int k = 0; k < kRadixItems; ++k) {
-    const bool valid = wbase + k * 32 + lane < n;
+    const bool valid = k * 32 + (int)lane < n_mine;
     const uint32_t d = valid ? (key[k] >> shift) & mask : mask + 1u;      // padding never matches a digit
-    const unsigned peers = __match_any_sync(0xffffffffu, d);
-    const int leader = __ffs(peers) - 1;
+    peers[k] = __match_any_sync(0xffffffffu, d);
+  }
+#pragma unroll
+  for (int k = 0; k < kRadixItems; ++k) {
+    const bool valid = k * 32 + (int)lane < n_mine;
+    const uint32_t d = (key[k] >> shift) & mask;
+    const int leader = __ffs(peers[k]) - 1;
     uint32_t before = 0;
-    if (valid && (int)lane == leader) { before = warp_cnt[w][d]; warp_cnt[w][d] = before + __popc(peers); }
+    if (valid && (int)lane == leader) { before = warp_cnt[w][d]; warp_cnt[w][d] = before + __popc(peers[k]); }
     before = __shfl_sync(0xffffffffu, before, leader);
-    rank[k] = before + __popc(peers & ((1u << lane) - 1u));
+    rank[k] = before + __popc(peers[k] & ((1u << lane) - 1u));
     __syncwarp();
   }
   __syncthreads();
@@ -157,7 +185,7 @@ __global__ void __launch_bounds__(kRadixThreads, 3) k_radix_scatter(RadixSrc src
   // 4. local reorder into shared memory
 #pragma unroll
   for (int k = 0; k < kRadixItems; ++k) {
-    if (wbase + k * 32 + lane < n) {
+    if (k * 32 + (int)lane < n_mine) {
       const uint32_t d = (key[k] >> shift) & mask;
       const uint32_t pos = digit_start[d] + warp_cnt[w][d] + rank[k];
       s_keys[pos] = key[k]; s_orig[pos] = og[k]; s_yt[pos] = yt[k];

@@ -247,7 +247,7 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
   Consts& c = t->consts;
   const int w = t->cap.grid_w;
   c.n_rows = nr; c.n_sr = g->n_sectors * nr; c.n_tb = t->cap.n_tb; c.n_pb = t->cap.n_pb; c.n_bins = t->cap.n_bins;
-  c.max_time = g->max_time_bin; c.inv_bin_w = (float)(1.0 / (double)w);
+  c.max_time = g->max_time_bin; c.inv_bin_w = (float)(1.0 / (double)w); c.inv_n_rows = (float)(1.0 / (double)nr);
   c.Z = g->time_bin_cm; c.inv_Z = (float)(1.0 / (double)g->time_bin_cm); c.P = g->pad_pitch_cm;
   const double w1 = (double)p->win_slope * pitch + (double)p->win_const;
   c.W1 = (float)w1;
