@@ -95,17 +95,27 @@ struct TrackOutputs {   // device pointers of tpc_tracks_t (include/tpc_tracker.
   int32_t* hit_index;
 };
 
-// track_idx / hit_off are the exclusive scans of flag / owned; their totals sit behind the last tile offset.
+// track_slot[track_idx[j]] = j for every tracklet that became a track: the emit kernel then runs one warp per TRACK
+// (1.8e6 in configs[3]) instead of one per tracklet slot (1.2e7, most of which had nothing to emit).
+__global__ void __launch_bounds__(256) k_selector_map(const int32_t* __restrict__ counters, const uint32_t* __restrict__ flag,
+                                                      const uint32_t* __restrict__ track_idx, uint32_t* __restrict__ track_slot) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j < counters[0] && flag[j]) track_slot[track_idx[j]] = (uint32_t)j;
+}
+
+// One warp per track.  track_idx / hit_off are the exclusive scans of flag / owned; their totals sit behind the last
+// tile offset.
 __global__ void __launch_bounds__(kSelectorThreads) k_selector_emit(
     TrackletStore tl, const int32_t* __restrict__ counters, const uint32_t* __restrict__ own_mask,
-    const uint32_t* __restrict__ flag_in, const uint32_t* __restrict__ track_idx, const uint32_t* __restrict__ hit_off,
+    const uint32_t* __restrict__ track_slot, const uint32_t* __restrict__ hit_off,
     const uint32_t* __restrict__ track_total, const uint32_t* __restrict__ hit_total,
     const uint32_t* __restrict__ orig, const uint16_t* __restrict__ hsr, const uint32_t* __restrict__ start_hits,
     const uint32_t* __restrict__ n_invalid, TrackOutputs o, const __grid_constant__ Consts c) {
   constexpr int kWords = kRowStride / 32;
-  const int j = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  if (j == 0 && lane_id() == 0) {
-    const uint32_t nt = *track_total, nh = *hit_total;
+  const uint32_t ti = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const uint32_t nt = *track_total;
+  if (ti == 0 && lane_id() == 0) {
+    const uint32_t nh = *hit_total;
     *o.n_tracks = (int32_t)nt;
     *o.n_track_hits = (int64_t)nh;
     int st = 0;
@@ -115,11 +125,9 @@ __global__ void __launch_bounds__(kSelectorThreads) k_selector_emit(
     if (*n_invalid) st |= 8;                                // TPC_STATUS_INVALID_CLUSTERS
     *o.status = st;
   }
-  if (j >= counters[0]) return;
-  if (flag_in[j] == 0) return;
-  const uint32_t ti = track_idx[j];
+  if (ti >= nt || (int64_t)ti >= (int64_t)o.max_tracks) return;
+  const int j = (int)track_slot[ti];
   const uint32_t off = hit_off[j];
-  if ((int64_t)ti >= (int64_t)o.max_tracks) return;
   const int* rows = tl.row_hit + (size_t)j * kRowStride;
   const uint32_t my_word = lane_id() < kWords ? own_mask[(size_t)j * kWords + lane_id()] : 0u;
   int n_owned = 0, own_first = -1, own_last = -1;

@@ -35,7 +35,7 @@ struct Ids {   // arena allocation ids
   int stage_in = -1, stage_out = -1;
   int bin_start, sort_keys, tmp_keys, tmp_orig, tmp_yt, sort_hist, yt, orig, hsr, link_up, link_down, link_up_clean, start_flag, cell_count, start_hits,
       counters, scan_a, scan_b, seeds_a, seeds_b, row_hit, tl_meta, tl_rec, tl_cur, claim, owned, own_mask,
-      flag, track_idx, hit_off;
+      flag, track_idx, hit_off, track_slot;
 };
 
 struct Capacities {
@@ -142,6 +142,7 @@ void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids
   id.flag = plan.add("selector_flag", 4 * T, S_COUNT, S_EMIT);
   id.track_idx = plan.add("selector_track_idx", 4 * T, S_SELECT_SCAN, S_EMIT);
   id.hit_off = plan.add("selector_hit_off", 4 * T, S_SELECT_SCAN, S_EMIT);
+  id.track_slot = plan.add("selector_track_slot", 4 * T, S_EMIT, S_EMIT);
   plan.plan();
 }
 
@@ -390,6 +391,7 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   uint32_t* flag = P.ptr<uint32_t>(A, id.flag);
   uint32_t* track_idx = P.ptr<uint32_t>(A, id.track_idx);
   uint32_t* hit_off = P.ptr<uint32_t>(A, id.hit_off);
+  uint32_t* track_slot = P.ptr<uint32_t>(A, id.track_slot);
   TrackletStore tl;
   tl.row_hit = P.ptr<int>(A, id.row_hit);
   tl.meta = P.ptr<int4>(A, id.tl_meta);
@@ -491,8 +493,10 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   to.hit_offset = o->hit_offset; to.x = o->x; to.y = o->y; to.z_rel = o->z_rel; to.time_ref = o->time_ref;
   to.sin_phi = o->sin_phi; to.dzds = o->dzds; to.q_pt = o->q_pt; to.cov9 = o->cov9; to.hit_index = o->hit_index;
   const int n_scan_tiles = (int)scan_tiles((size_t)T);
-  k_selector_emit<<<std::max(warp_ctas, 1), kSelectorThreads, 0, st>>>(tl, counters, own_mask, flag, track_idx, hit_off, scan_a + n_scan_tiles,
-                                                                       scan_b + n_scan_tiles, orig, hsr, start_hits, n_invalid, to, c); ++launches;
+  k_selector_map<<<(int)((tl_bound + 255) / 256), 256, 0, st>>>(counters, flag, track_idx, track_slot); ++launches;
+  const int64_t emit_warps = std::max<int64_t>(std::min<int64_t>(tl_bound, o->max_tracks), 1);      // warp 0 also writes the scalars
+  k_selector_emit<<<(int)((emit_warps * 32 + kSelectorThreads - 1) / kSelectorThreads), kSelectorThreads, 0, st>>>(
+      tl, counters, own_mask, track_slot, hit_off, scan_a + n_scan_tiles, scan_b + n_scan_tiles, orig, hsr, start_hits, n_invalid, to, c); ++launches;
   mark(N_STEPS);
   t->have_times = t->profile;
   t->last_launches = launches;
