@@ -170,11 +170,9 @@ def main():
     import numpy as np
     import torch
     import torch.distributed as dist
-    from paper_2102_08862_b200 import gen, tracker as T
+    from paper_2102_08862_b200 import gen, replicas, tracker as T
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local_rank = replicas.rank_world_local()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the tracker has no CPU fallback")
     torch.cuda.set_device(local_rank)
@@ -184,7 +182,7 @@ def main():
 
     # ---- synthetic time frame (one per rank; seeded) ----
     cid = args.config
-    cfg = gen.preset(cid, args.seed + rank, args.frame_us if cid >= 2 else None)
+    cfg = gen.preset(cid, replicas.frame_seed(args.seed, rank), args.frame_us if cid >= 2 else None)
     cfg.n_threads = max(1, (os.cpu_count() or 8) // max(world, 1))
     t_gen = time.perf_counter()
     tf = gen.generate(cfg, want_truth=False)
@@ -239,15 +237,8 @@ def main():
     trk.close()
     del trk, outs
 
-    t = torch.tensor([total_ms, float(n)], dtype=torch.float64, device=dev)
-    if world > 1:
-        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        total_ms_max, n_all = float(tmax[0]), float(tsum[1])
-    else:
-        total_ms_max, n_all = total_ms, float(n)
-    ms_per_step = total_ms_max / args.steps
-    value = n_all / (ms_per_step * 1e-3)
+    # whole-job numbers: time = max over ranks, work = sum over ranks (paper_2102_08862_b200/replicas.py)
+    ms_per_step, value, n_all = replicas.aggregate(total_ms, n, args.steps, world, device=dev)
 
     # ---- end to end through the C-ABI host entry point (pinned host buffers) ----
     # Every step copies the frame host->device, tracks it and copies the tracks back, all inside tpc_track_timeframe_host.
@@ -284,9 +275,7 @@ def main():
         barrier()
         k_e2e = k_each * n_fl
         ms = e0.elapsed_time(e1) / k_e2e
-        t2 = torch.tensor([ms], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(t2, op=dist.ReduceOp.MAX)
+        t2 = [replicas.max_over_ranks(ms, world, device=dev)]
         k = int(houts[0][0].n_tracks[0]); h = int(houts[0][0].n_track_hits[0])
         d2h = 16 + k * (8 + 5 * 4 + 7 * 4 + 36) + 4 * h
         e2e = {"value": n_all / (float(t2[0]) * 1e-3), "unit": "clusters/s", "ms_per_step": float(t2[0]),
