@@ -47,7 +47,10 @@ __device__ __forceinline__ Span grid_span(const uint32_t* __restrict__ bin_start
 }
 
 constexpr int kFinderThreads = 256;
-constexpr int kFinderSlots = 4;       // candidates kept per neighbour row in shared memory; more -> generic path
+#ifndef TPC_FINDER_SLOTS
+#define TPC_FINDER_SLOTS 6
+#endif
+constexpr int kFinderSlots = TPC_FINDER_SLOTS;       // candidates kept per neighbour row in shared memory; more -> generic path
 
 // SIMT shape: (1) ONE flat loop scans the candidates of both neighbour rows (each row: the spans of one or two pad
 // bins -- the create-time check guarantees that the search area is narrower than a pad bin) and appends those inside

@@ -47,6 +47,12 @@ struct Capacities {
 };
 
 constexpr int kDefaultGridTimeBins = 4, kDefaultGridPadBins = 8, kDefaultSliceTimeBins = 256;
+#ifndef TPC_FOLLOW_CTAS_PER_SM
+#define TPC_FOLLOW_CTAS_PER_SM 64
+#endif
+#ifndef TPC_FIT_CTAS_PER_SM
+#define TPC_FIT_CTAS_PER_SM 64
+#endif
 constexpr double kGridMarginCm = 0.01;   // superset margin of the pad-bin lookups (fp32 rounding of a difference is << this)
 
 bool valid_geometry(const tpc_geometry_t* g) {
@@ -278,17 +284,17 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    auto resident = [&](auto kernel) {
+    auto resident = [&](auto kernel, int cap) {
       int per_sm = 1;
       if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kTrackletThreads, 0) != cudaSuccess || per_sm < 1) {
         cudaGetLastError(); per_sm = 1;
       }
-      return sms * per_sm;
+      return sms * std::min(per_sm, cap);
     };
-    t->ctas_fit_up = resident(k_tracklet_fit<false>);
-    t->ctas_follow_up = resident(k_tracklet_follow<false>);
-    t->ctas_fit_down = resident(k_tracklet_fit<true>);
-    t->ctas_follow_down = resident(k_tracklet_follow<true>);
+    t->ctas_fit_up = resident(k_tracklet_fit<false>, TPC_FIT_CTAS_PER_SM);
+    t->ctas_follow_up = resident(k_tracklet_follow<false>, TPC_FOLLOW_CTAS_PER_SM);
+    t->ctas_fit_down = resident(k_tracklet_fit<true>, TPC_FIT_CTAS_PER_SM);
+    t->ctas_follow_down = resident(k_tracklet_follow<true>, TPC_FOLLOW_CTAS_PER_SM);
   }
   for (int i = 0; i <= N_STEPS; ++i)
     if (cudaEventCreate(&t->ev[i]) != cudaSuccess) { cudaGetLastError(); tpc_tracker_destroy(t); return TPC_ECUDA; }
