@@ -41,9 +41,9 @@ ALGO_LANE_INST_TRANSPORT, ALGO_LANE_INST_UPDATE, ALGO_LANE_INST_PER_CANDIDATE = 
 TRACKLET_PHASES = {"tracklet_fit_up": "fit_up", "tracklet_follow_up": "follow_up", "tracklet_fit_down": "fit_down",
                    "tracklet_follow_down": "follow_down"}     # step name -> work-counter group
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of configs[3], seed 1
-# (profiles/r01d_ncu_full_config3.md); reported as roofline.traffic for that workload only, null otherwise.
-NCU_TRAFFIC_BYTES_CONFIG3 = {"tracklet_follow_up": 17.898e9 + 5.659e9, "tracklet_follow_down": 19.050e9 + 5.010e9,
-                             "tracklet_fit_down": 6.705e9 + 0.783e9, "neighbours_finder": 3.815e9 + 1.278e9}
+# (profiles/r01e_ncu_full_config3.md); reported as roofline.traffic for that workload only, null otherwise.
+NCU_TRAFFIC_BYTES_CONFIG3 = {"tracklet_follow_up": 17.941e9 + 5.657e9, "tracklet_follow_down": 19.170e9 + 5.006e9,
+                             "tracklet_fit_down": 6.703e9 + 0.782e9, "neighbours_finder": 3.815e9 + 1.279e9}
 SM_COUNT, SMSP_PER_SM, LANES = 148, 4, 32      # B300_MICROARCH.md: 4 schedulers per SM, <= 1 warp instruction per cycle each
 
 
@@ -317,7 +317,7 @@ def main():
     dom = max(step_acc, key=step_acc.get)
     roof = {"kernel": dom, "ms": step_acc[dom], "share_of_step": step_acc[dom] / total_step_ms,
             "traffic": NCU_TRAFFIC_BYTES_CONFIG3.get(dom) if (cid == 3 and args.seed == 1 and not args.frame_us) else None,
-            "traffic_source": "profiles/r01d_ncu_full_config3.md (dram read + write bytes per launch)"}
+            "traffic_source": "profiles/r01e_ncu_full_config3.md (dram read + write bytes per launch)"}
     roof.update({k: v for k, v in kernels[dom].items() if k not in ("ms", "share_of_step")})
     roof["peak_source"] = alu_src if roof.get("bound") == "alu" else peak_src
     if "bound" not in roof:

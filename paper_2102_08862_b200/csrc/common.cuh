@@ -35,13 +35,13 @@ struct Consts {
 // superset of the hits with time in [t_lo, t_hi].  The grid only accelerates; every decision is re-made by
 // the exact fp32 predicate on the candidates.
 __device__ __forceinline__ int time_bin(float t, const Consts& c) {
-  int b = (int)floorf(t * c.inv_bin_w);
+  int b = __float2int_rd(t * c.inv_bin_w);         // = (int)floorf(.) in one instruction
   return min(max(b, 0), c.n_tb - 1);
 }
 
 // Grid pad bin of a local y in a row (yoff, pscale of that row): monotone non-decreasing in y for the same reason.
 __device__ __forceinline__ int pad_bin(float y, float yoff, float pscale, const Consts& c) {
-  int b = (int)floorf((y + yoff) * pscale);
+  int b = __float2int_rd((y + yoff) * pscale);
   return min(max(b, 0), c.n_pb - 1);
 }
 
