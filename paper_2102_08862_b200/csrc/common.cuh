@@ -29,6 +29,7 @@ struct Consts {
   const int* npads;                      // [n_rows]
   const float* yoff;                     // [n_rows] half width of the row in cm: pad bin = floor((y + yoff) * pscale)
   const float* pscale;                   // [n_rows] n_pb / (row width in cm)
+  const float4* rowtab;                  // [n_rows] (n_pads - 0.5, cr, yoff, pscale): one 16-byte load per cluster in the ingest
 };
 
 // Grid bin of a time value: monotone non-decreasing in t, so a lookup over [bin(t_lo), bin(t_hi)] is a

@@ -16,9 +16,12 @@
 
 namespace tpc {
 
-constexpr int kRadixThreads = 256;
+#ifndef TPC_RADIX_THREADS
+#define TPC_RADIX_THREADS 256
+#endif
+constexpr int kRadixThreads = TPC_RADIX_THREADS;
 constexpr int kRadixItems = 8;
-constexpr int kRadixTile = kRadixThreads * kRadixItems;   // 2048
+constexpr int kRadixTile = kRadixThreads * kRadixItems;   // 2048 (256 threads) or 4096 (512)
 constexpr int kRadixMaxBits = 8;
 constexpr int kRadixBuckets = 1 << kRadixMaxBits;
 constexpr size_t kRadixScatterSmem = (size_t)kRadixTile * 16 + (size_t)(kRadixThreads / 32 + 2) * kRadixBuckets * 4;
@@ -32,9 +35,10 @@ __device__ __forceinline__ uint32_t cluster_key(float rf, float pad, float time,
   // r = sr mod n_rows without an integer division: sr < 2^16 and n_rows <= 160, so (sr + 0.5) / n_rows is at least
   // 0.003 away from an integer while the fp32 product is off by < 1e-4
   const int r = sr - (int)(((float)sr + 0.5f) * c.inv_n_rows) * c.n_rows;
-  const bool ok = ok_row && pad >= -0.5f && pad < (float)__ldg(c.npads + r) - 0.5f && time >= 0.0f && time <= c.max_time;
-  y = ok ? (pad - __ldg(c.cr + r)) * c.P : 0.0f;                       // y(h) = (pad - c_r) * P
-  const uint32_t key = (uint32_t)((sr * c.n_pb + pad_bin(y, __ldg(c.yoff + r), __ldg(c.pscale + r), c)) * c.n_tb + time_bin(time, c));
+  const float4 rt = __ldg(c.rowtab + r);                                // (n_pads - 0.5 [exact in fp32], c_r, yoff, pscale)
+  const bool ok = ok_row && pad >= -0.5f && pad < rt.x && time >= 0.0f && time <= c.max_time;
+  y = ok ? (pad - rt.y) * c.P : 0.0f;                                   // y(h) = (pad - c_r) * P
+  const uint32_t key = (uint32_t)((sr * c.n_pb + pad_bin(y, rt.z, rt.w, c)) * c.n_tb + time_bin(time, c));
   return ok ? key : (uint32_t)c.n_bins;
 }
 

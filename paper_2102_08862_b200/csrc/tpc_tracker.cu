@@ -240,14 +240,18 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
   }
   int n_dev = 0;
   if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) { cudaGetLastError(); delete t; return TPC_ECUDA; }
-  const size_t tab_bytes = (size_t)nr * 20;
+  const size_t rowtab_off = ((size_t)nr * 20 + 15) / 16 * 16;      // float4 (npads - 0.5, cr, yoff, pscale) per row, for the ingest key
+  const size_t tab_bytes = rowtab_off + (size_t)nr * 16;
+  std::vector<float> rowtab((size_t)nr * 4);
+  for (int r = 0; r < nr; ++r) { rowtab[4 * r] = (float)npads[r] - 0.5f; rowtab[4 * r + 1] = cr[r]; rowtab[4 * r + 2] = yoff[r]; rowtab[4 * r + 3] = pscale[r]; }
   if (cudaMalloc(&t->tables, tab_bytes) != cudaSuccess) { cudaGetLastError(); delete t; return TPC_ECUDA; }
   char* tb = static_cast<char*>(t->tables);
   if (cudaMemcpy(tb, xr.data(), (size_t)nr * 4, cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaMemcpy(tb + (size_t)nr * 4, cr.data(), (size_t)nr * 4, cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaMemcpy(tb + (size_t)nr * 8, npads.data(), (size_t)nr * 4, cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaMemcpy(tb + (size_t)nr * 12, yoff.data(), (size_t)nr * 4, cudaMemcpyHostToDevice) != cudaSuccess ||
-      cudaMemcpy(tb + (size_t)nr * 16, pscale.data(), (size_t)nr * 4, cudaMemcpyHostToDevice) != cudaSuccess) {
+      cudaMemcpy(tb + (size_t)nr * 16, pscale.data(), (size_t)nr * 4, cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemcpy(tb + rowtab_off, rowtab.data(), (size_t)nr * 16, cudaMemcpyHostToDevice) != cudaSuccess) {
     cudaGetLastError(); cudaFree(t->tables); delete t; return TPC_ECUDA;
   }
 
@@ -274,6 +278,7 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
   c.npads = reinterpret_cast<const int*>(tb + (size_t)nr * 8);
   c.yoff = reinterpret_cast<const float*>(tb + (size_t)nr * 12);
   c.pscale = reinterpret_cast<const float*>(tb + (size_t)nr * 16);
+  c.rowtab = reinterpret_cast<const float4*>(tb + rowtab_off);
 
   t->profile = p->profile != 0;
   if (cudaFuncSetAttribute(k_radix_scatter<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRadixScatterSmem) != cudaSuccess ||

@@ -107,10 +107,10 @@ def test_invalid_clusters_are_ignored_and_flagged():
     assert o.stats["invalid_clusters"] > 500
 
 
-@pytest.mark.parametrize("copies", [2, 6])
+@pytest.mark.parametrize("copies", [2, 6, 9])
 def test_duplicate_hits_tie_break_on_original_index(copies):
     """Exact duplicates of whole tracks: every chi2 / distance tie must go to the lowest original index
-    (6 copies also overflow the finder's 4 candidate slots per row -> generic path)."""
+    (6 copies fill the finder's 6 candidate slots per row exactly, 9 overflow them -> generic path)."""
     rows = np.arange(N_ROWS)
     x = row_x(rows)
     parts = []
