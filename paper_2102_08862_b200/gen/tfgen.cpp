@@ -131,7 +131,7 @@ namespace {
 
 void gen_collision(const tfgen_config& c, const Collision& col, int32_t icol,
                    const std::vector<double>& xr, const std::vector<int>& npads,
-                   std::vector<Cluster>& out, tfgen_track* tracks) {
+                   std::vector<Cluster>& out, tfgen_track* tracks, double t_max) {
   const int n_phi_sectors = (c.n_sectors == 1) ? 1 : 18;
   const double two_pi = 2.0 * kPi;
   const double half = c.half_sector_deg * kPi / 180.0;
@@ -176,9 +176,11 @@ void gen_collision(const tfgen_config& c, const Collision& col, int32_t icol,
             const double ys = y + c.sigma_y_cm * gy;
             const double padf = ys / c.pad_pitch_cm + 0.5 * (npads[r] - 1);
             if (!(padf >= -0.5 && padf < npads[r] - 0.5)) continue;
+            // the tracker tests the fp32 values: a pad that rounds up onto the row's edge is outside the row
+            if (!((float)padf >= -0.5f && (float)padf < (float)npads[r] - 0.5f)) continue;
             const double drift = c.drift_len_cm - std::fabs(z) + c.sigma_z_cm * gz;
             const double tb = (col.t0_us * c.v_drift_cm_us + drift) / c.time_bin_cm;
-            if (!(tb >= 0.0)) continue;
+            if (!(tb >= 0.0 && (float)tb <= (float)t_max)) continue;      // beyond the frame's last time bin (> 4 sigma): not read out
             const int sector = (c.n_sectors == 1) ? 0 : (z >= 0 ? sec : 18 + sec);
             Cluster cl;
             cl.row = (float)(sector * c.n_rows + r);
@@ -251,7 +253,7 @@ int tfgen_generate(const tfgen_config* cfg, tfgen_frame** out_frame) {
       for (;;) {
         size_t i = next.fetch_add(1);
         if (i >= cols.size()) break;
-        gen_collision(c, cols[i], (int32_t)i, xr, npads, per_col[i], f->tracks.data());
+        gen_collision(c, cols[i], (int32_t)i, xr, npads, per_col[i], f->tracks.data(), f->max_time_bin);
       }
     };
     std::vector<std::thread> th;
