@@ -1,0 +1,182 @@
+// ORACLE -- TEST INFRASTRUCTURE ONLY.  Plain single-threaded C++ fp32 CPU implementation of step C7:
+// merging of the per-sector TPC tracks of C6 across SECTOR BOUNDARIES (first half:
+// the linking of track pieces; the global refit of a merged chain is not part of this step).
+//
+// What it follows:
+//   * PAPER.md L23 / L25: "full TPC tracking"; the per-sector tracker (Run 2 HLT design) is followed by a
+//     merger of the sector tracks.  The paper gives no listing and no cuts, so every definition below is a
+//     reading of this build, listed as M1..M8 in DESIGN.md §3 ("C7").
+//   * BASELINE.json L8: 36 sectors, A side 0-17, C side 18-35, 20 degree slices, each in its rotated local frame.
+// It is a HEURISTIC (greedy reciprocal best match), followed step by step; all decisions in fp32, one rounded
+// operation per statement, evaluated left to right, built with -O2 -ffp-contract=off.
+//
+// Definition (notation of DESIGN.md §3; a track is (sector S, first_row f, last_row l, seed id, state
+// (x; y, z, s, t, k) at its innermost point, time_ref)):
+//   Cd = (1 - T^2) / (1 + T^2), Sd = 2 T / (1 + T^2) with T = tan_half_sector: cos / sin of the sector angle,
+//   derived in double from the fp32 geometry value and rounded once (no libm).
+//   For a track A and a side sg in {+1, -1}, the neighbour sector is S' = side(S)*18 + ((S mod 18) + sg) mod 18;
+//   A's state in the frame of S' (rotation by sg * 20 degrees about the beam axis):
+//       c  = sqrtf(1 - s*s)
+//       x1 = x*Cd + sg*(y*Sd);   y1 = y*Cd - sg*(x*Sd);   s1 = s*Cd - sg*(c*Sd)       (z, t, k unchanged)
+//       skip the side unless |s1| < sin_phi_max
+//   A candidate continuation is a track B in S' with  f_B > f_A  and  l_A + 1 - overlap <= f_B <= l_A + 1 + gap.
+//   The rotated state is transported to x_B with the state part of the C5 transport (exact circle, 3-term arc
+//   length series; FAIL -> no candidate), giving (y2, z2, s2); then
+//       dy = y2 - y_B;  dz = (z2 - z_B) + (time_ref_A - time_ref_B)*Z;  ds = s2 - s_B;  dk = k_A - k_B
+//       require |dy| < cut_y, |dz| < cut_z, |ds| < cut_s, |dk| < cut_k
+//       d2 = (dy*dy)*wy + (dz*dz)*wz + (ds*ds)*ws + (dk*dk)*wk            w = (float)(1 / cut^2), from double
+//   out[A] = the candidate with the smallest d2 over both sides (ties -> smallest seed id of B);
+//   in[B]  = the A with the smallest d2(A, B) among all A that have B as a candidate (ties -> smallest seed id of A).
+//   A and B are LINKED (next[A] = B, prev[B] = A) iff out[A] == B and in[B] == A.
+//   root[i] = the first piece of i's chain (follow prev).  A geometry with fewer than 18 sectors has no neighbours.
+//
+// Pins (tests/test_merge_oracle_pins.py): M-R rotation against the double-precision helix in global coordinates
+// and there-and-back identity; M-H noise-free helices crossing one or two boundaries are linked into one chain
+// and nothing else is linked; M-I invariants (reciprocity, adjacency, row order, acyclic); M-E link efficiency and
+// purity against generator truth on configs[1].  Parity unpinned: the values of the cuts themselves.
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load this.  It
+// shares no code, header, table or constant generator with the CUDA path.
+#include <cmath>
+#include <cstdint>
+#include <vector>
+
+extern "C" {
+
+struct orc_merge_params {
+  int32_t n_sectors;
+  float tan_half_sector, time_bin_cm;
+  float sin_phi_max, inv_R_per_qpt;
+  float cut_y_cm, cut_z_cm, cut_sin_phi, cut_q_pt;
+  int32_t max_row_gap, max_row_overlap;
+};
+
+}  // extern "C"
+
+namespace {
+
+struct St { float x, y, z, s, t, k; };
+
+// State part of the C5 transport: same statements, same order; false = FAIL (state unchanged).
+bool transport_state(St& S, float xn, float cB, float sin_phi_max) {
+  const float dx = xn - S.x;
+  const float kc = cB * S.k;
+  const float sn = S.s + kc * dx;
+  if (!(std::fabs(sn) < sin_phi_max)) return false;
+  const float c = std::sqrt(1.0f - S.s * S.s);
+  const float cn = std::sqrt(1.0f - sn * sn);
+  const float ss = S.s + sn;
+  const float cc = c + cn;
+  const float icc = 1.0f / cc;
+  const float T = ss * icc;
+  const float q = 1.0f + T * T;
+  const float rq = std::sqrt(q);
+  const float u = kc * dx;
+  const float a = (u * u) * q;
+  const float dS = (dx * rq) * (1.0f + a * (0.041666668f + a * (0.0046875f + a * 0.00069754466f)));
+  S.y = S.y + dx * T;
+  S.z = S.z + S.t * dS;
+  S.s = sn;
+  S.x = xn;
+  return true;
+}
+
+struct Consts { float Cd, Sd, wy, wz, ws, wk; };
+
+Consts derive(const orc_merge_params& p) {
+  const double T = (double)p.tan_half_sector;
+  Consts c;
+  c.Cd = (float)((1.0 - T * T) / (1.0 + T * T));
+  c.Sd = (float)(2.0 * T / (1.0 + T * T));
+  c.wy = (float)(1.0 / ((double)p.cut_y_cm * (double)p.cut_y_cm));
+  c.wz = (float)(1.0 / ((double)p.cut_z_cm * (double)p.cut_z_cm));
+  c.ws = (float)(1.0 / ((double)p.cut_sin_phi * (double)p.cut_sin_phi));
+  c.wk = (float)(1.0 / ((double)p.cut_q_pt * (double)p.cut_q_pt));
+  return c;
+}
+
+// Rotation of a state into the neighbour frame on side sg (+1 / -1).
+St rotate(const St& A, float sg, const Consts& c) {
+  St R = A;
+  const float cs = std::sqrt(1.0f - A.s * A.s);
+  R.x = A.x * c.Cd + sg * (A.y * c.Sd);
+  R.y = A.y * c.Cd - sg * (A.x * c.Sd);
+  R.s = A.s * c.Cd - sg * (cs * c.Sd);
+  return R;
+}
+
+}  // namespace
+
+extern "C" {
+
+// par: [n*7] = (x, y, z_rel, sin_phi, dzds, q_pt, time_ref) as written by the tracker / orc_copy_tracks.
+// next, prev, root: [n] track indices (-1 = none; root[i] = i for an unmerged track).  Returns the number of links.
+int64_t orc_merge(const orc_merge_params* pp, int64_t n, const int32_t* seed, const int32_t* sector,
+                  const int32_t* first_row, const int32_t* last_row, const float* par,
+                  int32_t* next, int32_t* prev, int32_t* root, float* best_d2_out) {
+  const orc_merge_params& p = *pp;
+  const Consts c = derive(p);
+  std::vector<int32_t> out(n, -1), in(n, -1);
+  std::vector<float> d_out(n, 0.0f), d_in(n, 0.0f);
+  if (p.n_sectors >= 18) {
+    for (int64_t a = 0; a < n; ++a) {
+      const float* pa = par + 7 * a;
+      const St A{pa[0], pa[1], pa[2], pa[3], pa[4], pa[5]};
+      const int32_t side = sector[a] / 18, phi = sector[a] % 18;
+      for (int isg = 0; isg < 2; ++isg) {
+        const float sg = isg == 0 ? 1.0f : -1.0f;
+        const int32_t nb = side * 18 + (phi + (isg == 0 ? 1 : 17)) % 18;
+        if (nb >= p.n_sectors) continue;
+        const St R = rotate(A, sg, c);
+        if (!(std::fabs(R.s) < p.sin_phi_max)) continue;
+        for (int64_t b = 0; b < n; ++b) {            // brute force over all tracks: the definition, nothing else
+          if (sector[b] != nb) continue;
+          if (!(first_row[b] > first_row[a])) continue;
+          if (first_row[b] < last_row[a] + 1 - p.max_row_overlap || first_row[b] > last_row[a] + 1 + p.max_row_gap) continue;
+          const float* pb = par + 7 * b;
+          St S = R;
+          if (!transport_state(S, pb[0], p.inv_R_per_qpt, p.sin_phi_max)) continue;
+          const float dy = S.y - pb[1];
+          const float dz = (S.z - pb[2]) + (pa[6] - pb[6]) * p.time_bin_cm;
+          const float ds = S.s - pb[3];
+          const float dk = A.k - pb[5];
+          if (!(std::fabs(dy) < p.cut_y_cm && std::fabs(dz) < p.cut_z_cm && std::fabs(ds) < p.cut_sin_phi &&
+                std::fabs(dk) < p.cut_q_pt)) continue;
+          const float d2 = (dy * dy) * c.wy + (dz * dz) * c.wz + (ds * ds) * c.ws + (dk * dk) * c.wk;
+          if (out[a] < 0 || d2 < d_out[a] || (d2 == d_out[a] && (uint32_t)seed[b] < (uint32_t)seed[out[a]])) { out[a] = (int32_t)b; d_out[a] = d2; }
+          if (in[b] < 0 || d2 < d_in[b] || (d2 == d_in[b] && (uint32_t)seed[a] < (uint32_t)seed[in[b]])) { in[b] = (int32_t)a; d_in[b] = d2; }
+        }
+      }
+    }
+  }
+  int64_t n_links = 0;
+  for (int64_t i = 0; i < n; ++i) { next[i] = -1; prev[i] = -1; }
+  for (int64_t a = 0; a < n; ++a) {
+    const int32_t b = out[a];
+    if (b >= 0 && in[b] == (int32_t)a) { next[a] = b; prev[b] = (int32_t)a; ++n_links; }
+    if (best_d2_out) best_d2_out[a] = out[a] >= 0 ? d_out[a] : -1.0f;
+  }
+  for (int64_t i = 0; i < n; ++i) {
+    int32_t r = (int32_t)i;
+    while (prev[r] >= 0) r = prev[r];             // first_row strictly increases along a chain: no cycles
+    root[i] = r;
+  }
+  return n_links;
+}
+
+// Pin helpers: the rotation and the state-only transport on their own.  st = (x, y, z, s, t, k).
+void orc_merge_rotate(const orc_merge_params* p, float* st, int32_t side_sign) {
+  const Consts c = derive(*p);
+  const St A{st[0], st[1], st[2], st[3], st[4], st[5]};
+  const St R = rotate(A, side_sign >= 0 ? 1.0f : -1.0f, c);
+  st[0] = R.x; st[1] = R.y; st[2] = R.z; st[3] = R.s; st[4] = R.t; st[5] = R.k;
+}
+
+int orc_merge_transport(const orc_merge_params* p, float* st, float xn) {
+  St S{st[0], st[1], st[2], st[3], st[4], st[5]};
+  const bool ok = transport_state(S, xn, p->inv_R_per_qpt, p->sin_phi_max);
+  st[0] = S.x; st[1] = S.y; st[2] = S.z; st[3] = S.s; st[4] = S.t; st[5] = S.k;
+  return ok ? 1 : 0;
+}
+
+}  // extern "C"

@@ -1,0 +1,166 @@
+"""Pins of the C7 oracle (oracle/tpc_merge_oracle.cpp: sector-boundary merging of the per-sector tracks).
+
+The paper prints no worked example of the merger (PAPER.md L23/L25 only name "full TPC tracking"), so the pins are
+what geometry and the generator's truth fix: M-R the rotation against the double-precision helix in GLOBAL
+coordinates, M-T the state-only transport against the (separately pinned, K1) full transport, M-H noise-free helices
+that cross sector boundaries, M-I invariants, M-P independence of the input order, M-E efficiency / purity.
+"""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import merge as M
+from paper_2102_08862_b200 import gen
+
+import merge_eval as ME
+
+CB = 1.0 / 666.7
+
+
+def _local(X, Y, Phi, alpha):
+    """Global point / direction -> local frame of a sector whose axis points at angle alpha (generator convention)."""
+    return (X * math.cos(alpha) + Y * math.sin(alpha), -X * math.sin(alpha) + Y * math.cos(alpha), math.sin(Phi - alpha))
+
+
+@pytest.mark.parametrize("side_sign", [1, -1])
+@pytest.mark.parametrize("Phi_deg,k", [(35.0, 1.7), (52.0, -0.8), (41.0, 0.0), (28.0, 3.1)])
+def test_MR_rotation_matches_the_global_frame(side_sign, Phi_deg, k):
+    p = M.default_merge_params()
+    alpha = math.radians(30.0)                       # sector 1; neighbours at 50 and 10 degrees
+    alpha2 = alpha + side_sign * math.radians(20.0)
+    Phi = math.radians(Phi_deg)
+    # a point near the sector edge on that side, 150 cm from the beam axis
+    ang = alpha + side_sign * math.radians(9.0)
+    X, Y = 150.0 * math.cos(ang), 150.0 * math.sin(ang)
+    x, y, s = _local(X, Y, Phi, alpha)
+    st = M.rotate(p, [x, y, 12.5, s, 0.3, k], side_sign)
+    x2, y2, s2 = _local(X, Y, Phi, alpha2)
+    assert abs(st[0] - x2) < 2e-4 and abs(st[1] - y2) < 2e-4 and abs(st[3] - s2) < 2e-6
+    assert st[2] == np.float32(12.5) and st[4] == np.float32(0.3) and st[5] == np.float32(k)      # z, t, k unchanged
+    # there and back
+    back = M.rotate(p, st, -side_sign)
+    assert abs(back[0] - x) < 2e-4 and abs(back[1] - y) < 2e-4 and abs(back[3] - s) < 2e-6
+    # the rotated state, transported, stays on the SAME circle: compare with the exact circle in the new frame (double)
+    xn = x2 + 9.0
+    ok, tr = M.transport_state(p, st, xn)
+    assert ok
+    kc = CB * k
+    sn = s2 + kc * (xn - x2)
+    if k == 0.0:
+        y_exact = y2 + (xn - x2) * s2 / math.sqrt(1 - s2 * s2)
+        arc = (xn - x2) / math.sqrt(1 - s2 * s2)
+    else:
+        y_exact = y2 + (math.sqrt(1 - s2 * s2) - math.sqrt(1 - sn * sn)) / kc
+        arc = (math.asin(sn) - math.asin(s2)) / kc
+    assert abs(tr[1] - y_exact) < 3e-4 and abs(tr[3] - sn) < 2e-6 and abs(tr[2] - (12.5 + 0.3 * arc)) < 3e-4
+
+
+def test_MR_sector_angle_constants_are_twenty_degrees():
+    """Cd, Sd come from tan(10 deg) without libm: rotating (1, 0) must give (cos 20, -sin 20)."""
+    p = M.default_merge_params()
+    st = M.rotate(p, [1.0, 0.0, 0.0, 0.0, 0.0, 0.0], 1)
+    assert abs(st[0] - math.cos(math.radians(20.0))) < 1e-7 and abs(st[1] + math.sin(math.radians(20.0))) < 1e-7
+    assert abs(st[3] + math.sin(math.radians(20.0))) < 1e-7
+
+
+def test_MT_state_transport_is_the_state_part_of_the_C5_transport():
+    rng = np.random.default_rng(5)
+    p = M.default_merge_params()
+    tp = oracle.default_params()
+    n_ok = 0
+    for _ in range(400):
+        s0 = rng.uniform(-0.9, 0.9)
+        st = [rng.uniform(85, 240), rng.uniform(-30, 30), rng.uniform(-50, 50), s0, rng.uniform(-1.2, 1.2), rng.uniform(-6, 6)]
+        xn = st[0] + rng.uniform(-60, 60)
+        ok_m, a = M.transport_state(p, st, xn)
+        ok_f, b, _ = oracle.transport(tp, st, [1, 0, 0.1, 0, 0, 100, 1, 0, 0.1], xn)
+        assert ok_m == ok_f
+        np.testing.assert_array_equal(a, b)
+        n_ok += ok_m
+    assert n_ok > 200
+
+
+_cache = {}
+
+
+def _tracked(cid, seed, **kw):
+    key = (cid, seed, tuple(sorted(kw.items())))
+    if key not in _cache:
+        c = gen.preset(cid, seed)
+        for k, v in kw.items():
+            setattr(c, k, v)
+        tf = gen.generate(c)
+        res = oracle.track(oracle.default_geometry(36, tf.max_time_bin), oracle.default_params(max(c.sigma_y_cm, 0.08), max(c.sigma_z_cm, 0.12)),
+                           tf.row, tf.pad, tf.time)
+        mr = M.merge(M.default_merge_params(36), res.tr_seed, res.tr_sector, res.tr_first_row, res.tr_last_row, res.tr_par)
+        _cache[key] = (tf, res, mr)
+    return _cache[key]
+
+
+def _evaluate(tf, res, mr):
+    keys = ME.track_truth_keys(tf, res.tr_hit_offset, res.tr_n_hits, res.tr_hit_index)
+    return ME.evaluate_links(keys, res.tr_sector, res.tr_first_row, res.tr_last_row, mr.next)
+
+
+def test_MH_noise_free_helices_crossing_boundaries_are_linked_and_nothing_else():
+    tf, res, mr = _tracked(1, 4, fixed_tracks=600, sigma_y_cm=0.0, sigma_z_cm=0.0, dropout=0.0, noise_frac=0.0, pt_min=0.15)
+    rep = _evaluate(tf, res, mr)
+    assert rep["expected"] >= 150, rep
+    assert rep["got"] == rep["expected"], rep
+    assert rep["wrong"] == 0, rep
+    # chains: a particle crossing two boundaries gives a chain of three pieces with one root
+    assert (np.bincount(mr.root, minlength=len(mr.root)) >= 3).any()
+
+
+@pytest.mark.parametrize("seed", [1, 2])
+def test_MI_invariants(seed):
+    tf, res, mr = _tracked(1, seed)
+    n = len(res.tr_seed)
+    a = np.where(mr.next >= 0)[0]
+    b = mr.next[a]
+    assert mr.n_links == a.size and mr.n_links > 1000
+    np.testing.assert_array_equal(mr.prev[b], a)                                   # reciprocal
+    assert np.unique(b).size == b.size                                             # a track continues at most one track
+    sa, sb = res.tr_sector[a], res.tr_sector[b]
+    assert np.all(sa // 18 == sb // 18) and np.all(np.isin((sa % 18 - sb % 18) % 18, (1, 17)))   # adjacent, same side
+    assert np.all(res.tr_first_row[b] > res.tr_first_row[a])
+    assert np.all(res.tr_first_row[b] >= res.tr_last_row[a] - 1) and np.all(res.tr_first_row[b] <= res.tr_last_row[a] + 13)
+    # roots: fixed points of prev, and every chain member points at its chain's first piece
+    assert np.all(mr.prev[mr.root] == -1)
+    np.testing.assert_array_equal(mr.root[b], mr.root[a])
+    np.testing.assert_array_equal(mr.root[np.where(mr.prev < 0)[0]], np.where(mr.prev < 0)[0])
+    assert n - mr.n_links == np.unique(mr.root).size                               # merged tracks = tracks - links
+
+
+def test_MP_result_does_not_depend_on_the_input_order():
+    tf, res, mr = _tracked(1, 1)
+    n = len(res.tr_seed)
+    perm = np.random.default_rng(11).permutation(n)
+    m2 = M.merge(M.default_merge_params(36), res.tr_seed[perm], res.tr_sector[perm], res.tr_first_row[perm],
+                 res.tr_last_row[perm], res.tr_par[perm])
+    seed_next = np.where(mr.next >= 0, res.tr_seed[np.maximum(mr.next, 0)], -1)
+    seed_next2 = np.where(m2.next >= 0, res.tr_seed[perm][np.maximum(m2.next, 0)], -1)
+    np.testing.assert_array_equal(seed_next[perm], seed_next2)
+
+
+@pytest.mark.parametrize("seed", [1, 2])
+def test_ME_link_efficiency_and_purity_on_config1(seed):
+    tf, res, mr = _tracked(1, seed)
+    rep = _evaluate(tf, res, mr)
+    assert rep["expected"] >= 2000, rep
+    assert rep["efficiency"] >= 0.97, rep
+    assert rep["wrong_rate"] <= 0.02, rep
+
+
+def test_degenerate_inputs():
+    p = M.default_merge_params(36)
+    e = M.merge(p, [], [], [], [], np.zeros((0, 7), np.float32))
+    assert e.n_links == 0 and e.next.size == 0
+    # a single-sector geometry has no neighbours
+    tf, res, mr = _tracked(1, 1)
+    one = M.merge(M.default_merge_params(1), res.tr_seed, np.zeros_like(res.tr_sector), res.tr_first_row, res.tr_last_row, res.tr_par)
+    assert one.n_links == 0 and np.all(one.next == -1) and np.array_equal(one.root, np.arange(len(res.tr_seed)))
