@@ -20,7 +20,8 @@ _LIB = os.path.join(_HERE, "libtpcmergeoracle.so")
 
 
 class MergeParams(C.Structure):
-    _fields_ = [("n_sectors", C.c_int32), ("tan_half_sector", C.c_float), ("time_bin_cm", C.c_float),
+    _fields_ = [("n_sectors", C.c_int32), ("x0_cm", C.c_float), ("row_pitch_cm", C.c_float),
+                ("tan_half_sector", C.c_float), ("time_bin_cm", C.c_float),
                 ("sin_phi_max", C.c_float), ("inv_R_per_qpt", C.c_float),
                 ("cut_y_cm", C.c_float), ("cut_z_cm", C.c_float), ("cut_sin_phi", C.c_float), ("cut_q_pt", C.c_float),
                 ("max_row_gap", C.c_int32), ("max_row_overlap", C.c_int32)]
@@ -28,7 +29,7 @@ class MergeParams(C.Structure):
 
 def default_merge_params(n_sectors: int = 36) -> MergeParams:
     """DESIGN.md §3 C7 readings M4/M5: cuts 2 cm, 2 cm, 0.05, 0.5 (GeV/c)^-1; rows l_A - 1 .. l_A + 13."""
-    return MergeParams(n_sectors, math.tan(math.radians(10.0)), 0.516, 0.95, 1.0 / 666.7,
+    return MergeParams(n_sectors, 85.0, 1.07, math.tan(math.radians(10.0)), 0.516, 0.95, 1.0 / 666.7,
                        2.0, 2.0, 0.05, 0.5, 12, 2)
 
 

@@ -19,7 +19,8 @@
 //       c  = sqrtf(1 - s*s)
 //       x1 = x*Cd + sg*(y*Sd);   y1 = y*Cd - sg*(x*Sd);   s1 = s*Cd - sg*(c*Sd)       (z, t, k unchanged)
 //       skip the side unless |s1| < sin_phi_max
-//   A candidate continuation is a track B in S' with  f_B > f_A  and  l_A + 1 - overlap <= f_B <= l_A + 1 + gap.
+//   r_B = (int)floorf((x_B - x0) / pitch + 0.5f) is the pad row B's state sits on (its innermost tracklet hit; r_B <= f_B).
+//   A candidate continuation is a track B in S' with  r_B > f_A  and  l_A + 1 - overlap <= r_B <= l_A + 1 + gap.
 //   The rotated state is transported to x_B with the state part of the C5 transport (exact circle, 3-term arc
 //   length series; FAIL -> no candidate), giving (y2, z2, s2); then
 //       dy = y2 - y_B;  dz = (z2 - z_B) + (time_ref_A - time_ref_B)*Z;  ds = s2 - s_B;  dk = k_A - k_B
@@ -45,6 +46,7 @@ extern "C" {
 
 struct orc_merge_params {
   int32_t n_sectors;
+  float x0_cm, row_pitch_cm;
   float tan_half_sector, time_bin_cm;
   float sin_phi_max, inv_R_per_qpt;
   float cut_y_cm, cut_z_cm, cut_sin_phi, cut_q_pt;
@@ -131,9 +133,10 @@ int64_t orc_merge(const orc_merge_params* pp, int64_t n, const int32_t* seed, co
         if (!(std::fabs(R.s) < p.sin_phi_max)) continue;
         for (int64_t b = 0; b < n; ++b) {            // brute force over all tracks: the definition, nothing else
           if (sector[b] != nb) continue;
-          if (!(first_row[b] > first_row[a])) continue;
-          if (first_row[b] < last_row[a] + 1 - p.max_row_overlap || first_row[b] > last_row[a] + 1 + p.max_row_gap) continue;
           const float* pb = par + 7 * b;
+          const int32_t rb = (int32_t)std::floor((pb[0] - p.x0_cm) / p.row_pitch_cm + 0.5f);
+          if (!(rb > first_row[a])) continue;
+          if (rb < last_row[a] + 1 - p.max_row_overlap || rb > last_row[a] + 1 + p.max_row_gap) continue;
           St S = R;
           if (!transport_state(S, pb[0], p.inv_R_per_qpt, p.sin_phi_max)) continue;
           const float dy = S.y - pb[1];
@@ -158,7 +161,7 @@ int64_t orc_merge(const orc_merge_params* pp, int64_t n, const int32_t* seed, co
   }
   for (int64_t i = 0; i < n; ++i) {
     int32_t r = (int32_t)i;
-    while (prev[r] >= 0) r = prev[r];             // first_row strictly increases along a chain: no cycles
+    while (prev[r] >= 0) r = prev[r];             // r_B > f_A >= r_A: state rows strictly increase along a chain, no cycles
     root[i] = r;
   }
   return n_links;

@@ -127,8 +127,9 @@ def test_MI_invariants(seed):
     assert np.unique(b).size == b.size                                             # a track continues at most one track
     sa, sb = res.tr_sector[a], res.tr_sector[b]
     assert np.all(sa // 18 == sb // 18) and np.all(np.isin((sa % 18 - sb % 18) % 18, (1, 17)))   # adjacent, same side
-    assert np.all(res.tr_first_row[b] > res.tr_first_row[a])
-    assert np.all(res.tr_first_row[b] >= res.tr_last_row[a] - 1) and np.all(res.tr_first_row[b] <= res.tr_last_row[a] + 13)
+    rb = np.rint((res.tr_par[b, 0].astype(np.float64) - 85.0) / 1.07).astype(np.int64)     # row the state of B sits on
+    assert np.all(rb <= res.tr_first_row[b]) and np.all(rb > res.tr_first_row[a])
+    assert np.all(rb >= res.tr_last_row[a] - 1) and np.all(rb <= res.tr_last_row[a] + 13)
     # roots: fixed points of prev, and every chain member points at its chain's first piece
     assert np.all(mr.prev[mr.root] == -1)
     np.testing.assert_array_equal(mr.root[b], mr.root[a])
