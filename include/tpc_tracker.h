@@ -172,6 +172,41 @@ int tpc_tracker_arena_plan(const tpc_tracker_t* tracker, int32_t i, const char**
  * the decision arithmetic has to round like the definition, BASELINE.json L5).                              */
 int tpc_selftest_fast_math(void* cuda_stream, uint64_t* mismatches_out);
 
+/* ---- C7: sector-boundary merging of the per-sector tracks (DESIGN.md §3 "C7", readings M1..M8; PAPER.md L23 / L25:
+ * "full TPC tracking" -- the sector tracker is followed by a merger of the sector tracks; BASELINE.json L8: 36 sectors,
+ * each in its rotated local frame).  A widening step after the hot path (linking only: the
+ * refit of a merged chain and central-electrode crossings are not part of it).                                  */
+typedef struct {
+  float cut_y_cm, cut_z_cm;         /* 2, 2     : |dy|, |dz| between the extrapolated inner piece and the outer piece   */
+  float cut_sin_phi, cut_q_pt;      /* 0.05, 0.5: |d sin phi|, |d q/pT| [c/GeV]                            (reading M4) */
+  int32_t max_row_gap;              /* 12 : the outer piece's state row r_B <= last_row_A + 1 + max_row_gap (reading M5) */
+  int32_t max_row_overlap;          /* 2  : r_B >= last_row_A + 1 - max_row_overlap                                     */
+} tpc_merge_params_t;
+
+/* Caller-allocated DEVICE buffers, [tracks->max_tracks] each (entries >= *n_tracks are -1).                       */
+typedef struct {
+  int32_t* next;     /* track index of the outer continuation of track i, -1 = none                               */
+  int32_t* prev;     /* track index of the inner piece that track i continues, -1 = none                          */
+  int32_t* root;     /* first piece of i's chain (i itself for an unmerged track)                                  */
+  int32_t* n_links;  /* scalar: number of links (merged tracks = *n_tracks - *n_links)                             */
+} tpc_merged_t;
+
+/* Bytes of the tracker's arena that tpc_merge_tracks uses for `max_tracks` tracks (host arithmetic; 0 = invalid).  */
+size_t tpc_merge_scratch_bytes(const tpc_tracker_t* tracker, int64_t max_tracks);
+
+/* Links the tracks that `tracks` (DEVICE buffers, as written by tpc_track_timeframe of THIS tracker: geometry, row
+ * table and curvature constant are the handle's) holds across sector boundaries of the same TPC side.  Asynchronous on
+ * `cuda_stream`; reads *tracks->n_tracks on the device; never allocates: its scratch is the handle's arena, whose
+ * tracking scratch is dead once tpc_track_timeframe has been enqueued on the same stream (the two calls must not
+ * overlap on different streams).  The result does not depend on the order of the tracks.
+ * Errors: TPC_EINVAL (null pointer, non-positive cut), TPC_ENOMEM (arena smaller than tpc_merge_scratch_bytes),
+ * TPC_ECUDA.                                                                                                     */
+int tpc_merge_tracks(tpc_tracker_t* tracker, const tpc_merge_params_t* merge_params, const tpc_tracks_t* tracks,
+                     void* cuda_stream, tpc_merged_t* merged_out);
+
+/* Number of kernel launches the last tpc_merge_tracks call enqueued (memsets not counted).                        */
+int64_t tpc_merge_last_launches(const tpc_tracker_t* tracker);
+
 int tpc_tracker_destroy(tpc_tracker_t* tracker);
 
 const char* tpc_strerror(int code);

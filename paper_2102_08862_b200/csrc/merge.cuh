@@ -1,0 +1,175 @@
+// C7 sector-boundary merging of the per-sector tracks (DESIGN.md §3 "C7", readings M1..M8; "full TPC
+// tracking" -- the per-sector tracker is followed by a merger of the sector tracks; BASELINE.json L8: 36 sectors, each in
+// its rotated local frame).
+//
+// A track A is rotated into the frame of each neighbour sector (same side, +-20 degrees), transported to every pad row
+// r_B of the row window, and compared with the tracks B of that sector whose state sits on row r_B: reciprocal best
+// match in d2 = dy^2 wy + dz^2 wz + ds^2 ws + dk^2 wk inside the four cuts, every tie -> lowest seed id.
+//
+// Layout: the tracks are binned by (sector, state row, 32-time-bin cell of the state's time) with a counting sort
+// (histogram -> exclusive scan -> fill); the candidate records (y, z_rel, sin phi, q/pT | time_ref, seed) are stored in
+// cell order, so the candidates of one (row, time window) are one contiguous span.  One thread per track A: two
+// rotations, one state transport per row of the window (it serves every candidate of that row), a few candidates per
+// row.  in[B] is a 64-bit atomicMin on (d2 bits, seed of A) -- d2 >= 0, so its bit pattern orders like its value -- and
+// out[A] the same key kept in a register: the result does not depend on the order in which candidates are met.
+// All decision arithmetic is fp32 in the written order (--fmad=false).
+#pragma once
+#include "common.cuh"
+
+namespace tpc {
+
+constexpr int kMergeThreads = 128;
+constexpr int kMergeCellTimeBins = 32;
+
+struct MergeConsts {
+  int n_sectors, n_rows, n_tcell, gap, overlap, max_tracks;
+  float x0, pitch, Cd, Sd, Z, inv_Z, cB, sin_phi_max;
+  float cut_y, cut_z, cut_s, cut_k, wy, wz, ws, wk;
+  float inv_cell, t_window;      // 1 / kMergeCellTimeBins; half width of the time lookup = cut_z / Z + 0.5 bins
+  const float* xr;               // [n_rows] x of the pad row (the handle's table)
+};
+
+struct MergeTracks {   // device pointers of tpc_tracks_t
+  const int32_t *n_tracks, *seed, *sector, *first_row, *last_row;
+  const float *x, *y, *z, *time_ref, *s, *t, *k;
+};
+
+struct MergeScratch {
+  uint32_t* cell_start;          // [n_cells + 1] histogram, then its exclusive scan
+  uint32_t* cell_cursor;         // [n_cells]
+  uint32_t* cell_of;             // [max_tracks]
+  uint32_t* cand_idx;            // [max_tracks] track index, in cell order
+  float4* cand_a;                // [max_tracks] (y, z_rel, sin phi, q/pT), in cell order
+  float2* cand_b;                // [max_tracks] (time_ref, seed as bits), in cell order
+  unsigned long long* out_key;   // [max_tracks] (d2 bits << 32 | seed of B) of out[A]; all ones = none
+  int32_t* out_b;                // [max_tracks]
+  unsigned long long* in_key;    // [max_tracks] (d2 bits << 32 | seed of A) of in[B]; all ones = none
+};
+
+__device__ __forceinline__ int merge_n(const MergeTracks& T, const MergeConsts& c) { return min(*T.n_tracks, c.max_tracks); }
+
+// State part of the C5 transport (same statements, same order as tracklet.cuh::transport).
+__device__ __forceinline__ bool merge_transport(float& x, float& y, float& z, float& s, float t, float k, float xn, float cB, float spm) {
+  const float dx = xn - x;
+  const float kc = cB * k;
+  const float sn = s + kc * dx;
+  if (!(fabsf(sn) < spm)) return false;
+  const float c = sqrtf(1.0f - s * s);
+  const float cn = sqrtf(1.0f - sn * sn);
+  const float ss = s + sn;
+  const float cc = c + cn;
+  const float icc = 1.0f / cc;
+  const float T = ss * icc;
+  const float q = 1.0f + T * T;
+  const float rq = sqrtf(q);
+  const float u = kc * dx;
+  const float a = (u * u) * q;
+  const float dS = (dx * rq) * (1.0f + a * (0.041666668f + a * (0.0046875f + a * 0.00069754466f)));
+  y = y + dx * T;
+  z = z + t * dS;
+  s = sn;
+  x = xn;
+  return true;
+}
+
+__device__ __forceinline__ int merge_time_cell(float t, const MergeConsts& c) {
+  return min(max(__float2int_rd(t * c.inv_cell), 0), c.n_tcell - 1);
+}
+
+// Row the state of a track sits on (reading M5) and its cell.
+__global__ void __launch_bounds__(256) k_merge_cell_count(MergeTracks T, MergeScratch S, const __grid_constant__ MergeConsts c) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= merge_n(T, c)) return;
+  int rb = (int)floorf((T.x[i] - c.x0) / c.pitch + 0.5f);
+  rb = min(max(rb, 0), c.n_rows - 1);
+  const float tb = T.time_ref[i] + T.z[i] * c.inv_Z;
+  const int sec = min(max(T.sector[i], 0), c.n_sectors - 1);
+  const uint32_t cell = (uint32_t)((sec * c.n_rows + rb) * c.n_tcell + merge_time_cell(tb, c));
+  S.cell_of[i] = cell;
+  atomicAdd(S.cell_start + cell, 1u);
+}
+
+__global__ void __launch_bounds__(256) k_merge_cell_fill(MergeTracks T, MergeScratch S, const __grid_constant__ MergeConsts c) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= merge_n(T, c)) return;
+  const uint32_t cell = S.cell_of[i];
+  const uint32_t pos = S.cell_start[cell] + atomicAdd(S.cell_cursor + cell, 1u);    // order inside a cell is irrelevant (ties are decided on seeds)
+  S.cand_idx[pos] = (uint32_t)i;
+  S.cand_a[pos] = make_float4(T.y[i], T.z[i], T.s[i], T.k[i]);
+  S.cand_b[pos] = make_float2(T.time_ref[i], __int_as_float(T.seed[i]));
+}
+
+__global__ void __launch_bounds__(kMergeThreads) k_merge_match(MergeTracks T, MergeScratch S, const __grid_constant__ MergeConsts c) {
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= merge_n(T, c)) return;
+  unsigned long long best = ~0ull;
+  int best_b = -1;
+  if (c.n_sectors >= 18) {
+    const float ax = T.x[a], ay = T.y[a], az = T.z[a], as = T.s[a], at = T.t[a], ak = T.k[a], atr = T.time_ref[a];
+    const uint32_t aseed = (uint32_t)T.seed[a];
+    const int sec = T.sector[a], side = sec / 18, phi = sec % 18;
+    const int fa = T.first_row[a], la = T.last_row[a];
+    const int r_lo = max(la + 1 - c.overlap, fa + 1), r_hi = min(la + 1 + c.gap, c.n_rows - 1);
+    const float cs = sqrtf(1.0f - as * as);
+    for (int isg = 0; isg < 2; ++isg) {
+      const float sg = isg == 0 ? 1.0f : -1.0f;
+      const int nb = side * 18 + (phi + (isg == 0 ? 1 : 17)) % 18;
+      if (nb >= c.n_sectors) continue;
+      const float x1 = ax * c.Cd + sg * (ay * c.Sd);
+      const float y1 = ay * c.Cd - sg * (ax * c.Sd);
+      const float s1 = as * c.Cd - sg * (cs * c.Sd);
+      if (!(fabsf(s1) < c.sin_phi_max)) continue;
+      for (int rb = r_lo; rb <= r_hi; ++rb) {
+        float x2 = x1, y2 = y1, z2 = az, s2 = s1;
+        if (!merge_transport(x2, y2, z2, s2, at, ak, __ldg(c.xr + rb), c.cB, c.sin_phi_max)) continue;
+        const float tpred = atr + z2 * c.inv_Z;
+        const uint32_t base = (uint32_t)((nb * c.n_rows + rb) * c.n_tcell);
+        const uint32_t lo = __ldg(S.cell_start + base + merge_time_cell(tpred - c.t_window, c));
+        const uint32_t hi = __ldg(S.cell_start + base + merge_time_cell(tpred + c.t_window, c) + 1);
+        for (uint32_t q = lo; q < hi; ++q) {
+          const float4 ca = S.cand_a[q];
+          const float2 cb = S.cand_b[q];
+          const float dy = y2 - ca.x;
+          const float dz = (z2 - ca.y) + (atr - cb.x) * c.Z;
+          const float ds = s2 - ca.z;
+          const float dk = ak - ca.w;
+          if (!(fabsf(dy) < c.cut_y && fabsf(dz) < c.cut_z && fabsf(ds) < c.cut_s && fabsf(dk) < c.cut_k)) continue;
+          const float d2 = (dy * dy) * c.wy + (dz * dz) * c.wz + (ds * ds) * c.ws + (dk * dk) * c.wk;
+          const unsigned long long hi_bits = (unsigned long long)__float_as_uint(d2) << 32;
+          const unsigned long long key_b = hi_bits | (unsigned long long)(uint32_t)__float_as_int(cb.y);
+          if (key_b < best) { best = key_b; best_b = (int)S.cand_idx[q]; }
+          atomicMin(S.in_key + S.cand_idx[q], hi_bits | (unsigned long long)aseed);
+        }
+      }
+    }
+  }
+  S.out_key[a] = best;
+  S.out_b[a] = best_b;
+}
+
+// next / prev are pre-set to -1; *n_links to 0.
+__global__ void __launch_bounds__(256) k_merge_link(MergeTracks T, MergeScratch S, int32_t* __restrict__ next, int32_t* __restrict__ prev,
+                                                    int32_t* __restrict__ n_links, const __grid_constant__ MergeConsts c) {
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  bool linked = false;
+  if (a < merge_n(T, c)) {
+    const int b = S.out_b[a];
+    if (b >= 0) {
+      const unsigned long long key_a = (S.out_key[a] & 0xFFFFFFFF00000000ull) | (unsigned long long)(uint32_t)T.seed[a];
+      if (S.in_key[b] == key_a) { next[a] = b; prev[b] = a; linked = true; }
+    }
+  }
+  const unsigned m = __ballot_sync(0xffffffffu, linked);
+  if (lane_id() == 0 && m) atomicAdd(n_links, __popc(m));
+}
+
+__global__ void __launch_bounds__(256) k_merge_root(MergeTracks T, const int32_t* __restrict__ prev, int32_t* __restrict__ root,
+                                                    const __grid_constant__ MergeConsts c) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= merge_n(T, c)) return;
+  int r = i;
+  for (int p = prev[r]; p >= 0; p = prev[r]) r = p;      // state rows strictly increase along a chain: no cycles
+  root[i] = r;
+}
+
+}  // namespace tpc

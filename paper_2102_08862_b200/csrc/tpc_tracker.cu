@@ -14,6 +14,7 @@
 #include "finder.cuh"
 #include "ingest.cuh"
 #include "links.cuh"
+#include "merge.cuh"
 #include "scan.cuh"
 #include "selector.cuh"
 #include "tracklet.cuh"
@@ -154,6 +155,31 @@ void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids
 
 }  // namespace
 
+// C7 scratch (merge.cuh), carved from the start of the arena: the tracking scratch is dead by then.
+namespace {
+struct MergeLayout { size_t cell_start, cell_cursor, scan, cell_of, cand_idx, cand_a, cand_b, out_key, out_b, in_key, total; int n_tcell; size_t n_cells; };
+MergeLayout merge_layout(const tpc_geometry_t& g, int64_t max_tracks) {
+  MergeLayout L{};
+  L.n_tcell = (int)std::floor((double)g.max_time_bin / (double)kMergeCellTimeBins) + 2;
+  L.n_cells = (size_t)g.n_sectors * (size_t)g.n_rows * (size_t)L.n_tcell;
+  const size_t K = (size_t)std::max<int64_t>(max_tracks, 1);
+  size_t off = 0;
+  auto take = [&](size_t bytes) { const size_t o = off; off += (bytes + 255) / 256 * 256; return o; };
+  L.cell_start = take(4 * (L.n_cells + 1));
+  L.cell_cursor = take(4 * L.n_cells);
+  L.scan = take(4 * (scan_tiles(L.n_cells + 1) + 1));
+  L.cell_of = take(4 * K);
+  L.cand_idx = take(4 * K);
+  L.cand_a = take(16 * K);
+  L.cand_b = take(8 * K);
+  L.out_key = take(8 * K);
+  L.out_b = take(4 * K);
+  L.in_key = take(8 * K);
+  L.total = off;
+  return L;
+}
+}  // namespace
+
 struct tpc_tracker {
   tpc_geometry_t geom;
   tpc_params_t params;
@@ -164,7 +190,7 @@ struct tpc_tracker {
   void* tables = nullptr;          // device: xr | cr | npads
   cudaEvent_t ev[N_STEPS + 1] = {};
   bool profile = false, have_times = false;
-  int64_t last_launches = 0;
+  int64_t last_launches = 0, last_merge_launches = 0;
   int ctas_fit_up = 148, ctas_follow_up = 148, ctas_fit_down = 148, ctas_follow_down = 148;   // persistent grids: SMs x resident CTAs per SM
 };
 
@@ -208,7 +234,8 @@ size_t tpc_tracker_arena_bytes(const tpc_geometry_t* g, const tpc_params_t* p, i
   ArenaPlan plan;
   Ids id;
   build_plan(p, c, plan, id);
-  return plan.peak_bytes();
+  // the arena also serves tpc_merge_tracks (C7) for the default track capacity
+  return std::max(plan.peak_bytes(), merge_layout(*g, c.max_tracks).total);
 }
 
 int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_tracker_t** out) {
@@ -306,6 +333,74 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
   *out = t;
   return TPC_OK;
 }
+
+
+// ---- C7: sector-boundary merging of the tracks of one tpc_track_timeframe call (merge.cuh) ----
+
+size_t tpc_merge_scratch_bytes(const tpc_tracker_t* t, int64_t max_tracks) {
+  if (!t || max_tracks < 0 || max_tracks >= ((int64_t)1 << 31)) return 0;
+  return merge_layout(t->geom, max_tracks).total;
+}
+
+int tpc_merge_tracks(tpc_tracker_t* t, const tpc_merge_params_t* mp, const tpc_tracks_t* tr, void* cuda_stream, tpc_merged_t* out) {
+  if (!t || !mp || !tr || !out) return TPC_EINVAL;
+  if (!(mp->cut_y_cm > 0 && mp->cut_z_cm > 0 && mp->cut_sin_phi > 0 && mp->cut_q_pt > 0 && mp->max_row_gap >= 0 && mp->max_row_overlap >= 0)) return TPC_EINVAL;
+  if (tr->max_tracks < 0 || !tr->n_tracks || !out->next || !out->prev || !out->root || !out->n_links) return TPC_EINVAL;
+  if (tr->max_tracks > 0 && (!tr->seed_hit || !tr->sector || !tr->first_row || !tr->last_row || !tr->x || !tr->y || !tr->z_rel ||
+                             !tr->time_ref || !tr->sin_phi || !tr->dzds || !tr->q_pt)) return TPC_EINVAL;
+  const MergeLayout L = merge_layout(t->geom, tr->max_tracks);
+  if (!t->params.arena || L.total > t->params.arena_bytes) return TPC_ENOMEM;
+  if (L.n_cells + 1 >= 2147483000ull) return TPC_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* A = static_cast<char*>(t->params.arena);
+  const int K = tr->max_tracks;
+  MergeConsts c{};
+  c.n_sectors = t->geom.n_sectors; c.n_rows = t->geom.n_rows; c.n_tcell = L.n_tcell;
+  c.gap = mp->max_row_gap; c.overlap = mp->max_row_overlap; c.max_tracks = K;
+  c.x0 = t->geom.x0_cm; c.pitch = t->geom.row_pitch_cm;
+  {   // cos / sin of the sector angle from tan of its half, in double, rounded once (no libm: the oracle derives them the same way)
+    const double T = (double)t->geom.tan_half_sector;
+    c.Cd = (float)((1.0 - T * T) / (1.0 + T * T));
+    c.Sd = (float)(2.0 * T / (1.0 + T * T));
+  }
+  c.Z = t->consts.Z; c.inv_Z = t->consts.inv_Z; c.cB = t->consts.cB; c.sin_phi_max = t->consts.sin_phi_max;
+  c.cut_y = mp->cut_y_cm; c.cut_z = mp->cut_z_cm; c.cut_s = mp->cut_sin_phi; c.cut_k = mp->cut_q_pt;
+  c.wy = (float)(1.0 / ((double)mp->cut_y_cm * (double)mp->cut_y_cm));
+  c.wz = (float)(1.0 / ((double)mp->cut_z_cm * (double)mp->cut_z_cm));
+  c.ws = (float)(1.0 / ((double)mp->cut_sin_phi * (double)mp->cut_sin_phi));
+  c.wk = (float)(1.0 / ((double)mp->cut_q_pt * (double)mp->cut_q_pt));
+  c.inv_cell = 1.0f / (float)kMergeCellTimeBins;
+  c.t_window = (float)((double)mp->cut_z_cm / (double)t->geom.time_bin_cm + 0.5);
+  c.xr = t->consts.xr;
+  MergeTracks T{tr->n_tracks, tr->seed_hit, tr->sector, tr->first_row, tr->last_row, tr->x, tr->y, tr->z_rel, tr->time_ref, tr->sin_phi, tr->dzds, tr->q_pt};
+  MergeScratch S{reinterpret_cast<uint32_t*>(A + L.cell_start), reinterpret_cast<uint32_t*>(A + L.cell_cursor),
+                 reinterpret_cast<uint32_t*>(A + L.cell_of), reinterpret_cast<uint32_t*>(A + L.cand_idx),
+                 reinterpret_cast<float4*>(A + L.cand_a), reinterpret_cast<float2*>(A + L.cand_b),
+                 reinterpret_cast<unsigned long long*>(A + L.out_key), reinterpret_cast<int32_t*>(A + L.out_b),
+                 reinterpret_cast<unsigned long long*>(A + L.in_key)};
+  int64_t launches = 0;
+  cudaMemsetAsync(out->n_links, 0, 4, st);
+  if (K > 0) {
+    cudaMemsetAsync(out->next, 0xFF, 4 * (size_t)K, st);
+    cudaMemsetAsync(out->prev, 0xFF, 4 * (size_t)K, st);
+    cudaMemsetAsync(out->root, 0xFF, 4 * (size_t)K, st);
+    cudaMemsetAsync(S.cell_start, 0, 4 * (L.n_cells + 1), st);
+    cudaMemsetAsync(S.cell_cursor, 0, 4 * L.n_cells, st);
+    cudaMemsetAsync(S.in_key, 0xFF, 8 * (size_t)K, st);
+    const int g256 = (K + 255) / 256;
+    k_merge_cell_count<<<g256, 256, 0, st>>>(T, S, c); ++launches;
+    launches += exclusive_scan_u32(S.cell_start, S.cell_start, L.n_cells + 1, reinterpret_cast<uint32_t*>(A + L.scan), st);
+    k_merge_cell_fill<<<g256, 256, 0, st>>>(T, S, c); ++launches;
+    k_merge_match<<<(K + kMergeThreads - 1) / kMergeThreads, kMergeThreads, 0, st>>>(T, S, c); ++launches;
+    k_merge_link<<<g256, 256, 0, st>>>(T, S, out->next, out->prev, out->n_links, c); ++launches;
+    k_merge_root<<<g256, 256, 0, st>>>(T, out->prev, out->root, c); ++launches;
+  }
+  t->last_merge_launches = launches;
+  if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;
+  return TPC_OK;
+}
+
+int64_t tpc_merge_last_launches(const tpc_tracker_t* t) { return t ? t->last_merge_launches : -1; }
 
 int tpc_tracker_destroy(tpc_tracker_t* t) {
   if (!t) return TPC_EINVAL;

@@ -18,6 +18,7 @@ STATUS_TRACKLET_OVERFLOW, STATUS_TRACK_OVERFLOW, STATUS_TRACK_HIT_OVERFLOW, STAT
 EXPORTS = ("tpc_tracker_arena_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
            "tpc_tracker_step_ms", "tpc_tracker_step_name", "tpc_tracker_last_launches", "tpc_tracker_work_counters",
            "tpc_tracker_arena_plan", "tpc_selftest_fast_math",
+           "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_merge_last_launches",
            "tpc_tracker_destroy", "tpc_strerror")
 
 
@@ -57,6 +58,22 @@ class Tracks(C.Structure):
                 ("hit_index", C.c_void_p), ("link_up", C.c_void_p), ("link_down", C.c_void_p), ("is_start_hit", C.c_void_p),
                 ("max_tracklets", C.c_int32), ("n_tracklets", C.c_void_p), ("tracklet_seed", C.c_void_p),
                 ("tracklet_n_hits", C.c_void_p), ("tracklet_row_hit", C.c_void_p), ("tracklet_par", C.c_void_p)]
+
+
+class MergeParams(C.Structure):
+    """``tpc_merge_params_t``"""
+    _fields_ = [("cut_y_cm", C.c_float), ("cut_z_cm", C.c_float), ("cut_sin_phi", C.c_float), ("cut_q_pt", C.c_float),
+                ("max_row_gap", C.c_int32), ("max_row_overlap", C.c_int32)]
+
+
+class Merged(C.Structure):
+    """``tpc_merged_t``"""
+    _fields_ = [("next", C.c_void_p), ("prev", C.c_void_p), ("root", C.c_void_p), ("n_links", C.c_void_p)]
+
+
+def default_merge_params() -> MergeParams:
+    """DESIGN.md §3 C7 readings M4 / M5."""
+    return MergeParams(2.0, 2.0, 0.05, 0.5, 12, 2)
 
 
 def default_geometry(n_sectors: int = 36, max_time_bin: float = 487.0) -> Geometry:
@@ -101,6 +118,12 @@ def load_library(build_if_missing: bool = True):
         L.tpc_tracker_destroy.argtypes = [vp]
         L.tpc_selftest_fast_math.argtypes = [vp, C.POINTER(C.c_uint64)]
         L.tpc_selftest_fast_math.restype = C.c_int
+        L.tpc_merge_scratch_bytes.argtypes = [vp, C.c_int64]
+        L.tpc_merge_scratch_bytes.restype = C.c_size_t
+        L.tpc_merge_tracks.argtypes = [vp, C.POINTER(MergeParams), C.POINTER(Tracks), vp, C.POINTER(Merged)]
+        L.tpc_merge_tracks.restype = C.c_int
+        L.tpc_merge_last_launches.argtypes = [vp]
+        L.tpc_merge_last_launches.restype = C.c_int64
         L.tpc_strerror.argtypes = [C.c_int]
         L.tpc_strerror.restype = C.c_char_p
         for nm in ("tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host", "tpc_tracker_step_ms",
@@ -267,6 +290,28 @@ class Tracker:
         if rc != TPC_OK:
             raise TpcError(rc, "tpc_track_timeframe_host")
         return out
+
+    def tpc_merge_tracks(self, outputs, merge_params: MergeParams | None = None, merged=None, stream=None):
+        """C7 on the DEVICE outputs of ``tpc_track_timeframe`` (same stream); returns (next, prev, root, n_links) tensors."""
+        torch = self._torch
+        out, st = outputs
+        K = int(st.max_tracks)
+        if merged is None:
+            merged = tuple(torch.empty(max(K, 1), dtype=torch.int32, device=self.device) for _ in range(3)) + \
+                     (torch.empty(1, dtype=torch.int32, device=self.device),)
+        mp = merge_params if merge_params is not None else default_merge_params()
+        m = Merged(*(t.data_ptr() for t in merged))
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        rc = self.lib.tpc_merge_tracks(self.handle, C.byref(mp), C.byref(st), C.c_void_p(s.cuda_stream), C.byref(m))
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_merge_tracks")
+        return merged
+
+    def merge_scratch_bytes(self, max_tracks: int) -> int:
+        return int(self.lib.tpc_merge_scratch_bytes(self.handle, int(max_tracks)))
+
+    def last_merge_launches(self) -> int:
+        return int(self.lib.tpc_merge_last_launches(self.handle))
 
     def step_ms(self) -> dict:
         buf = (C.c_float * 32)()
