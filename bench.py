@@ -238,6 +238,23 @@ def main():
     n_track_hits = int(outs[0].n_track_hits[0])
     status = int(outs[0].status[0])
     arena_gb = trk.arena_bytes / 1e9
+    # ---- widening step C7 (sector-boundary merging of the tracks, not part of `value`): timed on its own ----
+    merge = None
+    if cfg.n_sectors >= 18:
+        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        merged = None
+        ms_m = 0.0
+        for _ in range(3):
+            with torch.cuda.stream(stream):
+                trk.tpc_track_timeframe(*devc, n=n, outputs=outs, stream=stream)      # the merger's input (and it reuses the arena)
+                m0.record(stream)
+                merged = trk.tpc_merge_tracks(outs, merged=merged, stream=stream)
+                m1.record(stream)
+            stream.synchronize()
+            ms_m = m0.elapsed_time(m1)                                                # last of three
+        merge = {"step": "sector_boundary_merge (C7, tpc_merge_tracks)", "ms": round(ms_m, 4), "n_links": int(merged[3][0]),
+                 "n_tracks": n_tracks, "tracks_per_s": n_tracks / (ms_m * 1e-3) if ms_m > 0 else None,
+                 "gpu_launches": trk.last_merge_launches(), "in_value": False}
     trk.close()
     del trk, outs
 
@@ -349,7 +366,7 @@ def main():
                              "working set may fit L2 (small config)", "gen_seconds": round(t_gen, 1)},
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches,
             "step_ms": {k: round(v, 4) for k, v in step_acc.items()}, "kernels": kernels,
-            "tracklet_constructor": constructor, "roofline": roof, "cpu_baseline": cpu}
+            "tracklet_constructor": constructor, "merge": merge, "roofline": roof, "cpu_baseline": cpu}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -130,3 +130,69 @@ def test_merge_rejects_bad_arguments():
     assert rc == T.TPC_ENOMEM
     torch.cuda.synchronize()
     trk.close()
+
+
+def test_full_10ms_frame_merge_invariants_and_sampled_oracle_parity():
+    """configs[3] at FULL size, default parameters: tpc_track_timeframe + tpc_merge_tracks as bench.py times them.
+    (a) Invariants of the links.  (b) Sampled parity: the oracle tracks and merges the sub-frame {sectors S-2 .. S+2,
+    2000-bin window +- 2200 bins}; for every track of sector S whose hits all lie inside the window, the link to its
+    continuation (and to the piece it continues) must be the same seed -> seed link as on the GPU (a candidate lies
+    within one drift length, 485 bins, of the track, a competitor within another 485: all at least 1200 bins inside
+    the sub-frame, where the sampled tracking parity of test_parity_gpu.py holds)."""
+    import torch
+    from paper_2102_08862_b200 import tracker as T
+    from test_parity_gpu import _full_frame, N_ROWS
+    import oracle
+    from oracle import merge as M
+    cfg, tf = _full_frame(3)
+    n = tf.n
+    trk = T.Tracker(T.default_geometry(36, tf.max_time_bin), T.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm, max_clusters=n))
+    d = [torch.from_numpy(a).to(trk.device) for a in (tf.row, tf.pad, tf.time)]
+    outs = trk.alloc_outputs(n)
+    out = trk.tpc_track_timeframe(*d, n=n, outputs=outs)
+    nxt, prv, root, n_links = trk.tpc_merge_tracks(outs)
+    torch.cuda.synchronize()
+    k, nh = int(out.n_tracks[0]), int(out.n_track_hits[0])
+    assert int(out.status[0]) & 7 == 0 and k > 1e6
+    seed, sec = out.seed_hit[:k].cpu().numpy(), out.sector[:k].cpu().numpy()
+    first_row, last_row = out.first_row[:k].cpu().numpy(), out.last_row[:k].cpu().numpy()
+    x = out.x[:k].cpu().numpy()
+    nxt, prv, root, n_links = nxt[:k].cpu().numpy(), prv[:k].cpu().numpy(), root[:k].cpu().numpy(), int(n_links[0])
+    trk.close()
+    del d, out, outs
+    # (a) invariants (as pin M-I)
+    a = np.nonzero(nxt >= 0)[0]
+    b = nxt[a]
+    assert n_links == a.size and n_links > 2e5
+    np.testing.assert_array_equal(prv[b], a)
+    assert np.unique(b).size == b.size
+    assert np.all(sec[a] // 18 == sec[b] // 18) and np.all(np.isin((sec[a] % 18 - sec[b] % 18) % 18, (1, 17)))
+    rb = np.rint((x[b].astype(np.float64) - 85.0) / 1.07).astype(np.int64)
+    assert np.all(rb > first_row[a]) and np.all(rb >= last_row[a] - 1) and np.all(rb <= last_row[a] + 13)
+    assert np.all(prv[root] == -1) and np.array_equal(root[b], root[a])
+    assert k - n_links == np.unique(root).size
+    # (b) sampled parity
+    S, t_lo, width, margin = 7, 20000.0, 2000.0, 2200.0
+    t_hi = t_lo + width
+    sectors = [(S + o) % 18 for o in (-2, -1, 0, 1, 2)]
+    srow = (tf.row.astype(np.int64) // N_ROWS)
+    sel = np.nonzero(np.isin(srow, sectors) & (tf.time >= t_lo - margin) & (tf.time <= t_hi + margin))[0]
+    assert sel.size > 1e6
+    o = oracle.track(oracle.default_geometry(36, tf.max_time_bin), oracle.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm),
+                     tf.row[sel], tf.pad[sel], tf.time[sel])
+    mr = M.merge(M.default_merge_params(36), o.tr_seed, o.tr_sector, o.tr_first_row, o.tr_last_row, o.tr_par)
+    o_t = tf.time[sel][o.tr_hit_index]
+    o_min = np.minimum.reduceat(o_t, o.tr_hit_offset); o_max = np.maximum.reduceat(o_t, o.tr_hit_offset)
+    core = np.nonzero((o.tr_sector == S) & (o_min >= t_lo) & (o_max <= t_hi))[0]
+    assert core.size > 300
+    o_seed_global = sel[o.tr_seed]
+    lookup = {int(s): i for i, s in enumerate(seed)}
+    n_with_link = 0
+    for i in core:
+        gi = lookup[int(o_seed_global[i])]                      # the same track exists on the GPU (sampled tracking parity)
+        for o_idx, g_idx in ((mr.next[i], nxt[gi]), (mr.prev[i], prv[gi])):
+            o_link = int(o_seed_global[o_idx]) if o_idx >= 0 else -1
+            g_link = int(seed[g_idx]) if g_idx >= 0 else -1
+            assert o_link == g_link, (int(o_seed_global[i]), o_link, g_link)
+            n_with_link += o_link >= 0
+    assert n_with_link > 50
