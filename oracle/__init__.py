@@ -79,6 +79,10 @@ def lib():
         L.orc_transport.restype = C.c_int
         L.orc_update.argtypes = [vp, vp, C.c_float, C.c_float, C.c_float, C.c_float]
         L.orc_tables.argtypes = [C.POINTER(Geometry), C.POINTER(Params), vp, vp, vp, vp]
+        L.orc_refit_chains.argtypes = [C.POINTER(Geometry), C.POINTER(Params), vp, vp, vp, C.c_int64] + [vp] * 12
+        L.orc_refit_chains.restype = None
+        L.orc_rotate_with_cov.argtypes = [C.POINTER(Geometry), C.POINTER(Params), vp, vp, C.c_int32]
+        L.orc_rotate_with_cov.restype = C.c_int
         for nm in ("orc_copy_links", "orc_copy_tracklets", "orc_copy_tracks", "orc_copy_stats", "orc_free",
                    "orc_update", "orc_tables"):
             getattr(L, nm).restype = None
@@ -188,3 +192,28 @@ def tables(geom: Geometry, params: Params):
     k = np.empty(8, np.float32)
     lib().orc_tables(C.byref(geom), C.byref(params), x.ctypes.data, npads.ctypes.data, cr.ctypes.data, k.ctypes.data)
     return x, npads, cr, dict(W1=k[0], Ay=k[1], Az=k[2], wy=k[3], wz=k[4], ry=k[5], rz=k[6])
+
+
+def refit_chains(geom: Geometry, params: Params, row, pad, time, res: "Result", nxt, prv):
+    """C8: refit of the chains linked by C7 (``oracle.merge``).  Returns (ok, chain_hits, chain_pieces, par[n,7], cov[n,9])."""
+    a = lambda v, t: np.ascontiguousarray(v, t)
+    row, pad, time = a(row, np.float32), a(pad, np.float32), a(time, np.float32)
+    nxt, prv = a(nxt, np.int32), a(prv, np.int32)
+    n = int(len(res.tr_seed))
+    ok, ch, cp = np.zeros(n, np.int32), np.zeros(n, np.int32), np.zeros(n, np.int32)
+    rp, rc = np.zeros((n, 7), np.float32), np.zeros((n, 9), np.float32)
+    sec, nh, off = a(res.tr_sector, np.int32), a(res.tr_n_hits, np.int32), a(res.tr_hit_offset, np.int64)
+    hi, par = a(res.tr_hit_index, np.int32), a(res.tr_par, np.float32)
+    lib().orc_refit_chains(C.byref(geom), C.byref(params), row.ctypes.data, pad.ctypes.data, time.ctypes.data, n,
+                           sec.ctypes.data, nh.ctypes.data, off.ctypes.data, hi.ctypes.data, par.ctypes.data,
+                           nxt.ctypes.data, prv.ctypes.data, ok.ctypes.data, ch.ctypes.data, cp.ctypes.data,
+                           rp.ctypes.data, rc.ctypes.data)
+    return ok, ch, cp, rp, rc
+
+
+def rotate_with_cov(geom: Geometry, params: Params, state6, cov9, q: int):
+    """C8 rotation of state and covariance by q * 20 degrees (pin F-J).  Returns (ok, state6, cov9)."""
+    st = np.array(state6, np.float32)
+    cv = np.array(cov9, np.float32)
+    rc = lib().orc_rotate_with_cov(C.byref(geom), C.byref(params), st.ctypes.data, cv.ctypes.data, int(q))
+    return rc == 0, st, cv

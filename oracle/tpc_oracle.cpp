@@ -499,6 +499,88 @@ void orc_copy_tracks(const orc_result* r, int32_t* seed, int32_t* sector, int32_
 void orc_copy_stats(const orc_result* r, double* out16) { std::memcpy(out16, r->stats, sizeof(r->stats)); }
 void orc_free(orc_result* r) { delete r; }
 
+// C8 rotation of a state and its covariance by q * (sector angle), q = +-1 (statement list in the C8 header below).
+static bool rotate_with_cov(State& S, float qd, float Cd, float Sd, float sin_phi_max) {
+  const float cs = std::sqrt(1.0f - S.s * S.s);
+  const float J = Cd + qd * ((S.s / cs) * Sd);
+  const float x1 = S.x * Cd + qd * (S.y * Sd);
+  const float y1 = S.y * Cd - qd * (S.x * Sd);
+  const float s1 = S.s * Cd - qd * (cs * Sd);
+  if (!(std::fabs(s1) < sin_phi_max)) return false;
+  S.x = x1; S.y = y1; S.s = s1;
+  S.c1 = S.c1 * J; S.c2 = (S.c2 * J) * J; S.c4 = S.c4 * J;
+  return true;
+}
+
+// ---- C8: refit of the chains linked by C7 (second half; DESIGN.md §3 "C8", readings F1..F6).
+// PAPER.md L23 / L25 name "full TPC tracking"; the paper gives no listing.  One Kalman pass per chain of >= 2 pieces
+// P0 -> P1 -> ... -> Pm (inner to outer), from the outermost hit of Pm inward to the innermost hit of P0, over the hits
+// each piece OWNS (C6), each piece in its own sector frame; at a piece boundary the state and its covariance are rotated
+// into the frame of the next inner piece and z is re-referenced to that piece's time_ref:
+//   S = state of Pm (its C6 parameters);  transport(S, x of Pm's outermost hit);  cov = diag(c0_y2, c0_s2, c0_k2 | c0_z2, c0_t2)
+//   for p = m .. 0:
+//       for the hits of Pp, outermost first:  transport(S, x_row(hit));  update(S, y(hit), (time(hit) - time_ref_p) * Z)
+//       if p > 0 (q = -sg, sg = side of the link P(p-1) -> Pp; Cd, Sd = cos, sin of the sector angle as in C7):
+//           cs = sqrtf(1 - s*s);  J = Cd + q*((s/cs)*Sd)                       # d s' / d s
+//           x' = x*Cd + q*(y*Sd);  y' = y*Cd - q*(x*Sd);  s' = s*Cd - q*(cs*Sd);  FAIL unless |s'| < sin_phi_max
+//           c1 = c1*J;  c2 = (c2*J)*J;  c4 = c4*J;   z = z + (time_ref_p - time_ref_(p-1)) * Z
+//   any transport FAIL -> the chain is flagged (ok = -1) and keeps the parameters of P0.
+// Output per root: state + covariance at P0's innermost hit (z relative to P0's time_ref), hits and pieces of the chain.
+void orc_refit_chains(const orc_geometry* gp, const orc_params* pp, const float* row, const float* pad, const float* time,
+                      int64_t n_tracks, const int32_t* sector, const int32_t* n_hits, const int64_t* hit_offset,
+                      const int32_t* hit_index, const float* par, const int32_t* next, const int32_t* prev,
+                      int32_t* ok, int32_t* chain_hits, int32_t* chain_pieces, float* rpar, float* rcov) {
+  const Derived D = derive(*gp, *pp);
+  const double T = (double)gp->tan_half_sector;
+  const float Cd = (float)((1.0 - T * T) / (1.0 + T * T)), Sd = (float)(2.0 * T / (1.0 + T * T));
+  const int nr = gp->n_rows;
+  for (int64_t i = 0; i < n_tracks; ++i) {
+    ok[i] = 0; chain_hits[i] = n_hits[i]; chain_pieces[i] = 1;
+    for (int k = 0; k < 7; ++k) rpar[7 * i + k] = par[7 * i + k];
+    for (int k = 0; k < 9; ++k) rcov[9 * i + k] = 0.0f;
+    if (prev[i] >= 0 || next[i] < 0) continue;
+    std::vector<int64_t> pieces;
+    for (int64_t p = i; p >= 0; p = next[p]) pieces.push_back(p);
+    int32_t total = 0;
+    for (int64_t p : pieces) total += n_hits[p];
+    chain_hits[i] = total; chain_pieces[i] = (int32_t)pieces.size();
+    const int64_t pm = pieces.back();
+    const float* q = par + 7 * pm;
+    State S{q[0], q[1], q[2], q[3], q[4], q[5], 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    bool good = true;
+    {
+      const int32_t h = hit_index[hit_offset[pm] + n_hits[pm] - 1];
+      good = transport(S, D.xr[(int)row[h] % nr], D.cB, pp->sin_phi_max);
+    }
+    S.c0 = pp->c0_y2; S.c1 = 0; S.c2 = pp->c0_s2; S.c3 = 0; S.c4 = 0; S.c5 = pp->c0_k2; S.d0 = pp->c0_z2; S.d1 = 0; S.d2 = pp->c0_t2;
+    for (int ip = (int)pieces.size() - 1; ip >= 0 && good; --ip) {
+      const int64_t p = pieces[ip];
+      const float tref = par[7 * p + 6];
+      for (int64_t j = hit_offset[p] + n_hits[p] - 1; j >= hit_offset[p] && good; --j) {
+        const int32_t h = hit_index[j];
+        const int r = (int)row[h] % nr;
+        good = transport(S, D.xr[r], D.cB, pp->sin_phi_max);
+        if (!good) break;
+        const float ym = (pad[h] - D.cr[r]) * D.P;
+        const float zm = (time[h] - tref) * D.Z;
+        update(S, ym, zm, D.ry, D.rz);
+      }
+      if (good && ip > 0) {
+        const int64_t pin = pieces[ip - 1];
+        const float sg = ((sector[p] % 18) == ((sector[pin] % 18) + 1) % 18) ? 1.0f : -1.0f;
+        if (!rotate_with_cov(S, -sg, Cd, Sd, pp->sin_phi_max)) { good = false; break; }
+        S.z = S.z + (tref - par[7 * pin + 6]) * D.Z;
+      }
+    }
+    if (good) {
+      ok[i] = 1;
+      put_state(S, par[7 * i + 6], rpar + 7 * i, rcov + 9 * i);
+    } else {
+      ok[i] = -1;
+    }
+  }
+}
+
 // ---- hooks for the pins (K1..K3, G1): the same functions the tracker uses, callable one at a time ----
 // state6 = (x, y, z, s, t, k); cov9 = (c0..c5, d0..d2).  Returns 0, or 1 on transport FAIL.
 int orc_transport(const orc_params* p, float* st, float* cv, float xn) {
@@ -514,6 +596,17 @@ void orc_update(float* st, float* cv, float ym, float zm, float ry, float rz) {
   update(S, ym, zm, ry, rz);
   put_state(S, 0.0f, nullptr, cv);
   st[0] = S.x; st[1] = S.y; st[2] = S.z; st[3] = S.s; st[4] = S.t; st[5] = S.k;
+}
+
+// C8 rotation on its own (pin F-J): q = +1 / -1.  Returns 0, or 1 when |s'| >= sin_phi_max (state unchanged).
+int orc_rotate_with_cov(const orc_geometry* g, const orc_params* p, float* st, float* cv, int32_t q) {
+  const double T = (double)g->tan_half_sector;
+  const float Cd = (float)((1.0 - T * T) / (1.0 + T * T)), Sd = (float)(2.0 * T / (1.0 + T * T));
+  State S{st[0], st[1], st[2], st[3], st[4], st[5], cv[0], cv[1], cv[2], cv[3], cv[4], cv[5], cv[6], cv[7], cv[8]};
+  const bool ok = rotate_with_cov(S, q >= 0 ? 1.0f : -1.0f, Cd, Sd, p->sin_phi_max);
+  put_state(S, 0.0f, nullptr, cv);
+  st[0] = S.x; st[1] = S.y; st[2] = S.z; st[3] = S.s; st[4] = S.t; st[5] = S.k;
+  return ok ? 0 : 1;
 }
 
 // x_r [n_rows], n_pads [n_rows], c_r [n_rows]; consts8 = (W1, Ay, Az, wy, wz, ry, rz, 0)
