@@ -204,6 +204,24 @@ size_t tpc_merge_scratch_bytes(const tpc_tracker_t* tracker, int64_t max_tracks)
 int tpc_merge_tracks(tpc_tracker_t* tracker, const tpc_merge_params_t* merge_params, const tpc_tracks_t* tracks,
                      void* cuda_stream, tpc_merged_t* merged_out);
 
+/* ---- C8: refit of the chains linked by C7 (DESIGN.md §3 "C8", readings F1..F6): one inward Kalman pass over the hits
+ * all pieces of a chain own, each piece in its own sector frame, state and covariance rotated at every boundary.      */
+typedef struct {   /* caller-allocated DEVICE buffers, indexed by track like tpc_tracks_t                              */
+  int32_t* ok;           /* [max_tracks] 1: root of a chain of >= 2 pieces, refitted; 0: anything else (values passed
+                            through); -1: root whose refit failed (a transport / rotation reached sin_phi_max)         */
+  int32_t* chain_hits;   /* [max_tracks] hits of the whole chain (roots), else the track's own n_hits                  */
+  int32_t* chain_pieces; /* [max_tracks] pieces of the chain (roots), else 1                                           */
+  float* par7;           /* [max_tracks*7] (x, y, z_rel, sin_phi, dzds, q_pt, time_ref) at the innermost hit of the root */
+  float* cov9;           /* [max_tracks*9] (yy, ys, ss, yk, sk, kk | zz, zt, tt); zeros unless ok == 1                  */
+} tpc_refit_t;
+
+/* `clusters` are the DEVICE arrays the frame was tracked from (the hits' coordinates are read from them), `tracks` the
+ * outputs of tpc_track_timeframe, `merged` those of tpc_merge_tracks; all on the same stream, after tpc_merge_tracks.
+ * Asynchronous; never allocates (4 bytes of arena per track).  Errors: TPC_EINVAL, TPC_ENOMEM, TPC_ECUDA.
+ * tpc_merge_last_launches() then reports this call's launches.                                                        */
+int tpc_refit_chains(tpc_tracker_t* tracker, const tpc_clusters_t* clusters, const tpc_tracks_t* tracks,
+                     const tpc_merged_t* merged, void* cuda_stream, tpc_refit_t* refit_out);
+
 /* Number of kernel launches the last tpc_merge_tracks call enqueued (memsets not counted).                        */
 int64_t tpc_merge_last_launches(const tpc_tracker_t* tracker);
 

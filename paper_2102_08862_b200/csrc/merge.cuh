@@ -15,6 +15,7 @@
 // All decision arithmetic is fp32 in the written order (--fmad=false).
 #pragma once
 #include "common.cuh"
+#include "tracklet.cuh"
 
 namespace tpc {
 
@@ -170,6 +171,109 @@ __global__ void __launch_bounds__(256) k_merge_root(MergeTracks T, const int32_t
   int r = i;
   for (int p = prev[r]; p >= 0; p = prev[r]) r = p;      // state rows strictly increase along a chain: no cycles
   root[i] = r;
+}
+
+// ---- C8: refit of the chains linked by C7 (DESIGN.md §3 "C8", readings F1..F6) ----
+// One Kalman pass per chain of >= 2 pieces, from the outermost hit of the outermost piece inward to the innermost hit
+// of the root piece, over the hits each piece owns, each piece in its own sector frame; state and covariance are
+// rotated at every boundary.  transport / kalman_update are the constructor's (tracklet.cuh): same statements, same order.
+struct RefitIo {
+  const float *row, *pad, *time;            // the frame's clusters (DEVICE, as passed to tpc_track_timeframe)
+  const int32_t *n_hits; const int64_t* hit_offset; const int32_t* hit_index;
+  const int32_t *next, *prev;               // C7 links
+  int32_t *ok, *chain_hits, *chain_pieces;  // [max_tracks]
+  float *rpar, *rcov;                       // [max_tracks * 7], [max_tracks * 9]
+};
+
+// Pass-through values for every track + the list of chain roots (order irrelevant: results are indexed by track).
+__global__ void __launch_bounds__(256) k_refit_roots(MergeTracks T, RefitIo io, uint32_t* __restrict__ root_list, uint32_t* __restrict__ n_roots,
+                                                     const __grid_constant__ MergeConsts c) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  bool is_root = false;
+  if (i < merge_n(T, c)) {
+    is_root = io.prev[i] < 0 && io.next[i] >= 0;
+    io.ok[i] = 0; io.chain_hits[i] = io.n_hits[i]; io.chain_pieces[i] = 1;
+    float* rp = io.rpar + 7 * (size_t)i;
+    rp[0] = T.x[i]; rp[1] = T.y[i]; rp[2] = T.z[i]; rp[3] = T.s[i]; rp[4] = T.t[i]; rp[5] = T.k[i]; rp[6] = T.time_ref[i];
+    float* rc = io.rcov + 9 * (size_t)i;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) rc[k] = 0.0f;
+  }
+  const unsigned m = __ballot_sync(0xffffffffu, is_root);
+  if (m) {
+    uint32_t base = 0;
+    const int leader = __ffs(m) - 1;
+    if ((int)lane_id() == leader) base = atomicAdd(n_roots, (uint32_t)__popc(m));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (is_root) root_list[base + __popc(m & ((1u << lane_id()) - 1u))] = (uint32_t)i;
+  }
+}
+
+__global__ void __launch_bounds__(kMergeThreads) k_refit_chains(MergeTracks T, RefitIo io, const uint32_t* __restrict__ root_list,
+                                                                 const uint32_t* __restrict__ n_roots, const __grid_constant__ MergeConsts c,
+                                                                 const __grid_constant__ Consts tc) {
+  __shared__ float xr[kRowStride], cr[kRowStride];
+  for (int r = threadIdx.x; r < tc.n_rows; r += blockDim.x) { xr[r] = tc.xr[r]; cr[r] = tc.cr[r]; }
+  __syncthreads();
+  const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= *n_roots) return;
+  const int root = (int)root_list[e];
+  int pm = root, pieces = 1, total = io.n_hits[root];
+  for (int p = io.next[pm]; p >= 0; p = io.next[pm]) { pm = p; ++pieces; total += io.n_hits[p]; }
+  io.chain_hits[root] = total;
+  io.chain_pieces[root] = pieces;
+  TrackState S;
+  S.x = T.x[pm]; S.y = T.y[pm]; S.z = T.z[pm]; S.s = T.s[pm]; S.t = T.t[pm]; S.k = T.k[pm];
+  S.c0 = S.c1 = S.c2 = S.c3 = S.c4 = S.c5 = 0.0f; S.d0 = S.d1 = S.d2 = 0.0f;
+  bool good;
+  {
+    const int32_t h = io.hit_index[io.hit_offset[pm] + io.n_hits[pm] - 1];
+    const int r = (int)io.row[h] % tc.n_rows;
+    good = transport(S, xr[r], tc.cB, tc.sin_phi_max);
+  }
+  S.c0 = tc.c0_y2; S.c1 = 0.0f; S.c2 = tc.c0_s2; S.c3 = 0.0f; S.c4 = 0.0f; S.c5 = tc.c0_k2; S.d0 = tc.c0_z2; S.d1 = 0.0f; S.d2 = tc.c0_t2;
+  for (int p = pm; good; ) {
+    const float tref = T.time_ref[p];
+    const int64_t off = io.hit_offset[p];
+    int64_t j = off + io.n_hits[p] - 1;
+    int32_t h = io.hit_index[j];
+    float hr = io.row[h], hp = io.pad[h], ht = io.time[h];
+    for (; j >= off; --j) {
+      float nr = 0.0f, np = 0.0f, nt = 0.0f;
+      if (j > off) {                                   // the next hit, one iteration ahead
+        const int32_t hn = io.hit_index[j - 1];
+        nr = io.row[hn]; np = io.pad[hn]; nt = io.time[hn];
+      }
+      const int r = (int)hr % tc.n_rows;
+      good = transport(S, xr[r], tc.cB, tc.sin_phi_max);
+      if (!good) break;
+      kalman_update(S, (hp - cr[r]) * tc.P, (ht - tref) * tc.Z, tc.ry, tc.rz);
+      hr = nr; hp = np; ht = nt;
+    }
+    if (!good || p == root) break;
+    const int pin = io.prev[p];
+    const float sg = ((T.sector[p] % 18) == ((T.sector[pin] % 18) + 1) % 18) ? 1.0f : -1.0f;
+    const float qd = -sg;
+    const float cs = sqrtf(1.0f - S.s * S.s);
+    const float J = c.Cd + qd * ((S.s / cs) * c.Sd);
+    const float x1 = S.x * c.Cd + qd * (S.y * c.Sd);
+    const float y1 = S.y * c.Cd - qd * (S.x * c.Sd);
+    const float s1 = S.s * c.Cd - qd * (cs * c.Sd);
+    if (!(fabsf(s1) < tc.sin_phi_max)) { good = false; break; }
+    S.x = x1; S.y = y1; S.s = s1;
+    S.c1 = S.c1 * J; S.c2 = (S.c2 * J) * J; S.c4 = S.c4 * J;
+    S.z = S.z + (tref - T.time_ref[pin]) * tc.Z;
+    p = pin;
+  }
+  if (good) {
+    io.ok[root] = 1;
+    float* rp = io.rpar + 7 * (size_t)root;
+    rp[0] = S.x; rp[1] = S.y; rp[2] = S.z; rp[3] = S.s; rp[4] = S.t; rp[5] = S.k;      // rp[6] = time_ref of the root: already there
+    float* rc = io.rcov + 9 * (size_t)root;
+    rc[0] = S.c0; rc[1] = S.c1; rc[2] = S.c2; rc[3] = S.c3; rc[4] = S.c4; rc[5] = S.c5; rc[6] = S.d0; rc[7] = S.d1; rc[8] = S.d2;
+  } else {
+    io.ok[root] = -1;
+  }
 }
 
 }  // namespace tpc

@@ -400,6 +400,42 @@ int tpc_merge_tracks(tpc_tracker_t* t, const tpc_merge_params_t* mp, const tpc_t
   return TPC_OK;
 }
 
+
+// ---- C8: refit of the chains linked by C7 (merge.cuh) ----
+int tpc_refit_chains(tpc_tracker_t* t, const tpc_clusters_t* cl, const tpc_tracks_t* tr, const tpc_merged_t* mg, void* cuda_stream,
+                     tpc_refit_t* out) {
+  if (!t || !cl || !tr || !mg || !out) return TPC_EINVAL;
+  if (tr->max_tracks < 0 || !tr->n_tracks || !out->ok || !out->chain_hits || !out->chain_pieces || !out->par7 || !out->cov9) return TPC_EINVAL;
+  if (tr->max_tracks > 0 && (!cl->row || !cl->pad || !cl->time || !tr->sector || !tr->n_hits || !tr->hit_offset || !tr->hit_index || !tr->x ||
+                             !tr->y || !tr->z_rel || !tr->time_ref || !tr->sin_phi || !tr->dzds || !tr->q_pt || !mg->next || !mg->prev)) return TPC_EINVAL;
+  const int K = tr->max_tracks;
+  const size_t need = 256 + 4 * (size_t)std::max(K, 1);
+  if (!t->params.arena || need > t->params.arena_bytes) return TPC_ENOMEM;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* A = static_cast<char*>(t->params.arena);
+  uint32_t* n_roots = reinterpret_cast<uint32_t*>(A);
+  uint32_t* root_list = reinterpret_cast<uint32_t*>(A + 256);
+  MergeConsts c{};
+  c.n_sectors = t->geom.n_sectors; c.n_rows = t->geom.n_rows; c.max_tracks = K;
+  {
+    const double T = (double)t->geom.tan_half_sector;
+    c.Cd = (float)((1.0 - T * T) / (1.0 + T * T));
+    c.Sd = (float)(2.0 * T / (1.0 + T * T));
+  }
+  MergeTracks T{tr->n_tracks, tr->seed_hit, tr->sector, tr->first_row, tr->last_row, tr->x, tr->y, tr->z_rel, tr->time_ref, tr->sin_phi, tr->dzds, tr->q_pt};
+  RefitIo io{cl->row, cl->pad, cl->time, tr->n_hits, tr->hit_offset, tr->hit_index, mg->next, mg->prev,
+             out->ok, out->chain_hits, out->chain_pieces, out->par7, out->cov9};
+  int64_t launches = 0;
+  cudaMemsetAsync(n_roots, 0, 4, st);
+  if (K > 0) {
+    k_refit_roots<<<(K + 255) / 256, 256, 0, st>>>(T, io, root_list, n_roots, c); ++launches;
+    k_refit_chains<<<(K + kMergeThreads - 1) / kMergeThreads, kMergeThreads, 0, st>>>(T, io, root_list, n_roots, c, t->consts); ++launches;
+  }
+  t->last_merge_launches = launches;
+  if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;
+  return TPC_OK;
+}
+
 int64_t tpc_merge_last_launches(const tpc_tracker_t* t) { return t ? t->last_merge_launches : -1; }
 
 int tpc_tracker_destroy(tpc_tracker_t* t) {

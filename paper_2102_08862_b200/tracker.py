@@ -18,7 +18,7 @@ STATUS_TRACKLET_OVERFLOW, STATUS_TRACK_OVERFLOW, STATUS_TRACK_HIT_OVERFLOW, STAT
 EXPORTS = ("tpc_tracker_arena_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
            "tpc_tracker_step_ms", "tpc_tracker_step_name", "tpc_tracker_last_launches", "tpc_tracker_work_counters",
            "tpc_tracker_arena_plan", "tpc_selftest_fast_math",
-           "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_merge_last_launches",
+           "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_refit_chains", "tpc_merge_last_launches",
            "tpc_tracker_destroy", "tpc_strerror")
 
 
@@ -69,6 +69,11 @@ class MergeParams(C.Structure):
 class Merged(C.Structure):
     """``tpc_merged_t``"""
     _fields_ = [("next", C.c_void_p), ("prev", C.c_void_p), ("root", C.c_void_p), ("n_links", C.c_void_p)]
+
+
+class Refit(C.Structure):
+    """``tpc_refit_t``"""
+    _fields_ = [("ok", C.c_void_p), ("chain_hits", C.c_void_p), ("chain_pieces", C.c_void_p), ("par7", C.c_void_p), ("cov9", C.c_void_p)]
 
 
 def default_merge_params() -> MergeParams:
@@ -122,6 +127,8 @@ def load_library(build_if_missing: bool = True):
         L.tpc_merge_scratch_bytes.restype = C.c_size_t
         L.tpc_merge_tracks.argtypes = [vp, C.POINTER(MergeParams), C.POINTER(Tracks), vp, C.POINTER(Merged)]
         L.tpc_merge_tracks.restype = C.c_int
+        L.tpc_refit_chains.argtypes = [vp, C.POINTER(Clusters), C.POINTER(Tracks), C.POINTER(Merged), vp, C.POINTER(Refit)]
+        L.tpc_refit_chains.restype = C.c_int
         L.tpc_merge_last_launches.argtypes = [vp]
         L.tpc_merge_last_launches.restype = C.c_int64
         L.tpc_strerror.argtypes = [C.c_int]
@@ -306,6 +313,23 @@ class Tracker:
         if rc != TPC_OK:
             raise TpcError(rc, "tpc_merge_tracks")
         return merged
+
+    def tpc_refit_chains(self, row, pad, time, outputs, merged, refit=None, stream=None):
+        """C8 on the DEVICE clusters, track outputs and C7 links (same stream); returns (ok, chain_hits, chain_pieces, par7, cov9)."""
+        torch = self._torch
+        out, st = outputs
+        K = max(int(st.max_tracks), 1)
+        if refit is None:
+            e = lambda shape, dt: torch.empty(shape, dtype=dt, device=self.device)
+            refit = (e(K, torch.int32), e(K, torch.int32), e(K, torch.int32), e((K, 7), torch.float32), e((K, 9), torch.float32))
+        cl = Clusters(row.data_ptr(), pad.data_ptr(), time.data_ptr(), None)
+        m = Merged(*(t.data_ptr() for t in merged))
+        r = Refit(*(t.data_ptr() for t in refit))
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        rc = self.lib.tpc_refit_chains(self.handle, C.byref(cl), C.byref(st), C.byref(m), C.c_void_p(s.cuda_stream), C.byref(r))
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_refit_chains")
+        return refit
 
     def merge_scratch_bytes(self, max_tracks: int) -> int:
         return int(self.lib.tpc_merge_scratch_bytes(self.handle, int(max_tracks)))

@@ -23,11 +23,13 @@ def _gpu_track_and_merge(tf, cfg, n_sectors=36, merge_params=None):
     d = [torch.from_numpy(np.ascontiguousarray(a, np.float32)).to(trk.device) for a in (tf.row, tf.pad, tf.time)]
     outs = trk.alloc_outputs(n)
     out = trk.tpc_track_timeframe(*d, n=n, outputs=outs)
-    nxt, prv, root, n_links = trk.tpc_merge_tracks(outs, merge_params)
+    nxt, prv, root, n_links = merged = trk.tpc_merge_tracks(outs, merge_params)
+    launches_merge = trk.last_merge_launches()
+    rf = trk.tpc_refit_chains(*d, outs, merged)
     torch.cuda.synchronize()
     k = int(out.n_tracks[0])
-    res = dict(k=k, seed=out.seed_hit[:k].cpu().numpy(), next=nxt.cpu().numpy(), prev=prv.cpu().numpy(), root=root.cpu().numpy(),
-               n_links=int(n_links[0]), launches=trk.last_merge_launches(), status=int(out.status[0]),
+    res = dict(k=k, refit=tuple(t[:k].cpu().numpy() for t in rf), launches_refit=trk.last_merge_launches(), seed=out.seed_hit[:k].cpu().numpy(), next=nxt.cpu().numpy(), prev=prv.cpu().numpy(), root=root.cpu().numpy(),
+               n_links=int(n_links[0]), launches=launches_merge, status=int(out.status[0]),
                sector=out.sector[:k].cpu().numpy(), first_row=out.first_row[:k].cpu().numpy(), last_row=out.last_row[:k].cpu().numpy())
     trk.close()
     return res
@@ -36,10 +38,12 @@ def _gpu_track_and_merge(tf, cfg, n_sectors=36, merge_params=None):
 def _oracle_track_and_merge(tf, cfg, n_sectors=36, mp=None):
     import oracle
     from oracle import merge as M
-    res = oracle.track(oracle.default_geometry(n_sectors, tf.max_time_bin), oracle.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm),
-                       tf.row, tf.pad, tf.time)
+    g, p = oracle.default_geometry(n_sectors, tf.max_time_bin), oracle.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm)
+    res = oracle.track(g, p, tf.row, tf.pad, tf.time)
     mp = mp if mp is not None else M.default_merge_params(n_sectors)
-    return res, M.merge(mp, res.tr_seed, res.tr_sector, res.tr_first_row, res.tr_last_row, res.tr_par)
+    mr = M.merge(mp, res.tr_seed, res.tr_sector, res.tr_first_row, res.tr_last_row, res.tr_par)
+    mr.refit = oracle.refit_chains(g, p, tf.row, tf.pad, tf.time, res, mr.next, mr.prev)
+    return res, mr
 
 
 def _as_seed_links(seed, idx):
@@ -57,6 +61,16 @@ def _compare(g, res, mr):
     assert g["n_links"] == mr.n_links
     assert np.all(g["next"][k:] == -1) and np.all(g["prev"][k:] == -1) and np.all(g["root"][k:] == -1)
     assert g["launches"] >= 8
+    # C8: refit of the chains -- flags and counts exact, fits within the stated tolerances (in fact bit-identical)
+    ok, ch, cp, rp, rc = (a[go] for a in g["refit"])
+    o_ok, o_ch, o_cp, o_rp, o_rc = (a[oo] for a in mr.refit)
+    np.testing.assert_array_equal(ok, o_ok, err_msg="refit ok")
+    np.testing.assert_array_equal(ch, o_ch, err_msg="chain hits")
+    np.testing.assert_array_equal(cp, o_cp, err_msg="chain pieces")
+    from parity_util import _check_par
+    _check_par(rp, o_rp, "refit")
+    assert np.array_equal(rp, o_rp) and np.array_equal(rc, o_rc), "refit not bit-identical"
+    assert g["launches_refit"] == 2
 
 
 @pytest.mark.parametrize("seed", [1, 2, 3])
