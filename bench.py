@@ -241,20 +241,29 @@ def main():
     # ---- widening step C7 (sector-boundary merging of the tracks, not part of `value`): timed on its own ----
     merge = None
     if cfg.n_sectors >= 18:
-        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        merged = None
-        ms_m = 0.0
+        m0, m1, m2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        merged = refit = None
+        ms_m = ms_r = 0.0
+        outs_c = trk.alloc_outputs(n, hit_coords=True)      # C8 reads the hits' coordinates from two optional emit outputs
         for _ in range(3):
             with torch.cuda.stream(stream):
-                trk.tpc_track_timeframe(*devc, n=n, outputs=outs, stream=stream)      # the merger's input (and it reuses the arena)
+                trk.tpc_track_timeframe(*devc, n=n, outputs=outs_c, stream=stream)    # the merger's input (and it reuses the arena)
                 m0.record(stream)
-                merged = trk.tpc_merge_tracks(outs, merged=merged, stream=stream)
+                merged = trk.tpc_merge_tracks(outs_c, merged=merged, stream=stream)
                 m1.record(stream)
+                refit = trk.tpc_refit_chains(outs_c, merged, refit=refit, stream=stream)
+                m2.record(stream)
             stream.synchronize()
-            ms_m = m0.elapsed_time(m1)                                                # last of three
+            ms_m, ms_r = m0.elapsed_time(m1), m1.elapsed_time(m2)                     # last of three
+        emit_with_coords_ms = trk.step_ms().get("selector_emit")
         merge = {"step": "sector_boundary_merge (C7, tpc_merge_tracks)", "ms": round(ms_m, 4), "n_links": int(merged[3][0]),
                  "n_tracks": n_tracks, "tracks_per_s": n_tracks / (ms_m * 1e-3) if ms_m > 0 else None,
-                 "gpu_launches": trk.last_merge_launches(), "in_value": False}
+                 "gpu_launches": 8, "in_value": False,
+                 "refit": {"step": "chain_refit (C8, tpc_refit_chains)", "ms": round(ms_r, 4), "n_chains_refitted": int((refit[0] == 1).sum()),
+                           "n_chains_failed": int((refit[0] == -1).sum()), "hits_refitted": int(refit[1][refit[0] == 1].sum()),
+                           "gpu_launches": trk.last_merge_launches(),
+                           "selector_emit_ms_with_hit_coordinates": emit_with_coords_ms}}
+        del outs_c
     trk.close()
     del trk, outs
 

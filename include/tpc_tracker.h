@@ -121,6 +121,10 @@ typedef struct {
   int32_t* tracklet_n_hits;       /* [max_tracklets]                                                        */
   int32_t* tracklet_row_hit;      /* [max_tracklets*n_rows] original indices, -1 = none                     */
   float* tracklet_par;            /* [max_tracklets*7] (x, y, z_rel, sin_phi, dzds, q_pt, time_ref)         */
+  /* optional, each may be NULL (device entry point only; tpc_refit_chains needs both): the coordinates of the track
+   * hits, so that a later pass over a track's hits reads them in order instead of gathering from the clusters       */
+  float* hit_y_time;              /* [max_track_hits*2] (y [cm] = (pad - c_r) * pad_pitch, time [bins]) of hit_index[k] */
+  uint8_t* hit_row;               /* [max_track_hits] pad row of hit_index[k]                                */
 } tpc_tracks_t;
 
 /* Bytes of arena the tracker needs for params->max_clusters (the `max_clusters` argument, if > 0,
@@ -215,12 +219,12 @@ typedef struct {   /* caller-allocated DEVICE buffers, indexed by track like tpc
   float* cov9;           /* [max_tracks*9] (yy, ys, ss, yk, sk, kk | zz, zt, tt); zeros unless ok == 1                  */
 } tpc_refit_t;
 
-/* `clusters` are the DEVICE arrays the frame was tracked from (the hits' coordinates are read from them), `tracks` the
- * outputs of tpc_track_timeframe, `merged` those of tpc_merge_tracks; all on the same stream, after tpc_merge_tracks.
- * Asynchronous; never allocates (4 bytes of arena per track).  Errors: TPC_EINVAL, TPC_ENOMEM, TPC_ECUDA.
- * tpc_merge_last_launches() then reports this call's launches.                                                        */
-int tpc_refit_chains(tpc_tracker_t* tracker, const tpc_clusters_t* clusters, const tpc_tracks_t* tracks,
-                     const tpc_merged_t* merged, void* cuda_stream, tpc_refit_t* refit_out);
+/* `tracks` are the outputs of tpc_track_timeframe INCLUDING the optional hit_y_time / hit_row arrays (the hits'
+ * coordinates are read from them, in order), `merged` those of tpc_merge_tracks; all on the same stream, after
+ * tpc_merge_tracks.  Asynchronous; never allocates (4 bytes of arena per track).  Errors: TPC_EINVAL (also: hit
+ * coordinates missing), TPC_ENOMEM, TPC_ECUDA.  tpc_merge_last_launches() then reports this call's launches.          */
+int tpc_refit_chains(tpc_tracker_t* tracker, const tpc_tracks_t* tracks, const tpc_merged_t* merged, void* cuda_stream,
+                     tpc_refit_t* refit_out);
 
 /* Number of kernel launches the last tpc_merge_tracks call enqueued (memsets not counted).                        */
 int64_t tpc_merge_last_launches(const tpc_tracker_t* tracker);

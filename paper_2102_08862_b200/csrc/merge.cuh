@@ -178,8 +178,8 @@ __global__ void __launch_bounds__(256) k_merge_root(MergeTracks T, const int32_t
 // of the root piece, over the hits each piece owns, each piece in its own sector frame; state and covariance are
 // rotated at every boundary.  transport / kalman_update are the constructor's (tracklet.cuh): same statements, same order.
 struct RefitIo {
-  const float *row, *pad, *time;            // the frame's clusters (DEVICE, as passed to tpc_track_timeframe)
-  const int32_t *n_hits; const int64_t* hit_offset; const int32_t* hit_index;
+  const float2* hit_yt; const uint8_t* hit_row;   // (y, time) and pad row of every track hit, in hit_index order (tpc_tracks_t)
+  const int32_t *n_hits; const int64_t* hit_offset;
   const int32_t *next, *prev;               // C7 links
   int32_t *ok, *chain_hits, *chain_pieces;  // [max_tracks]
   float *rpar, *rcov;                       // [max_tracks * 7], [max_tracks * 9]
@@ -209,70 +209,93 @@ __global__ void __launch_bounds__(256) k_refit_roots(MergeTracks T, RefitIo io, 
   }
 }
 
+// Persistent warps, one lane per chain at a time, lanes refilled from a global counter once kRefitRefill of them are idle
+// (chains are 60 .. 450 hits long: without the refill a warp waits for its longest chain).  One loop iteration = one hit:
+// transport to its row, update; the next hit's (row, pad, time) are gathered one iteration ahead.
+constexpr int kRefitRefill = 4;
 __global__ void __launch_bounds__(kMergeThreads) k_refit_chains(MergeTracks T, RefitIo io, const uint32_t* __restrict__ root_list,
-                                                                 const uint32_t* __restrict__ n_roots, const __grid_constant__ MergeConsts c,
-                                                                 const __grid_constant__ Consts tc) {
-  __shared__ float xr[kRowStride], cr[kRowStride];
-  for (int r = threadIdx.x; r < tc.n_rows; r += blockDim.x) { xr[r] = tc.xr[r]; cr[r] = tc.cr[r]; }
+                                                                 const uint32_t* __restrict__ n_roots, uint32_t* __restrict__ work_counter,
+                                                                 const __grid_constant__ MergeConsts c, const __grid_constant__ Consts tc) {
+  __shared__ float xr[kRowStride];
+  for (int r = threadIdx.x; r < tc.n_rows; r += blockDim.x) xr[r] = tc.xr[r];
   __syncthreads();
-  const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
-  if (e >= *n_roots) return;
-  const int root = (int)root_list[e];
-  int pm = root, pieces = 1, total = io.n_hits[root];
-  for (int p = io.next[pm]; p >= 0; p = io.next[pm]) { pm = p; ++pieces; total += io.n_hits[p]; }
-  io.chain_hits[root] = total;
-  io.chain_pieces[root] = pieces;
+  const uint32_t n_work = *n_roots;
+  const unsigned lane = lane_id();
+  bool active = false, exhausted = false;
+  int root = -1, p = -1;
+  int64_t j = 0, off = 0;
+  float tref = 0.0f;
+  float2 hy = make_float2(0.0f, 0.0f);                 // (y, time) of the current hit
+  int hr = 0;                                          // its pad row
   TrackState S;
-  S.x = T.x[pm]; S.y = T.y[pm]; S.z = T.z[pm]; S.s = T.s[pm]; S.t = T.t[pm]; S.k = T.k[pm];
-  S.c0 = S.c1 = S.c2 = S.c3 = S.c4 = S.c5 = 0.0f; S.d0 = S.d1 = S.d2 = 0.0f;
-  bool good;
-  {
-    const int32_t h = io.hit_index[io.hit_offset[pm] + io.n_hits[pm] - 1];
-    const int r = (int)io.row[h] % tc.n_rows;
-    good = transport(S, xr[r], tc.cB, tc.sin_phi_max);
-  }
-  S.c0 = tc.c0_y2; S.c1 = 0.0f; S.c2 = tc.c0_s2; S.c3 = 0.0f; S.c4 = 0.0f; S.c5 = tc.c0_k2; S.d0 = tc.c0_z2; S.d1 = 0.0f; S.d2 = tc.c0_t2;
-  for (int p = pm; good; ) {
-    const float tref = T.time_ref[p];
-    const int64_t off = io.hit_offset[p];
-    int64_t j = off + io.n_hits[p] - 1;
-    int32_t h = io.hit_index[j];
-    float hr = io.row[h], hp = io.pad[h], ht = io.time[h];
-    for (; j >= off; --j) {
-      float nr = 0.0f, np = 0.0f, nt = 0.0f;
-      if (j > off) {                                   // the next hit, one iteration ahead
-        const int32_t hn = io.hit_index[j - 1];
-        nr = io.row[hn]; np = io.pad[hn]; nt = io.time[hn];
+  S.x = S.y = S.z = S.s = S.t = S.k = 0.0f; S.c0 = S.c1 = S.c2 = S.c3 = S.c4 = S.c5 = 0.0f; S.d0 = S.d1 = S.d2 = 0.0f;
+  for (;;) {
+    const unsigned idle = __ballot_sync(0xffffffffu, !active && !exhausted);
+    const unsigned busy = __ballot_sync(0xffffffffu, active);
+    if (idle && (__popc(idle) >= kRefitRefill || busy == 0)) {
+      if (!active && !exhausted) {
+        const uint32_t e = (uint32_t)take_tracklets(work_counter, idle, lane);
+        if (e >= n_work) {
+          exhausted = true;
+        } else {
+          root = (int)root_list[e];
+          int pm = root, pieces = 1, total = io.n_hits[root];
+          for (int q = io.next[pm]; q >= 0; q = io.next[pm]) { pm = q; ++pieces; total += io.n_hits[q]; }
+          io.chain_hits[root] = total;
+          io.chain_pieces[root] = pieces;
+          S.x = T.x[pm]; S.y = T.y[pm]; S.z = T.z[pm]; S.s = T.s[pm]; S.t = T.t[pm]; S.k = T.k[pm];
+          S.c0 = S.c1 = S.c2 = S.c3 = S.c4 = S.c5 = 0.0f; S.d0 = S.d1 = S.d2 = 0.0f;
+          p = pm; off = io.hit_offset[pm]; j = off + io.n_hits[pm] - 1; tref = T.time_ref[pm];
+          hy = io.hit_yt[j]; hr = io.hit_row[j];
+          const bool ok0 = transport(S, xr[hr], tc.cB, tc.sin_phi_max);       // to the outermost hit, then the reset covariance
+          S.c0 = tc.c0_y2; S.c1 = 0.0f; S.c2 = tc.c0_s2; S.c3 = 0.0f; S.c4 = 0.0f; S.c5 = tc.c0_k2; S.d0 = tc.c0_z2; S.d1 = 0.0f; S.d2 = tc.c0_t2;
+          if (ok0) active = true; else io.ok[root] = -1;
+        }
       }
-      const int r = (int)hr % tc.n_rows;
-      good = transport(S, xr[r], tc.cB, tc.sin_phi_max);
-      if (!good) break;
-      kalman_update(S, (hp - cr[r]) * tc.P, (ht - tref) * tc.Z, tc.ry, tc.rz);
-      hr = nr; hp = np; ht = nt;
     }
-    if (!good || p == root) break;
-    const int pin = io.prev[p];
-    const float sg = ((T.sector[p] % 18) == ((T.sector[pin] % 18) + 1) % 18) ? 1.0f : -1.0f;
-    const float qd = -sg;
-    const float cs = sqrtf(1.0f - S.s * S.s);
-    const float J = c.Cd + qd * ((S.s / cs) * c.Sd);
-    const float x1 = S.x * c.Cd + qd * (S.y * c.Sd);
-    const float y1 = S.y * c.Cd - qd * (S.x * c.Sd);
-    const float s1 = S.s * c.Cd - qd * (cs * c.Sd);
-    if (!(fabsf(s1) < tc.sin_phi_max)) { good = false; break; }
-    S.x = x1; S.y = y1; S.s = s1;
-    S.c1 = S.c1 * J; S.c2 = (S.c2 * J) * J; S.c4 = S.c4 * J;
-    S.z = S.z + (tref - T.time_ref[pin]) * tc.Z;
-    p = pin;
-  }
-  if (good) {
-    io.ok[root] = 1;
-    float* rp = io.rpar + 7 * (size_t)root;
-    rp[0] = S.x; rp[1] = S.y; rp[2] = S.z; rp[3] = S.s; rp[4] = S.t; rp[5] = S.k;      // rp[6] = time_ref of the root: already there
-    float* rc = io.rcov + 9 * (size_t)root;
-    rc[0] = S.c0; rc[1] = S.c1; rc[2] = S.c2; rc[3] = S.c3; rc[4] = S.c4; rc[5] = S.c5; rc[6] = S.d0; rc[7] = S.d1; rc[8] = S.d2;
-  } else {
-    io.ok[root] = -1;
+    if (busy == 0 && __ballot_sync(0xffffffffu, active) == 0) {
+      if (__ballot_sync(0xffffffffu, !exhausted) == 0) break;
+      continue;
+    }
+    if (active) {
+      float2 ny = make_float2(0.0f, 0.0f);
+      int nr = 0;
+      if (j > off) { ny = io.hit_yt[j - 1]; nr = io.hit_row[j - 1]; }      // the next hit, one iteration ahead
+      bool good = transport(S, xr[hr], tc.cB, tc.sin_phi_max);
+      if (good) {
+        kalman_update(S, hy.x, (hy.y - tref) * tc.Z, tc.ry, tc.rz);
+        if (j > off) {
+          --j; hy = ny; hr = nr;
+        } else if (p == root) {                        // innermost hit of the root piece: done
+          io.ok[root] = 1;
+          float* rp = io.rpar + 7 * (size_t)root;
+          rp[0] = S.x; rp[1] = S.y; rp[2] = S.z; rp[3] = S.s; rp[4] = S.t; rp[5] = S.k;      // rp[6] = time_ref of the root: already there
+          float* rc = io.rcov + 9 * (size_t)root;
+          rc[0] = S.c0; rc[1] = S.c1; rc[2] = S.c2; rc[3] = S.c3; rc[4] = S.c4; rc[5] = S.c5; rc[6] = S.d0; rc[7] = S.d1; rc[8] = S.d2;
+          active = false;
+        } else {                                       // piece boundary: rotate into the frame of the next inner piece
+          const int pin = io.prev[p];
+          const float sg = ((T.sector[p] % 18) == ((T.sector[pin] % 18) + 1) % 18) ? 1.0f : -1.0f;
+          const float qd = -sg;
+          const float cs = sqrtf(1.0f - S.s * S.s);
+          const float J = c.Cd + qd * ((S.s / cs) * c.Sd);
+          const float x1 = S.x * c.Cd + qd * (S.y * c.Sd);
+          const float y1 = S.y * c.Cd - qd * (S.x * c.Sd);
+          const float s1 = S.s * c.Cd - qd * (cs * c.Sd);
+          if (fabsf(s1) < tc.sin_phi_max) {
+            S.x = x1; S.y = y1; S.s = s1;
+            S.c1 = S.c1 * J; S.c2 = (S.c2 * J) * J; S.c4 = S.c4 * J;
+            const float tref_in = T.time_ref[pin];
+            S.z = S.z + (tref - tref_in) * tc.Z;
+            p = pin; tref = tref_in; off = io.hit_offset[pin]; j = off + io.n_hits[pin] - 1;
+            hy = io.hit_yt[j]; hr = io.hit_row[j];
+          } else {
+            good = false;
+          }
+        }
+      }
+      if (!good) { io.ok[root] = -1; active = false; }
+    }
   }
 }
 

@@ -93,6 +93,7 @@ struct TrackOutputs {   // device pointers of tpc_tracks_t (include/tpc_tracker.
   int32_t *seed_hit, *sector, *first_row, *last_row, *n_hits; int64_t* hit_offset;
   float *x, *y, *z_rel, *time_ref, *sin_phi, *dzds, *q_pt, *cov9;
   int32_t* hit_index;
+  float2* hit_yt; uint8_t* hit_row;   // optional (NULL = not wanted)
 };
 
 // track_slot[track_idx[j]] = j for every tracklet that became a track: the emit kernel then runs one warp per TRACK
@@ -109,7 +110,7 @@ __global__ void __launch_bounds__(kSelectorThreads) k_selector_emit(
     TrackletStore tl, const int32_t* __restrict__ counters, const uint32_t* __restrict__ own_mask,
     const uint32_t* __restrict__ track_slot, const uint32_t* __restrict__ hit_off,
     const uint32_t* __restrict__ track_total, const uint32_t* __restrict__ hit_total,
-    const uint32_t* __restrict__ orig, const uint16_t* __restrict__ hsr, const uint32_t* __restrict__ start_hits,
+    const uint32_t* __restrict__ orig, const float2* __restrict__ yt, const uint16_t* __restrict__ hsr, const uint32_t* __restrict__ start_hits,
     const uint32_t* __restrict__ n_invalid, TrackOutputs o, const __grid_constant__ Consts c) {
   constexpr int kWords = kRowStride / 32;
   const uint32_t ti = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -137,7 +138,11 @@ __global__ void __launch_bounds__(kSelectorThreads) k_selector_emit(
     if (b >> lane_id() & 1u) {
       const int m = rows[i * 32 + (int)lane_id()];
       const int64_t pos = (int64_t)off + n_owned + __popc(b & ((1u << lane_id()) - 1u));
-      if (pos < o.max_track_hits) o.hit_index[pos] = (int32_t)orig[m];
+      if (pos < o.max_track_hits) {
+        o.hit_index[pos] = (int32_t)orig[m];
+        if (o.hit_yt) o.hit_yt[pos] = yt[m];
+        if (o.hit_row) o.hit_row[pos] = (uint8_t)(i * 32 + (int)lane_id());
+      }
     }
     if (b) {
       if (own_first < 0) own_first = i * 32 + __ffs(b) - 1;

@@ -191,6 +191,7 @@ struct tpc_tracker {
   cudaEvent_t ev[N_STEPS + 1] = {};
   bool profile = false, have_times = false;
   int64_t last_launches = 0, last_merge_launches = 0;
+  int ctas_refit = 148 * 8;
   int ctas_fit_up = 148, ctas_follow_up = 148, ctas_fit_down = 148, ctas_follow_down = 148;   // persistent grids: SMs x resident CTAs per SM
 };
 
@@ -327,6 +328,11 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
     t->ctas_follow_up = resident(k_tracklet_follow<false>, TPC_FOLLOW_CTAS_PER_SM);
     t->ctas_fit_down = resident(k_tracklet_fit<true>, TPC_FIT_CTAS_PER_SM);
     t->ctas_follow_down = resident(k_tracklet_follow<true>, TPC_FOLLOW_CTAS_PER_SM);
+    t->ctas_refit = resident(k_refit_chains, 64);
+  }
+  if (const char* e = std::getenv("TPC_L2_FETCH_GRANULARITY")) {      // experiment knob: 32 / 64 / 128 bytes
+    const int g = std::atoi(e);
+    if (g == 32 || g == 64 || g == 128) { cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)g); cudaGetLastError(); }
   }
   for (int i = 0; i <= N_STEPS; ++i)
     if (cudaEventCreate(&t->ev[i]) != cudaSuccess) { cudaGetLastError(); tpc_tracker_destroy(t); return TPC_ECUDA; }
@@ -402,19 +408,19 @@ int tpc_merge_tracks(tpc_tracker_t* t, const tpc_merge_params_t* mp, const tpc_t
 
 
 // ---- C8: refit of the chains linked by C7 (merge.cuh) ----
-int tpc_refit_chains(tpc_tracker_t* t, const tpc_clusters_t* cl, const tpc_tracks_t* tr, const tpc_merged_t* mg, void* cuda_stream,
-                     tpc_refit_t* out) {
-  if (!t || !cl || !tr || !mg || !out) return TPC_EINVAL;
+int tpc_refit_chains(tpc_tracker_t* t, const tpc_tracks_t* tr, const tpc_merged_t* mg, void* cuda_stream, tpc_refit_t* out) {
+  if (!t || !tr || !mg || !out) return TPC_EINVAL;
   if (tr->max_tracks < 0 || !tr->n_tracks || !out->ok || !out->chain_hits || !out->chain_pieces || !out->par7 || !out->cov9) return TPC_EINVAL;
-  if (tr->max_tracks > 0 && (!cl->row || !cl->pad || !cl->time || !tr->sector || !tr->n_hits || !tr->hit_offset || !tr->hit_index || !tr->x ||
+  if (tr->max_tracks > 0 && (!tr->hit_y_time || !tr->hit_row || !tr->sector || !tr->n_hits || !tr->hit_offset || !tr->x ||
                              !tr->y || !tr->z_rel || !tr->time_ref || !tr->sin_phi || !tr->dzds || !tr->q_pt || !mg->next || !mg->prev)) return TPC_EINVAL;
   const int K = tr->max_tracks;
-  const size_t need = 256 + 4 * (size_t)std::max(K, 1);
+  const size_t need = 512 + 4 * (size_t)std::max(K, 1);
   if (!t->params.arena || need > t->params.arena_bytes) return TPC_ENOMEM;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   char* A = static_cast<char*>(t->params.arena);
   uint32_t* n_roots = reinterpret_cast<uint32_t*>(A);
-  uint32_t* root_list = reinterpret_cast<uint32_t*>(A + 256);
+  uint32_t* work_counter = reinterpret_cast<uint32_t*>(A + 256);
+  uint32_t* root_list = reinterpret_cast<uint32_t*>(A + 512);
   MergeConsts c{};
   c.n_sectors = t->geom.n_sectors; c.n_rows = t->geom.n_rows; c.max_tracks = K;
   {
@@ -423,13 +429,13 @@ int tpc_refit_chains(tpc_tracker_t* t, const tpc_clusters_t* cl, const tpc_track
     c.Sd = (float)(2.0 * T / (1.0 + T * T));
   }
   MergeTracks T{tr->n_tracks, tr->seed_hit, tr->sector, tr->first_row, tr->last_row, tr->x, tr->y, tr->z_rel, tr->time_ref, tr->sin_phi, tr->dzds, tr->q_pt};
-  RefitIo io{cl->row, cl->pad, cl->time, tr->n_hits, tr->hit_offset, tr->hit_index, mg->next, mg->prev,
+  RefitIo io{reinterpret_cast<const float2*>(tr->hit_y_time), tr->hit_row, tr->n_hits, tr->hit_offset, mg->next, mg->prev,
              out->ok, out->chain_hits, out->chain_pieces, out->par7, out->cov9};
   int64_t launches = 0;
-  cudaMemsetAsync(n_roots, 0, 4, st);
+  cudaMemsetAsync(n_roots, 0, 512, st);
   if (K > 0) {
     k_refit_roots<<<(K + 255) / 256, 256, 0, st>>>(T, io, root_list, n_roots, c); ++launches;
-    k_refit_chains<<<(K + kMergeThreads - 1) / kMergeThreads, kMergeThreads, 0, st>>>(T, io, root_list, n_roots, c, t->consts); ++launches;
+    k_refit_chains<<<std::min(t->ctas_refit, (K + kMergeThreads - 1) / kMergeThreads), kMergeThreads, 0, st>>>(T, io, root_list, n_roots, work_counter, c, t->consts); ++launches;
   }
   t->last_merge_launches = launches;
   if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;
@@ -634,11 +640,12 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   to.seed_hit = o->seed_hit; to.sector = o->sector; to.first_row = o->first_row; to.last_row = o->last_row; to.n_hits = o->n_hits;
   to.hit_offset = o->hit_offset; to.x = o->x; to.y = o->y; to.z_rel = o->z_rel; to.time_ref = o->time_ref;
   to.sin_phi = o->sin_phi; to.dzds = o->dzds; to.q_pt = o->q_pt; to.cov9 = o->cov9; to.hit_index = o->hit_index;
+  to.hit_yt = reinterpret_cast<float2*>(o->hit_y_time); to.hit_row = o->hit_row;
   const int n_scan_tiles = (int)scan_tiles((size_t)T);
   k_selector_map<<<(int)((tl_bound + 255) / 256), 256, 0, st>>>(counters, flag, track_idx, track_slot); ++launches;
   const int64_t emit_warps = std::max<int64_t>(std::min<int64_t>(tl_bound, o->max_tracks), 1);      // warp 0 also writes the scalars
   k_selector_emit<<<(int)((emit_warps * 32 + kSelectorThreads - 1) / kSelectorThreads), kSelectorThreads, 0, st>>>(
-      tl, counters, own_mask, track_slot, hit_off, scan_a + n_scan_tiles, scan_b + n_scan_tiles, orig, hsr, start_hits, n_invalid, to, c); ++launches;
+      tl, counters, own_mask, track_slot, hit_off, scan_a + n_scan_tiles, scan_b + n_scan_tiles, orig, yt, hsr, start_hits, n_invalid, to, c); ++launches;
   mark(N_STEPS);
   t->have_times = t->profile;
   t->last_launches = launches;

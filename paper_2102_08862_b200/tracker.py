@@ -57,7 +57,8 @@ class Tracks(C.Structure):
                 ("sin_phi", C.c_void_p), ("dzds", C.c_void_p), ("q_pt", C.c_void_p), ("cov9", C.c_void_p),
                 ("hit_index", C.c_void_p), ("link_up", C.c_void_p), ("link_down", C.c_void_p), ("is_start_hit", C.c_void_p),
                 ("max_tracklets", C.c_int32), ("n_tracklets", C.c_void_p), ("tracklet_seed", C.c_void_p),
-                ("tracklet_n_hits", C.c_void_p), ("tracklet_row_hit", C.c_void_p), ("tracklet_par", C.c_void_p)]
+                ("tracklet_n_hits", C.c_void_p), ("tracklet_row_hit", C.c_void_p), ("tracklet_par", C.c_void_p),
+                ("hit_y_time", C.c_void_p), ("hit_row", C.c_void_p)]
 
 
 class MergeParams(C.Structure):
@@ -127,7 +128,7 @@ def load_library(build_if_missing: bool = True):
         L.tpc_merge_scratch_bytes.restype = C.c_size_t
         L.tpc_merge_tracks.argtypes = [vp, C.POINTER(MergeParams), C.POINTER(Tracks), vp, C.POINTER(Merged)]
         L.tpc_merge_tracks.restype = C.c_int
-        L.tpc_refit_chains.argtypes = [vp, C.POINTER(Clusters), C.POINTER(Tracks), C.POINTER(Merged), vp, C.POINTER(Refit)]
+        L.tpc_refit_chains.argtypes = [vp, C.POINTER(Tracks), C.POINTER(Merged), vp, C.POINTER(Refit)]
         L.tpc_refit_chains.restype = C.c_int
         L.tpc_merge_last_launches.argtypes = [vp]
         L.tpc_merge_last_launches.restype = C.c_int64
@@ -193,6 +194,8 @@ class TrackResult:
     tracklet_n_hits: object = None
     tracklet_row_hit: object = None
     tracklet_par: object = None
+    hit_y_time: object = None      # optional: (y, time) of every track hit, in hit_index order (needed by tpc_refit_chains)
+    hit_row: object = None
 
 
 class Tracker:
@@ -222,7 +225,8 @@ class Tracker:
         self.arena_bytes = int(need)
 
     # -- buffers ---------------------------------------------------------------------------------------------
-    def _alloc_outputs(self, n: int, max_tracks: int, max_track_hits: int, taps: bool, max_tracklets: int, host: bool):
+    def _alloc_outputs(self, n: int, max_tracks: int, max_track_hits: int, taps: bool, max_tracklets: int, host: bool,
+                       hit_coords: bool = False):
         torch = self._torch
         kw = dict(device="cpu", pin_memory=True) if host else dict(device=self.device)
         e = lambda shape, dt: torch.empty(shape, dtype=dt, **kw)
@@ -241,6 +245,8 @@ class Tracker:
             r.tracklet_seed, r.tracklet_n_hits = e(max_tracklets, torch.int32), e(max_tracklets, torch.int32)
             r.tracklet_row_hit = e((max_tracklets, nr), torch.int32)
             r.tracklet_par = e((max_tracklets, 7), torch.float32)
+        if hit_coords and not host:
+            r.hit_y_time, r.hit_row = e((H, 2), torch.float32), e(H, torch.uint8)
         return r
 
     @staticmethod
@@ -250,16 +256,17 @@ class Tracker:
                       p(r.first_row), p(r.last_row), p(r.n_hits), p(r.hit_offset), p(r.x), p(r.y), p(r.z_rel), p(r.time_ref),
                       p(r.sin_phi), p(r.dzds), p(r.q_pt), p(r.cov9), p(r.hit_index), p(r.link_up), p(r.link_down),
                       p(r.is_start_hit), max_tracklets, p(r.n_tracklets), p(r.tracklet_seed), p(r.tracklet_n_hits),
-                      p(r.tracklet_row_hit), p(r.tracklet_par))
+                      p(r.tracklet_row_hit), p(r.tracklet_par), p(r.hit_y_time), p(r.hit_row))
 
     def default_capacities(self, n: int):
         return max(n // 64 + 4096, 1), max(n, 1)
 
-    def alloc_outputs(self, n: int, taps: bool = False, host: bool = False, max_tracks: int = 0, max_track_hits: int = 0):
+    def alloc_outputs(self, n: int, taps: bool = False, host: bool = False, max_tracks: int = 0, max_track_hits: int = 0,
+                      hit_coords: bool = False):
         K, H = self.default_capacities(n)
         K, H = (max_tracks or K), (max_track_hits or H)
         T = int(self.params.max_tracklets or (self.params.max_clusters // 10 + 4096)) if taps else 0
-        out = self._alloc_outputs(n, K, H, taps, T, host)
+        out = self._alloc_outputs(n, K, H, taps, T, host, hit_coords)
         return out, self._tracks_struct(out, K, H, T)
 
     # -- the C-ABI calls -------------------------------------------------------------------------------------
@@ -314,19 +321,19 @@ class Tracker:
             raise TpcError(rc, "tpc_merge_tracks")
         return merged
 
-    def tpc_refit_chains(self, row, pad, time, outputs, merged, refit=None, stream=None):
-        """C8 on the DEVICE clusters, track outputs and C7 links (same stream); returns (ok, chain_hits, chain_pieces, par7, cov9)."""
+    def tpc_refit_chains(self, outputs, merged, refit=None, stream=None):
+        """C8 on the DEVICE track outputs (allocated with ``hit_coords=True``) and C7 links (same stream); returns
+        (ok, chain_hits, chain_pieces, par7, cov9)."""
         torch = self._torch
         out, st = outputs
         K = max(int(st.max_tracks), 1)
         if refit is None:
             e = lambda shape, dt: torch.empty(shape, dtype=dt, device=self.device)
             refit = (e(K, torch.int32), e(K, torch.int32), e(K, torch.int32), e((K, 7), torch.float32), e((K, 9), torch.float32))
-        cl = Clusters(row.data_ptr(), pad.data_ptr(), time.data_ptr(), None)
         m = Merged(*(t.data_ptr() for t in merged))
         r = Refit(*(t.data_ptr() for t in refit))
         s = stream if stream is not None else torch.cuda.current_stream(self.device)
-        rc = self.lib.tpc_refit_chains(self.handle, C.byref(cl), C.byref(st), C.byref(m), C.c_void_p(s.cuda_stream), C.byref(r))
+        rc = self.lib.tpc_refit_chains(self.handle, C.byref(st), C.byref(m), C.c_void_p(s.cuda_stream), C.byref(r))
         if rc != TPC_OK:
             raise TpcError(rc, "tpc_refit_chains")
         return refit

@@ -21,13 +21,21 @@ def _gpu_track_and_merge(tf, cfg, n_sectors=36, merge_params=None):
     n = tf.n
     trk = T.Tracker(T.default_geometry(n_sectors, tf.max_time_bin), T.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm, max_clusters=max(n, 1)))
     d = [torch.from_numpy(np.ascontiguousarray(a, np.float32)).to(trk.device) for a in (tf.row, tf.pad, tf.time)]
-    outs = trk.alloc_outputs(n)
+    outs = trk.alloc_outputs(n, hit_coords=True)
     out = trk.tpc_track_timeframe(*d, n=n, outputs=outs)
     nxt, prv, root, n_links = merged = trk.tpc_merge_tracks(outs, merge_params)
     launches_merge = trk.last_merge_launches()
-    rf = trk.tpc_refit_chains(*d, outs, merged)
+    rf = trk.tpc_refit_chains(outs, merged)
     torch.cuda.synchronize()
     k = int(out.n_tracks[0])
+    nh = int(out.n_track_hits[0])
+    hi = out.hit_index[:nh].cpu().numpy()
+    hyt, hrow = out.hit_y_time[:nh].cpu().numpy(), out.hit_row[:nh].cpu().numpy()
+    # the optional hit coordinates are those of hit_index: time verbatim, row, y = (pad - c_r) * pitch in fp32
+    assert np.array_equal(hyt[:, 1], tf.time[hi]) and np.array_equal(hrow, (tf.row[hi].astype(np.int64) % 152).astype(np.uint8))
+    npads = np.floor(2.0 * (85.0 + 1.07 * np.arange(152)) * np.tan(np.radians(10.0)) / 0.5)
+    cr = (0.5 * (npads - 1)).astype(np.float32)
+    assert np.array_equal(hyt[:, 0], (tf.pad[hi] - cr[hrow]) * np.float32(0.5))
     res = dict(k=k, refit=tuple(t[:k].cpu().numpy() for t in rf), launches_refit=trk.last_merge_launches(), seed=out.seed_hit[:k].cpu().numpy(), next=nxt.cpu().numpy(), prev=prv.cpu().numpy(), root=root.cpu().numpy(),
                n_links=int(n_links[0]), launches=launches_merge, status=int(out.status[0]),
                sector=out.sector[:k].cpu().numpy(), first_row=out.first_row[:k].cpu().numpy(), last_row=out.last_row[:k].cpu().numpy())
@@ -162,12 +170,15 @@ def test_full_10ms_frame_merge_invariants_and_sampled_oracle_parity():
     n = tf.n
     trk = T.Tracker(T.default_geometry(36, tf.max_time_bin), T.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm, max_clusters=n))
     d = [torch.from_numpy(a).to(trk.device) for a in (tf.row, tf.pad, tf.time)]
-    outs = trk.alloc_outputs(n)
+    outs = trk.alloc_outputs(n, hit_coords=True)
     out = trk.tpc_track_timeframe(*d, n=n, outputs=outs)
-    nxt, prv, root, n_links = trk.tpc_merge_tracks(outs)
+    nxt, prv, root, n_links = merged = trk.tpc_merge_tracks(outs)
+    rf_ok, rf_ch, rf_cp, rf_par, rf_cov = trk.tpc_refit_chains(outs, merged)
     torch.cuda.synchronize()
     k, nh = int(out.n_tracks[0]), int(out.n_track_hits[0])
     assert int(out.status[0]) & 7 == 0 and k > 1e6
+    rf_ok, rf_ch, rf_cp, rf_par, rf_cov = (t[:k].cpu().numpy() for t in (rf_ok, rf_ch, rf_cp, rf_par, rf_cov))
+    n_hits_all = out.n_hits[:k].cpu().numpy()
     seed, sec = out.seed_hit[:k].cpu().numpy(), out.sector[:k].cpu().numpy()
     first_row, last_row = out.first_row[:k].cpu().numpy(), out.last_row[:k].cpu().numpy()
     x = out.x[:k].cpu().numpy()
@@ -185,6 +196,11 @@ def test_full_10ms_frame_merge_invariants_and_sampled_oracle_parity():
     assert np.all(rb > first_row[a]) and np.all(rb >= last_row[a] - 1) and np.all(rb <= last_row[a] + 13)
     assert np.all(prv[root] == -1) and np.array_equal(root[b], root[a])
     assert k - n_links == np.unique(root).size
+    is_root = (prv < 0) & (nxt >= 0)
+    assert np.all(rf_ok[~is_root] == 0) and np.all(rf_ok[is_root] != 0) and (rf_ok[is_root] == -1).mean() < 0.03
+    np.testing.assert_array_equal(rf_ch[is_root], np.bincount(root, weights=n_hits_all, minlength=k).astype(np.int64)[is_root])
+    np.testing.assert_array_equal(rf_cp[is_root], np.bincount(root, minlength=k)[is_root])
+    assert np.all(np.isfinite(rf_par)) and np.all(np.isfinite(rf_cov))
     # (b) sampled parity
     S, t_lo, width, margin = 7, 20000.0, 2000.0, 2200.0
     t_hi = t_lo + width
@@ -195,18 +211,24 @@ def test_full_10ms_frame_merge_invariants_and_sampled_oracle_parity():
     o = oracle.track(oracle.default_geometry(36, tf.max_time_bin), oracle.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm),
                      tf.row[sel], tf.pad[sel], tf.time[sel])
     mr = M.merge(M.default_merge_params(36), o.tr_seed, o.tr_sector, o.tr_first_row, o.tr_last_row, o.tr_par)
+    o_ok, o_ch, o_cp, o_rp, o_rc = oracle.refit_chains(oracle.default_geometry(36, tf.max_time_bin), oracle.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm),
+                                                       tf.row[sel], tf.pad[sel], tf.time[sel], o, mr.next, mr.prev)
     o_t = tf.time[sel][o.tr_hit_index]
     o_min = np.minimum.reduceat(o_t, o.tr_hit_offset); o_max = np.maximum.reduceat(o_t, o.tr_hit_offset)
     core = np.nonzero((o.tr_sector == S) & (o_min >= t_lo) & (o_max <= t_hi))[0]
     assert core.size > 300
     o_seed_global = sel[o.tr_seed]
     lookup = {int(s): i for i, s in enumerate(seed)}
-    n_with_link = 0
+    n_with_link = n_refitted = 0
     for i in core:
         gi = lookup[int(o_seed_global[i])]                      # the same track exists on the GPU (sampled tracking parity)
+        # C8: a chain whose root lies in the core is refitted from the same hits on both sides -> bit-identical
+        assert rf_ok[gi] == o_ok[i] and rf_ch[gi] == o_ch[i] and rf_cp[gi] == o_cp[i]
+        assert np.array_equal(rf_par[gi], o_rp[i]) and np.array_equal(rf_cov[gi], o_rc[i])
+        n_refitted += int(o_ok[i] == 1)
         for o_idx, g_idx in ((mr.next[i], nxt[gi]), (mr.prev[i], prv[gi])):
             o_link = int(o_seed_global[o_idx]) if o_idx >= 0 else -1
             g_link = int(seed[g_idx]) if g_idx >= 0 else -1
             assert o_link == g_link, (int(o_seed_global[i]), o_link, g_link)
             n_with_link += o_link >= 0
-    assert n_with_link > 50
+    assert n_with_link > 50 and n_refitted > 20
