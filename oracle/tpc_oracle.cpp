@@ -21,6 +21,9 @@
 // N2 noise-free straight track links; N3 reciprocity; K1 transport round trip / composition / exact
 // circle; K2 arc-length series vs asin; K3 KF == weighted least-squares line; K4 noise-free helix
 // end to end; S1 selector == sort-by-key first-come-first-served; E1 efficiency >= 95 % (pT > 0.2).
+// Also holds C8 (orc_refit_chains, further down: refit of the chains linked by the C7 oracle tpc_merge_oracle.cpp), pinned by
+// tests/test_refit_oracle_pins.py: F-J rotation Jacobian vs numerical derivative, F-H noise-free helices, F-N resolution and
+// pull width against generator truth, F-I bookkeeping.
 // Parity unpinned (no external truth exists): absolute fitted values on noisy data.
 #include <algorithm>
 #include <chrono>
