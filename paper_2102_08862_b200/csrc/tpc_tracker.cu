@@ -330,10 +330,6 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
     t->ctas_follow_down = resident(k_tracklet_follow<true>, TPC_FOLLOW_CTAS_PER_SM);
     t->ctas_refit = resident(k_refit_chains, 64);
   }
-  if (const char* e = std::getenv("TPC_L2_FETCH_GRANULARITY")) {      // experiment knob: 32 / 64 / 128 bytes
-    const int g = std::atoi(e);
-    if (g == 32 || g == 64 || g == 128) { cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)g); cudaGetLastError(); }
-  }
   for (int i = 0; i <= N_STEPS; ++i)
     if (cudaEventCreate(&t->ev[i]) != cudaSuccess) { cudaGetLastError(); tpc_tracker_destroy(t); return TPC_ECUDA; }
   *out = t;
