@@ -226,6 +226,15 @@ typedef struct {   /* caller-allocated DEVICE buffers, indexed by track like tpc
 int tpc_refit_chains(tpc_tracker_t* tracker, const tpc_tracks_t* tracks, const tpc_merged_t* merged, void* cuda_stream,
                      tpc_refit_t* refit_out);
 
+/* ---- C9: where and when a track passes the beam line (DESIGN.md §3 "C9"; z is only known once the
+ * collision time is).  Every state of `par7` (DEVICE, [max_tracks*7] = (x, y, z_rel, sin_phi, dzds, q_pt, time_ref): the
+ * par7 of tpc_refit_chains, or the same seven values of tpc_tracks_t) is transported to x = 0, the beam axis in every
+ * sector frame: vertex_time = time_ref + z / time_bin_cm [time bins] = (t0 v_drift + drift_len - side z_vertex) / time_bin_cm
+ * for a primary track, vertex_y [cm] its offset from the axis; ok = 0 (outputs 0) when sin phi would reach sin_phi_max.
+ * Outputs: DEVICE, [max_tracks].  Asynchronous, reads *n_tracks on the device.  Errors: TPC_EINVAL, TPC_ECUDA.          */
+int tpc_vertex_time(tpc_tracker_t* tracker, const int32_t* n_tracks, int32_t max_tracks, const float* par7,
+                    void* cuda_stream, int32_t* ok, float* vertex_time, float* vertex_y);
+
 /* Number of kernel launches the last tpc_merge_tracks call enqueued (memsets not counted).                        */
 int64_t tpc_merge_last_launches(const tpc_tracker_t* tracker);
 

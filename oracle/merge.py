@@ -53,6 +53,8 @@ def lib():
         L.orc_merge_rotate.restype = None
         L.orc_merge_transport.argtypes = [C.POINTER(MergeParams), vp, C.c_float]
         L.orc_merge_transport.restype = C.c_int
+        L.orc_vertex_time.argtypes = [C.POINTER(MergeParams), C.c_int64, vp, vp, vp, vp]
+        L.orc_vertex_time.restype = None
         _lib = L
     return _lib
 
@@ -90,3 +92,12 @@ def transport_state(p: MergeParams, state6, xn: float):
     st = np.array(state6, np.float32)
     ok = lib().orc_merge_transport(C.byref(p), st.ctypes.data, float(xn))
     return bool(ok), st
+
+
+def vertex_time(p: MergeParams, par):
+    """C9: (ok, vertex_time [time bins], vertex_y [cm]) of every state in ``par`` (float32[n, 7]) transported to the beam line."""
+    par = np.ascontiguousarray(par, np.float32).reshape(-1, 7)
+    n = int(par.shape[0])
+    ok, t, y = np.zeros(n, np.int32), np.zeros(n, np.float32), np.zeros(n, np.float32)
+    lib().orc_vertex_time(C.byref(p), n, par.ctypes.data, ok.ctypes.data, t.ctypes.data, y.ctypes.data)
+    return ok, t, y

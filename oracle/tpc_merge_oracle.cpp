@@ -182,4 +182,22 @@ int orc_merge_transport(const orc_merge_params* p, float* st, float xn) {
   return ok ? 1 : 0;
 }
 
+// ---- C9: time and offset at which a track passes the beam line ("t0 / vertex-z estimation from the
+// time coordinate"; the z position is only known once the collision time is).  The beam axis is x = y = 0 in
+// every sector frame, so the state (x; y, z, s, t, k | time_ref) is transported to x = 0 with the state part of the C5
+// transport:  ok = transport(S, 0);  vertex_time = time_ref + S.z / Z  [time bins];  vertex_y = S.y  [cm].
+// With time = (t0 * v_drift + drift_len - |z|) / Z this is (t0 * v_drift + drift_len - side * z_vertex) / Z for a primary
+// track (side = +1 on the A side, -1 on the C side): the collision time up to the (few cm) vertex spread.  FAIL (|sin phi| would reach sin_phi_max): ok = 0, outputs 0.
+// par: [n*7] as in orc_merge.  Pin (tests/test_merge_oracle_pins.py::test_MV_*): generator truth of t0 and z_vertex.
+void orc_vertex_time(const orc_merge_params* p, int64_t n, const float* par, int32_t* ok, float* vertex_time, float* vertex_y) {
+  for (int64_t i = 0; i < n; ++i) {
+    const float* q = par + 7 * i;
+    St S{q[0], q[1], q[2], q[3], q[4], q[5]};
+    const bool good = transport_state(S, 0.0f, p->inv_R_per_qpt, p->sin_phi_max);
+    ok[i] = good ? 1 : 0;
+    vertex_time[i] = good ? q[6] + S.z / p->time_bin_cm : 0.0f;
+    vertex_y[i] = good ? S.y : 0.0f;
+  }
+}
+
 }  // extern "C"

@@ -299,4 +299,19 @@ __global__ void __launch_bounds__(kMergeThreads) k_refit_chains(MergeTracks T, R
   }
 }
 
+// ---- C9: time and offset at which a track passes the beam line (DESIGN.md §3 "C9") ----
+// One thread per state: transport to x = 0 (the beam axis in every sector frame); vertex_time = time_ref + z / Z.
+__global__ void __launch_bounds__(256) k_vertex_time(const int32_t* __restrict__ n_tracks, int max_tracks, const float* __restrict__ par7,
+                                                     int32_t* __restrict__ ok, float* __restrict__ vertex_time, float* __restrict__ vertex_y,
+                                                     float Z, float cB, float sin_phi_max) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= min(*n_tracks, max_tracks)) return;
+  const float* q = par7 + 7 * (size_t)i;
+  float x = q[0], y = q[1], z = q[2], s = q[3];
+  const bool good = merge_transport(x, y, z, s, q[4], q[5], 0.0f, cB, sin_phi_max);
+  ok[i] = good ? 1 : 0;
+  vertex_time[i] = good ? q[6] + z / Z : 0.0f;
+  vertex_y[i] = good ? y : 0.0f;
+}
+
 }  // namespace tpc

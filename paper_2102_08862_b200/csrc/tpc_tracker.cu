@@ -438,6 +438,20 @@ int tpc_refit_chains(tpc_tracker_t* t, const tpc_tracks_t* tr, const tpc_merged_
   return TPC_OK;
 }
 
+
+// ---- C9: beam-line time / offset of every state in par7 (merge.cuh) ----
+int tpc_vertex_time(tpc_tracker_t* t, const int32_t* n_tracks, int32_t max_tracks, const float* par7, void* cuda_stream,
+                    int32_t* ok, float* vertex_time, float* vertex_y) {
+  if (!t || !n_tracks || max_tracks < 0 || !ok || !vertex_time || !vertex_y || (max_tracks > 0 && !par7)) return TPC_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (max_tracks > 0)
+    k_vertex_time<<<(max_tracks + 255) / 256, 256, 0, st>>>(n_tracks, max_tracks, par7, ok, vertex_time, vertex_y, t->consts.Z, t->consts.cB,
+                                                          t->consts.sin_phi_max);
+  t->last_merge_launches = max_tracks > 0 ? 1 : 0;
+  if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;
+  return TPC_OK;
+}
+
 int64_t tpc_merge_last_launches(const tpc_tracker_t* t) { return t ? t->last_merge_launches : -1; }
 
 int tpc_tracker_destroy(tpc_tracker_t* t) {

@@ -18,7 +18,7 @@ STATUS_TRACKLET_OVERFLOW, STATUS_TRACK_OVERFLOW, STATUS_TRACK_HIT_OVERFLOW, STAT
 EXPORTS = ("tpc_tracker_arena_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
            "tpc_tracker_step_ms", "tpc_tracker_step_name", "tpc_tracker_last_launches", "tpc_tracker_work_counters",
            "tpc_tracker_arena_plan", "tpc_selftest_fast_math",
-           "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_refit_chains", "tpc_merge_last_launches",
+           "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_refit_chains", "tpc_vertex_time", "tpc_merge_last_launches",
            "tpc_tracker_destroy", "tpc_strerror")
 
 
@@ -130,6 +130,8 @@ def load_library(build_if_missing: bool = True):
         L.tpc_merge_tracks.restype = C.c_int
         L.tpc_refit_chains.argtypes = [vp, C.POINTER(Tracks), C.POINTER(Merged), vp, C.POINTER(Refit)]
         L.tpc_refit_chains.restype = C.c_int
+        L.tpc_vertex_time.argtypes = [vp, vp, C.c_int32, vp, vp, vp, vp, vp]
+        L.tpc_vertex_time.restype = C.c_int
         L.tpc_merge_last_launches.argtypes = [vp]
         L.tpc_merge_last_launches.restype = C.c_int64
         L.tpc_strerror.argtypes = [C.c_int]
@@ -337,6 +339,20 @@ class Tracker:
         if rc != TPC_OK:
             raise TpcError(rc, "tpc_refit_chains")
         return refit
+
+    def tpc_vertex_time(self, n_tracks, par7, stream=None):
+        """C9: (ok, vertex_time [time bins], vertex_y [cm]) of the DEVICE states ``par7`` (float32[K, 7]); ``n_tracks`` is the
+        1-element device tensor written by ``tpc_track_timeframe``."""
+        torch = self._torch
+        K = int(par7.shape[0])
+        ok = torch.empty(max(K, 1), dtype=torch.int32, device=self.device)
+        vt, vy = (torch.empty(max(K, 1), dtype=torch.float32, device=self.device) for _ in range(2))
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        rc = self.lib.tpc_vertex_time(self.handle, n_tracks.data_ptr(), K, par7.data_ptr(), C.c_void_p(s.cuda_stream),
+                                      ok.data_ptr(), vt.data_ptr(), vy.data_ptr())
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_vertex_time")
+        return ok, vt, vy
 
     def merge_scratch_bytes(self, max_tracks: int) -> int:
         return int(self.lib.tpc_merge_scratch_bytes(self.handle, int(max_tracks)))

@@ -26,6 +26,8 @@ def _gpu_track_and_merge(tf, cfg, n_sectors=36, merge_params=None):
     nxt, prv, root, n_links = merged = trk.tpc_merge_tracks(outs, merge_params)
     launches_merge = trk.last_merge_launches()
     rf = trk.tpc_refit_chains(outs, merged)
+    launches_refit = trk.last_merge_launches()
+    vtx = trk.tpc_vertex_time(out.n_tracks, rf[3])
     torch.cuda.synchronize()
     k = int(out.n_tracks[0])
     nh = int(out.n_track_hits[0])
@@ -36,7 +38,7 @@ def _gpu_track_and_merge(tf, cfg, n_sectors=36, merge_params=None):
     npads = np.floor(2.0 * (85.0 + 1.07 * np.arange(152)) * np.tan(np.radians(10.0)) / 0.5)
     cr = (0.5 * (npads - 1)).astype(np.float32)
     assert np.array_equal(hyt[:, 0], (tf.pad[hi] - cr[hrow]) * np.float32(0.5))
-    res = dict(k=k, refit=tuple(t[:k].cpu().numpy() for t in rf), launches_refit=trk.last_merge_launches(), seed=out.seed_hit[:k].cpu().numpy(), next=nxt.cpu().numpy(), prev=prv.cpu().numpy(), root=root.cpu().numpy(),
+    res = dict(k=k, vertex=tuple(t[:int(out.n_tracks[0])].cpu().numpy() for t in vtx), refit=tuple(t[:k].cpu().numpy() for t in rf), launches_refit=launches_refit, seed=out.seed_hit[:k].cpu().numpy(), next=nxt.cpu().numpy(), prev=prv.cpu().numpy(), root=root.cpu().numpy(),
                n_links=int(n_links[0]), launches=launches_merge, status=int(out.status[0]),
                sector=out.sector[:k].cpu().numpy(), first_row=out.first_row[:k].cpu().numpy(), last_row=out.last_row[:k].cpu().numpy())
     trk.close()
@@ -79,6 +81,12 @@ def _compare(g, res, mr):
     _check_par(rp, o_rp, "refit")
     assert np.array_equal(rp, o_rp) and np.array_equal(rc, o_rc), "refit not bit-identical"
     assert g["launches_refit"] == 2
+    # C9: beam-line time / offset of the refitted states -- one transport each, bit-identical
+    from oracle import merge as M
+    o_vok, o_vt, o_vy = M.vertex_time(M.default_merge_params(36), o_rp)
+    vok, vt, vy = (a[go] for a in g["vertex"])
+    np.testing.assert_array_equal(vok, o_vok, err_msg="vertex ok")
+    assert np.array_equal(vt, o_vt) and np.array_equal(vy, o_vy), "vertex time / offset not bit-identical"
 
 
 @pytest.mark.parametrize("seed", [1, 2, 3])

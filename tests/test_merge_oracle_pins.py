@@ -157,6 +157,26 @@ def test_ME_link_efficiency_and_purity_on_config1(seed):
     assert rep["wrong_rate"] <= 0.02, rep
 
 
+@pytest.mark.parametrize("seed", [1, 2])
+def test_MV_vertex_time_and_offset_against_generator_truth(seed):
+    """C9: a primary track transported to the beam line arrives at time (t0 v + L - side z_v) / Z with |y| ~ 0."""
+    tf, res, mr = _tracked(1, seed)
+    ok, vt, vy = M.vertex_time(M.default_merge_params(36), res.tr_par)
+    keys = ME.track_truth_keys(tf, res.tr_hit_offset, res.tr_n_hits, res.tr_hit_index)
+    tr = tf.tracks[np.where(keys >= 0, keys // (64 * 16), 0)]
+    side = np.where(res.tr_sector < 18, 1.0, -1.0)
+    t_true = (tr["t0_us"] * 2.58 + 250.0 - side * tr["z_v"]) / 0.516
+    sel = (keys >= 0) & (keys % 16 == 0) & (mr.prev < 0) & (tr["pt"] > 0.3)          # first outgoing arc, innermost piece
+    assert sel.sum() > 2000 and np.all(ok[sel] == 1)
+    d = (vt - t_true)[sel]
+    assert abs(np.median(d)) < 0.02 and np.median(np.abs(d)) < 0.15 and np.percentile(np.abs(d), 99) < 1.0, (np.median(d), np.median(np.abs(d)))
+    assert np.median(np.abs(vy[sel])) < 0.2 and np.percentile(np.abs(vy[sel]), 95) < 1.0
+    # a state that cannot reach x = 0 below sin_phi_max is flagged and zeroed
+    st = np.array([[150.0, 0.0, 0.0, 0.5, 0.2, 8.0, 100.0]], np.float32)                # s - k cB x = 0.5 - 1.8 < -0.95
+    ok1, t1, y1 = M.vertex_time(M.default_merge_params(36), st)
+    assert ok1[0] == 0 and t1[0] == 0.0 and y1[0] == 0.0
+
+
 def test_degenerate_inputs():
     p = M.default_merge_params(36)
     e = M.merge(p, [], [], [], [], np.zeros((0, 7), np.float32))
