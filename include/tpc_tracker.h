@@ -212,7 +212,8 @@ int tpc_merge_tracks(tpc_tracker_t* tracker, const tpc_merge_params_t* merge_par
  * all pieces of a chain own, each piece in its own sector frame, state and covariance rotated at every boundary.      */
 typedef struct {   /* caller-allocated DEVICE buffers, indexed by track like tpc_tracks_t                              */
   int32_t* ok;           /* [max_tracks] 1: root of a chain of >= 2 pieces, refitted; 0: anything else (values passed
-                            through); -1: root whose refit failed (a transport / rotation reached sin_phi_max)         */
+                            through); -1: root whose refit failed (a transport / rotation reached sin_phi_max, or a
+                            hit list of the chain was cut by TPC_STATUS_TRACK_HIT_OVERFLOW)                            */
   int32_t* chain_hits;   /* [max_tracks] hits of the whole chain (roots), else the track's own n_hits                  */
   int32_t* chain_pieces; /* [max_tracks] pieces of the chain (roots), else 1                                           */
   float* par7;           /* [max_tracks*7] (x, y, z_rel, sin_phi, dzds, q_pt, time_ref) at the innermost hit of the root */

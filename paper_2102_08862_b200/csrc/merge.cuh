@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(256) k_merge_root(MergeTracks T, const int32_t
 // rotated at every boundary.  transport / kalman_update are the constructor's (tracklet.cuh): same statements, same order.
 struct RefitIo {
   const float2* hit_yt; const uint8_t* hit_row;   // (y, time) and pad row of every track hit, in hit_index order (tpc_tracks_t)
-  const int32_t *n_hits; const int64_t* hit_offset;
+  const int32_t *n_hits; const int64_t* hit_offset; int64_t max_track_hits;
   const int32_t *next, *prev;               // C7 links
   int32_t *ok, *chain_hits, *chain_pieces;  // [max_tracks]
   float *rpar, *rcov;                       // [max_tracks * 7], [max_tracks * 9]
@@ -240,16 +240,21 @@ __global__ void __launch_bounds__(kMergeThreads) k_refit_chains(MergeTracks T, R
         } else {
           root = (int)root_list[e];
           int pm = root, pieces = 1, total = io.n_hits[root];
-          for (int q = io.next[pm]; q >= 0; q = io.next[pm]) { pm = q; ++pieces; total += io.n_hits[q]; }
+          bool complete = io.hit_offset[root] + io.n_hits[root] <= io.max_track_hits;      // hit list not cut by TPC_STATUS_TRACK_HIT_OVERFLOW
+          for (int q = io.next[pm]; q >= 0; q = io.next[pm]) {
+            pm = q; ++pieces; total += io.n_hits[q];
+            complete = complete && io.hit_offset[q] + io.n_hits[q] <= io.max_track_hits;
+          }
           io.chain_hits[root] = total;
           io.chain_pieces[root] = pieces;
+          if (!complete) io.ok[root] = -1;
           S.x = T.x[pm]; S.y = T.y[pm]; S.z = T.z[pm]; S.s = T.s[pm]; S.t = T.t[pm]; S.k = T.k[pm];
           S.c0 = S.c1 = S.c2 = S.c3 = S.c4 = S.c5 = 0.0f; S.d0 = S.d1 = S.d2 = 0.0f;
           p = pm; off = io.hit_offset[pm]; j = off + io.n_hits[pm] - 1; tref = T.time_ref[pm];
-          hy = io.hit_yt[j]; hr = io.hit_row[j];
+          if (complete) { hy = io.hit_yt[j]; hr = io.hit_row[j]; } else { hr = 0; }
           const bool ok0 = transport(S, xr[hr], tc.cB, tc.sin_phi_max);       // to the outermost hit, then the reset covariance
           S.c0 = tc.c0_y2; S.c1 = 0.0f; S.c2 = tc.c0_s2; S.c3 = 0.0f; S.c4 = 0.0f; S.c5 = tc.c0_k2; S.d0 = tc.c0_z2; S.d1 = 0.0f; S.d2 = tc.c0_t2;
-          if (ok0) active = true; else io.ok[root] = -1;
+          if (ok0 && complete) active = true; else io.ok[root] = -1;
         }
       }
     }

@@ -425,7 +425,7 @@ int tpc_refit_chains(tpc_tracker_t* t, const tpc_tracks_t* tr, const tpc_merged_
     c.Sd = (float)(2.0 * T / (1.0 + T * T));
   }
   MergeTracks T{tr->n_tracks, tr->seed_hit, tr->sector, tr->first_row, tr->last_row, tr->x, tr->y, tr->z_rel, tr->time_ref, tr->sin_phi, tr->dzds, tr->q_pt};
-  RefitIo io{reinterpret_cast<const float2*>(tr->hit_y_time), tr->hit_row, tr->n_hits, tr->hit_offset, mg->next, mg->prev,
+  RefitIo io{reinterpret_cast<const float2*>(tr->hit_y_time), tr->hit_row, tr->n_hits, tr->hit_offset, tr->max_track_hits, mg->next, mg->prev,
              out->ok, out->chain_hits, out->chain_pieces, out->par7, out->cov9};
   int64_t launches = 0;
   cudaMemsetAsync(n_roots, 0, 512, st);

@@ -240,3 +240,29 @@ def test_full_10ms_frame_merge_invariants_and_sampled_oracle_parity():
             assert o_link == g_link, (int(o_seed_global[i]), o_link, g_link)
             n_with_link += o_link >= 0
     assert n_with_link > 50 and n_refitted > 20
+
+
+def test_refit_with_truncated_hit_lists_flags_the_chains_instead_of_reading_past_the_buffers():
+    import torch
+    from paper_2102_08862_b200 import tracker as T
+    cfg = gen.preset(1, 2)
+    tf = gen.generate(cfg)
+    n = tf.n
+    trk = T.Tracker(T.default_geometry(36, tf.max_time_bin), T.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm, max_clusters=n))
+    d = [torch.from_numpy(np.ascontiguousarray(a, np.float32)).to(trk.device) for a in (tf.row, tf.pad, tf.time)]
+    outs = trk.alloc_outputs(n, hit_coords=True, max_track_hits=200_000)          # the frame has ~7e5 track hits
+    out = trk.tpc_track_timeframe(*d, n=n, outputs=outs)
+    merged = trk.tpc_merge_tracks(outs)
+    ok, ch, cp, rp, rc = trk.tpc_refit_chains(outs, merged)
+    torch.cuda.synchronize()
+    k = int(out.n_tracks[0])
+    assert int(out.status[0]) & T.STATUS_TRACK_HIT_OVERFLOW and int(out.n_track_hits[0]) > 200_000
+    ok, ch = ok[:k].cpu().numpy(), ch[:k].cpu().numpy()
+    off, nh = out.hit_offset[:k].cpu().numpy(), out.n_hits[:k].cpu().numpy()
+    nxt, prv, root = (t[:k].cpu().numpy() for t in merged[:3])
+    roots = np.nonzero((prv < 0) & (nxt >= 0))[0]
+    cut = (off + nh) > 200_000                                                      # tracks whose hit list was cut
+    chain_cut = np.bincount(root, weights=cut, minlength=k) > 0
+    assert np.all(ok[roots[chain_cut[roots]]] == -1) and (ok[roots[~chain_cut[roots]]] == 1).sum() > 100
+    assert np.all(np.isfinite(rp[:k].cpu().numpy()))
+    trk.close()
