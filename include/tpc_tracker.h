@@ -9,6 +9,8 @@
  * The entry points and their argument lists are fixed by BASELINE.json L5 (north_star):
  *   tpc_tracker_create(geometry, params), tpc_track_timeframe(clusters, n, stream, tracks_out),
  *   tpc_tracker_destroy.  The exact operations (steps C1..C6) are defined in DESIGN.md §3.
+ * After the hot path, three widening steps are separate calls on the tracker's outputs:
+ *   tpc_merge_tracks (C7), tpc_refit_chains (C8), tpc_vertex_time (C9); DESIGN.md §3 defines them too.
  *
  * Conventions
  *   - Plain C, no torch types.  Every pointer is marked DEVICE or HOST.
