@@ -122,6 +122,33 @@ def _cpu_oracle_run(cid, seed, frame_us):
     return tf.n, dt, len(r.tr_seed)
 
 
+def _cpu_oracle_run_all_cores(cid, seed, frame_us):
+    """The same unchanged oracle, one call per sector (sectors are independent), from a thread pool: BASELINE.md §3 (2).
+    ctypes releases the GIL during the call.  Returns (clusters, seconds, threads used, tracks)."""
+    import numpy as np
+    from concurrent.futures import ThreadPoolExecutor
+    import oracle
+    from paper_2102_08862_b200 import gen
+    cfg = gen.preset(cid, seed, frame_us if cid >= 2 else None)
+    tf = gen.generate(cfg, want_truth=False)
+    n_rows = 152
+    sec = (tf.row.astype(np.int64) // n_rows)
+    parts = []
+    for s_ in range(cfg.n_sectors):                      # split outside the timed region (the input of a per-sector tracker)
+        m = np.nonzero(sec == s_)[0]
+        parts.append((np.ascontiguousarray(tf.row[m] - np.float32(s_ * n_rows)), np.ascontiguousarray(tf.pad[m]),
+                      np.ascontiguousarray(tf.time[m])))
+    g1 = oracle.default_geometry(1, tf.max_time_bin)
+    p = oracle.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm)
+    threads = max(1, min(len(parts), os.cpu_count() or 1))
+    oracle.lib()
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(threads) as ex:
+        res = list(ex.map(lambda a: len(oracle.track(g1, p, *a).tr_seed), parts))
+    dt = time.perf_counter() - t0
+    return tf.n, dt, threads, int(sum(res))
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle on the box's host cores, same metric; each step a bounded sample."""
     rank = int(os.environ.get("RANK", "0"))
@@ -363,6 +390,10 @@ def main():
         sample = (f"{CONFIG_NAMES[cid]} generator, seed {args.seed}, frame cut to {args.cpu_sample_us:g} us ({cn} clusters)"
                   if cid >= 2 else f"{CONFIG_NAMES[cid]} ({cn} clusters)")
         cpu = {"value": cn / cdt, "unit": "clusters/s", "cores": 1, "kind": "oracle", "sample": sample, "seconds": cdt}
+        if cfg.n_sectors > 1:                            # the unchanged oracle, one sector per thread
+            an, adt, athreads, _ = _cpu_oracle_run_all_cores(cid, args.seed, args.cpu_sample_us)
+            cpu["all_cores"] = {"value": an / adt, "unit": "clusters/s", "cores": athreads, "host_cpus": os.cpu_count(),
+                                "kind": "oracle, one call per sector from a thread pool", "seconds": adt}
 
     line = {"metric": "tpc_clusters_tracked_per_s", "value": value, "unit": "clusters/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,

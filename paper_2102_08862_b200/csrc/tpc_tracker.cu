@@ -128,7 +128,7 @@ void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids
   id.tmp_orig = plan.add("sort_tmp_orig", 4 * N, S_SORT, S_SORT);
   id.tmp_yt = plan.add("sort_tmp_y_time", 8 * N, S_SORT, S_SORT);
   id.sort_hist = plan.add("sort_tile_histograms", 4 * hist_len, S_SORT, S_SORT);
-  id.yt = plan.add("hits_y_time(float2)", 8 * N, S_SORT, S_FOLLOW_DOWN);
+  id.yt = plan.add("hits_y_time(float2)", 8 * N, S_SORT, S_EMIT);      // the emit kernel copies the track hits' (y, time) on request
   id.orig = plan.add("hits_orig_index", 4 * N, S_SORT, S_EMIT);
   id.hsr = plan.add("hits_sector_row(u16)", 2 * N, S_GRID, S_EMIT);
   id.link_up = plan.add("link_up_raw", 4 * N, S_FINDER, S_CLEAN_START);
