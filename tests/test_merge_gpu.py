@@ -99,10 +99,15 @@ def test_merge_config1_full_tpc(seed):
     assert mr.n_links > 2000
 
 
-@pytest.mark.parametrize("cid,seed,us", [(2, 1, 150.0), (4, 2, 100.0)])
-def test_merge_continuous_readout_short_frames(cid, seed, us):
-    """Several overlapping collisions: the time cells of the candidate index and the time_ref differences matter."""
+@pytest.mark.parametrize("cid,seed,us,over", [(2, 1, 150.0, {}), (4, 2, 100.0, {}),
+                                              (3, 22091, 120.0, dict(dropout=0.0, noise_frac=0.5))])
+def test_merge_continuous_readout_short_frames(cid, seed, us, over):
+    """Several overlapping collisions: the time cells of the candidate index and the time_ref differences matter.
+    (The third case is the one a randomized sweep found: with this cluster / grid size ratio the arena planner used to put
+    the claim array on top of hits_y_time, which the emit kernel reads for the optional hit coordinates.)"""
     cfg = gen.preset(cid, seed, us)
+    for k_, v_ in over.items():
+        setattr(cfg, k_, v_)
     tf = gen.generate(cfg)
     g = _gpu_track_and_merge(tf, cfg)
     res, mr = _oracle_track_and_merge(tf, cfg)
