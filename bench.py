@@ -406,7 +406,7 @@ def main():
                              "working set may fit L2 (small config)", "gen_seconds": round(t_gen, 1)},
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches,
             "step_ms": {k: round(v, 4) for k, v in step_acc.items()}, "kernels": kernels,
-            "tracklet_constructor": constructor, "merge": merge, "roofline": roof, "cpu_baseline": cpu}
+            "tracklet_constructor": constructor, "rare_paths": work.get("rare_paths"), "merge": merge, "roofline": roof, "cpu_baseline": cpu}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -163,7 +163,10 @@ int64_t tpc_tracker_last_launches(const tpc_tracker_t* tracker);
  * tracklet constructor, [4] Kalman updates, [5] candidates scanned by its window searches (each the sum over the
  * four phase kernels), then [6 + 3 p + k] the same three counts (k = 0 row steps, 1 updates, 2 candidates) of phase
  * p = 0 chain fit, 1 follow up, 2 refit down, 3 follow down.  These are the units of the constructor's roofline
- * (DESIGN.md §6).  Returns the number of counters (18) or a negative status.                                 */
+ * (DESIGN.md §6).  Then the rare paths taken: [18] refits replayed after a failed transport that followed a hole,
+ * [19] refits that failed before their first update (the up pass's state is the result), [20] window searches that met
+ * an exact fp32 tie of the smallest distance (decided on the original index).  Returns the number of counters (21) or
+ * a negative status.                                                                                                 */
 int tpc_tracker_work_counters(tpc_tracker_t* tracker, void* cuda_stream, int64_t* out, int32_t capacity);
 
 /* Arena plan: for allocation i writes name, offset, bytes, first and last step of its lifetime.

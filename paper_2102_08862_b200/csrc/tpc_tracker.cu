@@ -484,14 +484,15 @@ int tpc_tracker_work_counters(tpc_tracker_t* t, void* cuda_stream, int64_t* out,
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (cudaMemcpyAsync(&h, t->plan.ptr<char>(t->params.arena, t->id.counters), 256, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
       cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return TPC_ECUDA; }
-  int64_t v[18] = {h.i32[kCntTracklets], h.i32[kCntStartHits], (int64_t)(uint32_t)h.i32[kCntInvalid], 0, 0, 0};
+  int64_t v[21] = {h.i32[kCntTracklets], h.i32[kCntStartHits], (int64_t)(uint32_t)h.i32[kCntInvalid], 0, 0, 0};
   for (int ph = 0; ph < 4; ++ph)
     for (int k = 0; k < 3; ++k) {
       v[6 + 3 * ph + k] = (int64_t)h.u64[kCnt64Phase0 - 4 + 3 * ph + k];
       v[3 + k] += v[6 + 3 * ph + k];
     }
-  for (int i = 0; i < 18 && i < capacity; ++i) out[i] = v[i];
-  return 18;
+  for (int k = 0; k < 3; ++k) v[18 + k] = (int64_t)h.u64[kCnt64Rare0 - 4 + k];
+  for (int i = 0; i < 21 && i < capacity; ++i) out[i] = v[i];
+  return 21;
 }
 
 int tpc_tracker_step_ms(tpc_tracker_t* t, float* ms_out, int32_t capacity) {

@@ -372,14 +372,15 @@ class Tracker:
 
     def work_counters(self, stream=None) -> dict:
         s = stream if stream is not None else self._torch.cuda.current_stream(self.device)
-        buf = (C.c_int64 * 18)()
-        k = self.lib.tpc_tracker_work_counters(self.handle, C.c_void_p(s.cuda_stream), buf, 18)
+        buf = (C.c_int64 * 21)()
+        k = self.lib.tpc_tracker_work_counters(self.handle, C.c_void_p(s.cuda_stream), buf, 21)
         if k < 0:
             raise TpcError(k, "tpc_tracker_work_counters")
         names = ("tracklets", "start_hits", "invalid_clusters", "row_steps", "updates", "candidates")
         out = {nm: int(buf[i]) for i, nm in enumerate(names)}
         for p, ph in enumerate(("fit_up", "follow_up", "fit_down", "follow_down")):
             out[ph] = {nm: int(buf[6 + 3 * p + i]) for i, nm in enumerate(("row_steps", "updates", "candidates"))}
+        out["rare_paths"] = {"refit_replays": int(buf[18]), "refits_without_update": int(buf[19]), "search_ties": int(buf[20])}
         return out
 
     def arena_plan(self) -> list:

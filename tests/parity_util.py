@@ -27,6 +27,7 @@ def run_gpu(row, pad, time, n_sectors, max_time_bin, sigma_y=0.08, sigma_z=0.12,
     torch.cuda.synchronize()
     res = {k: (v.cpu().numpy() if v is not None else None) for k, v in out.__dict__.items()}
     res["launches"] = trk.last_launches()
+    res["work"] = trk.work_counters()
     trk.close()
     return res
 

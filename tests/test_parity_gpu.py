@@ -55,6 +55,17 @@ def test_continuous_readout_short_frames(cid, seed):
     assert rep["n_tracks"] > 1000
 
 
+def test_rare_paths_of_the_constructor_are_taken_and_agree():
+    """The refit's replay (a failed transport after a hole) and the refit that fails before its first update (the up
+    pass's state is the result) are rare; this input takes both (device counters), and parity holds on it."""
+    cfg, tf = _frame(1, 2, pt_min=0.05)
+    g, o = _both(tf, cfg)
+    rep = PU.compare(g, o)
+    assert rep["track_par_bit_identical"] and rep["tracklet_par_bit_identical"] and rep["track_cov_bit_identical"]
+    rare = g["work"]["rare_paths"]
+    assert rare["refit_replays"] >= 1 and rare["refits_without_update"] >= 20, rare
+
+
 def test_time_coordinate_at_the_end_of_a_10ms_frame():
     """fp32 time values near 5e4 bins (ulp 2^-8 bin): all z arithmetic is on differences of raw time values."""
     cfg, tf = _frame(3, 5, frame_us=100.0)
@@ -127,6 +138,7 @@ def test_duplicate_hits_tie_break_on_original_index(copies):
     o = PU.run_oracle(row, pad, time, 1, 487.0)
     rep = PU.compare(g, o)
     assert rep["n_tracks"] >= 4
+    assert g["work"]["rare_paths"]["search_ties"] > 0          # the follower's exact-tie path ran
 
 
 def test_runs_are_deterministic_including_output_order():
