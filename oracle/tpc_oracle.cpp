@@ -96,7 +96,7 @@ bool transport(State& S, float xn, float cB, float sin_phi_max) {
   const float dx = xn - S.x;
   const float kc = cB * S.k;
   const float sn = S.s + kc * dx;
-  if (!(std::fabs(sn) < sin_phi_max)) return false;
+  if (!(std::fabs(S.s) < sin_phi_max && std::fabs(sn) < sin_phi_max)) return false;   // A12: at BOTH ends (an update may have pushed s past the limit)
   const float c = std::sqrt(1.0f - S.s * S.s);
   const float cn = std::sqrt(1.0f - sn * sn);
   const float ss = S.s + sn;

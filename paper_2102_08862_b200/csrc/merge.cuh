@@ -54,7 +54,7 @@ __device__ __forceinline__ bool merge_transport(float& x, float& y, float& z, fl
   const float dx = xn - x;
   const float kc = cB * k;
   const float sn = s + kc * dx;
-  if (!(fabsf(sn) < spm)) return false;
+  if (!(fabsf(s) < spm && fabsf(sn) < spm)) return false;
   const float c = sqrtf(1.0f - s * s);
   const float cn = sqrtf(1.0f - sn * sn);
   const float ss = s + sn;

@@ -96,6 +96,25 @@ def test_K1_transport_fails_beyond_sin_phi_max_and_keeps_state():
     np.testing.assert_array_equal(cv1, np.array(cv, np.float32))
 
 
+def test_K1_transport_never_leaves_the_domain_of_the_circle():
+    """Reading A12 on both ends: whatever an update did to sin phi (even |s| >= 1, where sqrt(1 - s^2) does not exist),
+    a transport either FAILs and keeps the state or returns finite numbers."""
+    rng = np.random.default_rng(17)
+    p = oracle.default_params()
+    p.sin_phi_max = 0.99
+    n_fail = n_ok = 0
+    for _ in range(3000):
+        st = [rng.uniform(85, 245), rng.uniform(-40, 40), rng.uniform(-100, 100), rng.uniform(-1.3, 1.3), rng.uniform(-1.5, 1.5), rng.uniform(-30, 30)]
+        ok, a, c = oracle.transport(p, st, [1, 0, 0.1, 0, 0, 100, 1, 0, 0.1], st[0] + rng.uniform(-12, 12))
+        assert np.all(np.isfinite(a)) and np.all(np.isfinite(c))
+        if abs(st[3]) >= 0.99:
+            assert not ok
+        if not ok:
+            np.testing.assert_array_equal(a, np.array(st, np.float32))
+        n_fail += (not ok); n_ok += ok
+    assert n_fail > 300 and n_ok > 300
+
+
 def test_K1_covariance_transport_is_F_C_Ft():
     """The staged covariance lines equal F C F^T with the Jacobian taken by finite differences in double."""
     p = oracle.default_params()
