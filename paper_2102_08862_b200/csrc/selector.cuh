@@ -11,7 +11,10 @@
 
 namespace tpc {
 
-constexpr int kSelectorThreads = 256;   // 8 tracklets per CTA
+#ifndef TPC_SELECTOR_THREADS
+#define TPC_SELECTOR_THREADS 256
+#endif
+constexpr int kSelectorThreads = TPC_SELECTOR_THREADS;   // 8 tracklets per CTA at 256
 
 // One warp per tracklet; the five row words are loaded back to back, then the atomics are fired (no return value).
 // (Claiming from inside the constructor when a tracklet retires was measured: it stalls the whole warp on the row
