@@ -397,3 +397,135 @@ def test_E1_efficiency_at_least_95_percent(cid, seed):
     assert e["n_findable"] >= 50
     assert e["efficiency"] >= 0.95, e
     assert e["fake_rate"] <= 0.02 and e["clone_rate"] <= 0.02, e
+
+
+# ----------------------------------------------------------------------------- P1..P4: hand-built pins of the cuts
+# Each of these exists because a plausible one-token mistake in the oracle survived every pin above (round-1 review):
+# the follower's stop rule, the growth of its window over missed rows, the two bounds of the finder's search area and
+# the seed's dz/ds.  All inputs are noise-free straight lines, so the expected outcome follows from BASELINE.json L7's
+# cuts ("0.05*dx + 0.5 cm" windows, "miss limit of 10 consecutive missed rows") by hand.
+def _line(rows, slope_y=0.02, slope_z=0.3, y_at=0.0, z_at=150.0, dy=0.0, dz=0.0):
+    """Clusters of the straight line y = y_at + slope_y (x - x0), z = z_at + slope_z (x - x0) at the given rows,
+    every one displaced by (dy, dz)."""
+    rows = np.asarray(rows)
+    x = row_x(rows)
+    return clusters_from_xyz(rows, y_at + slope_y * (x - X0) + dy, z_at + slope_z * (x - X0) + dz)
+
+
+def _track_one(parts, **params):
+    row, pad, time = concat(parts)
+    p = oracle.default_params()
+    for k, v in params.items():
+        setattr(p, k, v)
+    return oracle.track(_geom(), p, row, pad, time), row
+
+
+@pytest.mark.parametrize("gap,bridged", [(9, True), (10, False)])
+def test_P1_miss_limit_upward_is_the_tenth_consecutive_missed_row(gap, bridged):
+    """BASELINE.json L7 "a miss limit of 10 consecutive missed rows ends track following" (reading A11): a gap of 9 rows
+    is crossed, the 10th consecutive missed row ends the direction.  Above the gap only two hits (no chain of three, so
+    nothing but the follower of the lower piece can pick them up)."""
+    lower = np.arange(20, 61)
+    upper = np.array([61 + gap, 62 + gap])
+    r, row = _track_one([_line(lower), _line(upper)])
+    assert len(r.tl_seed) == 1 and len(r.tr_seed) == 1
+    got = np.sort((row[r.track_hits(0)]).astype(int))
+    want = np.concatenate([lower, upper]) if bridged else lower
+    np.testing.assert_array_equal(got, want)
+
+
+@pytest.mark.parametrize("gap,bridged", [(9, True), (10, False)])
+def test_P1_miss_limit_downward_is_the_tenth_consecutive_missed_row(gap, bridged):
+    """The same rule in the down pass below the seed row."""
+    upper = np.arange(80, 121)
+    lower = np.array([78 - gap, 79 - gap])
+    r, row = _track_one([_line(upper), _line(lower)])
+    assert len(r.tl_seed) == 1 and len(r.tr_seed) == 1
+    got = np.sort((row[r.track_hits(0)]).astype(int))
+    want = np.concatenate([lower, upper]) if bridged else upper
+    np.testing.assert_array_equal(got, want)
+
+
+def test_P1_a_hit_resets_the_miss_count_and_holes_in_the_refit_are_not_misses():
+    """Three gaps of 9 rows in a row: the count is of CONSECUTIVE misses (a hit resets it), and in the down pass the 27
+    holes inside the collected range do not count at all (reading A11, second half)."""
+    rows = np.concatenate([np.arange(10, 51), [60], [70], [80, 81]])
+    r, row = _track_one([_line(rows)])
+    assert len(r.tr_seed) == 1
+    np.testing.assert_array_equal(np.sort(row[r.track_hits(0)].astype(int)), rows)
+
+
+@pytest.mark.parametrize("axis", ["y", "z"])
+@pytest.mark.parametrize("k_missed,disp,attached", [(5, 0.70, True), (5, 0.90, False), (0, 0.50, True), (0, 0.60, False),
+                                                    (8, 0.90, True), (8, 1.06, False)])
+def test_P2_follower_window_grows_with_the_distance_since_the_last_hit(axis, k_missed, disp, attached):
+    """BASELINE.json L7 "0.05*dx + 0.5 cm" with dx = distance since the last attached hit (reading A1): after k missed
+    rows the window is W = 0.05 * 1.07 (k + 1) + 0.5 (0.5535, 0.821, 0.9815 for k = 0, 5, 8).  A single hit displaced
+    by `disp` from the line is attached iff disp < W, in y and in z alike."""
+    lower = np.arange(20, 61)
+    far = np.array([61 + k_missed])
+    w = 0.05 * 1.07 * (k_missed + 1) + 0.5
+    assert (disp < w) == attached and abs(disp - w) > 0.04          # the case is not marginal
+    kw = {"dy": disp} if axis == "y" else {"dz": disp}
+    r, row = _track_one([_line(lower), _line(far, **kw)])
+    assert len(r.tr_seed) == 1
+    got = np.sort(row[r.track_hits(0)].astype(int))
+    np.testing.assert_array_equal(got, np.concatenate([lower, far]) if attached else lower)
+
+
+def test_P3_search_area_bounds_y_and_z_separately():
+    """The finder's search area is |dy| < A_y = slope_y_max*1.07 + W1 (1.6235) and |dz| < A_z = slope_z_max*1.07 + W1
+    (2.1585) (reading A1).  A perfect straight line stepping 1.9 cm per row links when the step is
+    in z and does not when it is in y; 1.5 cm links in both; 2.3 cm in neither."""
+    rows = np.arange(40, 47)
+    for step, in_y, in_z in ((1.9, False, True), (1.5, True, True), (2.3, False, False)):
+        for axis, expect in (("y", in_y), ("z", in_z)):
+            kw = dict(slope_y=step / PITCH, slope_z=0.0, y_at=-5.0 - 40 * step) if axis == "y" else dict(slope_y=0.0, slope_z=step / PITCH)
+            row, pad, time = _line(rows, **kw)
+            r = oracle.track(_geom(1, 1200.0), oracle.default_params(), row, pad, time)
+            linked = r.up_raw[1:-1] >= 0
+            assert linked.all() == expect and linked.any() == expect, (step, axis)
+            if expect:
+                np.testing.assert_array_equal(r.up_raw[1:-1], np.arange(2, rows.size))
+                np.testing.assert_array_equal(r.down_raw[1:-1], np.arange(0, rows.size - 2))
+
+
+def test_N1_brute_force_on_steep_tracks():
+    """N1 again on hand-made steep lines (|dy/dx| up to 1.4, |dz/dx| up to 1.9: candidates between the two bounds of
+    the search area exist) plus uniform noise, against the independent numpy all-pairs evaluation."""
+    rng = np.random.default_rng(21)
+    rows = np.arange(30, 52)
+    parts = []
+    for sy, sz in ((1.4, 0.2), (-1.3, 1.9), (0.9, -1.7), (1.45, 1.45), (0.1, 1.95), (-1.0, -0.4)):
+        parts.append(_line(rows, slope_y=sy, slope_z=sz, y_at=-sy * (row_x(41) - X0), z_at=120.0))
+    nr = rng.integers(30, 52, 250)
+    parts.append(((nr).astype(np.float32), rng.uniform(5, 60, 250).astype(np.float32), rng.uniform(150, 330, 250).astype(np.float32)))
+    row, pad, time = concat(parts)
+    g, p = _geom(1, 600.0), oracle.default_params()
+    fast = oracle.track(g, p, row, pad, time)
+    _, npads_tab, _, consts = oracle.tables(g, p)
+    up, dn = _numpy_all_pairs_links(row, pad, time, consts, npads_tab, np.float32(9.0))
+    np.testing.assert_array_equal(fast.up_raw, up)
+    np.testing.assert_array_equal(fast.down_raw, dn)
+    assert (up >= 0).sum() >= 6 * 18
+    # the steep-in-y lines link (1.4 * 1.07 + noise-free < A_y), so candidates beyond A_y but inside A_z were rejected
+    x = row_x(rows)
+    assert 1.45 * PITCH < 1.6235 < 1.9 * PITCH < 2.1585
+
+
+def test_P4_seed_state_is_direction_cosines_of_the_first_two_hits():
+    """C5 step 1 (reading A7): s = dy/L, t = dz/L with L = sqrt(dx^2 + dy^2) -- BOTH over the path length in the bending
+    plane.  With sin_phi_max lowered below the seed's sin phi the very first transport FAILs, so the tracklet's output
+    IS the init state: x = x_r0, y = y(h0), z = 0, s = 0.6, t = 0.8, k = 0 for a line with dy/dx = 0.75, dz/dx = 1."""
+    rows = np.arange(10, 15)
+    row, pad, time = _line(rows, slope_y=0.75, slope_z=1.0, y_at=-12.0, z_at=100.0)
+    p = oracle.default_params()
+    p.sin_phi_max = 0.5
+    r = oracle.track(_geom(), p, row, pad, time)
+    assert len(r.tl_seed) == 1 and r.tl_seed[0] == 1 and r.tl_n_hits[0] == 1      # start hit = row 11 (row 10 is linkless)
+    par = r.tl_par[0].astype(np.float64)
+    y0 = (float(pad[1]) - 0.5 * (n_pads(11) - 1)) * 0.5
+    assert abs(par[0] - row_x(11)) < 1e-4 and abs(par[1] - y0) < 1e-5 and par[2] == 0.0 and par[5] == 0.0
+    assert abs(par[3] - 0.6) < 2e-4           # pads are fp32: the line is reproduced to ~1e-5 cm
+    assert abs(par[4] - 0.8) < 2e-4           # dz/dx (= 1.0) here would be the mistake
+    assert par[6] == time[1]
