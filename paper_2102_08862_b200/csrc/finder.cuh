@@ -57,7 +57,7 @@ constexpr int kFinderSlots = TPC_FINDER_SLOTS;       // candidates kept per neig
 // the search area to two small per-thread lists in shared memory ([slot][thread]: conflict-free); (2) ONE flat loop
 // over the nu x nd pairs.  Both trip counts are the maximum over the warp of a small number, and the bodies are
 // branch-free apart from the rare exact-tie case.  The nested "for u: for d" form over the raw spans ran at 4.5 of
-// 32 lanes (profiles/r01a_ncu_full_baseline.md).
+// 32 lanes (round-1 ncu capture).
 __global__ void __launch_bounds__(kFinderThreads) k_neighbours_finder(const float2* __restrict__ yt, const uint32_t* __restrict__ orig,
                                                                       const uint16_t* __restrict__ hsr, const uint32_t* __restrict__ bin_start,
                                                                       int* __restrict__ link_up, int* __restrict__ link_down,
