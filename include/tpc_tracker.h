@@ -60,7 +60,8 @@ typedef struct {
   float tan_half_sector; /* (float)tan(10 deg); pads_r = floor(2 x_r tan / pad_pitch) in double         */
   float time_bin_cm;     /* 0.516 = 2.58 cm/us * 0.2 us                                                 */
   float drift_len_cm;    /* 250 (informative)                                                           */
-  float max_time_bin;    /* upper bound of the time coordinate in a frame; sizes the grid               */
+  float max_time_bin;    /* upper bound of the time coordinate in a frame; sizes the grid; < 2^19 bins
+                            (the grid lookups' absolute fp32 margins hold up to there), else TPC_EINVAL */
 } tpc_geometry_t;
 
 typedef struct {
@@ -110,8 +111,10 @@ typedef struct {
   int32_t* status;       /* scalar: TPC_STATUS_* bits                                                       */
   int32_t *seed_hit, *sector, *first_row, *last_row, *n_hits; /* [max_tracks]                               */
   int64_t* hit_offset;   /* [max_tracks] first entry of the track in hit_index                              */
-  float *x, *y, *z_rel, *time_ref, *sin_phi, *dzds, *q_pt;    /* [max_tracks] state at the innermost hit;
-                            z_rel [cm] is relative to time_ref [time bins] (reading A2)           */
+  float *x, *y, *z_rel, *time_ref, *sin_phi, *dzds, *q_pt;    /* [max_tracks] state after the tracklet's last Kalman
+                            update: at its innermost hit, unless the downward refit FAILed early (about 1 track in
+                            1000: the state then sits on a higher pad row -- x says which).  z_rel [cm] is relative
+                            to time_ref [time bins] (reading A2)                                      */
   float* cov9;           /* [max_tracks*9] (yy, ys, ss, yk, sk, kk | zz, zt, tt); may be NULL               */
   int32_t* hit_index;    /* [max_track_hits] original cluster indices, ascending row, per track contiguous  */
   /* parity taps, each may be NULL (device entry point only): */
@@ -158,7 +161,9 @@ const char* tpc_tracker_step_name(int32_t step);
 /* Number of kernel launches the last tpc_track_timeframe call enqueued (memsets not counted).              */
 int64_t tpc_tracker_last_launches(const tpc_tracker_t* tracker);
 
-/* Work counters of the last completed call, read back from the device (synchronises `cuda_stream`):
+/* Work counters of the last completed tpc_track_timeframe call, read back from the device (synchronises
+ * `cuda_stream`).  The block lives in memory the handle owns, not in the arena, so it stays valid after
+ * tpc_merge_tracks / tpc_refit_chains (which reuse the arena):
  * out[0] tracklets constructed, [1] start hits found, [2] invalid clusters, [3] row steps (transports) of the
  * tracklet constructor, [4] Kalman updates, [5] candidates scanned by its window searches (each the sum over the
  * four phase kernels), then [6 + 3 p + k] the same three counts (k = 0 row steps, 1 updates, 2 candidates) of phase
@@ -188,7 +193,8 @@ int tpc_selftest_fast_math(void* cuda_stream, uint64_t* mismatches_out);
 typedef struct {
   float cut_y_cm, cut_z_cm;         /* 2, 2     : |dy|, |dz| between the extrapolated inner piece and the outer piece   */
   float cut_sin_phi, cut_q_pt;      /* 0.05, 0.5: |d sin phi|, |d q/pT| [c/GeV]                            (reading M4) */
-  int32_t max_row_gap;              /* 12 : the outer piece's state row r_B <= last_row_A + 1 + max_row_gap (reading M5) */
+  int32_t max_row_gap;              /* 12 : the outer piece's state row r_B <= last_row_A + 1 + max_row_gap (reading M5);
+                                       always r_B > max(first_row_A, state row of A) and r_B <= first_row_B (M7)        */
   int32_t max_row_overlap;          /* 2  : r_B >= last_row_A + 1 - max_row_overlap                                     */
 } tpc_merge_params_t;
 

@@ -19,8 +19,11 @@
 //       c  = sqrtf(1 - s*s)
 //       x1 = x*Cd + sg*(y*Sd);   y1 = y*Cd - sg*(x*Sd);   s1 = s*Cd - sg*(c*Sd)       (z, t, k unchanged)
 //       skip the side unless |s1| < sin_phi_max
-//   r_B = (int)floorf((x_B - x0) / pitch + 0.5f) is the pad row B's state sits on (its innermost tracklet hit; r_B <= f_B).
-//   A candidate continuation is a track B in S' with  r_B > f_A  and  l_A + 1 - overlap <= r_B <= l_A + 1 + gap.
+//   r_X = (int)floorf((x_X - x0) / pitch + 0.5f) is the pad row the state of track X sits on: the row of the tracklet's last
+//   Kalman update -- normally its innermost hit (r_X <= f_X), but a down refit that FAILs early leaves the state higher up.
+//   A candidate continuation is a track B in S' whose state really is at its inner end,  r_B <= f_B,  with
+//   r_B > max(f_A, r_A)  and  l_A + 1 - overlap <= r_B <= l_A + 1 + gap   (reading M7: state rows strictly increase along
+//   a chain, so chains are acyclic and hold at most n_rows pieces).
 //   The rotated state is transported to x_B with the state part of the C5 transport (exact circle, 3-term arc
 //   length series; FAIL -> no candidate), giving (y2, z2, s2); then
 //       dy = y2 - y_B;  dz = (z2 - z_B) + (time_ref_A - time_ref_B)*Z;  ds = s2 - s_B;  dk = k_A - k_B
@@ -135,7 +138,9 @@ int64_t orc_merge(const orc_merge_params* pp, int64_t n, const int32_t* seed, co
           if (sector[b] != nb) continue;
           const float* pb = par + 7 * b;
           const int32_t rb = (int32_t)std::floor((pb[0] - p.x0_cm) / p.row_pitch_cm + 0.5f);
-          if (!(rb > first_row[a])) continue;
+          const int32_t ra = (int32_t)std::floor((pa[0] - p.x0_cm) / p.row_pitch_cm + 0.5f);
+          if (!(rb > first_row[a] && rb > ra)) continue;
+          if (!(rb <= first_row[b])) continue;       // B's state must sit at its inner end (M7)
           if (rb < last_row[a] + 1 - p.max_row_overlap || rb > last_row[a] + 1 + p.max_row_gap) continue;
           St S = R;
           if (!transport_state(S, pb[0], p.inv_R_per_qpt, p.sin_phi_max)) continue;
@@ -161,7 +166,7 @@ int64_t orc_merge(const orc_merge_params* pp, int64_t n, const int32_t* seed, co
   }
   for (int64_t i = 0; i < n; ++i) {
     int32_t r = (int32_t)i;
-    while (prev[r] >= 0) r = prev[r];             // r_B > f_A >= r_A: state rows strictly increase along a chain, no cycles
+    for (int steps = 0; prev[r] >= 0 && steps < 1024; ++steps) r = prev[r];   // r_B > r_A: state rows strictly increase along a chain, no cycles (the bound is never reached)
     root[i] = r;
   }
   return n_links;

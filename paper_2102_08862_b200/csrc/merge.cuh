@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(256) k_merge_cell_count(MergeTracks T, MergeSc
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= merge_n(T, c)) return;
   int rb = (int)floorf((T.x[i] - c.x0) / c.pitch + 0.5f);
-  rb = min(max(rb, 0), c.n_rows - 1);
+  if (rb < 0 || rb >= c.n_rows || rb > T.first_row[i]) { S.cell_of[i] = 0xFFFFFFFFu; return; }   // reading M7: only a state at the inner end of its track is a candidate B
   const float tb = T.time_ref[i] + T.z[i] * c.inv_Z;
   const int sec = min(max(T.sector[i], 0), c.n_sectors - 1);
   const uint32_t cell = (uint32_t)((sec * c.n_rows + rb) * c.n_tcell + merge_time_cell(tb, c));
@@ -94,6 +94,7 @@ __global__ void __launch_bounds__(256) k_merge_cell_fill(MergeTracks T, MergeScr
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= merge_n(T, c)) return;
   const uint32_t cell = S.cell_of[i];
+  if (cell == 0xFFFFFFFFu) return;
   const uint32_t pos = S.cell_start[cell] + atomicAdd(S.cell_cursor + cell, 1u);    // order inside a cell is irrelevant (ties are decided on seeds)
   S.cand_idx[pos] = (uint32_t)i;
   S.cand_a[pos] = make_float4(T.y[i], T.z[i], T.s[i], T.k[i]);
@@ -110,7 +111,8 @@ __global__ void __launch_bounds__(kMergeThreads) k_merge_match(MergeTracks T, Me
     const uint32_t aseed = (uint32_t)T.seed[a];
     const int sec = T.sector[a], side = sec / 18, phi = sec % 18;
     const int fa = T.first_row[a], la = T.last_row[a];
-    const int r_lo = max(la + 1 - c.overlap, fa + 1), r_hi = min(la + 1 + c.gap, c.n_rows - 1);
+    const int ra = (int)floorf((ax - c.x0) / c.pitch + 0.5f);            // row A's own state sits on
+    const int r_lo = max(la + 1 - c.overlap, max(fa, ra) + 1), r_hi = min(la + 1 + c.gap, c.n_rows - 1);
     const float cs = sqrtf(1.0f - as * as);
     for (int isg = 0; isg < 2; ++isg) {
       const float sg = isg == 0 ? 1.0f : -1.0f;
@@ -169,7 +171,8 @@ __global__ void __launch_bounds__(256) k_merge_root(MergeTracks T, const int32_t
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= merge_n(T, c)) return;
   int r = i;
-  for (int p = prev[r]; p >= 0; p = prev[r]) r = p;      // state rows strictly increase along a chain: no cycles
+  int steps = 0;
+  for (int p = prev[r]; p >= 0 && steps < c.n_rows; p = prev[r], ++steps) r = p;      // state rows strictly increase along a chain (M7): no cycles, <= n_rows pieces
   root[i] = r;
 }
 
@@ -242,6 +245,7 @@ __global__ void __launch_bounds__(kMergeThreads) k_refit_chains(MergeTracks T, R
           int pm = root, pieces = 1, total = io.n_hits[root];
           bool complete = io.hit_offset[root] + io.n_hits[root] <= io.max_track_hits;      // hit list not cut by TPC_STATUS_TRACK_HIT_OVERFLOW
           for (int q = io.next[pm]; q >= 0; q = io.next[pm]) {
+            if (pieces >= c.n_rows) { complete = false; break; }          // cannot happen (M7); never walk a corrupted link list for ever
             pm = q; ++pieces; total += io.n_hits[q];
             complete = complete && io.hit_offset[q] + io.n_hits[q] <= io.max_track_hits;
           }

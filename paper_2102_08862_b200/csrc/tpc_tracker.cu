@@ -35,7 +35,7 @@ const char* const kStepNames[N_STEPS] = {
 struct Ids {   // arena allocation ids
   int stage_in = -1, stage_out = -1;
   int bin_start, sort_keys, tmp_keys, tmp_orig, tmp_yt, sort_hist, yt, orig, hsr, link_up, link_down, link_up_clean, start_flag, cell_count, start_hits,
-      counters, scan_a, scan_b, seeds_a, seeds_b, row_hit, tl_meta, tl_rec, tl_cur, claim, owned, own_mask,
+      scan_a, scan_b, seeds_a, seeds_b, row_hit, tl_meta, tl_rec, tl_cur, claim, owned, own_mask,
       flag, track_idx, hit_off, track_slot;
 };
 
@@ -54,12 +54,17 @@ constexpr int kDefaultGridTimeBins = 4, kDefaultGridPadBins = 8, kDefaultSliceTi
 #ifndef TPC_FIT_CTAS_PER_SM
 #define TPC_FIT_CTAS_PER_SM 64
 #endif
+// The grid lookups add ABSOLUTE superset margins to their time windows (0.05 / 0.02 time bins, tracklet.cuh / finder.cuh)
+// that must exceed the rounding of a predicted fp32 time: half an ulp at 2^19 bins is 0.03, so frames are limited to
+// 2^19 time bins (104 ms; the paper's frame is 10 ms = 5e4 bins).
+constexpr float kMaxTimeBin = 524288.0f;
 constexpr double kGridMarginCm = 0.01;   // superset margin of the pad-bin lookups (fp32 rounding of a difference is << this)
 
 bool valid_geometry(const tpc_geometry_t* g) {
   return g && g->n_sectors >= 1 && g->n_rows >= 3 && g->n_rows <= kRowStride &&
          (int64_t)g->n_sectors * g->n_rows <= 65535 && g->row_pitch_cm > 0 && g->pad_pitch_cm > 0 &&
-         g->tan_half_sector > 0 && g->time_bin_cm > 0 && g->max_time_bin >= 0 && std::isfinite(g->max_time_bin);
+         g->tan_half_sector > 0 && g->time_bin_cm > 0 && g->max_time_bin >= 0 && std::isfinite(g->max_time_bin) &&
+         g->max_time_bin < kMaxTimeBin;
 }
 
 bool valid_params(const tpc_params_t* p) {
@@ -119,7 +124,6 @@ void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids
   }
   const size_t hist_len = (size_t)kRadixBuckets * (size_t)c.sort_tiles + 1;
   const size_t scan_len = std::max(std::max(scan_tiles(hist_len), scan_tiles((size_t)c.n_cells + 1)), scan_tiles(T)) + 2;
-  id.counters = plan.add("counters", 256, S_SORT, S_EMIT);
   id.scan_a = plan.add("scan_tile_sums_a", 4 * scan_len, S_SORT, S_EMIT);
   id.scan_b = plan.add("scan_tile_sums_b", 4 * scan_len, S_SORT, S_EMIT);
   id.bin_start = plan.add("grid_bin_start", 4 * B, S_GRID, S_FOLLOW_DOWN);
@@ -188,6 +192,8 @@ struct tpc_tracker {
   Ids id;
   Consts consts;
   void* tables = nullptr;          // device: xr | cr | npads
+  int32_t* counters = nullptr;     // device: the 256-byte counter block of the last tpc_track_timeframe call (inside `tables`, NOT in
+                                   // the arena: tpc_merge_tracks / tpc_refit_chains reuse the arena from offset 0)
   cudaEvent_t ev[N_STEPS + 1] = {};
   bool profile = false, have_times = false;
   int64_t last_launches = 0, last_merge_launches = 0;
@@ -269,7 +275,8 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
   int n_dev = 0;
   if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) { cudaGetLastError(); delete t; return TPC_ECUDA; }
   const size_t rowtab_off = ((size_t)nr * 20 + 15) / 16 * 16;      // float4 (npads - 0.5, cr, yoff, pscale) per row, for the ingest key
-  const size_t tab_bytes = rowtab_off + (size_t)nr * 16;
+  const size_t counters_off = (rowtab_off + (size_t)nr * 16 + 255) / 256 * 256;
+  const size_t tab_bytes = counters_off + 256;
   std::vector<float> rowtab((size_t)nr * 4);
   for (int r = 0; r < nr; ++r) { rowtab[4 * r] = (float)npads[r] - 0.5f; rowtab[4 * r + 1] = cr[r]; rowtab[4 * r + 2] = yoff[r]; rowtab[4 * r + 3] = pscale[r]; }
   if (cudaMalloc(&t->tables, tab_bytes) != cudaSuccess) { cudaGetLastError(); delete t; return TPC_ECUDA; }
@@ -283,6 +290,8 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
     cudaGetLastError(); cudaFree(t->tables); delete t; return TPC_ECUDA;
   }
 
+  t->counters = reinterpret_cast<int32_t*>(tb + counters_off);
+  if (cudaMemset(t->counters, 0, 256) != cudaSuccess) { cudaGetLastError(); cudaFree(t->tables); delete t; return TPC_ECUDA; }
   Consts& c = t->consts;
   const int w = t->cap.grid_w;
   c.n_rows = nr; c.n_sr = g->n_sectors * nr; c.n_tb = t->cap.n_tb; c.n_pb = t->cap.n_pb; c.n_bins = t->cap.n_bins;
@@ -482,7 +491,7 @@ int tpc_tracker_work_counters(tpc_tracker_t* t, void* cuda_stream, int64_t* out,
   struct { int32_t i32[8]; unsigned long long u64[28]; } h;     // the 256-byte counter block
   static_assert(sizeof(h) == 256, "counter block");
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  if (cudaMemcpyAsync(&h, t->plan.ptr<char>(t->params.arena, t->id.counters), 256, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+  if (cudaMemcpyAsync(&h, t->counters, 256, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
       cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return TPC_ECUDA; }
   int64_t v[21] = {h.i32[kCntTracklets], h.i32[kCntStartHits], (int64_t)(uint32_t)h.i32[kCntInvalid], 0, 0, 0};
   for (int ph = 0; ph < 4; ++ph)
@@ -537,7 +546,7 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   uint8_t* start_flag = P.ptr<uint8_t>(A, id.start_flag);
   uint32_t* cell_count = P.ptr<uint32_t>(A, id.cell_count);
   uint32_t* start_hits = P.ptr<uint32_t>(A, id.start_hits);
-  int32_t* counters = P.ptr<int32_t>(A, id.counters);          // layout: kCnt* in tracklet.cuh
+  int32_t* counters = t->counters;                             // layout: kCnt* in tracklet.cuh
   uint32_t* n_invalid = reinterpret_cast<uint32_t*>(counters + kCntInvalid);
   TrackletSeeds seeds;
   seeds.a = P.ptr<int4>(A, id.seeds_a);

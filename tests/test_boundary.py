@@ -54,6 +54,9 @@ def test_invalid_arguments_are_rejected_on_the_host():
     bad = T.default_geometry()
     bad.n_rows = 500
     assert T.tpc_tracker_arena_bytes(bad, p) == 0
+    long_frame = T.default_geometry(1, 524288.0)            # >= 2^19 time bins: the lookups' fp32 margins no longer hold
+    assert T.tpc_tracker_arena_bytes(long_frame, p) == 0
+    assert T.tpc_tracker_arena_bytes(T.default_geometry(1, 524287.0), p) > 0
     badp = T.default_params(max_clusters=1000)
     badp.sin_phi_max = 1.5
     assert T.tpc_tracker_arena_bytes(g, badp) == 0

@@ -185,3 +185,42 @@ def test_degenerate_inputs():
     tf, res, mr = _tracked(1, 1)
     one = M.merge(M.default_merge_params(1), res.tr_seed, np.zeros_like(res.tr_sector), res.tr_first_row, res.tr_last_row, res.tr_par)
     assert one.n_links == 0 and np.all(one.next == -1) and np.array_equal(one.root, np.arange(len(res.tr_seed)))
+
+
+def _pair_across_boundary(state_row_b, first_row_b, state_row_a=40, first_row_a=40, last_row_a=99):
+    """Two hand-made tracks on ONE straight radial line through the boundary between sectors 0 and 1: A in sector 0
+    (rows first_row_a..last_row_a), B in sector 1; each state is the exact line at the row it claims to sit on."""
+    x0, pitch = 85.0, 1.07
+    T = math.tan(math.radians(10.0))
+    Phi = math.radians(17.0)                                  # global direction; the line passes the boundary (20 deg) near row 100
+    xa = x0 + pitch * state_row_a
+    # global line through the point P = 192 cm * (cos 20, sin 20) with direction Phi
+    P = (192.0 * math.cos(math.radians(20.0)), 192.0 * math.sin(math.radians(20.0)))
+    def local_state(alpha_deg, x_local):
+        al = math.radians(alpha_deg)
+        px, py, ph = _local(P[0], P[1], Phi, al)
+        tanl = math.tan(Phi - al)
+        return [x_local, py + (x_local - px) * tanl, 0.0, math.sin(Phi - al), 0.0, 0.0, 100.0]
+    a = local_state(10.0, xa)
+    b = local_state(30.0, x0 + pitch * state_row_b)
+    par = np.array([a, b], np.float32)
+    return ([11, 22], [0, 1], [first_row_a, first_row_b], [last_row_a, 140], par)
+
+
+def test_MC_a_state_above_its_first_row_is_never_a_continuation_and_chains_are_acyclic():
+    """Reading M7: B is a candidate only if its state sits at its inner end (r_B <= f_B) and above A's own state row."""
+    p = M.default_merge_params(36)
+    ok = M.merge(p, *_pair_across_boundary(state_row_b=101, first_row_b=101))
+    assert ok.n_links == 1 and ok.next[0] == 1 and ok.prev[1] == 0 and ok.root[1] == 0
+    # the same B, but its hits start at row 95 and its state (failed down refit) stayed on row 101: not a candidate
+    bad = M.merge(p, *_pair_across_boundary(state_row_b=101, first_row_b=95))
+    assert bad.n_links == 0 and np.all(bad.next == -1) and np.array_equal(bad.root, [0, 1])
+    # A's own state sits ABOVE the candidate's row (A's refit failed part-way, state on row 105): r_B > r_A fails
+    bad2 = M.merge(p, *_pair_across_boundary(state_row_b=101, first_row_b=101, state_row_a=105))
+    assert bad2.n_links == 0
+    # real data: along every chain the state rows strictly increase
+    tf, res, mr = _tracked(1, 1)
+    rs = np.floor((res.tr_par[:, 0] - np.float32(85.0)) / np.float32(1.07) + np.float32(0.5)).astype(np.int64)
+    a = np.where(mr.next >= 0)[0]
+    assert np.all(rs[mr.next[a]] > rs[a]) and np.all(rs[mr.next[a]] <= res.tr_first_row[mr.next[a]])
+    assert (rs > res.tr_first_row).sum() >= 1            # the input does hold tracks whose state is not at the inner end
