@@ -228,7 +228,7 @@ class Tracker:
 
     # -- buffers ---------------------------------------------------------------------------------------------
     def _alloc_outputs(self, n: int, max_tracks: int, max_track_hits: int, taps: bool, max_tracklets: int, host: bool,
-                       hit_coords: bool = False):
+                       hit_coords: bool = False, tap_row_hit: bool = True):
         torch = self._torch
         kw = dict(device="cpu", pin_memory=True) if host else dict(device=self.device)
         e = lambda shape, dt: torch.empty(shape, dtype=dt, **kw)
@@ -245,7 +245,7 @@ class Tracker:
             r.link_up, r.link_down, r.is_start_hit = e(n, torch.int32), e(n, torch.int32), e(n, torch.uint8)
             r.n_tracklets = e(1, torch.int32)
             r.tracklet_seed, r.tracklet_n_hits = e(max_tracklets, torch.int32), e(max_tracklets, torch.int32)
-            r.tracklet_row_hit = e((max_tracklets, nr), torch.int32)
+            r.tracklet_row_hit = e((max_tracklets, nr), torch.int32) if tap_row_hit else None
             r.tracklet_par = e((max_tracklets, 7), torch.float32)
         if hit_coords and not host:
             r.hit_y_time, r.hit_row = e((H, 2), torch.float32), e(H, torch.uint8)
@@ -264,11 +264,11 @@ class Tracker:
         return max(n // 64 + 4096, 1), max(n, 1)
 
     def alloc_outputs(self, n: int, taps: bool = False, host: bool = False, max_tracks: int = 0, max_track_hits: int = 0,
-                      hit_coords: bool = False):
+                      hit_coords: bool = False, tap_row_hit: bool = True):
         K, H = self.default_capacities(n)
         K, H = (max_tracks or K), (max_track_hits or H)
         T = int(self.params.max_tracklets or (self.params.max_clusters // 10 + 4096)) if taps else 0
-        out = self._alloc_outputs(n, K, H, taps, T, host, hit_coords)
+        out = self._alloc_outputs(n, K, H, taps, T, host, hit_coords, tap_row_hit)
         return out, self._tracks_struct(out, K, H, T)
 
     # -- the C-ABI calls -------------------------------------------------------------------------------------

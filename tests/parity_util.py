@@ -99,3 +99,79 @@ def _check_par(g, o, what):
     den = np.maximum(np.abs(o[:, 5]), 1e-3)
     assert np.max(np.abs(g[:, 5] - o[:, 5]) / den) <= QPT_REL_TOL, f"{what} q/pT"
     assert np.array_equal(g[:, 6], o[:, 6]), f"{what} time_ref"
+
+
+def run_oracle_per_sector(row, pad, time, n_sectors, max_time_bin, sigma_y=0.08, sigma_z=0.12, threads=None, n_rows=152):
+    """The unchanged oracle, one call per sector from a thread pool (ctypes releases the GIL), results mapped back to
+    whole-frame cluster indices.  Sectors are independent (reading A16) and a sub-frame keeps the cluster order, so
+    every original-index tie-break and tracklet id maps through the selection.  Returns a dict of whole-frame arrays;
+    per-sector results are reduced at once (the tracklets' row->hit tables are dropped: 10 GB for a 10 ms frame)."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    import oracle
+    n = int(len(row))
+    sec = (row.astype(np.int32) // n_rows)
+    order = np.argsort(sec, kind="stable")                      # ascending cluster index inside a sector
+    bounds = np.searchsorted(sec[order], np.arange(n_sectors + 1))
+    g1 = oracle.default_geometry(1, max_time_bin)
+    p = oracle.default_params(sigma_y, sigma_z)
+    oracle.lib()
+    up = np.full(n, -1, np.int32); down = np.full(n, -1, np.int32); start = np.zeros(n, np.uint8)
+
+    def one(s):
+        sel = order[bounds[s]:bounds[s + 1]]
+        if sel.size == 0:
+            return None
+        r = oracle.track(g1, p, row[sel] - np.float32(s * n_rows), pad[sel], time[sel])
+        sel32 = sel.astype(np.int32)
+        up[sel] = np.where(r.link_up >= 0, sel32[np.maximum(r.link_up, 0)], -1)
+        down[sel] = np.where(r.link_down >= 0, sel32[np.maximum(r.link_down, 0)], -1)
+        start[sel] = r.is_start_hit
+        return dict(tl_seed=sel32[r.tl_seed], tl_n_hits=r.tl_n_hits, tl_par=r.tl_par,
+                    tr_seed=sel32[r.tr_seed], tr_sector=np.full(len(r.tr_seed), s, np.int32), tr_first_row=r.tr_first_row,
+                    tr_last_row=r.tr_last_row, tr_n_hits=r.tr_n_hits, tr_par=r.tr_par, tr_cov=r.tr_cov,
+                    tr_hit_index=sel32[r.tr_hit_index])
+
+    threads = threads or max(1, min(n_sectors, os.cpu_count() or 1))
+    with ThreadPoolExecutor(threads) as ex:
+        parts = [q for q in ex.map(one, range(n_sectors)) if q is not None]
+    res = {k: np.concatenate([q[k] for q in parts]) for k in parts[0]} if parts else {}
+    res.update(link_up=up, link_down=down, is_start_hit=start)
+    return res
+
+
+def _ragged_gather(values, offsets, counts):
+    """Concatenation of values[offsets[i] : offsets[i] + counts[i]] over i, vectorised."""
+    counts = counts.astype(np.int64)
+    total = int(counts.sum())
+    starts = np.concatenate([[0], np.cumsum(counts[:-1])]) if counts.size else np.zeros(0, np.int64)
+    idx = np.arange(total, dtype=np.int64) - np.repeat(starts, counts) + np.repeat(offsets.astype(np.int64), counts)
+    return values[idx]
+
+
+def compare_whole_frame(gpu: dict, orc: dict) -> dict:
+    """Bit-for-bit comparison of a whole frame (arrays by original cluster index / joined on the seed)."""
+    np.testing.assert_array_equal(gpu["link_up"], orc["link_up"], err_msg="link_up")
+    np.testing.assert_array_equal(gpu["link_down"], orc["link_down"], err_msg="link_down")
+    np.testing.assert_array_equal(gpu["is_start_hit"], orc["is_start_hit"], err_msg="is_start_hit")
+    nt = int(gpu["n_tracklets"][0])
+    assert nt == len(orc["tl_seed"]), (nt, len(orc["tl_seed"]))
+    go, oo = np.argsort(gpu["tracklet_seed"][:nt], kind="stable"), np.argsort(orc["tl_seed"], kind="stable")
+    np.testing.assert_array_equal(gpu["tracklet_seed"][:nt][go], orc["tl_seed"][oo], err_msg="tracklet seeds")
+    np.testing.assert_array_equal(gpu["tracklet_n_hits"][:nt][go], orc["tl_n_hits"][oo], err_msg="tracklet n_hits")
+    assert np.array_equal(gpu["tracklet_par"][:nt][go].view(np.uint32), orc["tl_par"][oo].view(np.uint32)), "tracklet parameters"
+    k = int(gpu["n_tracks"][0])
+    assert k == len(orc["tr_seed"]), (k, len(orc["tr_seed"]))
+    go, oo = np.argsort(gpu["seed_hit"][:k], kind="stable"), np.argsort(orc["tr_seed"], kind="stable")
+    np.testing.assert_array_equal(gpu["seed_hit"][:k][go], orc["tr_seed"][oo], err_msg="track seeds")
+    for name, ref in (("sector", "tr_sector"), ("first_row", "tr_first_row"), ("last_row", "tr_last_row"), ("n_hits", "tr_n_hits")):
+        np.testing.assert_array_equal(gpu[name][:k][go], orc[ref][oo], err_msg=f"track {name}")
+    o_off = np.concatenate([[0], np.cumsum(orc["tr_n_hits"][:-1], dtype=np.int64)]) if k else np.zeros(0, np.int64)
+    gh = _ragged_gather(gpu["hit_index"], gpu["hit_offset"][:k][go], gpu["n_hits"][:k][go])
+    oh = _ragged_gather(orc["tr_hit_index"], o_off[oo], orc["tr_n_hits"][oo])
+    np.testing.assert_array_equal(gh, oh, err_msg="track hit lists")
+    gpar = np.stack([gpu[nm][:k][go] for nm in ("x", "y", "z_rel", "sin_phi", "dzds", "q_pt", "time_ref")], 1)
+    assert np.array_equal(gpar.view(np.uint32), orc["tr_par"][oo].view(np.uint32)), "track parameters"
+    assert np.array_equal(gpu["cov9"][:k][go].view(np.uint32), orc["tr_cov"][oo].view(np.uint32)), "track covariance"
+    return dict(n_tracks_compared=k, n_tracks_oracle=len(orc["tr_seed"]), n_track_hits_compared=int(gh.size),
+                n_tracklets_compared=nt, n_links_compared=int(gpu["link_up"].size))

@@ -232,79 +232,56 @@ _FULL = {}
 
 
 def _full_frame(cid):
-    """The full 10 ms frame of configs[cid], seed 1 (the one bench.py times); generated once per test session."""
+    """The full frame of configs[cid], seed 1 (the one bench.py times); one multi-GB frame in host memory at a time."""
     if cid not in _FULL:
-        _FULL.clear()                                  # one 2 GB frame in host memory at a time
+        _FULL.clear()
         c = gen.preset(cid, 1)
         _FULL[cid] = (c, gen.generate(c, want_truth=False))
     return _FULL[cid]
 
 
-@pytest.mark.parametrize("cid,sector,t_lo", [(3, 7, 20000.0), (3, 29, 41000.0), (4, 16, 9000.0)])
-def test_full_10ms_frame_invariants_and_sampled_oracle_parity(cid, sector, t_lo):
-    """BASELINE.json configs[3] / configs[4] at FULL size (1.6e8 clusters), in the launch configuration bench.py times
-    (default parameters, no taps).  (a) Properties that hold at any size.  (b) Sampled parity: the tracks of one sector
-    whose hits all lie inside a 3000-bin time window must equal, hit for hit and bit for bit, the tracks the oracle finds
-    on the sub-frame {that sector, window +- 1200 bins} (a track spans <= 485 bins of drift and every decision that
-    touches it -- links, start hits, window searches, the one-pass hit claims -- involves only hits within a few bins of
-    a tracklet that shares a hit with it, i.e. within ~1000 bins; cluster order is kept, so original-index tie-breaks
-    and tracklet ids order the same way)."""
+@pytest.mark.parametrize("cid", [2, 3, 4])
+def test_whole_frame_oracle_parity_at_full_size(cid):
+    """BASELINE.json L5 "GPU tracks identical to the oracle ... on all five configs": configs[2] (2 ms, 4e7 clusters),
+    configs[3] and configs[4] (10 ms, 1.6e8 clusters) at FULL size, in the launch configuration bench.py times (default
+    parameters; the link / start-hit / tracklet-summary taps add three small kernels' worth of writes).  The oracle runs
+    unchanged, once per sector from a thread pool (sectors are independent -- reading A16 -- and a per-sector sub-frame
+    keeps the cluster order, so original-index tie-breaks and tracklet ids map through the selection).  Compared bit
+    for bit, over the WHOLE frame: every cleaned link and start hit, every tracklet's (seed, n_hits, 7 parameters),
+    every track's hit list, rows, parameters and covariance.  (The tracklets' row->hit tables are 10 GB at this size;
+    they are compared in full on configs[0], [1] and the short frames -- here the tracklet parameters, which depend on
+    every attached hit in order, stand in for them.)"""
     import torch
     from paper_2102_08862_b200 import tracker as T
     cfg, tf = _full_frame(cid)
     n = tf.n
-    assert n > 1.2e8
+    assert n > (3e7 if cid == 2 else 1.2e8)
     g = T.default_geometry(cfg.n_sectors, tf.max_time_bin)
     trk = T.Tracker(g, T.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm, max_clusters=n))
     d = [torch.from_numpy(a).to(trk.device) for a in (tf.row, tf.pad, tf.time)]
-    out = trk.tpc_track_timeframe(*d, n=n)
+    outs = trk.alloc_outputs(n, taps=True, tap_row_hit=False)
+    out = trk.tpc_track_timeframe(*d, n=n, outputs=outs)
     torch.cuda.synchronize()
-    k, nh, status = int(out.n_tracks[0]), int(out.n_track_hits[0]), int(out.status[0])
-    assert status & 7 == 0 and k > 1e6
-    n_hits = out.n_hits[:k].cpu().numpy()
-    off = out.hit_offset[:k].cpu().numpy()
-    hit_index = out.hit_index[:nh].cpu().numpy()
-    sec = out.sector[:k].cpu().numpy()
-    first_row, last_row = out.first_row[:k].cpu().numpy(), out.last_row[:k].cpu().numpy()
-    seed = out.seed_hit[:k].cpu().numpy()
-    par = np.stack([getattr(out, nm)[:k].cpu().numpy() for nm in ("x", "y", "z_rel", "sin_phi", "dzds", "q_pt", "time_ref")], 1)
-    cov = out.cov9[:k].cpu().numpy()
+    gpu = {k: (v.cpu().numpy() if v is not None else None) for k, v in out.__dict__.items()}
     trk.close()
-    del d, out
-    # (a) invariants
+    del d, out, outs
+    torch.cuda.empty_cache()
+    k, nh, status = int(gpu["n_tracks"][0]), int(gpu["n_track_hits"][0]), int(gpu["status"][0])
+    assert status == 0 and k > (2e5 if cid == 2 else 1e6)
+    orc = PU.run_oracle_per_sector(tf.row, tf.pad, tf.time, cfg.n_sectors, tf.max_time_bin, cfg.sigma_y_cm, cfg.sigma_z_cm)
+    rep = PU.compare_whole_frame(gpu, orc)
+    assert rep["n_tracks_compared"] == k == rep["n_tracks_oracle"]
+    assert rep["n_track_hits_compared"] == nh
+    assert rep["n_tracklets_compared"] == int(gpu["n_tracklets"][0])
+    assert rep["n_links_compared"] == n
+    # properties that hold at any size (hit rows ascend inside a track, a hit in at most one track, offsets are the scan)
+    n_hits, off, hit_index = gpu["n_hits"][:k], gpu["hit_offset"][:k], gpu["hit_index"][:nh]
     assert n_hits.min() >= 30 and n_hits.max() <= N_ROWS
     np.testing.assert_array_equal(off, np.concatenate([[0], np.cumsum(n_hits[:-1], dtype=np.int64)]))
-    assert int(n_hits.sum()) == nh
-    cnt = np.bincount(hit_index, minlength=n)
-    assert cnt.max() == 1, "a hit belongs to more than one track"
+    assert np.bincount(hit_index, minlength=n).max() == 1, "a hit belongs to more than one track"
     hrow = tf.row[hit_index].astype(np.int64)
-    track_of = np.repeat(np.arange(k), n_hits)
-    assert np.array_equal(hrow // N_ROWS, sec[track_of]), "a track holds hits of another sector"
+    assert np.array_equal(hrow // N_ROWS, np.repeat(gpu["sector"][:k], n_hits)), "a track holds hits of another sector"
     r_in = hrow % N_ROWS
-    inner = np.ones(nh, bool); inner[off] = False                      # not the first hit of its track
+    inner = np.ones(nh, bool); inner[off] = False
     assert np.all(r_in[inner] > r_in[np.nonzero(inner)[0] - 1]), "hit rows must ascend inside a track"
-    assert np.array_equal(r_in[off], first_row) and np.array_equal(r_in[off + n_hits - 1], last_row)
-    assert np.all(np.isfinite(par)) and np.all(np.isfinite(cov))
-    # (b) sampled parity
-    width, margin = 3000.0, 1200.0
-    t_hi = t_lo + width
-    sel = np.nonzero((tf.row >= sector * N_ROWS) & (tf.row < (sector + 1) * N_ROWS) &
-                     (tf.time >= t_lo - margin) & (tf.time <= t_hi + margin))[0]            # ascending: order kept
-    assert sel.size > 1e5
-    sub_row = tf.row[sel] - np.float32(sector * N_ROWS)
-    # time values are passed unshifted: every difference of two time values stays bit-identical
-    o = PU.run_oracle(sub_row, tf.pad[sel], tf.time[sel], 1, tf.max_time_bin, cfg.sigma_y_cm, cfg.sigma_z_cm)
-    ht = tf.time[hit_index]
-    tmin = np.minimum.reduceat(ht, off); tmax = np.maximum.reduceat(ht, off)
-    g_in = np.nonzero((sec == sector) & (tmin >= t_lo) & (tmax <= t_hi))[0]
-    o_t = tf.time[sel][o.tr_hit_index]
-    o_min = np.minimum.reduceat(o_t, o.tr_hit_offset); o_max = np.maximum.reduceat(o_t, o.tr_hit_offset)
-    o_in = np.nonzero((o_min >= t_lo) & (o_max <= t_hi))[0]
-    assert g_in.size > 200 and g_in.size == o_in.size, (g_in.size, o_in.size)
-    g_in = g_in[np.argsort(seed[g_in])]
-    o_seed = sel[o.tr_seed[o_in]]
-    o_in = o_in[np.argsort(o_seed)]
-    np.testing.assert_array_equal(seed[g_in], sel[o.tr_seed[o_in]])
-    for a, b in zip(g_in, o_in):
-        np.testing.assert_array_equal(hit_index[off[a]:off[a] + n_hits[a]], sel[o.track_hits(int(b))])
-    assert np.array_equal(par[g_in], o.tr_par[o_in]) and np.array_equal(cov[g_in], o.tr_cov[o_in])
+    assert np.array_equal(r_in[off], gpu["first_row"][:k]) and np.array_equal(r_in[off + n_hits - 1], gpu["last_row"][:k])
