@@ -101,8 +101,9 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def _tracker_params(T, cfg, n, host_staging, profile, grid=(0, 0, 0)):
+def _tracker_params(T, cfg, n, host_staging, profile, grid=(0, 0, 0), follower=0):
     p = T.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm, max_clusters=n)
+    p.follower = int(follower)
     p.host_staging, p.profile, p.grid_time_bins, p.grid_pad_bins = int(host_staging), int(profile), int(grid[0]), int(grid[1])
     p.slice_time_bins = int(grid[2])
     return p
@@ -189,6 +190,7 @@ def main():
     ap.add_argument("--grid-time-bins", type=int, default=0, help="grid bin width in time bins (0 = library default)")
     ap.add_argument("--slice-time-bins", type=int, default=0, help="processing-order time slice (0 = library default)")
     ap.add_argument("--grid-pad-bins", type=int, default=0, help="grid bins across a pad row (0 = library default)")
+    ap.add_argument("--follower", type=int, default=0, help="0 = per-lane follower (default), 1 = row-synchronous follower (A/B)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-inflight", type=int, default=2, help="time frames in flight in the end-to-end measurement")
@@ -224,7 +226,7 @@ def main():
     torch.cuda.synchronize()
 
     g = T.default_geometry(cfg.n_sectors, tf.max_time_bin)
-    trk = T.Tracker(g, _tracker_params(T, cfg, n, False, True, (args.grid_time_bins, args.grid_pad_bins, args.slice_time_bins)), device=str(dev))
+    trk = T.Tracker(g, _tracker_params(T, cfg, n, False, True, (args.grid_time_bins, args.grid_pad_bins, args.slice_time_bins), args.follower), device=str(dev))
     outs = trk.alloc_outputs(n)
     stream = torch.cuda.Stream(device=dev)
 
@@ -305,7 +307,7 @@ def main():
     if not args.no_e2e:
         n_fl = max(1, args.e2e_inflight)
         gp = (args.grid_time_bins, args.grid_pad_bins, args.slice_time_bins)
-        trks = [T.Tracker(g, _tracker_params(T, cfg, n, True, False, gp), device=str(dev)) for _ in range(n_fl)]
+        trks = [T.Tracker(g, _tracker_params(T, cfg, n, True, False, gp, args.follower), device=str(dev)) for _ in range(n_fl)]
         houts = [t.alloc_outputs(n, host=True) for t in trks]
         streams = [torch.cuda.Stream(device=dev) for _ in range(n_fl)]
         k_each = max(2, (max(3, args.steps // 2) + n_fl - 1) // n_fl)

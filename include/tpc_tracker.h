@@ -80,7 +80,10 @@ typedef struct {
                                      results do not depend on either value.                                  */
   int32_t slice_time_bins;        /* tracklets are constructed in (sector, time slice, row) order for cache
                                      locality; width of a slice in time bins; 0 = default (256)              */
-  int32_t reserved0;
+  int32_t follower;               /* 0 = one lane per tracklet, persistent warps with lane refill, lookups in global
+                                     memory (csrc/tracklet.cuh); 1 = row-synchronous: a CTA sweeps the pad rows in lock
+                                     step with the row's grid offsets and hits staged in shared memory by bulk copies
+                                     (csrc/follow_rows.cuh; measured slower; kept for A/B).  Same results. */
   int64_t max_clusters;           /* capacity: largest n of any tpc_track_timeframe call                    */
   int64_t max_tracklets;          /* capacity of the tracklet store; 0 = max_clusters/10 + 4096             */
   int64_t max_tracks;             /* host entry point only: staging capacity; 0 = max_clusters/64 + 4096    */
@@ -170,8 +173,9 @@ int64_t tpc_tracker_last_launches(const tpc_tracker_t* tracker);
  * p = 0 chain fit, 1 follow up, 2 refit down, 3 follow down.  These are the units of the constructor's roofline
  * (DESIGN.md §6).  Then the rare paths taken: [18] refits replayed after a failed transport that followed a hole,
  * [19] refits that failed before their first update (the up pass's state is the result), [20] window searches that met
- * an exact fp32 tie of the smallest distance (decided on the original index).  Returns the number of counters (21) or
- * a negative status.                                                                                                 */
+ * an exact fp32 tie of the smallest distance (decided on the original index), [21] window searches of the row-synchronous
+ * follower that were served from global memory because the staged range did not cover them.  Returns the number of
+ * counters (22) or a negative status.                                                                                                 */
 int tpc_tracker_work_counters(tpc_tracker_t* tracker, void* cuda_stream, int64_t* out, int32_t capacity);
 
 /* Arena plan: for allocation i writes name, offset, bytes, first and last step of its lifetime.
@@ -185,6 +189,15 @@ int tpc_tracker_arena_plan(const tpc_tracker_t* tracker, int32_t i, const char**
  * (HOST, 2 entries) receives the number of differing bit patterns for sqrt and for the reciprocal (both must be 0:
  * the decision arithmetic has to round like the definition, BASELINE.json L5).                              */
 int tpc_selftest_fast_math(void* cuda_stream, uint64_t* mismatches_out);
+
+/* Micro-benchmark of the bound the tracklet constructor is accounted against ("measure it with a
+ * micro-benchmark, do not quote a datasheet number"): dependency-free streams of fp32 multiplies and adds -- no FMA
+ * contraction, like the constructor's arithmetic (--fmad=false) -- on every SM, timed with CUDA events on
+ * `cuda_stream` (synchronises it).  lane_inst_per_s_out (HOST, 2 entries): [0] scalar FMUL / FADD instructions,
+ * in lane-instructions per second (warp instructions x 32) -- the "alu" peak of the roofline; [1] the same arithmetic
+ * issued as packed mul.f32x2 / add.f32x2 (two fp32 operations per lane-instruction), in fp32 operations per second.
+ * Returns TPC_OK or TPC_ECUDA.                                                                              */
+int tpc_selftest_alu_peak(void* cuda_stream, double* lane_inst_per_s_out);
 
 /* ---- C7: sector-boundary merging of the per-sector tracks (DESIGN.md §3 "C7", readings M1..M8; PAPER.md L23 / L25:
  * "full TPC tracking" -- the sector tracker is followed by a merger of the sector tracks; BASELINE.json L8: 36 sectors,

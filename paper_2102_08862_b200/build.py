@@ -26,7 +26,8 @@ def build_cuda(force: bool = False, verbose: bool = False) -> str:
     newest = max(os.path.getmtime(p) for p in _sources())
     if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < newest:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB,
+        extra = os.environ.get("TPC_NVCC_EXTRA", "").split()      # build-time knobs (-DTPC_...); default: none
+        cmd = [nvcc, *NVCC_FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB,
                os.path.join(CSRC, "tpc_tracker.cu")]
         subprocess.check_call(cmd)
     return LIB

@@ -12,7 +12,7 @@ constexpr uint32_t kInvalidRank = 0xFFFFFFFFu;
 // on the host in double from the fp32 parameter values and rounded once ("Notation").
 struct Consts {
   // geometry
-  int n_rows, n_sr, n_tb, n_pb, n_bins;  // rows per sector, sector-rows, time bins and pad bins per sector-row, n_sr*n_pb*n_tb
+  int n_rows, n_sr, n_tb, n_pb, n_bins;  // rows per sector, sector-rows, time bins and pad bins per sector-row, n_sr*n_tb*n_pb
   float max_time, inv_bin_w;             // validity bound of the time coordinate; 1 / grid bin width (time)
   float inv_n_rows;                      // (float)(1 / n_rows), for row = sector_row mod n_rows without a division
   float Z, inv_Z, P;                     // time-bin size [cm], its inverse (grid lookups only), pad pitch
@@ -44,6 +44,14 @@ __device__ __forceinline__ int time_bin(float t, const Consts& c) {
 __device__ __forceinline__ int pad_bin(float y, float yoff, float pscale, const Consts& c) {
   int b = __float2int_rd((y + yoff) * pscale);
   return min(max(b, 0), c.n_pb - 1);
+}
+
+// Grid bin index.  Inside a sector-row the bins are TIME-MAJOR: ((sector_row * n_tb + time_bin) * n_pb + pad_bin), so
+// that (a) all hits of a sector-row inside a time range are ONE contiguous span of the sorted hit arrays -- what a CTA
+// stages into shared memory with one bulk copy -- and (b) the pad bins pb0..pb1 of one time bin are contiguous: a
+// lookup window is one span per grid time bin it touches.
+__device__ __forceinline__ uint32_t grid_bin(int sr, int tb, int pb, const Consts& c) {
+  return (uint32_t)((sr * c.n_tb + tb) * c.n_pb + pb);
 }
 
 __device__ __forceinline__ unsigned lane_id() { return threadIdx.x & 31u; }

@@ -4,8 +4,8 @@
 // differences ey, ez lie inside the window W1 with the smallest mid-point deviation chi2 < chi2_cut
 // (DESIGN.md §3 C2).  Ties go to the smallest original index of u, then of d.
 //
-// Layout: hits sorted by (sector-row, time bin); the candidates of one neighbour row are ONE contiguous span
-// [binStart[b(t-A)], binStart[b(t+A)+1]) of the float2 (y, time) array, so a thread streams ~64 B per row.
+// Layout: hits sorted by (sector-row, time bin, pad bin); the candidates of one neighbour row are one contiguous span of
+// the float2 (y, time) array per grid time bin the search area touches.
 // All decision arithmetic is fp32 in the written order, compiled with --fmad=false.
 #pragma once
 #include "common.cuh"
@@ -38,31 +38,40 @@ __device__ __forceinline__ bool in_search_area(const float2 me, const float2 cq,
   return fabsf(dy) < c.Ay && fabsf(dz) < c.Az;
 }
 
-// Candidate span of one (sector-row, pad bin): the hits of the time bins [tb_lo, tb_hi].
-struct Span { uint32_t lo, n; };
-__device__ __forceinline__ Span grid_span(const uint32_t* __restrict__ bin_start, int sr, int pb, int tb_lo, int tb_hi, const Consts& c) {
-  const uint32_t* bs = bin_start + ((size_t)sr * c.n_pb + pb) * c.n_tb;
-  const uint32_t lo = __ldg(bs + tb_lo);
-  return Span{lo, __ldg(bs + tb_hi + 1) - lo};
-}
-
 constexpr int kFinderThreads = 256;
 #ifndef TPC_FINDER_SLOTS
 #define TPC_FINDER_SLOTS 6
 #endif
 constexpr int kFinderSlots = TPC_FINDER_SLOTS;       // candidates kept per neighbour row in shared memory; more -> generic path
 
-// SIMT shape: (1) ONE flat loop scans the candidates of both neighbour rows (each row: the spans of one or two pad
-// bins -- the create-time check guarantees that the search area is narrower than a pad bin) and appends those inside
-// the search area to two small per-thread lists in shared memory ([slot][thread]: conflict-free); (2) ONE flat loop
-// over the nu x nd pairs.  Both trip counts are the maximum over the warp of a small number, and the bodies are
-// branch-free apart from the rare exact-tie case.  The nested "for u: for d" form over the raw spans ran at 4.5 of
-// 32 lanes (round-1 ncu capture).
+// Scans the candidates of one neighbour row (sector-row srn) inside the search area of hit `me`: for every grid time
+// bin the lookup touches, the pad bins pb0..pb1 are one contiguous span (time-major grid, common.cuh::grid_bin).
+// Candidates inside the area are appended to the thread's slot list; returns how many were inside (may exceed the slots).
+__device__ __forceinline__ int finder_collect(const float2* __restrict__ yt, const uint32_t* __restrict__ bin_start, const float2 me,
+                                              int srn, int tb_lo, int tb_hi, int pb0, int pb1, float2 (*s_val)[kFinderThreads],
+                                              uint32_t (*s_idx)[kFinderThreads], int slot0, const Consts& c) {
+  int n_in = 0;
+  for (int tb = tb_lo; tb <= tb_hi; ++tb) {
+    const uint32_t b = grid_bin(srn, tb, pb0, c);
+    const uint32_t lo = __ldg(bin_start + b), hi = __ldg(bin_start + b + (uint32_t)(pb1 - pb0) + 1u);
+    for (uint32_t q = lo; q < hi; ++q) {
+      const float2 cq = yt[q];
+      if (!in_search_area(me, cq, c)) continue;
+      if (n_in < kFinderSlots) { s_val[slot0 + n_in][threadIdx.x] = cq; s_idx[slot0 + n_in][threadIdx.x] = q; }
+      ++n_in;
+    }
+  }
+  return n_in;
+}
+
+// SIMT shape: the candidates of both neighbour rows that lie inside the search area go to two small per-thread lists in
+// shared memory ([slot][thread]: conflict-free); then ONE flat loop over the nu x nd pairs, branch-free apart from the rare
+// exact-tie case.  A crowded area (more than kFinderSlots candidates in a row) takes generic nested loops.
 __global__ void __launch_bounds__(kFinderThreads) k_neighbours_finder(const float2* __restrict__ yt, const uint32_t* __restrict__ orig,
                                                                       const uint16_t* __restrict__ hsr, const uint32_t* __restrict__ bin_start,
                                                                       int* __restrict__ link_up, int* __restrict__ link_down,
                                                                       const __grid_constant__ Consts c) {
-  __shared__ float2 s_val[2 * kFinderSlots][kFinderThreads];      // rows 0..3: up candidates, 4..7: down candidates
+  __shared__ float2 s_val[2 * kFinderSlots][kFinderThreads];      // slots [0, kFinderSlots): up candidates, then down candidates
   __shared__ uint32_t s_idx[2 * kFinderSlots][kFinderThreads];
   const uint32_t n_valid = __ldg(bin_start + c.n_bins);
   const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
@@ -77,37 +86,8 @@ __global__ void __launch_bounds__(kFinderThreads) k_neighbours_finder(const floa
     const float yo_d = __ldg(c.yoff + r - 1), ps_d = __ldg(c.pscale + r - 1);
     const int pu0 = pad_bin(me.x - c.finder_yw, yo_u, ps_u, c), pu1 = pad_bin(me.x + c.finder_yw, yo_u, ps_u, c);
     const int pd0 = pad_bin(me.x - c.finder_yw, yo_d, ps_d, c), pd1 = pad_bin(me.x + c.finder_yw, yo_d, ps_d, c);
-    // spans: u0, u1 (row r+1), d0, d1 (row r-1); the second span of a row is empty unless the area straddles two pad bins
-    const Span u0 = grid_span(bin_start, sr + 1, pu0, tb_lo, tb_hi, c);
-    const Span d0 = grid_span(bin_start, sr - 1, pd0, tb_lo, tb_hi, c);
-    Span u1{0u, 0u}, d1{0u, 0u};
-    if (pu1 != pu0) u1 = grid_span(bin_start, sr + 1, pu1, tb_lo, tb_hi, c);
-    if (pd1 != pd0) d1 = grid_span(bin_start, sr - 1, pd1, tb_lo, tb_hi, c);
-    const uint32_t e0 = u0.n, e1 = e0 + u1.n, e2 = e1 + d0.n, n_all = e2 + d1.n;   // up candidates: i < e1
-    // flat index i -> sorted-hit index: base of the span that holds i, minus the span's first i
-    const uint32_t b0 = u0.lo, b1 = u1.lo - e0, b2 = d0.lo - e1, b3 = d1.lo - e2;
-    int nu = 0, nd = 0;
-    for (uint32_t ib = 0; ib < n_all; ib += 2) {     // two independent loads per trip
-      uint32_t qq[2];
-      float2 cq[2];
-#pragma unroll
-      for (int k = 0; k < 2; ++k) {
-        const uint32_t i = min(ib + k, n_all - 1);
-        qq[k] = (i < e1 ? (i < e0 ? b0 : b1) : (i < e2 ? b2 : b3)) + i;
-        cq[k] = yt[qq[k]];
-      }
-#pragma unroll
-      for (int k = 0; k < 2; ++k) {
-        const uint32_t i = ib + k;
-        if (i < n_all && in_search_area(me, cq[k], c)) {
-          const bool up = i < e1;
-          const int slot = up ? nu : kFinderSlots + nd;
-          if ((up ? nu : nd) < kFinderSlots) { s_val[slot][threadIdx.x] = cq[k]; s_idx[slot][threadIdx.x] = qq[k]; }
-          nu += up ? 1 : 0;
-          nd += up ? 0 : 1;
-        }
-      }
-    }
+    const int nu = finder_collect(yt, bin_start, me, sr + 1, tb_lo, tb_hi, pu0, pu1, s_val, s_idx, 0, c);
+    const int nd = finder_collect(yt, bin_start, me, sr - 1, tb_lo, tb_hi, pd0, pd1, s_val, s_idx, kFinderSlots, c);
     float best = 0.0f;
     if (nu <= kFinderSlots && nd <= kFinderSlots) {
       const int n_pairs = nu * nd;
@@ -118,16 +98,21 @@ __global__ void __launch_bounds__(kFinderThreads) k_neighbours_finder(const floa
         if (++b == nd) { b = 0; ++a; }
       }
     } else {   // crowded area: generic nested loops over the spans (ties are decided on the original index)
-      auto index_of = [&](uint32_t i) -> uint32_t { return (i < e1 ? (i < e0 ? b0 : b1) : (i < e2 ? b2 : b3)) + i; };
-      for (uint32_t iu = 0; iu < e1; ++iu) {
-        const uint32_t qu = index_of(iu);
-        const float2 cu = yt[qu];
-        if (!in_search_area(me, cu, c)) continue;
-        for (uint32_t id = e1; id < n_all; ++id) {
-          const uint32_t qd = index_of(id);
-          const float2 cd = yt[qd];
-          if (!in_search_area(me, cd, c)) continue;
-          finder_try_pair(me, cu, cd, qu, qd, orig, c, best, bu, bd);
+      for (int tu = tb_lo; tu <= tb_hi; ++tu) {
+        const uint32_t b_u = grid_bin(sr + 1, tu, pu0, c);
+        const uint32_t ulo = __ldg(bin_start + b_u), uhi = __ldg(bin_start + b_u + (uint32_t)(pu1 - pu0) + 1u);
+        for (uint32_t qu = ulo; qu < uhi; ++qu) {
+          const float2 cu = yt[qu];
+          if (!in_search_area(me, cu, c)) continue;
+          for (int td = tb_lo; td <= tb_hi; ++td) {
+            const uint32_t b_d = grid_bin(sr - 1, td, pd0, c);
+            const uint32_t dlo = __ldg(bin_start + b_d), dhi = __ldg(bin_start + b_d + (uint32_t)(pd1 - pd0) + 1u);
+            for (uint32_t qd = dlo; qd < dhi; ++qd) {
+              const float2 cd = yt[qd];
+              if (!in_search_area(me, cd, c)) continue;
+              finder_try_pair(me, cu, cd, qu, qd, orig, c, best, bu, bd);
+            }
+          }
         }
       }
     }

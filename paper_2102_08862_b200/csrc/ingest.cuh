@@ -1,9 +1,10 @@
 // C1 cluster ingest (BASELINE.json L5 item 1: "sorts clusters into per-(sector, row) grids of (pad, time) bins by
 // radix sort and prefix scan"; PAPER.md L23 native coordinates).
 //
-// key(i) = ((sector*n_rows + row) * n_pb + pad_bin(y)) * n_tb + time_bin(time)   (= grid bin index; n_bins for
-// clusters outside the geometry, which therefore sort to the end).  A stable least-significant-digit radix sort on the key orders the
-// frame by (sector-row, time bin) and, inside a bin, by original index -- the layout is deterministic.
+// key(i) = ((sector*n_rows + row) * n_tb + time_bin(time)) * n_pb + pad_bin(y)   (= grid bin index, common.cuh::grid_bin;
+// n_bins for clusters outside the geometry, which therefore sort to the end).  A stable least-significant-digit radix sort
+// on the key orders the frame by (sector-row, time bin, pad bin) and, inside a bin, by original index -- the layout is
+// deterministic.
 // One pass = k_radix_histogram (digit counts per 2048-element tile) -> exclusive prefix scan over
 // (digit, tile) -> k_radix_scatter (stable in-tile ranking by warp match, local reorder in shared memory, then
 // every digit's run is written contiguously: coalesced writes instead of 4..8-byte random scatters).
@@ -38,7 +39,7 @@ __device__ __forceinline__ uint32_t cluster_key(float rf, float pad, float time,
   const float4 rt = __ldg(c.rowtab + r);                                // (n_pads - 0.5 [exact in fp32], c_r, yoff, pscale)
   const bool ok = ok_row && pad >= -0.5f && pad < rt.x && time >= 0.0f && time <= c.max_time;
   y = ok ? (pad - rt.y) * c.P : 0.0f;                                   // y(h) = (pad - c_r) * P
-  const uint32_t key = (uint32_t)((sr * c.n_pb + pad_bin(y, rt.z, rt.w, c)) * c.n_tb + time_bin(time, c));
+  const uint32_t key = grid_bin(sr, time_bin(time, c), pad_bin(y, rt.z, rt.w, c), c);
   return ok ? key : (uint32_t)c.n_bins;
 }
 

@@ -45,24 +45,22 @@ __global__ void __launch_bounds__(kLinkThreads) k_clean_links_find_starts(
 
 // Start-hit compaction in PROCESSING order.  The constructor's in-flight tracklets should be close in space and
 // time so that the hits and grid bins they touch stay in L2: start hits are therefore listed by
-// (sector, time slice, row, pad bin) instead of the hits' own (sector, row, pad bin, time) order.  A cell
-// (sector, slice, row, pad bin) is one contiguous range of sorted hits, so the compaction is: one thread per cell
+// (sector, time slice, row) instead of the hits' own (sector, row, time) order.  A cell (sector, slice, row) is one
+// contiguous range of sorted hits (the grid is time-major inside a sector-row), so the compaction is: one thread per cell
 // counts its flags -> exclusive scan over the cells in processing order -> the same thread writes its start hits.
 // Deterministic (no atomics).
 struct StartCells { int n_slices, slice_bins; uint32_t n_cells; };   // slice_bins: grid time bins per slice
 
 __device__ __forceinline__ void start_cell_range(uint32_t cell, const StartCells sc, const uint32_t* __restrict__ bin_start,
                                                  const Consts& c, uint32_t& lo, uint32_t& hi) {
-  const int p = (int)(cell % (uint32_t)c.n_pb);
-  uint32_t q = cell / (uint32_t)c.n_pb;
-  const int r = (int)(q % (uint32_t)c.n_rows);
-  q /= (uint32_t)c.n_rows;
+  const int r = (int)(cell % (uint32_t)c.n_rows);
+  const uint32_t q = cell / (uint32_t)c.n_rows;
   const int slice = (int)(q % (uint32_t)sc.n_slices);
   const int sector = (int)(q / (uint32_t)sc.n_slices);
-  const uint32_t* bs = bin_start + ((size_t)(sector * c.n_rows + r) * c.n_pb + p) * c.n_tb;
+  const int sr = sector * c.n_rows + r;
   const int t0 = slice * sc.slice_bins;
-  lo = __ldg(bs + t0);
-  hi = __ldg(bs + min(t0 + sc.slice_bins, c.n_tb));
+  lo = __ldg(bin_start + grid_bin(sr, t0, 0, c));
+  hi = __ldg(bin_start + grid_bin(sr, min(t0 + sc.slice_bins, c.n_tb), 0, c));      // (sr, n_tb, 0) == (sr + 1, 0, 0)
 }
 
 __global__ void __launch_bounds__(kLinkThreads) k_start_cell_count(const uint8_t* __restrict__ start_flag,

@@ -12,6 +12,7 @@
 #include "arena.h"
 #include "common.cuh"
 #include "finder.cuh"
+#include "follow_rows.cuh"
 #include "ingest.cuh"
 #include "links.cuh"
 #include "merge.cuh"
@@ -36,14 +37,14 @@ struct Ids {   // arena allocation ids
   int stage_in = -1, stage_out = -1;
   int bin_start, sort_keys, tmp_keys, tmp_orig, tmp_yt, sort_hist, yt, orig, hsr, link_up, link_down, link_up_clean, start_flag, cell_count, start_hits,
       scan_a, scan_b, seeds_a, seeds_b, row_hit, tl_meta, tl_rec, tl_cur, claim, owned, own_mask,
-      flag, track_idx, hit_off, track_slot;
+      flag, track_idx, hit_off, track_slot, chunks;
 };
 
 struct Capacities {
   int64_t max_clusters, max_tracklets, max_tracks, max_track_hits;
   int n_tb, n_pb, grid_w, n_bins, n_link_ctas;
   int n_slices, slice_bins;     // start-hit processing order: time slices of slice_bins grid time bins
-  int64_t n_cells;
+  int64_t n_cells, max_chunks;
   int sort_passes, sort_digit_bits, sort_tiles;
 };
 
@@ -104,8 +105,9 @@ bool capacities(const tpc_geometry_t* g, const tpc_params_t* p, int64_t max_clus
   const int slice_tb = p->slice_time_bins > 0 ? p->slice_time_bins : kDefaultSliceTimeBins;
   c.slice_bins = std::max(1, slice_tb / c.grid_w);
   c.n_slices = (c.n_tb + c.slice_bins - 1) / c.slice_bins;
-  c.n_cells = (int64_t)g->n_sectors * g->n_rows * c.n_pb * c.n_slices;
+  c.n_cells = (int64_t)g->n_sectors * g->n_rows * c.n_slices;
   if (c.n_cells >= 2147483000) return false;
+  c.max_chunks = c.max_tracklets / kFrChunk + (int64_t)g->n_sectors * c.n_slices + 2;      // follow_rows.cuh: chunks never straddle a (sector, slice) group
   int bits = 1;
   while (((int64_t)1 << bits) <= (int64_t)c.n_bins) ++bits;          // the sentinel key n_bins must be representable
   c.sort_passes = (bits + kRadixMaxBits - 1) / kRadixMaxBits;
@@ -141,6 +143,7 @@ void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids
   id.start_flag = plan.add("start_flag(u8)", N, S_CLEAN_START, S_COMPACT);
   id.cell_count = plan.add("start_cell_count", 4 * ((size_t)c.n_cells + 2), S_COMPACT, S_COMPACT);
   id.start_hits = plan.add("start_hits", 4 * T, S_COMPACT, S_EMIT);
+  id.chunks = plan.add("follower_chunks(uint2)", 8 * (size_t)c.max_chunks, S_COMPACT, S_FOLLOW_DOWN);
   id.seeds_a = plan.add("tracklet_seeds_a(int4)", 16 * T, S_TL_INIT, S_FOLLOW_DOWN);
   id.seeds_b = plan.add("tracklet_seeds_b(float4)", 16 * T, S_TL_INIT, S_FOLLOW_DOWN);
   id.row_hit = plan.add("tracklet_row_hit", 4 * (size_t)kRowStride * T, S_TL_INIT, S_EMIT);
@@ -199,6 +202,8 @@ struct tpc_tracker {
   int64_t last_launches = 0, last_merge_launches = 0;
   int ctas_refit = 148 * 8;
   int ctas_fit_up = 148, ctas_follow_up = 148, ctas_fit_down = 148, ctas_follow_down = 148;   // persistent grids: SMs x resident CTAs per SM
+  int ctas_rows_up = 148, ctas_rows_down = 148;
+  bool follow_rows = false;        // row-synchronous follower (follow_rows.cuh) instead of the per-lane one
 };
 
 // Exhaustive check of sqrt_rn_normal / rcp_rn_normal (tracklet.cuh) against sqrtf() / (1.0f / x) over every fp32 bit
@@ -218,6 +223,47 @@ __global__ void __launch_bounds__(256) k_selftest_fast_math(unsigned long long* 
   bad_sqrt = __reduce_add_sync(0xffffffffu, (unsigned)bad_sqrt);
   bad_rcp = __reduce_add_sync(0xffffffffu, (unsigned)bad_rcp);
   if (lane_id() == 0) { if (bad_sqrt) atomicAdd(mismatches, bad_sqrt); if (bad_rcp) atomicAdd(mismatches + 1, bad_rcp); }
+}
+
+// fp32 issue-rate micro-benchmarks (tpc_selftest_alu_peak): 8 independent chains per thread, alternating multiply and add,
+// compiled with --fmad=false like the rest of the file, so nothing contracts into FMA.
+constexpr int kAluIters = 2048, kAluChains = 8;
+__global__ void __launch_bounds__(256) k_alu_peak_scalar(float* __restrict__ sink, float a, float b) {
+  float v[kAluChains];
+#pragma unroll
+  for (int k = 0; k < kAluChains; ++k) v[k] = (float)(threadIdx.x + k) * 1.0e-3f;
+  for (int i = 0; i < kAluIters; ++i) {
+#pragma unroll
+    for (int k = 0; k < kAluChains; ++k) v[k] = v[k] * a;
+#pragma unroll
+    for (int k = 0; k < kAluChains; ++k) v[k] = v[k] + b;
+  }
+  float s = 0.0f;
+#pragma unroll
+  for (int k = 0; k < kAluChains; ++k) s += v[k];
+  if (s == 123.456f) sink[blockIdx.x] = s;             // never true: keeps the chains alive
+}
+// Packed form: every multiply is fma.rn.f32x2(a, b, -0) and every add fma.rn.f32x2(a, 1, c) -- exactly RN(a*b) and RN(a+c)
+// in both halves (IEEE), written as explicit FMAs because ptxas contracts a mul.rn.f32x2 feeding an add.rn.f32x2 into one
+// FFMA2 even under --fmad=false (seen in the SASS), and an explicit fma is never re-fused.
+__global__ void __launch_bounds__(256) k_alu_peak_packed(float* __restrict__ sink, float a, float b) {
+  unsigned long long v[kAluChains], pa, pb, one, nz;
+  asm("mov.b64 %0, {%1, %1};" : "=l"(pa) : "f"(a));
+  asm("mov.b64 %0, {%1, %1};" : "=l"(pb) : "f"(b));
+  asm("mov.b64 %0, {%1, %1};" : "=l"(one) : "f"(1.0f));
+  asm("mov.b64 %0, {%1, %1};" : "=l"(nz) : "f"(-0.0f));
+#pragma unroll
+  for (int k = 0; k < kAluChains; ++k) { const float x = (float)(threadIdx.x + k) * 1.0e-3f; asm("mov.b64 %0, {%1, %1};" : "=l"(v[k]) : "f"(x)); }
+  for (int i = 0; i < kAluIters; ++i) {
+#pragma unroll
+    for (int k = 0; k < kAluChains; ++k) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(v[k]) : "l"(pa), "l"(nz));
+#pragma unroll
+    for (int k = 0; k < kAluChains; ++k) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(v[k]) : "l"(one), "l"(pb));
+  }
+  float s = 0.0f;
+#pragma unroll
+  for (int k = 0; k < kAluChains; ++k) { float lo, hi; asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v[k])); s += lo + hi; }
+  if (s == 123.456f) sink[blockIdx.x] = s;
 }
 
 extern "C" {
@@ -338,6 +384,20 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
     t->ctas_fit_down = resident(k_tracklet_fit<true>, TPC_FIT_CTAS_PER_SM);
     t->ctas_follow_down = resident(k_tracklet_follow<true>, TPC_FOLLOW_CTAS_PER_SM);
     t->ctas_refit = resident(k_refit_chains, 64);
+    t->follow_rows = p->follower == 1 && p->miss_limit <= 255;      // the packed per-tracklet counters are 8 bits wide
+    if (cudaFuncSetAttribute(k_follow_rows<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FrSmem)) != cudaSuccess ||
+        cudaFuncSetAttribute(k_follow_rows<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FrSmem)) != cudaSuccess) {
+      cudaGetLastError(); tpc_tracker_destroy(t); return TPC_ECUDA;
+    }
+    auto resident_rows = [&](auto kernel) {
+      int per_sm = 1;
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kFrThreads, sizeof(FrSmem)) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError(); per_sm = 1;
+      }
+      return sms * per_sm;
+    };
+    t->ctas_rows_up = resident_rows(k_follow_rows<false>);
+    t->ctas_rows_down = resident_rows(k_follow_rows<true>);
   }
   for (int i = 0; i <= N_STEPS; ++i)
     if (cudaEventCreate(&t->ev[i]) != cudaSuccess) { cudaGetLastError(); tpc_tracker_destroy(t); return TPC_ECUDA; }
@@ -493,15 +553,15 @@ int tpc_tracker_work_counters(tpc_tracker_t* t, void* cuda_stream, int64_t* out,
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (cudaMemcpyAsync(&h, t->counters, 256, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
       cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return TPC_ECUDA; }
-  int64_t v[21] = {h.i32[kCntTracklets], h.i32[kCntStartHits], (int64_t)(uint32_t)h.i32[kCntInvalid], 0, 0, 0};
+  int64_t v[22] = {h.i32[kCntTracklets], h.i32[kCntStartHits], (int64_t)(uint32_t)h.i32[kCntInvalid], 0, 0, 0};
   for (int ph = 0; ph < 4; ++ph)
     for (int k = 0; k < 3; ++k) {
       v[6 + 3 * ph + k] = (int64_t)h.u64[kCnt64Phase0 - 4 + 3 * ph + k];
       v[3 + k] += v[6 + 3 * ph + k];
     }
-  for (int k = 0; k < 3; ++k) v[18 + k] = (int64_t)h.u64[kCnt64Rare0 - 4 + k];
-  for (int i = 0; i < 21 && i < capacity; ++i) out[i] = v[i];
-  return 21;
+  for (int k = 0; k < 4; ++k) v[18 + k] = (int64_t)h.u64[kCnt64Rare0 - 4 + k];
+  for (int i = 0; i < 22 && i < capacity; ++i) out[i] = v[i];
+  return 22;
 }
 
 int tpc_tracker_step_ms(tpc_tracker_t* t, float* ms_out, int32_t capacity) {
@@ -546,6 +606,7 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   uint8_t* start_flag = P.ptr<uint8_t>(A, id.start_flag);
   uint32_t* cell_count = P.ptr<uint32_t>(A, id.cell_count);
   uint32_t* start_hits = P.ptr<uint32_t>(A, id.start_hits);
+  uint2* chunks = P.ptr<uint2>(A, id.chunks);
   int32_t* counters = t->counters;                             // layout: kCnt* in tracklet.cuh
   uint32_t* n_invalid = reinterpret_cast<uint32_t*>(counters + kCntInvalid);
   TrackletSeeds seeds;
@@ -619,6 +680,10 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
     launches += exclusive_scan_u32(cell_count, cell_count, n_cells, scan_a, st);
     k_start_cell_write<<<cell_ctas, kLinkThreads, 0, st>>>(start_flag, bin_start, sc, cell_count, scan_a + scan_tiles(n_cells), start_hits,
                                                            (uint32_t)T, counters, c); ++launches;
+    if (t->follow_rows) {    // work units of the row-synchronous follower: <= kFrChunk tracklets of one (sector, slice) group each
+      k_follow_chunk_list<<<1, kScanThreads, 0, st>>>(cell_count, scan_a + scan_tiles(n_cells), t->geom.n_sectors * t->cap.n_slices, c.n_rows,
+                                                      chunks, counters); ++launches;
+    }
   }
 
   // ---- C5 tracklet constructor ----
@@ -627,14 +692,17 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   k_tracklet_init<<<(int)((tl_bound + 255) / 256), 256, 0, st>>>(yt, hsr, link_up_clean, start_hits, counters, seeds, tl.row_hit, c); ++launches;
   {
     const int need = (int)((tl_bound + kTrackletThreads - 1) / kTrackletThreads);
+    const int64_t rows_need = std::max<int64_t>(1, std::min<int64_t>(t->cap.max_chunks, tl_bound / kFrChunk + (int64_t)t->geom.n_sectors * t->cap.n_slices + 1));
     mark(S_FIT_UP);
     k_tracklet_fit<false><<<std::min(t->ctas_fit_up, need), kTrackletThreads, 0, st>>>(yt, orig, seeds, counters, tl, c);
     mark(S_FOLLOW_UP);
-    k_tracklet_follow<false><<<std::min(t->ctas_follow_up, need), kTrackletThreads, 0, st>>>(yt, orig, bin_start, seeds, counters, tl, c);
+    if (t->follow_rows) k_follow_rows<false><<<(int)std::min<int64_t>(t->ctas_rows_up, rows_need), kFrThreads, sizeof(FrSmem), st>>>(yt, orig, bin_start, seeds, counters, chunks, tl, c);
+    else k_tracklet_follow<false><<<std::min(t->ctas_follow_up, need), kTrackletThreads, 0, st>>>(yt, orig, bin_start, seeds, counters, tl, c);
     mark(S_FIT_DOWN);
     k_tracklet_fit<true><<<std::min(t->ctas_fit_down, need), kTrackletThreads, 0, st>>>(yt, orig, seeds, counters, tl, c);
     mark(S_FOLLOW_DOWN);
-    k_tracklet_follow<true><<<std::min(t->ctas_follow_down, need), kTrackletThreads, 0, st>>>(yt, orig, bin_start, seeds, counters, tl, c);
+    if (t->follow_rows) k_follow_rows<true><<<(int)std::min<int64_t>(t->ctas_rows_down, rows_need), kFrThreads, sizeof(FrSmem), st>>>(yt, orig, bin_start, seeds, counters, chunks, tl, c);
+    else k_tracklet_follow<true><<<std::min(t->ctas_follow_down, need), kTrackletThreads, 0, st>>>(yt, orig, bin_start, seeds, counters, tl, c);
     launches += 4;
   }
   const int warp_ctas = (int)((tl_bound * 32 + kSelectorThreads - 1) / kSelectorThreads);
@@ -685,6 +753,38 @@ int tpc_selftest_fast_math(void* cuda_stream, uint64_t* mismatches_out) {
   cudaFree(d);
   if (!ok) { cudaGetLastError(); return TPC_ECUDA; }
   mismatches_out[0] = h[0]; mismatches_out[1] = h[1];
+  return TPC_OK;
+}
+
+int tpc_selftest_alu_peak(void* cuda_stream, double* out) {
+  if (!out) return TPC_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  int dev = 0, sms = 148;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return TPC_ECUDA; }
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const int ctas = sms * 8 * 4;                        // 4 waves of 8 resident CTAs of 256 threads per SM
+  float* sink = nullptr;
+  cudaEvent_t e[3] = {};
+  bool ok = cudaMalloc(&sink, (size_t)ctas * 4) == cudaSuccess;
+  for (int i = 0; i < 3 && ok; ++i) ok = cudaEventCreate(&e[i]) == cudaSuccess;
+  float ms[2] = {0.0f, 0.0f};
+  if (ok) {
+    k_alu_peak_scalar<<<ctas, 256, 0, st>>>(sink, 1.0000001f, 1.0e-9f);     // warm-up (clocks, instruction cache)
+    k_alu_peak_packed<<<ctas, 256, 0, st>>>(sink, 1.0000001f, 1.0e-9f);
+    cudaEventRecord(e[0], st);
+    k_alu_peak_scalar<<<ctas, 256, 0, st>>>(sink, 1.0000001f, 1.0e-9f);
+    cudaEventRecord(e[1], st);
+    k_alu_peak_packed<<<ctas, 256, 0, st>>>(sink, 1.0000001f, 1.0e-9f);
+    cudaEventRecord(e[2], st);
+    ok = cudaStreamSynchronize(st) == cudaSuccess && cudaEventElapsedTime(&ms[0], e[0], e[1]) == cudaSuccess &&
+         cudaEventElapsedTime(&ms[1], e[1], e[2]) == cudaSuccess && cudaGetLastError() == cudaSuccess;
+  }
+  for (int i = 0; i < 3; ++i) if (e[i]) cudaEventDestroy(e[i]);
+  if (sink) cudaFree(sink);
+  if (!ok || ms[0] <= 0.0f || ms[1] <= 0.0f) { cudaGetLastError(); return TPC_ECUDA; }
+  const double lane_inst = (double)ctas * 256.0 * (double)kAluIters * (double)(2 * kAluChains);
+  out[0] = lane_inst / ((double)ms[0] * 1.0e-3);
+  out[1] = 2.0 * lane_inst / ((double)ms[1] * 1.0e-3);
   return TPC_OK;
 }
 

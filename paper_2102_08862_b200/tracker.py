@@ -17,7 +17,7 @@ STATUS_TRACKLET_OVERFLOW, STATUS_TRACK_OVERFLOW, STATUS_TRACK_HIT_OVERFLOW, STAT
 
 EXPORTS = ("tpc_tracker_arena_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
            "tpc_tracker_step_ms", "tpc_tracker_step_name", "tpc_tracker_last_launches", "tpc_tracker_work_counters",
-           "tpc_tracker_arena_plan", "tpc_selftest_fast_math",
+           "tpc_tracker_arena_plan", "tpc_selftest_fast_math", "tpc_selftest_alu_peak",
            "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_refit_chains", "tpc_vertex_time", "tpc_merge_last_launches",
            "tpc_tracker_destroy", "tpc_strerror")
 
@@ -36,7 +36,7 @@ class Params(C.Structure):
                 ("slope_y_max", C.c_float), ("slope_z_max", C.c_float), ("seed_min_hits", C.c_int32),
                 ("sin_phi_max", C.c_float), ("inv_R_per_qpt", C.c_float),
                 ("c0_y2", C.c_float), ("c0_s2", C.c_float), ("c0_k2", C.c_float), ("c0_z2", C.c_float), ("c0_t2", C.c_float),
-                ("grid_time_bins", C.c_int32), ("grid_pad_bins", C.c_int32), ("slice_time_bins", C.c_int32), ("reserved0", C.c_int32),
+                ("grid_time_bins", C.c_int32), ("grid_pad_bins", C.c_int32), ("slice_time_bins", C.c_int32), ("follower", C.c_int32),
                 ("max_clusters", C.c_int64), ("max_tracklets", C.c_int64),
                 ("max_tracks", C.c_int64), ("max_track_hits", C.c_int64), ("arena", C.c_void_p), ("arena_bytes", C.c_size_t),
                 ("host_staging", C.c_int32), ("profile", C.c_int32)]
@@ -92,7 +92,7 @@ def default_params(sigma_y: float = 0.08, sigma_z: float = 0.12, max_clusters: i
     return Params(win_slope=0.05, win_const=0.5, chi2_cut=9.0, miss_limit=10, min_hits=30,
                   sigma_y_cm=sigma_y, sigma_z_cm=sigma_z, slope_y_max=1.0, slope_z_max=1.5, seed_min_hits=3,
                   sin_phi_max=0.95, inv_R_per_qpt=1.0 / 666.7, c0_y2=1.0, c0_s2=0.1, c0_k2=100.0, c0_z2=1.0, c0_t2=0.1,
-                  grid_time_bins=0, grid_pad_bins=0, slice_time_bins=0, reserved0=0, max_clusters=max_clusters, max_tracklets=0, max_tracks=0, max_track_hits=0,
+                  grid_time_bins=0, grid_pad_bins=0, slice_time_bins=0, follower=0, max_clusters=max_clusters, max_tracklets=0, max_tracks=0, max_track_hits=0,
                   arena=None, arena_bytes=0, host_staging=0, profile=0)
 
 
@@ -124,6 +124,8 @@ def load_library(build_if_missing: bool = True):
         L.tpc_tracker_destroy.argtypes = [vp]
         L.tpc_selftest_fast_math.argtypes = [vp, C.POINTER(C.c_uint64)]
         L.tpc_selftest_fast_math.restype = C.c_int
+        L.tpc_selftest_alu_peak.argtypes = [vp, C.POINTER(C.c_double)]
+        L.tpc_selftest_alu_peak.restype = C.c_int
         L.tpc_merge_scratch_bytes.argtypes = [vp, C.c_int64]
         L.tpc_merge_scratch_bytes.restype = C.c_size_t
         L.tpc_merge_tracks.argtypes = [vp, C.POINTER(MergeParams), C.POINTER(Tracks), vp, C.POINTER(Merged)]
@@ -161,6 +163,20 @@ def tpc_selftest_fast_math(stream=None) -> tuple:
     if rc != TPC_OK:
         raise TpcError(rc, "tpc_selftest_fast_math")
     return int(out[0]), int(out[1])
+
+
+def tpc_selftest_alu_peak(stream=None) -> tuple:
+    """(scalar fp32 multiply / add lane-instructions per second, fp32 operations per second issued as packed f32x2)
+    measured by the library's micro-benchmark (include/tpc_tracker.h): the "alu" peak of the constructor's roofline."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("tpc_selftest_alu_peak needs a CUDA device")
+    s = stream if stream is not None else torch.cuda.current_stream()
+    out = (C.c_double * 2)()
+    rc = load_library().tpc_selftest_alu_peak(C.c_void_p(s.cuda_stream), out)
+    if rc != TPC_OK:
+        raise TpcError(rc, "tpc_selftest_alu_peak")
+    return float(out[0]), float(out[1])
 
 
 def tpc_tracker_arena_bytes(geometry: Geometry, params: Params, max_clusters: int = 0) -> int:
@@ -372,15 +388,16 @@ class Tracker:
 
     def work_counters(self, stream=None) -> dict:
         s = stream if stream is not None else self._torch.cuda.current_stream(self.device)
-        buf = (C.c_int64 * 21)()
-        k = self.lib.tpc_tracker_work_counters(self.handle, C.c_void_p(s.cuda_stream), buf, 21)
+        buf = (C.c_int64 * 22)()
+        k = self.lib.tpc_tracker_work_counters(self.handle, C.c_void_p(s.cuda_stream), buf, 22)
         if k < 0:
             raise TpcError(k, "tpc_tracker_work_counters")
         names = ("tracklets", "start_hits", "invalid_clusters", "row_steps", "updates", "candidates")
         out = {nm: int(buf[i]) for i, nm in enumerate(names)}
         for p, ph in enumerate(("fit_up", "follow_up", "fit_down", "follow_down")):
             out[ph] = {nm: int(buf[6 + 3 * p + i]) for i, nm in enumerate(("row_steps", "updates", "candidates"))}
-        out["rare_paths"] = {"refit_replays": int(buf[18]), "refits_without_update": int(buf[19]), "search_ties": int(buf[20])}
+        out["rare_paths"] = {"refit_replays": int(buf[18]), "refits_without_update": int(buf[19]), "search_ties": int(buf[20]),
+                             "searches_in_global_memory": int(buf[21])}
         return out
 
     def arena_plan(self) -> list:
