@@ -29,10 +29,14 @@ CONFIG_NAMES = {0: "configs[0] single sector, 300 tracks", 1: "configs[1] full T
                 2: "configs[2] 2 ms continuous readout at 50 kHz", 3: "configs[3] 10 ms continuous readout at 50 kHz",
                 4: "configs[4] 10 ms high-occupancy stress frame"}
 
-# Algorithmic HBM bytes per cluster of each step -- what the method must move, not what it moves.
+# Algorithmic HBM bytes per cluster of each step: SURVEY.md §8(d)'s per-unit figures (what the METHOD must move, whatever
+# sort or layout this implementation uses).  ingest: 12 read + 12 read again + 12 write (+ 4 grid) = 40, split
+# over its two kernels; finder 24; cleaner + start hits 24, split over its two steps; tracklet_init: seeds + chain walk
+# (32 B + 6.8 chain hits x 16 B per tracklet, 0.076 tracklets per cluster) = 11; selector 60 = claim 30 + count 26 + emit 4.
 ALGO_BYTES_PER_CLUSTER = {
-    "ingest_radix_sort": 4 * (4 + 16 + 16), "grid_build": 4 + 4 + 2,
-    "neighbours_finder": 10 + 8 + 8, "cleaner_start_hits": 8 + 4 + 1, "start_hit_compaction": 1,
+    "ingest_radix_sort": 36, "grid_build": 4,
+    "neighbours_finder": 24, "cleaner_start_hits": 20, "start_hit_compaction": 4, "tracklet_init": 11,
+    "selector_claim": 30, "selector_count": 26, "selector_scan": 0, "selector_emit": 4,
 }
 # Tracklet constructor: bound by plain fp32 ALU issue.  Algorithmic lane-instructions of one row step
 # (= one transport [+ search] [+ update]) counted from the statement lists of DESIGN.md §3 with IEEE division and
@@ -40,10 +44,27 @@ ALGO_BYTES_PER_CLUSTER = {
 ALGO_LANE_INST_TRANSPORT, ALGO_LANE_INST_UPDATE, ALGO_LANE_INST_PER_CANDIDATE = 123, 52, 12
 TRACKLET_PHASES = {"tracklet_fit_up": "fit_up", "tracklet_follow_up": "follow_up", "tracklet_fit_down": "fit_down",
                    "tracklet_follow_down": "follow_down"}     # step name -> work-counter group
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of configs[3], seed 1
-# (profiles/r01e_ncu_full_config3.md); reported as roofline.traffic for that workload only, null otherwise.
-NCU_TRAFFIC_BYTES_CONFIG3 = {"tracklet_follow_up": 17.941e9 + 5.657e9, "tracklet_follow_down": 19.170e9 + 5.006e9,
-                             "tracklet_fit_down": 6.703e9 + 0.782e9, "neighbours_finder": 3.815e9 + 1.279e9}
+# roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch, read from the committed summary of the
+# `ncu --set full` capture of configs[3], seed 1 (profiles/NCU_TRAFFIC_CSV; its .md names the command and the commit it was
+# taken at).  Reported for that workload only, null otherwise.
+NCU_TRAFFIC_CSV = "r02_ncu_traffic_config3.csv"
+STEP_KERNEL = {"tracklet_follow_up": "k_tracklet_follow<0>", "tracklet_follow_down": "k_tracklet_follow<1>",
+               "tracklet_fit_up": "k_tracklet_fit<0>", "tracklet_fit_down": "k_tracklet_fit<1>", "neighbours_finder": "k_neighbours_finder",
+               "selector_claim": "k_selector_claim", "selector_count": "k_selector_count", "tracklet_init": "k_tracklet_init"}
+
+
+def _ncu_traffic():
+    """{kernel name: (bytes per launch, commit)} from profiles/NCU_TRAFFIC_CSV; {} if the file is missing."""
+    out = {}
+    try:
+        with open(os.path.join(ROOT, "profiles", NCU_TRAFFIC_CSV)) as f:
+            for line in f:
+                q = [x.strip() for x in line.split(",")]
+                if len(q) >= 4 and q[0] != "kernel" and not q[0].startswith("#"):
+                    out[q[0]] = (float(q[1]) + float(q[2]), q[3])
+    except OSError:
+        pass
+    return out
 SM_COUNT, SMSP_PER_SM, LANES = 148, 4, 32      # B300_MICROARCH.md: 4 schedulers per SM, <= 1 warp instruction per cycle each
 
 
@@ -123,15 +144,17 @@ def _cpu_oracle_run(cid, seed, frame_us):
     return tf.n, dt, len(r.tr_seed)
 
 
-def _cpu_oracle_run_all_cores(cid, seed, frame_us):
+def _cpu_oracle_run_all_cores(cid, seed, frame_us, tf=None):
     """The same unchanged oracle, one call per sector (sectors are independent), from a thread pool: BASELINE.md §3 (2).
-    ctypes releases the GIL during the call.  Returns (clusters, seconds, threads used, tracks)."""
+    ctypes releases the GIL during the call.  Returns (clusters, seconds, threads used, tracks).  `tf`: a frame that is
+    already generated (the WHOLE benchmark frame); else the generator's frame cut to frame_us."""
     import numpy as np
     from concurrent.futures import ThreadPoolExecutor
     import oracle
     from paper_2102_08862_b200 import gen
     cfg = gen.preset(cid, seed, frame_us if cid >= 2 else None)
-    tf = gen.generate(cfg, want_truth=False)
+    if tf is None:
+        tf = gen.generate(cfg, want_truth=False)
     n_rows = 152
     sec = (tf.row.astype(np.int64) // n_rows)
     parts = []
@@ -151,15 +174,20 @@ def _cpu_oracle_run_all_cores(cid, seed, frame_us):
 
 
 def run_reference(args):
-    """--impl reference: the CPU oracle on the box's host cores, same metric; each step a bounded sample."""
+    """--impl reference: the CPU oracle, as it stands, on the box's host cores (one unchanged call per sector from a thread
+    pool: sectors are independent), same metric; each step a bounded sample of the workload (the frame cut to
+    --ref-frame-us) so that the whole run ends within a few minutes."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
     cid = args.config
     sample_us = args.ref_frame_us
-    total_n, total_t = 0, 0.0
+    total_n, total_t, cores = 0, 0.0, 1
     for i in range(args.warmup + args.steps):
-        n, dt, _ = _cpu_oracle_run(cid, 1000 + i, sample_us)
+        if cid >= 1:
+            n, dt, cores, _ = _cpu_oracle_run_all_cores(cid, 1000 + i, sample_us)
+        else:
+            n, dt, _ = _cpu_oracle_run(cid, 1000 + i, sample_us)
         if i >= args.warmup:
             total_n += n; total_t += dt
     value = total_n / total_t
@@ -169,7 +197,7 @@ def run_reference(args):
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_t / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": CONFIG_NAMES[cid], "sample": sample, "clusters_per_step": total_n // args.steps},
-            "cpu_baseline": {"value": value, "unit": "clusters/s", "cores": 1, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": "clusters/s", "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": "clusters/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -185,8 +213,9 @@ def main():
     ap.add_argument("--frame-us", type=float, default=None, help="override the frame length (smoke runs only)")
     ap.add_argument("--seed", type=int, default=1)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--ref-frame-us", type=float, default=60.0, help="frame length of one reference-arm step")
-    ap.add_argument("--cpu-sample-us", type=float, default=150.0, help="frame length of the cpu_baseline sample")
+    ap.add_argument("--ref-frame-us", type=float, default=1000.0, help="frame length of one reference-arm step")
+    ap.add_argument("--cpu-sample-us", type=float, default=150.0, help="frame length of the single-core cpu_baseline sample")
+    ap.add_argument("--cpu-whole-frame", type=int, default=1, help="1: time the all-cores oracle on the WHOLE benchmark frame (about 20 s)")
     ap.add_argument("--grid-time-bins", type=int, default=0, help="grid bin width in time bins (0 = library default)")
     ap.add_argument("--slice-time-bins", type=int, default=0, help="processing-order time slice (0 = library default)")
     ap.add_argument("--grid-pad-bins", type=int, default=0, help="grid bins across a pad row (0 = library default)")
@@ -226,7 +255,8 @@ def main():
     torch.cuda.synchronize()
 
     g = T.default_geometry(cfg.n_sectors, tf.max_time_bin)
-    trk = T.Tracker(g, _tracker_params(T, cfg, n, False, True, (args.grid_time_bins, args.grid_pad_bins, args.slice_time_bins), args.follower), device=str(dev))
+    gp = (args.grid_time_bins, args.grid_pad_bins, args.slice_time_bins)
+    trk = T.Tracker(g, _tracker_params(T, cfg, n, False, False, gp, args.follower), device=str(dev))     # `value`: no per-step events
     outs = trk.alloc_outputs(n)
     stream = torch.cuda.Stream(device=dev)
 
@@ -253,8 +283,11 @@ def main():
         barrier()
     total_ms = e0.elapsed_time(e1)
     launches = trk.last_launches() * args.steps
-    # per-kernel durations: CUDA events recorded by the library on the same stream (params.profile = 1),
-    # averaged over a few extra steps
+    trk.close()
+    del trk
+    # per-kernel durations: CUDA events recorded by the library on the same stream (a second handle with
+    # params.profile = 1), averaged over a few extra steps
+    trk = T.Tracker(g, _tracker_params(T, cfg, n, False, True, gp, args.follower), device=str(dev))
     n_prof = min(args.steps, 5)
     for _ in range(n_prof):
         with torch.cuda.stream(stream):
@@ -267,6 +300,7 @@ def main():
     n_track_hits = int(outs[0].n_track_hits[0])
     status = int(outs[0].status[0])
     arena_gb = trk.arena_bytes / 1e9
+    alu_measured = T.tpc_selftest_alu_peak(stream)       # (scalar fp32 lane-inst/s, packed f32x2 fp32 ops/s), this GPU, now
     # ---- widening step C7 (sector-boundary merging of the tracks, not part of `value`): timed on its own ----
     merge = None
     if cfg.n_sectors >= 18:
@@ -305,43 +339,46 @@ def main():
     # processing node double-buffers time frames: the PCIe copies of one frame overlap the kernels of the other.
     e2e = None
     if not args.no_e2e:
+        def measure_e2e(n_fl):
+            trks = [T.Tracker(g, _tracker_params(T, cfg, n, True, False, gp, args.follower), device=str(dev)) for _ in range(n_fl)]
+            houts = [t.alloc_outputs(n, host=True) for t in trks]
+            streams = [torch.cuda.Stream(device=dev) for _ in range(n_fl)]
+            k_each = max(2, (max(3, args.steps // 2) + n_fl - 1) // n_fl)
+
+            def run_frames(i, k):
+                torch.cuda.set_device(local_rank)
+                for _ in range(k):
+                    trks[i].tpc_track_timeframe_host(*host, n=n, outputs=houts[i], stream=streams[i])
+
+            def run_all(k):
+                th = [threading.Thread(target=run_frames, args=(i, k)) for i in range(n_fl)]
+                for t_ in th:
+                    t_.start()
+                for t_ in th:
+                    t_.join()
+
+            run_all(1)                                   # warm-up
+            barrier()
+            e0.record(streams[0])
+            run_all(k_each)
+            for s_ in streams[1:]:
+                streams[0].wait_stream(s_)
+            e1.record(streams[0])
+            barrier()
+            k_e2e = k_each * n_fl
+            ms = replicas.max_over_ranks(e0.elapsed_time(e1) / k_e2e, world, device=dev)
+            k = int(houts[0][0].n_tracks[0]); h = int(houts[0][0].n_track_hits[0])
+            d2h = 16 + k * (8 + 5 * 4 + 7 * 4 + 36) + 4 * h
+            for t_ in trks:
+                t_.close()
+            return {"value": n_all / (float(ms) * 1e-3), "unit": "clusters/s", "ms_per_step": float(ms),
+                    "h2d_bytes_per_step": 12 * n, "d2h_bytes_per_step": d2h, "steps": k_e2e, "frames_in_flight": n_fl}
+
         n_fl = max(1, args.e2e_inflight)
-        gp = (args.grid_time_bins, args.grid_pad_bins, args.slice_time_bins)
-        trks = [T.Tracker(g, _tracker_params(T, cfg, n, True, False, gp, args.follower), device=str(dev)) for _ in range(n_fl)]
-        houts = [t.alloc_outputs(n, host=True) for t in trks]
-        streams = [torch.cuda.Stream(device=dev) for _ in range(n_fl)]
-        k_each = max(2, (max(3, args.steps // 2) + n_fl - 1) // n_fl)
-
-        def run_frames(i, k):
-            torch.cuda.set_device(local_rank)
-            for _ in range(k):
-                trks[i].tpc_track_timeframe_host(*host, n=n, outputs=houts[i], stream=streams[i])
-
-        def run_all(k):
-            th = [threading.Thread(target=run_frames, args=(i, k)) for i in range(n_fl)]
-            for t_ in th:
-                t_.start()
-            for t_ in th:
-                t_.join()
-
-        run_all(1)                                       # warm-up
-        barrier()
-        e0.record(streams[0])
-        run_all(k_each)
-        for s_ in streams[1:]:
-            streams[0].wait_stream(s_)
-        e1.record(streams[0])
-        barrier()
-        k_e2e = k_each * n_fl
-        ms = e0.elapsed_time(e1) / k_e2e
-        t2 = [replicas.max_over_ranks(ms, world, device=dev)]
-        k = int(houts[0][0].n_tracks[0]); h = int(houts[0][0].n_track_hits[0])
-        d2h = 16 + k * (8 + 5 * 4 + 7 * 4 + 36) + 4 * h
-        e2e = {"value": n_all / (float(t2[0]) * 1e-3), "unit": "clusters/s", "ms_per_step": float(t2[0]),
-               "h2d_bytes_per_step": 12 * n, "d2h_bytes_per_step": d2h, "steps": k_e2e, "frames_in_flight": n_fl}
-        for t_ in trks:
-            t_.close()
-        del trks, houts
+        e2e = measure_e2e(n_fl)                          # the headline: frames double-buffered the way a processing node runs
+        if n_fl != 1:                                    # ... and the latency-bound figure beside it: one frame at a time
+            one = measure_e2e(1)
+            e2e["one_frame_in_flight"] = {k: one[k] for k in ("value", "ms_per_step", "steps")}
 
     if rank != 0:
         if world > 1:
@@ -352,15 +389,20 @@ def main():
     peak, peak_src = _peaks()
     clk = clocks.summary()
     mhz = clk["sm_mhz"] or clk["sm_max_mhz"] or 1965.0
-    alu_peak = SM_COUNT * SMSP_PER_SM * LANES * mhz * 1e6 / 1e12          # T lane-instructions / s at the clock under load
-    alu_src = f"148 SMs x 4 schedulers x 32 lanes x {mhz:.0f} MHz (SM clock under load)"
+    alu_derived = SM_COUNT * SMSP_PER_SM * LANES * mhz * 1e6 / 1e12          # T lane-instructions / s at the clock under load
+    alu_peak = alu_measured[0] / 1e12                                        # measured on this GPU in this run
+    alu_src = (f"measured: tpc_selftest_alu_peak, dependency-free scalar FMUL/FADD streams on all SMs, no FMA contraction "
+               f"({alu_peak:.2f} T lane-inst/s = {alu_peak / alu_derived:.3f} of 148 SMs x 4 schedulers x 32 lanes x {mhz:.0f} MHz); "
+               f"the same arithmetic issued as packed f32x2 FFMA2 runs at {alu_measured[1] / 1e12:.2f} T fp32 op/s")
     total_step_ms = sum(step_acc.values())
+    traffic = _ncu_traffic() if (cid == 3 and args.seed == 1 and not args.frame_us and args.follower == 0) else {}
     kernels = {}
     for k, ms in step_acc.items():
         row = {"ms": round(ms, 4), "share_of_step": round(ms / total_step_ms, 4)}
-        if ALGO_BYTES_PER_CLUSTER.get(k) and ms > 0:
+        if k in ALGO_BYTES_PER_CLUSTER and ms > 0:
             a = ALGO_BYTES_PER_CLUSTER[k] * n / (ms * 1e-3) / 1e9
-            row.update({"bound": "hbm", "achieved": round(a, 1), "peak": peak, "unit": "GB/s", "frac": round(a / peak, 4)})
+            row.update({"bound": "hbm", "achieved": round(a, 1), "peak": peak, "unit": "GB/s", "frac": round(a / peak, 4),
+                        "algo_bytes_per_cluster": ALGO_BYTES_PER_CLUSTER[k]})
         elif k in TRACKLET_PHASES and ms > 0:
             w = work[TRACKLET_PHASES[k]]
             inst = (ALGO_LANE_INST_TRANSPORT * w["row_steps"] + ALGO_LANE_INST_UPDATE * w["updates"] +
@@ -368,12 +410,16 @@ def main():
             a = inst / (ms * 1e-3) / 1e12
             row.update({"bound": "alu", "achieved": round(a, 3), "peak": round(alu_peak, 3), "unit": "T lane-inst/s",
                         "frac": round(a / alu_peak, 4), "units": w})
+        t = traffic.get(STEP_KERNEL.get(k, ""))
+        if t:
+            row["traffic"] = t[0]
         kernels[k] = row
     dom = max(step_acc, key=step_acc.get)
+    t = traffic.get(STEP_KERNEL.get(dom, ""))
     roof = {"kernel": dom, "ms": step_acc[dom], "share_of_step": step_acc[dom] / total_step_ms,
-            "traffic": NCU_TRAFFIC_BYTES_CONFIG3.get(dom) if (cid == 3 and args.seed == 1 and not args.frame_us) else None,
-            "traffic_source": "profiles/r01e_ncu_full_config3.md (dram read + write bytes per launch)"}
-    roof.update({k: v for k, v in kernels[dom].items() if k not in ("ms", "share_of_step")})
+            "traffic": t[0] if t else None,
+            "traffic_source": (f"profiles/{NCU_TRAFFIC_CSV} (dram read + write bytes per launch, ncu --set full at commit {t[1]})" if t else None)}
+    roof.update({k: v for k, v in kernels[dom].items() if k not in ("ms", "share_of_step", "traffic")})
     roof["peak_source"] = alu_src if roof.get("bound") == "alu" else peak_src
     if "bound" not in roof:
         roof.update({"bound": "hbm", "achieved": None, "peak": peak, "unit": "GB/s", "frac": None})
@@ -385,17 +431,28 @@ def main():
                    "achieved": round(c_inst / (c_ms * 1e-3) / 1e12, 3) if c_ms > 0 else None, "peak": round(alu_peak, 3),
                    "unit": "T lane-inst/s", "frac": round(c_inst / (c_ms * 1e-3) / 1e12 / alu_peak, 4) if c_ms > 0 else None,
                    "units": {k: work[k] for k in ("tracklets", "row_steps", "updates", "candidates")}}
+    # the frame against the sum of its floors (HBM-bound steps at the measured copy bandwidth + the constructor at the ALU peak)
+    floor_ms = sum(ALGO_BYTES_PER_CLUSTER.get(k, 0) for k in step_acc) * n / (peak * 1e9) * 1e3 + c_inst / (alu_peak * 1e12) * 1e3
+    frame = {"sum_of_floors_ms": round(floor_ms, 3), "frac": round(floor_ms / total_step_ms, 4),
+             "algorithmic_bytes_per_cluster": sum(ALGO_BYTES_PER_CLUSTER.get(k, 0) for k in step_acc)}
 
     cpu = None
     if not args.no_cpu_baseline:
+        # (1) one core, a bounded sample (the paper's "speed-up vs 1 CPU core" convention)
         cn, cdt, _ = _cpu_oracle_run(cid, args.seed, args.cpu_sample_us)
         sample = (f"{CONFIG_NAMES[cid]} generator, seed {args.seed}, frame cut to {args.cpu_sample_us:g} us ({cn} clusters)"
                   if cid >= 2 else f"{CONFIG_NAMES[cid]} ({cn} clusters)")
-        cpu = {"value": cn / cdt, "unit": "clusters/s", "cores": 1, "kind": "oracle", "sample": sample, "seconds": cdt}
-        if cfg.n_sectors > 1:                            # the unchanged oracle, one sector per thread
-            an, adt, athreads, _ = _cpu_oracle_run_all_cores(cid, args.seed, args.cpu_sample_us)
-            cpu["all_cores"] = {"value": an / adt, "unit": "clusters/s", "cores": athreads, "host_cpus": os.cpu_count(),
-                                "kind": "oracle, one call per sector from a thread pool", "seconds": adt}
+        one_core = {"value": cn / cdt, "unit": "clusters/s", "cores": 1, "kind": "oracle", "sample": sample, "seconds": cdt}
+        cpu = dict(one_core)
+        if cfg.n_sectors > 1:
+            # (2) all host cores (the unchanged oracle, one call per sector from a thread pool), on the
+            # WHOLE frame the GPU arm timed -- the same configuration, about 20 s for a 10 ms frame on 16 cores
+            whole = bool(args.cpu_whole_frame) and not args.frame_us
+            an, adt, athreads, atracks = _cpu_oracle_run_all_cores(cid, args.seed, args.cpu_sample_us, tf=tf if whole else None)
+            cpu = {"value": an / adt, "unit": "clusters/s", "cores": athreads, "host_cpus": os.cpu_count(),
+                   "kind": "oracle", "how": "the unchanged oracle, one call per sector from a thread pool",
+                   "sample": (f"the whole frame the GPU arm timed ({an} clusters, same configuration)" if whole else sample),
+                   "same_config": whole, "seconds": adt, "n_tracks": atracks, "one_core": one_core}
 
     line = {"metric": "tpc_clusters_tracked_per_s", "value": value, "unit": "clusters/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
@@ -408,7 +465,8 @@ def main():
                              "working set may fit L2 (small config)", "gen_seconds": round(t_gen, 1)},
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches,
             "step_ms": {k: round(v, 4) for k, v in step_acc.items()}, "kernels": kernels,
-            "tracklet_constructor": constructor, "rare_paths": work.get("rare_paths"), "merge": merge, "roofline": roof, "cpu_baseline": cpu}
+            "tracklet_constructor": constructor, "frame_vs_floors": frame, "rare_paths": work.get("rare_paths"), "merge": merge,
+            "roofline": roof, "cpu_baseline": cpu}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
