@@ -36,7 +36,7 @@ const char* const kStepNames[N_STEPS] = {
 struct Ids {   // arena allocation ids
   int stage_in = -1, stage_out = -1;
   int bin_start, sort_keys, tmp_keys, tmp_orig, tmp_yt, sort_hist, yt, orig, hsr, link_up, link_down, link_up_clean, start_flag, cell_count, start_hits,
-      scan_a, scan_b, seeds_a, seeds_b, row_hit, tl_meta, tl_rec, tl_cur, claim, owned, own_mask,
+      scan_a, scan_b, seeds_a, seeds_b, row_hit, tl_meta, tl_rec, tl_cur, claim, owned,
       flag, track_idx, hit_off, track_slot, chunks;
 };
 
@@ -72,7 +72,7 @@ bool valid_params(const tpc_params_t* p) {
   return p && p->miss_limit >= 1 && p->min_hits >= 1 && p->seed_min_hits >= 2 && p->sigma_y_cm > 0 &&
          p->sigma_z_cm > 0 && p->sin_phi_max > 0 && p->sin_phi_max < 1 && p->grid_time_bins >= 0 && p->slice_time_bins >= 0 && p->grid_pad_bins >= 0 && p->grid_pad_bins <= 64 &&
          p->max_clusters >= 0 && p->max_clusters < ((int64_t)1 << 31) && p->max_tracklets >= 0 &&
-         p->max_tracklets < ((int64_t)1 << 31) / kRowStride * 32 && p->max_tracks >= 0 && p->max_track_hits >= 0 &&
+         p->max_tracklets <= ((int64_t)1 << kKeySlotBits) && p->max_tracks >= 0 && p->max_track_hits >= 0 &&
          p->win_const > 0 && p->win_slope >= 0 && p->chi2_cut > 0;
 }
 
@@ -80,7 +80,7 @@ bool capacities(const tpc_geometry_t* g, const tpc_params_t* p, int64_t max_clus
   c.max_clusters = max_clusters > 0 ? max_clusters : p->max_clusters;
   if (c.max_clusters < 1) c.max_clusters = 1;
   if (c.max_clusters >= ((int64_t)1 << 31)) return false;
-  c.max_tracklets = p->max_tracklets > 0 ? p->max_tracklets : c.max_clusters / 10 + 4096;
+  c.max_tracklets = p->max_tracklets > 0 ? p->max_tracklets : std::min<int64_t>(c.max_clusters / 10 + 4096, (int64_t)1 << kKeySlotBits);   // a claim word carries the slot in 24 bits
   c.max_tracks = p->max_tracks > 0 ? p->max_tracks : c.max_clusters / 64 + 4096;
   c.max_track_hits = p->max_track_hits > 0 ? p->max_track_hits : c.max_clusters;
   c.grid_w = p->grid_time_bins > 0 ? p->grid_time_bins : kDefaultGridTimeBins;
@@ -128,7 +128,7 @@ void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids
   const size_t scan_len = std::max(std::max(scan_tiles(hist_len), scan_tiles((size_t)c.n_cells + 1)), scan_tiles(T)) + 2;
   id.scan_a = plan.add("scan_tile_sums_a", 4 * scan_len, S_SORT, S_EMIT);
   id.scan_b = plan.add("scan_tile_sums_b", 4 * scan_len, S_SORT, S_EMIT);
-  id.bin_start = plan.add("grid_bin_start", 4 * B, S_GRID, S_FOLLOW_DOWN);
+  id.bin_start = plan.add("grid_bin_start", 4 * B, S_GRID, S_COUNT);        // its last entry (= number of valid hits) is read up to the count step
   id.sort_keys = plan.add("sort_keys", 4 * N, S_SORT, S_GRID);
   id.tmp_keys = plan.add("sort_tmp_keys", 4 * N, S_SORT, S_SORT);
   id.tmp_orig = plan.add("sort_tmp_orig", 4 * N, S_SORT, S_SORT);
@@ -150,8 +150,7 @@ void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids
   id.tl_meta = plan.add("tracklet_meta(int4)", 16 * T, S_FIT_UP, S_EMIT);
   id.tl_rec = plan.add("tracklet_record(4 x float4)", 64 * T, S_FIT_UP, S_EMIT);
   id.tl_cur = plan.add("tracklet_handover(2 x float4)", 32 * T, S_FOLLOW_UP, S_FIT_DOWN);
-  id.claim = plan.add("selector_claim(u64)", 8 * N, S_CLAIM, S_COUNT);
-  id.own_mask = plan.add("selector_own_mask", 4 * (size_t)(kRowStride / 32) * T, S_COUNT, S_EMIT);
+  id.claim = plan.add("selector_claim(u64)", 8 * N, S_CLAIM, S_EMIT);      // emit re-reads the claims of the tracks' hits
   id.owned = plan.add("selector_owned", 4 * T, S_COUNT, S_EMIT);
   id.flag = plan.add("selector_flag", 4 * T, S_COUNT, S_EMIT);
   id.track_idx = plan.add("selector_track_idx", 4 * T, S_SELECT_SCAN, S_EMIT);
@@ -616,7 +615,6 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   uint32_t* scan_b = P.ptr<uint32_t>(A, id.scan_b);
   unsigned long long* claim = P.ptr<unsigned long long>(A, id.claim);
   uint32_t* owned = P.ptr<uint32_t>(A, id.owned);
-  uint32_t* own_mask = P.ptr<uint32_t>(A, id.own_mask);
   uint32_t* flag = P.ptr<uint32_t>(A, id.flag);
   uint32_t* track_idx = P.ptr<uint32_t>(A, id.track_idx);
   uint32_t* hit_off = P.ptr<uint32_t>(A, id.hit_off);
@@ -716,8 +714,9 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   if (n > 0) cudaMemsetAsync(claim, 0, 8 * (size_t)n, st);
   k_selector_claim<<<warp_ctas, kSelectorThreads, 0, st>>>(tl, counters, claim, c); ++launches;
   mark(S_COUNT);
-  const int cap_warp_ctas = (int)(((int64_t)T * 32 + kSelectorThreads - 1) / kSelectorThreads);
-  k_selector_count<<<cap_warp_ctas, kSelectorThreads, 0, st>>>(tl, counters, claim, owned, flag, own_mask, T, c); ++launches;
+  cudaMemsetAsync(owned, 0, 4 * (size_t)T, st);
+  k_selector_count_hits<<<hit_ctas, 256, 0, st>>>(claim, bin_start, owned, c); ++launches;
+  k_selector_flag<<<(T + 255) / 256, 256, 0, st>>>(owned, flag, T, c); ++launches;
   mark(S_SELECT_SCAN);
   launches += exclusive_scan_u32(flag, track_idx, (size_t)T, scan_a, st);
   launches += exclusive_scan_u32(owned, hit_off, (size_t)T, scan_b, st);
@@ -733,7 +732,7 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   k_selector_map<<<(int)((tl_bound + 255) / 256), 256, 0, st>>>(counters, flag, track_idx, track_slot); ++launches;
   const int64_t emit_warps = std::max<int64_t>(std::min<int64_t>(tl_bound, o->max_tracks), 1);      // warp 0 also writes the scalars
   k_selector_emit<<<(int)((emit_warps * 32 + kSelectorThreads - 1) / kSelectorThreads), kSelectorThreads, 0, st>>>(
-      tl, counters, own_mask, track_slot, hit_off, scan_a + n_scan_tiles, scan_b + n_scan_tiles, orig, yt, hsr, start_hits, n_invalid, to, c); ++launches;
+      tl, counters, claim, track_slot, hit_off, scan_a + n_scan_tiles, scan_b + n_scan_tiles, orig, yt, hsr, start_hits, n_invalid, to, c); ++launches;
   mark(N_STEPS);
   t->have_times = t->profile;
   t->last_launches = launches;
