@@ -205,4 +205,89 @@ void orc_vertex_time(const orc_merge_params* p, int64_t n, const float* par, int
   }
 }
 
+
+// ---- C10: merging across the CENTRAL ELECTRODE ("sector-boundary and central-electrode track
+// merging"; the z position of a hit is only known through its time, so a track that crosses z = 0 continues in
+// the mirror sector of the other TPC side with the time coordinate REFLECTED).  Readings CE1..CE6, DESIGN.md §3 "C10":
+//   BASELINE.json L8/L9: sector S (A side, z > 0) and S + 18 (C side) share one local frame; time = (t0 v + L - |z|) / Z.
+//   Moving outward towards the electrode |z| falls, so the time coordinate RISES (dz/ds = t > 0); behind the electrode it
+//   falls again with the mirrored slope.  x, y, sin phi and q/pT are continuous.
+//   For a track A (sector S, rows [f, l], state on row r_A, t_A > 0) the candidates are the tracks B of the mirror sector
+//   (S + 18) mod 36 with the row window of C7:  r_B <= f_B,  r_B > max(f_A, r_A),  l_A + 1 - overlap <= r_B <= l_A + 1 + gap.
+//       L = transport(A, x of row l_A)            (FAIL -> A has no candidate)
+//       E = transport(L, x_B)                     (FAIL -> no candidate)
+//       dy = E.y - y_B;  ds = E.s - s_B;  dk = k_A - k_B;  dt = t_A + t_B                       (mirrored slope)
+//       dzm = (E.z - z_B) + (time_ref_A - time_ref_B) * Z      # A extrapolated THROUGH the electrode minus B, time-derived cm
+//       zg  = E.z - L.z;   hi = zg + zg  (0 unless zg > 0)     # twice what A's z advances between its last row and x_B
+//       ez  = dzm            if dzm < 0                        # the crossing must lie between A's last row and x_B:
+//           = dzm - hi       if dzm > hi                       #   0 <= dzm <= hi;  ez = distance from that interval
+//           = 0              otherwise
+//       require |dy| < cut_y, |ez| < cut_z, |ds| < cut_s, |dk| < cut_k, |dt| < cut_t
+//       d2 = (dy*dy)*wy + (ez*ez)*wz + (ds*ds)*ws + (dk*dk)*wk + (dt*dt)*wt          w = (float)(1 / cut^2), from double
+//   Reciprocal best match exactly as in C7 (ties -> lowest seed id).  For a linked A:
+//       cl = min(max(dzm, 0), hi);   t_ce[A] = time_ref_B + (z_B + 0.5f*cl) / Z       # time coordinate of the crossing
+//   = (t0 v + L) / Z: the collision time itself, with no vertex assumption.  Unlinked tracks: t_ce = 0.
+// Pins (tests/test_merge_oracle_pins.py): CE-L closed form on hand-made mirrored lines (link, t_ce), CE-S the sign and
+// mirror conditions, CE-H noise-free helices through the electrode against generator truth, CE-T t_ce against the
+// generator's t0, CE-I invariants, CE-P order independence.  Parity unpinned: the values of the cuts.
+struct orc_ce_params {
+  int32_t n_sectors, n_rows;
+  float x0_cm, row_pitch_cm, time_bin_cm, sin_phi_max, inv_R_per_qpt;
+  float cut_y_cm, cut_z_cm, cut_sin_phi, cut_q_pt, cut_dzds;
+  int32_t max_row_gap, max_row_overlap;
+};
+
+int64_t orc_merge_ce(const orc_ce_params* pp, int64_t n, const int32_t* seed, const int32_t* sector, const int32_t* first_row,
+                     const int32_t* last_row, const float* par, int32_t* next, int32_t* prev, float* t_ce) {
+  const orc_ce_params& p = *pp;
+  const float wy = (float)(1.0 / ((double)p.cut_y_cm * (double)p.cut_y_cm)), wz = (float)(1.0 / ((double)p.cut_z_cm * (double)p.cut_z_cm));
+  const float ws = (float)(1.0 / ((double)p.cut_sin_phi * (double)p.cut_sin_phi)), wk = (float)(1.0 / ((double)p.cut_q_pt * (double)p.cut_q_pt));
+  const float wt = (float)(1.0 / ((double)p.cut_dzds * (double)p.cut_dzds));
+  std::vector<int32_t> out(n, -1), in(n, -1);
+  std::vector<float> d_out(n, 0.0f), d_in(n, 0.0f), t_out(n, 0.0f);
+  if (p.n_sectors == 36) {
+    for (int64_t a = 0; a < n; ++a) {
+      const float* pa = par + 7 * a;
+      if (!(pa[4] > 0.0f)) continue;                                    // CE2: only a track approaching the electrode can cross it
+      St L{pa[0], pa[1], pa[2], pa[3], pa[4], pa[5]};
+      const float x_l = (float)((double)p.x0_cm + (double)p.row_pitch_cm * (double)last_row[a]);
+      if (!transport_state(L, x_l, p.inv_R_per_qpt, p.sin_phi_max)) continue;
+      const int32_t ra = (int32_t)std::floor((pa[0] - p.x0_cm) / p.row_pitch_cm + 0.5f);
+      const int32_t nb = (sector[a] + 18) % 36;
+      for (int64_t b = 0; b < n; ++b) {
+        if (sector[b] != nb) continue;
+        const float* pb = par + 7 * b;
+        const int32_t rb = (int32_t)std::floor((pb[0] - p.x0_cm) / p.row_pitch_cm + 0.5f);
+        if (!(rb > first_row[a] && rb > ra)) continue;
+        if (!(rb <= first_row[b])) continue;
+        if (rb < last_row[a] + 1 - p.max_row_overlap || rb > last_row[a] + 1 + p.max_row_gap) continue;
+        St E = L;
+        if (!transport_state(E, pb[0], p.inv_R_per_qpt, p.sin_phi_max)) continue;
+        const float dy = E.y - pb[1];
+        const float ds = E.s - pb[3];
+        const float dk = pa[5] - pb[5];
+        const float dt = pa[4] + pb[4];
+        const float dzm = (E.z - pb[2]) + (pa[6] - pb[6]) * p.time_bin_cm;
+        const float zg = E.z - L.z;
+        const float hi = zg > 0.0f ? zg + zg : 0.0f;
+        const float ez = dzm < 0.0f ? dzm : (dzm > hi ? dzm - hi : 0.0f);
+        if (!(std::fabs(dy) < p.cut_y_cm && std::fabs(ez) < p.cut_z_cm && std::fabs(ds) < p.cut_sin_phi && std::fabs(dk) < p.cut_q_pt &&
+              std::fabs(dt) < p.cut_dzds)) continue;
+        const float d2 = (dy * dy) * wy + (ez * ez) * wz + (ds * ds) * ws + (dk * dk) * wk + (dt * dt) * wt;
+        const float cl = std::fmin(std::fmax(dzm, 0.0f), hi);
+        const float tce = pb[6] + (pb[2] + 0.5f * cl) / p.time_bin_cm;
+        if (out[a] < 0 || d2 < d_out[a] || (d2 == d_out[a] && (uint32_t)seed[b] < (uint32_t)seed[out[a]])) { out[a] = (int32_t)b; d_out[a] = d2; t_out[a] = tce; }
+        if (in[b] < 0 || d2 < d_in[b] || (d2 == d_in[b] && (uint32_t)seed[a] < (uint32_t)seed[in[b]])) { in[b] = (int32_t)a; d_in[b] = d2; }
+      }
+    }
+  }
+  int64_t n_links = 0;
+  for (int64_t i = 0; i < n; ++i) { next[i] = -1; prev[i] = -1; t_ce[i] = 0.0f; }
+  for (int64_t a = 0; a < n; ++a) {
+    const int32_t b = out[a];
+    if (b >= 0 && in[b] == (int32_t)a) { next[a] = b; prev[b] = (int32_t)a; t_ce[a] = t_out[a]; ++n_links; }
+  }
+  return n_links;
+}
+
 }  // extern "C"

@@ -224,3 +224,124 @@ def test_MC_a_state_above_its_first_row_is_never_a_continuation_and_chains_are_a
     a = np.where(mr.next >= 0)[0]
     assert np.all(rs[mr.next[a]] > rs[a]) and np.all(rs[mr.next[a]] <= res.tr_first_row[mr.next[a]])
     assert (rs > res.tr_first_row).sum() >= 1            # the input does hold tracks whose state is not at the inner end
+
+
+# ----------------------------------------------------------------------------- C10: central-electrode merging
+def _ce_pair(x_c=150.0, t_a=0.4, rows_a=(40, 58), row_b=63, sec_a=3, slope=0.05, k=0.0, t_b=None, shift_b=0.0):
+    """Two hand-made tracks on ONE straight line of the common local frame of sectors sec_a / sec_a + 18: A holds rows
+    rows_a with its state on its first row, B starts on row_b in the mirror sector.  The time-derived coordinate rises with
+    slope t_a per unit path up to the crossing at x = x_c and falls with the mirrored slope behind it."""
+    x0, pitch = 85.0, 1.07
+    ds_dx = math.sqrt(1.0 + slope * slope)            # path per unit x of a straight line
+    s = slope / ds_dx
+    xa, xb = x0 + pitch * rows_a[0], x0 + pitch * row_b
+    z_of = lambda x: (x - x_c) * ds_dx * t_a if x <= x_c else -(x - x_c) * ds_dx * t_a     # relative to the crossing, cm
+    t_cross = 5000.0                                  # time coordinate of the crossing [bins]
+    tb = -t_a if t_b is None else t_b
+    a = [xa, slope * xa, 0.0, s, t_a, k, t_cross + z_of(xa) / 0.516]                       # z_rel = 0 at its own time_ref
+    b = [xb, slope * xb, 0.0, s, tb, k, t_cross + (z_of(xb) + shift_b) / 0.516]
+    par = np.array([a, b], np.float32)
+    return ([11, 22], [sec_a, (sec_a + 18) % 36], [rows_a[0], row_b], [rows_a[1], 140], par), t_cross
+
+
+def test_CEL_mirrored_line_is_linked_and_the_crossing_time_is_the_closed_form():
+    p = M.default_ce_params(36)
+    for x_c in (149.0, 150.5, 152.0):                 # anywhere between A's last row (x = 147.06) and B's state (x = 152.41)
+        args, t_cross = _ce_pair(x_c=x_c)
+        r = M.merge_ce(p, *args)
+        assert r.n_links == 1 and r.next[0] == 1 and r.prev[1] == 0 and r.next[1] == -1
+        assert abs(float(r.t_ce[0]) - t_cross) < 2e-3 and r.t_ce[1] == 0.0
+    # a C-side track that crosses to the A side links the same way (the mirror of sector 21 is sector 3)
+    args, t_cross = _ce_pair(sec_a=21)
+    r = M.merge_ce(p, *args)
+    assert r.n_links == 1 and abs(float(r.t_ce[0]) - t_cross) < 2e-3
+
+
+def test_CES_sign_mirror_and_interval_conditions():
+    p = M.default_ce_params(36)
+    link = lambda **kw: M.merge_ce(p, *_ce_pair(**kw)[0]).n_links
+    assert link() == 1
+    assert link(t_a=-0.4) == 0                        # CE2: a track moving away from the electrode cannot cross it
+    assert link(t_b=0.4) == 0                         # the slope behind the electrode must be mirrored (dt = t_A + t_B)
+    assert link(t_b=-0.35) == 1 and link(t_b=-0.25) == 0          # ... within cut_dzds = 0.1
+    assert link(x_c=140.0) == 0                       # crossing 7 cm BEFORE A's last row: dzm exceeds twice the gap advance by > 2 cm
+    # the allowed interval of dzm is [0, 2 * 0.4 * 5.36] = [0, 4.28] cm and dzm = 1.93 cm here; |ez| < cut_z = 2 cm beyond it
+    assert link(shift_b=3.5) == 1 and link(shift_b=4.5) == 0 and link(shift_b=-4.0) == 1 and link(shift_b=-5.0) == 0
+    # same sector pairing only: B in a different phi slice does not link
+    args, _ = _ce_pair()
+    args[1][1] = 22
+    assert M.merge_ce(p, *args).n_links == 0
+    assert M.merge_ce(M.default_ce_params(18), *_ce_pair()[0]).n_links == 0       # half a TPC has no mirror sectors
+
+
+def _ce_expected(res, keys):
+    """Pairs (i, j) of tracks that belong to the same (particle, arc), sit in mirror sectors and satisfy C10's row window."""
+    from collections import defaultdict
+    groups = defaultdict(list)
+    for i, k in enumerate(keys):
+        if k >= 0:
+            groups[(k // (64 * 16), k % 16)].append(i)
+    exp = set()
+    for v in groups.values():
+        for i in v:
+            for j in v:
+                if (res.tr_sector[j] == (res.tr_sector[i] + 18) % 36 and res.tr_par[i, 4] > 0 and
+                        res.tr_last_row[i] - 1 <= res.tr_first_row[j] <= res.tr_last_row[i] + 13 and res.tr_first_row[j] > res.tr_first_row[i]):
+                    exp.add((i, j))
+    return exp
+
+
+def _ce_frame(seed, noise_free):
+    c = gen.preset(1, seed)
+    c.fixed_tracks, c.zv_sigma_cm, c.eta_max, c.pt_min = 3000, 30.0, 0.3, 0.3      # many tracks through the electrode INSIDE the TPC
+    if noise_free:
+        c.sigma_y_cm = c.sigma_z_cm = c.dropout = c.noise_frac = 0.0
+    tf = gen.generate(c)
+    res = oracle.track(oracle.default_geometry(36, tf.max_time_bin), oracle.default_params(), tf.row, tf.pad, tf.time)
+    return tf, res, M.merge_ce(M.default_ce_params(36), res.tr_seed, res.tr_sector, res.tr_first_row, res.tr_last_row, res.tr_par)
+
+
+def test_CEH_noise_free_helices_through_the_electrode_and_CET_crossing_time():
+    tf, res, r = _ce_frame(3, noise_free=True)
+    keys = ME.track_truth_keys(tf, res.tr_hit_offset, res.tr_n_hits, res.tr_hit_index)
+    a = np.where(r.next >= 0)[0]
+    got = set(zip(a.tolist(), r.next[a].tolist()))
+    exp = _ce_expected(res, keys)
+    assert len(exp) >= 250
+    assert got <= exp, "a link that generator truth does not have"
+    assert len(got) >= 0.95 * len(exp), (len(got), len(exp))
+    # CE-T: the crossing time is the collision time: (t0 v_drift + drift length) / time bin
+    tr = tf.tracks[keys[a] // (64 * 16)]
+    t_true = (tr["t0_us"] * 2.58 + 250.0) / 0.516
+    err = np.abs(r.t_ce[a] - t_true)
+    assert np.median(err) < 1e-4 and np.mean(err < 0.05) > 0.98 and err.max() < 1.5       # a crossing inside the last rows of A is clamped to the interval
+    assert np.all(r.t_ce[r.next < 0] == 0.0)
+
+
+def test_CEI_invariants_CEP_order_independence_and_purity_with_noise():
+    tf, res, r = _ce_frame(4, noise_free=False)
+    keys = ME.track_truth_keys(tf, res.tr_hit_offset, res.tr_n_hits, res.tr_hit_index)
+    a = np.where(r.next >= 0)[0]
+    b = r.next[a]
+    assert r.n_links == a.size >= 150
+    np.testing.assert_array_equal(r.prev[b], a)
+    assert np.unique(b).size == b.size
+    np.testing.assert_array_equal(res.tr_sector[b], (res.tr_sector[a] + 18) % 36)
+    assert np.all(res.tr_par[a, 4] > 0)
+    rs = np.floor((res.tr_par[:, 0] - np.float32(85.0)) / np.float32(1.07) + np.float32(0.5)).astype(np.int64)
+    assert np.all(rs[b] > rs[a]) and np.all(rs[b] <= res.tr_first_row[b]) and np.all(rs[b] >= res.tr_last_row[a] - 1)
+    exp = _ce_expected(res, keys)
+    got = set(zip(a.tolist(), b.tolist()))
+    assert len(got & exp) >= 0.85 * len(exp), (len(got & exp), len(exp))
+    assert len(got - exp) <= 0.03 * len(got), (len(got - exp), len(got))
+    tr = tf.tracks[np.maximum(keys[a], 0) // (64 * 16)]
+    ok = np.array([(i, j) in exp for i, j in zip(a, b)])
+    t_true = (tr["t0_us"] * 2.58 + 250.0) / 0.516
+    assert np.median(np.abs(r.t_ce[a] - t_true)[ok]) < 0.5
+    # order independence
+    perm = np.random.default_rng(5).permutation(len(res.tr_seed))
+    r2 = M.merge_ce(M.default_ce_params(36), res.tr_seed[perm], res.tr_sector[perm], res.tr_first_row[perm], res.tr_last_row[perm], res.tr_par[perm])
+    s1 = np.where(r.next >= 0, res.tr_seed[np.maximum(r.next, 0)], -1)
+    s2 = np.where(r2.next >= 0, res.tr_seed[perm][np.maximum(r2.next, 0)], -1)
+    np.testing.assert_array_equal(s1[perm], s2)
+    np.testing.assert_array_equal(r.t_ce[perm], r2.t_ce)
