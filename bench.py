@@ -304,9 +304,9 @@ def main():
     # ---- widening step C7 (sector-boundary merging of the tracks, not part of `value`): timed on its own ----
     merge = None
     if cfg.n_sectors >= 18:
-        m0, m1, m2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
-        merged = refit = None
-        ms_m = ms_r = 0.0
+        m0, m1, m2, m3 = (torch.cuda.Event(enable_timing=True) for _ in range(4))
+        merged = refit = ce = None
+        ms_m = ms_r = ms_c = 0.0
         outs_c = trk.alloc_outputs(n, hit_coords=True)      # C8 reads the hits' coordinates from two optional emit outputs
         for _ in range(3):
             with torch.cuda.stream(stream):
@@ -316,8 +316,10 @@ def main():
                 m1.record(stream)
                 refit = trk.tpc_refit_chains(outs_c, merged, refit=refit, stream=stream)
                 m2.record(stream)
+                ce = trk.tpc_merge_central_electrode(outs_c, merged=ce, stream=stream)
+                m3.record(stream)
             stream.synchronize()
-            ms_m, ms_r = m0.elapsed_time(m1), m1.elapsed_time(m2)                     # last of three
+            ms_m, ms_r, ms_c = m0.elapsed_time(m1), m1.elapsed_time(m2), m2.elapsed_time(m3)      # last of three
         emit_with_coords_ms = trk.step_ms().get("selector_emit")
         merge = {"step": "sector_boundary_merge (C7, tpc_merge_tracks)", "ms": round(ms_m, 4), "n_links": int(merged[3][0]),
                  "n_tracks": n_tracks, "tracks_per_s": n_tracks / (ms_m * 1e-3) if ms_m > 0 else None,
@@ -325,7 +327,9 @@ def main():
                  "refit": {"step": "chain_refit (C8, tpc_refit_chains)", "ms": round(ms_r, 4), "n_chains_refitted": int((refit[0] == 1).sum()),
                            "n_chains_failed": int((refit[0] == -1).sum()), "hits_refitted": int(refit[1][refit[0] == 1].sum()),
                            "gpu_launches": trk.last_merge_launches(),
-                           "selector_emit_ms_with_hit_coordinates": emit_with_coords_ms}}
+                           "selector_emit_ms_with_hit_coordinates": emit_with_coords_ms},
+                 "central_electrode": {"step": "central_electrode_merge (C10, tpc_merge_central_electrode)", "ms": round(ms_c, 4),
+                                       "n_links": int(ce[3][0]), "gpu_launches": trk.last_merge_launches()}}
         del outs_c
     trk.close()
     del trk, outs

@@ -232,6 +232,31 @@ size_t tpc_merge_scratch_bytes(const tpc_tracker_t* tracker, int64_t max_tracks)
 int tpc_merge_tracks(tpc_tracker_t* tracker, const tpc_merge_params_t* merge_params, const tpc_tracks_t* tracks,
                      void* cuda_stream, tpc_merged_t* merged_out);
 
+/* ---- C10: merging across the CENTRAL ELECTRODE (DESIGN.md §3 "C10", readings CE1..CE6; PAPER.md L23:
+ * the z of a hit is only known through its time).  A track that approaches the electrode (dz/ds > 0 in the time-derived
+ * coordinate) continues in the mirror sector (S + 18) mod 36 of the other TPC side: x, y, sin phi, q/pT continuous, the time
+ * coordinate reflected.  Row window and reciprocal best match as in C7; needs the 36-sector geometry (else nothing links). */
+typedef struct {
+  float cut_y_cm, cut_z_cm;         /* 2, 2     : |dy|; distance of the crossing from the gap between the two pieces [cm]    */
+  float cut_sin_phi, cut_q_pt;      /* 0.05, 0.5                                                                             */
+  float cut_dzds;                   /* 0.1      : |dz/ds of A + dz/ds of B| (mirrored slopes)                   (reading CE5) */
+  int32_t max_row_gap, max_row_overlap;   /* 12, 2 : as in tpc_merge_params_t                                                 */
+} tpc_ce_params_t;
+
+typedef struct {   /* caller-allocated DEVICE buffers, [tracks->max_tracks] each                                               */
+  int32_t* next;     /* the continuation of track i behind the electrode, -1 = none                                          */
+  int32_t* prev;     /* the piece in front of the electrode that track i continues, -1 = none                                */
+  float* t_ce;       /* time coordinate [time bins] at which linked track i crosses the electrode = (t0 v_drift + drift
+                        length) / time bin: the collision time, with no vertex assumption; 0 for unlinked tracks             */
+  int32_t* n_links;  /* scalar                                                                                               */
+} tpc_ce_merged_t;
+
+/* Same calling rules as tpc_merge_tracks (asynchronous, scratch = the handle's arena, tpc_merge_scratch_bytes of it, after
+ * tpc_track_timeframe on the same stream; it may follow tpc_merge_tracks, whose scratch it overwrites).  Errors: TPC_EINVAL,
+ * TPC_ENOMEM, TPC_ECUDA.  tpc_merge_last_launches() then reports this call's launches.                                       */
+int tpc_merge_central_electrode(tpc_tracker_t* tracker, const tpc_ce_params_t* ce_params, const tpc_tracks_t* tracks,
+                                void* cuda_stream, tpc_ce_merged_t* merged_out);
+
 /* ---- C8: refit of the chains linked by C7 (DESIGN.md §3 "C8", readings F1..F6): one inward Kalman pass over the hits
  * all pieces of a chain own, each piece in its own sector frame, state and covariance rotated at every boundary.      */
 typedef struct {   /* caller-allocated DEVICE buffers, indexed by track like tpc_tracks_t                              */

@@ -176,6 +176,85 @@ __global__ void __launch_bounds__(256) k_merge_root(MergeTracks T, const int32_t
   root[i] = r;
 }
 
+// ---- C10: merging across the central electrode (DESIGN.md §3 "C10", readings CE1..CE6) ----
+// A track that approaches the electrode (dz/ds > 0 in the time-derived coordinate) continues in the mirror sector
+// (S + 18) mod 36 of the other side with x, y, sin phi, q/pT unchanged and the time coordinate reflected.  Same binning,
+// same row window, same reciprocal best match as C7; the state of A is carried to its last row and from there to the row
+// of the candidate, which bounds where the crossing can be.
+struct MergeCeConsts { float cut_t, wt; };
+
+__global__ void __launch_bounds__(kMergeThreads) k_merge_ce_match(MergeTracks T, MergeScratch S, float* __restrict__ out_t,
+                                                                   const __grid_constant__ MergeConsts c, const MergeCeConsts ce) {
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= merge_n(T, c)) return;
+  unsigned long long best = ~0ull;
+  int best_b = -1;
+  float best_t = 0.0f;
+  const float at = T.t[a];
+  if (c.n_sectors == 36 && at > 0.0f) {                // CE2: only a track approaching the electrode can cross it
+    const float ak = T.k[a], atr = T.time_ref[a];
+    const uint32_t aseed = (uint32_t)T.seed[a];
+    const int sec = T.sector[a], nb = (sec + 18) % 36;
+    const int fa = T.first_row[a], la = T.last_row[a];
+    float lx = T.x[a], ly = T.y[a], lz = T.z[a], ls = T.s[a];
+    const int ra = (int)floorf((lx - c.x0) / c.pitch + 0.5f);
+    const int r_lo = max(la + 1 - c.overlap, max(fa, ra) + 1), r_hi = min(la + 1 + c.gap, c.n_rows - 1);
+    if (la >= 0 && la < c.n_rows && merge_transport(lx, ly, lz, ls, at, ak, __ldg(c.xr + la), c.cB, c.sin_phi_max)) {
+      for (int rb = r_lo; rb <= r_hi; ++rb) {
+        float x2 = lx, y2 = ly, z2 = lz, s2 = ls;
+        if (!merge_transport(x2, y2, z2, s2, at, ak, __ldg(c.xr + rb), c.cB, c.sin_phi_max)) continue;
+        const float zg = z2 - lz;
+        const float hi = zg > 0.0f ? zg + zg : 0.0f;
+        const float tpred = atr + z2 * c.inv_Z;        // A extrapolated through the electrode; B lies up to (hi + cut) / Z EARLIER
+        const uint32_t base = (uint32_t)((nb * c.n_rows + rb) * c.n_tcell);
+        const uint32_t lo = __ldg(S.cell_start + base + merge_time_cell(tpred - (hi + c.cut_z) * c.inv_Z - 0.5f, c));
+        const uint32_t hi_q = __ldg(S.cell_start + base + merge_time_cell(tpred + c.t_window, c) + 1);
+        for (uint32_t q = lo; q < hi_q; ++q) {
+          const float4 ca = S.cand_a[q];               // (y, z_rel, sin phi, q/pT)
+          const float2 cb = S.cand_b[q];               // (time_ref, seed)
+          const float bt = T.t[S.cand_idx[q]];
+          const float dy = y2 - ca.x;
+          const float ds = s2 - ca.z;
+          const float dk = ak - ca.w;
+          const float dt = at + bt;
+          const float dzm = (z2 - ca.y) + (atr - cb.x) * c.Z;
+          const float ez = dzm < 0.0f ? dzm : (dzm > hi ? dzm - hi : 0.0f);
+          if (!(fabsf(dy) < c.cut_y && fabsf(ez) < c.cut_z && fabsf(ds) < c.cut_s && fabsf(dk) < c.cut_k && fabsf(dt) < ce.cut_t)) continue;
+          const float d2 = (dy * dy) * c.wy + (ez * ez) * c.wz + (ds * ds) * c.ws + (dk * dk) * c.wk + (dt * dt) * ce.wt;
+          const unsigned long long hi_bits = (unsigned long long)__float_as_uint(d2) << 32;
+          const unsigned long long key_b = hi_bits | (unsigned long long)(uint32_t)__float_as_int(cb.y);
+          if (key_b < best) {
+            best = key_b; best_b = (int)S.cand_idx[q];
+            const float cl = fminf(fmaxf(dzm, 0.0f), hi);
+            best_t = cb.x + (ca.y + 0.5f * cl) / c.Z;
+          }
+          atomicMin(S.in_key + S.cand_idx[q], hi_bits | (unsigned long long)aseed);
+        }
+      }
+    }
+  }
+  S.out_key[a] = best;
+  S.out_b[a] = best_b;
+  out_t[a] = best_t;
+}
+
+// next / prev are pre-set to -1, t_ce to 0, *n_links to 0.
+__global__ void __launch_bounds__(256) k_merge_ce_link(MergeTracks T, MergeScratch S, const float* __restrict__ out_t, int32_t* __restrict__ next,
+                                                       int32_t* __restrict__ prev, float* __restrict__ t_ce, int32_t* __restrict__ n_links,
+                                                       const __grid_constant__ MergeConsts c) {
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  bool linked = false;
+  if (a < merge_n(T, c)) {
+    const int b = S.out_b[a];
+    if (b >= 0) {
+      const unsigned long long key_a = (S.out_key[a] & 0xFFFFFFFF00000000ull) | (unsigned long long)(uint32_t)T.seed[a];
+      if (S.in_key[b] == key_a) { next[a] = b; prev[b] = a; t_ce[a] = out_t[a]; linked = true; }
+    }
+  }
+  const unsigned m = __ballot_sync(0xffffffffu, linked);
+  if (lane_id() == 0 && m) atomicAdd(n_links, __popc(m));
+}
+
 // ---- C8: refit of the chains linked by C7 (DESIGN.md §3 "C8", readings F1..F6) ----
 // One Kalman pass per chain of >= 2 pieces, from the outermost hit of the outermost piece inward to the innermost hit
 // of the root piece, over the hits each piece owns, each piece in its own sector frame; state and covariance are

@@ -163,7 +163,7 @@ void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids
 
 // C7 scratch (merge.cuh), carved from the start of the arena: the tracking scratch is dead by then.
 namespace {
-struct MergeLayout { size_t cell_start, cell_cursor, scan, cell_of, cand_idx, cand_a, cand_b, out_key, out_b, in_key, total; int n_tcell; size_t n_cells; };
+struct MergeLayout { size_t cell_start, cell_cursor, scan, cell_of, cand_idx, cand_a, cand_b, out_key, out_b, in_key, out_t, total; int n_tcell; size_t n_cells; };
 MergeLayout merge_layout(const tpc_geometry_t& g, int64_t max_tracks) {
   MergeLayout L{};
   L.n_tcell = (int)std::floor((double)g.max_time_bin / (double)kMergeCellTimeBins) + 2;
@@ -181,6 +181,7 @@ MergeLayout merge_layout(const tpc_geometry_t& g, int64_t max_tracks) {
   L.out_key = take(8 * K);
   L.out_b = take(4 * K);
   L.in_key = take(8 * K);
+  L.out_t = take(4 * K);
   L.total = off;
   return L;
 }
@@ -464,6 +465,63 @@ int tpc_merge_tracks(tpc_tracker_t* t, const tpc_merge_params_t* mp, const tpc_t
     k_merge_match<<<(K + kMergeThreads - 1) / kMergeThreads, kMergeThreads, 0, st>>>(T, S, c); ++launches;
     k_merge_link<<<g256, 256, 0, st>>>(T, S, out->next, out->prev, out->n_links, c); ++launches;
     k_merge_root<<<g256, 256, 0, st>>>(T, out->prev, out->root, c); ++launches;
+  }
+  t->last_merge_launches = launches;
+  if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;
+  return TPC_OK;
+}
+
+
+// ---- C10: merging across the central electrode (merge.cuh) ----
+int tpc_merge_central_electrode(tpc_tracker_t* t, const tpc_ce_params_t* mp, const tpc_tracks_t* tr, void* cuda_stream, tpc_ce_merged_t* out) {
+  if (!t || !mp || !tr || !out) return TPC_EINVAL;
+  if (!(mp->cut_y_cm > 0 && mp->cut_z_cm > 0 && mp->cut_sin_phi > 0 && mp->cut_q_pt > 0 && mp->cut_dzds > 0 && mp->max_row_gap >= 0 &&
+        mp->max_row_overlap >= 0)) return TPC_EINVAL;
+  if (tr->max_tracks < 0 || !tr->n_tracks || !out->next || !out->prev || !out->t_ce || !out->n_links) return TPC_EINVAL;
+  if (tr->max_tracks > 0 && (!tr->seed_hit || !tr->sector || !tr->first_row || !tr->last_row || !tr->x || !tr->y || !tr->z_rel ||
+                             !tr->time_ref || !tr->sin_phi || !tr->dzds || !tr->q_pt)) return TPC_EINVAL;
+  const MergeLayout L = merge_layout(t->geom, tr->max_tracks);
+  if (!t->params.arena || L.total > t->params.arena_bytes) return TPC_ENOMEM;
+  if (L.n_cells + 1 >= 2147483000ull) return TPC_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* A = static_cast<char*>(t->params.arena);
+  const int K = tr->max_tracks;
+  MergeConsts c{};
+  c.n_sectors = t->geom.n_sectors; c.n_rows = t->geom.n_rows; c.n_tcell = L.n_tcell;
+  c.gap = mp->max_row_gap; c.overlap = mp->max_row_overlap; c.max_tracks = K;
+  c.x0 = t->geom.x0_cm; c.pitch = t->geom.row_pitch_cm;
+  c.Z = t->consts.Z; c.inv_Z = t->consts.inv_Z; c.cB = t->consts.cB; c.sin_phi_max = t->consts.sin_phi_max;
+  c.cut_y = mp->cut_y_cm; c.cut_z = mp->cut_z_cm; c.cut_s = mp->cut_sin_phi; c.cut_k = mp->cut_q_pt;
+  c.wy = (float)(1.0 / ((double)mp->cut_y_cm * (double)mp->cut_y_cm));
+  c.wz = (float)(1.0 / ((double)mp->cut_z_cm * (double)mp->cut_z_cm));
+  c.ws = (float)(1.0 / ((double)mp->cut_sin_phi * (double)mp->cut_sin_phi));
+  c.wk = (float)(1.0 / ((double)mp->cut_q_pt * (double)mp->cut_q_pt));
+  c.inv_cell = 1.0f / (float)kMergeCellTimeBins;
+  c.t_window = (float)((double)mp->cut_z_cm / (double)t->geom.time_bin_cm + 0.5);
+  c.xr = t->consts.xr;
+  const MergeCeConsts ce{mp->cut_dzds, (float)(1.0 / ((double)mp->cut_dzds * (double)mp->cut_dzds))};
+  MergeTracks T{tr->n_tracks, tr->seed_hit, tr->sector, tr->first_row, tr->last_row, tr->x, tr->y, tr->z_rel, tr->time_ref, tr->sin_phi, tr->dzds, tr->q_pt};
+  MergeScratch S{reinterpret_cast<uint32_t*>(A + L.cell_start), reinterpret_cast<uint32_t*>(A + L.cell_cursor),
+                 reinterpret_cast<uint32_t*>(A + L.cell_of), reinterpret_cast<uint32_t*>(A + L.cand_idx),
+                 reinterpret_cast<float4*>(A + L.cand_a), reinterpret_cast<float2*>(A + L.cand_b),
+                 reinterpret_cast<unsigned long long*>(A + L.out_key), reinterpret_cast<int32_t*>(A + L.out_b),
+                 reinterpret_cast<unsigned long long*>(A + L.in_key)};
+  float* out_t = reinterpret_cast<float*>(A + L.out_t);
+  int64_t launches = 0;
+  cudaMemsetAsync(out->n_links, 0, 4, st);
+  if (K > 0) {
+    cudaMemsetAsync(out->next, 0xFF, 4 * (size_t)K, st);
+    cudaMemsetAsync(out->prev, 0xFF, 4 * (size_t)K, st);
+    cudaMemsetAsync(out->t_ce, 0, 4 * (size_t)K, st);
+    cudaMemsetAsync(S.cell_start, 0, 4 * (L.n_cells + 1), st);
+    cudaMemsetAsync(S.cell_cursor, 0, 4 * L.n_cells, st);
+    cudaMemsetAsync(S.in_key, 0xFF, 8 * (size_t)K, st);
+    const int g256 = (K + 255) / 256;
+    k_merge_cell_count<<<g256, 256, 0, st>>>(T, S, c); ++launches;
+    launches += exclusive_scan_u32(S.cell_start, S.cell_start, L.n_cells + 1, reinterpret_cast<uint32_t*>(A + L.scan), st);
+    k_merge_cell_fill<<<g256, 256, 0, st>>>(T, S, c); ++launches;
+    k_merge_ce_match<<<(K + kMergeThreads - 1) / kMergeThreads, kMergeThreads, 0, st>>>(T, S, out_t, c, ce); ++launches;
+    k_merge_ce_link<<<g256, 256, 0, st>>>(T, S, out_t, out->next, out->prev, out->t_ce, out->n_links, c); ++launches;
   }
   t->last_merge_launches = launches;
   if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;

@@ -18,7 +18,7 @@ STATUS_TRACKLET_OVERFLOW, STATUS_TRACK_OVERFLOW, STATUS_TRACK_HIT_OVERFLOW, STAT
 EXPORTS = ("tpc_tracker_arena_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
            "tpc_tracker_step_ms", "tpc_tracker_step_name", "tpc_tracker_last_launches", "tpc_tracker_work_counters",
            "tpc_tracker_arena_plan", "tpc_selftest_fast_math", "tpc_selftest_alu_peak",
-           "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_refit_chains", "tpc_vertex_time", "tpc_merge_last_launches",
+           "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_merge_central_electrode", "tpc_refit_chains", "tpc_vertex_time", "tpc_merge_last_launches",
            "tpc_tracker_destroy", "tpc_strerror")
 
 
@@ -70,6 +70,22 @@ class MergeParams(C.Structure):
 class Merged(C.Structure):
     """``tpc_merged_t``"""
     _fields_ = [("next", C.c_void_p), ("prev", C.c_void_p), ("root", C.c_void_p), ("n_links", C.c_void_p)]
+
+
+class CeParams(C.Structure):
+    """``tpc_ce_params_t``"""
+    _fields_ = [("cut_y_cm", C.c_float), ("cut_z_cm", C.c_float), ("cut_sin_phi", C.c_float), ("cut_q_pt", C.c_float),
+                ("cut_dzds", C.c_float), ("max_row_gap", C.c_int32), ("max_row_overlap", C.c_int32)]
+
+
+class CeMerged(C.Structure):
+    """``tpc_ce_merged_t``"""
+    _fields_ = [("next", C.c_void_p), ("prev", C.c_void_p), ("t_ce", C.c_void_p), ("n_links", C.c_void_p)]
+
+
+def default_ce_params() -> CeParams:
+    """DESIGN.md §3 C10 reading CE5."""
+    return CeParams(2.0, 2.0, 0.05, 0.5, 0.1, 12, 2)
 
 
 class Refit(C.Structure):
@@ -130,6 +146,8 @@ def load_library(build_if_missing: bool = True):
         L.tpc_merge_scratch_bytes.restype = C.c_size_t
         L.tpc_merge_tracks.argtypes = [vp, C.POINTER(MergeParams), C.POINTER(Tracks), vp, C.POINTER(Merged)]
         L.tpc_merge_tracks.restype = C.c_int
+        L.tpc_merge_central_electrode.argtypes = [vp, C.POINTER(CeParams), C.POINTER(Tracks), vp, C.POINTER(CeMerged)]
+        L.tpc_merge_central_electrode.restype = C.c_int
         L.tpc_refit_chains.argtypes = [vp, C.POINTER(Tracks), C.POINTER(Merged), vp, C.POINTER(Refit)]
         L.tpc_refit_chains.restype = C.c_int
         L.tpc_vertex_time.argtypes = [vp, vp, C.c_int32, vp, vp, vp, vp, vp]
@@ -337,6 +355,22 @@ class Tracker:
         rc = self.lib.tpc_merge_tracks(self.handle, C.byref(mp), C.byref(st), C.c_void_p(s.cuda_stream), C.byref(m))
         if rc != TPC_OK:
             raise TpcError(rc, "tpc_merge_tracks")
+        return merged
+
+    def tpc_merge_central_electrode(self, outputs, ce_params: CeParams | None = None, merged=None, stream=None):
+        """C10 on the DEVICE outputs of ``tpc_track_timeframe`` (same stream); returns (next, prev, t_ce, n_links) tensors."""
+        torch = self._torch
+        out, st = outputs
+        K = max(int(st.max_tracks), 1)
+        if merged is None:
+            e = lambda dt: torch.empty(K, dtype=dt, device=self.device)
+            merged = (e(torch.int32), e(torch.int32), e(torch.float32), torch.empty(1, dtype=torch.int32, device=self.device))
+        mp = ce_params if ce_params is not None else default_ce_params()
+        m = CeMerged(*(t.data_ptr() for t in merged))
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        rc = self.lib.tpc_merge_central_electrode(self.handle, C.byref(mp), C.byref(st), C.c_void_p(s.cuda_stream), C.byref(m))
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_merge_central_electrode")
         return merged
 
     def tpc_refit_chains(self, outputs, merged, refit=None, stream=None):

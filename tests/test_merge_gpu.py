@@ -187,9 +187,12 @@ def test_full_10ms_frame_merge_invariants_and_sampled_oracle_parity():
     out = trk.tpc_track_timeframe(*d, n=n, outputs=outs)
     nxt, prv, root, n_links = merged = trk.tpc_merge_tracks(outs)
     rf_ok, rf_ch, rf_cp, rf_par, rf_cov = trk.tpc_refit_chains(outs, merged)
+    ce_next, ce_prev, ce_t, ce_n = trk.tpc_merge_central_electrode(outs)        # C10 at full size: invariants below
     torch.cuda.synchronize()
     k, nh = int(out.n_tracks[0]), int(out.n_track_hits[0])
     assert int(out.status[0]) & 7 == 0 and k > 1e6
+    ce_next, ce_prev, ce_t, ce_n = ce_next[:k].cpu().numpy(), ce_prev[:k].cpu().numpy(), ce_t[:k].cpu().numpy(), int(ce_n[0])
+    dzds_all = out.dzds[:k].cpu().numpy()
     rf_ok, rf_ch, rf_cp, rf_par, rf_cov = (t[:k].cpu().numpy() for t in (rf_ok, rf_ch, rf_cp, rf_par, rf_cov))
     n_hits_all = out.n_hits[:k].cpu().numpy()
     seed, sec = out.seed_hit[:k].cpu().numpy(), out.sector[:k].cpu().numpy()
@@ -198,6 +201,15 @@ def test_full_10ms_frame_merge_invariants_and_sampled_oracle_parity():
     nxt, prv, root, n_links = nxt[:k].cpu().numpy(), prv[:k].cpu().numpy(), root[:k].cpu().numpy(), int(n_links[0])
     trk.close()
     del d, out, outs
+    # (a') C10 invariants (as pin CE-I): reciprocal, mirror sectors, approaching the electrode, crossing inside the frame
+    ca = np.nonzero(ce_next >= 0)[0]
+    cb = ce_next[ca]
+    assert ce_n == ca.size and ce_n > 100
+    np.testing.assert_array_equal(ce_prev[cb], ca)
+    assert np.unique(cb).size == cb.size
+    np.testing.assert_array_equal(sec[cb], (sec[ca] + 18) % 36)
+    assert np.all(dzds_all[ca] > 0)
+    assert np.all(ce_t[ca] > 400.0) and np.all(ce_t[ca] < tf.max_time_bin + 10.0) and np.all(ce_t[ce_next < 0] == 0)
     # (a) invariants (as pin M-I)
     a = np.nonzero(nxt >= 0)[0]
     b = nxt[a]
