@@ -209,16 +209,40 @@ __global__ void __launch_bounds__(kRadixThreads, TPC_SCATTER_CTAS) k_radix_scatt
 }
 
 // Grid bin offsets from the sorted keys: bin_start[b] = first position whose key >= b, for b in [0, n_bins].
-// Thread i (0 <= i <= n) fills the bins in (key[i-1], key[i]]; also writes the hit's sector-row (u16).
+// Thread i (0 <= i <= n) fills the bins in (key[i-1], key[i]]; also writes the hit's sector-row (u16).  On a dense frame a
+// gap is one or two bins.  A gap longer than kGridGapInline (an empty or sparse frame on a long-frame grid: up to all 2.8e8
+// bins) is not written by the one thread but cut into segments of kGridGapSegment bins that k_grid_fill_gaps fills with a
+// CTA each -- no thread ever writes more than kGridGapInline entries one by one.
+constexpr int kGridGapInline = 64, kGridGapSegment = 4096;
 __global__ void __launch_bounds__(256) k_grid_build(const uint32_t* __restrict__ keys, int64_t n, uint32_t* __restrict__ bin_start,
-                                                    uint16_t* __restrict__ hsr, const __grid_constant__ Consts c) {
+                                                    uint16_t* __restrict__ hsr, uint4* __restrict__ gap_list, uint32_t* __restrict__ n_gaps,
+                                                    const __grid_constant__ Consts c) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i > n) return;
   const uint32_t nb = (uint32_t)c.n_bins;
   const int64_t kprev = i == 0 ? -1 : (int64_t)min(keys[i - 1], nb);
   const uint32_t kcur = i == n ? nb : min(keys[i], nb);
   if (i < n && kcur < nb) hsr[i] = (uint16_t)(kcur / (uint32_t)(c.n_tb * c.n_pb));
-  for (int64_t b = kprev + 1; b <= (int64_t)kcur; ++b) bin_start[b] = (uint32_t)i;
+  const int64_t len = (int64_t)kcur - kprev;
+  if (len <= kGridGapInline) {
+    for (int64_t b = kprev + 1; b <= (int64_t)kcur; ++b) bin_start[b] = (uint32_t)i;
+  } else {
+    const uint32_t n_seg = (uint32_t)((len + kGridGapSegment - 1) / kGridGapSegment);
+    const uint32_t base = atomicAdd(n_gaps, n_seg);
+    for (uint32_t s = 0; s < n_seg; ++s) {
+      const int64_t b0 = kprev + 1 + (int64_t)s * kGridGapSegment;
+      gap_list[base + s] = make_uint4((uint32_t)b0, (uint32_t)min(b0 + kGridGapSegment, (int64_t)kcur + 1), (uint32_t)i, 0u);
+    }
+  }
+}
+// bin_start[b0 .. b1) = value for every listed segment (any order: the segments are disjoint)
+__global__ void __launch_bounds__(256) k_grid_fill_gaps(const uint4* __restrict__ gap_list, const uint32_t* __restrict__ n_gaps,
+                                                        uint32_t* __restrict__ bin_start) {
+  const uint32_t n = *n_gaps;
+  for (uint32_t s = blockIdx.x; s < n; s += gridDim.x) {
+    const uint4 g = gap_list[s];
+    for (uint32_t b = g.x + threadIdx.x; b < g.y; b += blockDim.x) bin_start[b] = g.z;
+  }
 }
 
 }  // namespace tpc

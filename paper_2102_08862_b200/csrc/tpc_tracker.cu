@@ -37,7 +37,7 @@ struct Ids {   // arena allocation ids
   int stage_in = -1, stage_out = -1;
   int bin_start, sort_keys, tmp_keys, tmp_orig, tmp_yt, sort_hist, yt, orig, hsr, link_up, link_down, link_up_clean, start_flag, cell_count, start_hits,
       scan_a, scan_b, seeds_a, seeds_b, row_hit, tl_meta, tl_rec, tl_cur, claim, owned,
-      flag, track_idx, hit_off, track_slot, chunks;
+      flag, track_idx, hit_off, track_slot, chunks, gap_list;
 };
 
 struct Capacities {
@@ -130,6 +130,8 @@ void build_plan(const tpc_params_t* p, const Capacities& c, ArenaPlan& plan, Ids
   id.scan_b = plan.add("scan_tile_sums_b", 4 * scan_len, S_SORT, S_EMIT);
   id.bin_start = plan.add("grid_bin_start", 4 * B, S_GRID, S_COUNT);        // its last entry (= number of valid hits) is read up to the count step
   id.sort_keys = plan.add("sort_keys", 4 * N, S_SORT, S_GRID);
+  // long runs of empty bins, cut into segments: <= one per kGridGapSegment bins + one per run longer than kGridGapInline
+  id.gap_list = plan.add("grid_gap_segments(uint4)", 16 * ((size_t)c.n_bins / kGridGapSegment + std::min<size_t>(N + 1, (size_t)c.n_bins / kGridGapInline) + 2), S_GRID, S_GRID);
   id.tmp_keys = plan.add("sort_tmp_keys", 4 * N, S_SORT, S_SORT);
   id.tmp_orig = plan.add("sort_tmp_orig", 4 * N, S_SORT, S_SORT);
   id.tmp_yt = plan.add("sort_tmp_y_time", 8 * N, S_SORT, S_SORT);
@@ -716,7 +718,12 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
     }
   }
   mark(S_GRID);
-  k_grid_build<<<(int)((n + 1 + 255) / 256), 256, 0, st>>>(sort_keys, n, bin_start, hsr, c); ++launches;
+  {
+    uint4* gap_list = P.ptr<uint4>(A, id.gap_list);
+    uint32_t* n_gaps = reinterpret_cast<uint32_t*>(counters + kCntGridGaps);
+    k_grid_build<<<(int)((n + 1 + 255) / 256), 256, 0, st>>>(sort_keys, n, bin_start, hsr, gap_list, n_gaps, c); ++launches;
+    k_grid_fill_gaps<<<148 * 8, 256, 0, st>>>(gap_list, n_gaps, bin_start); ++launches;
+  }
 
   // ---- C2 neighbours finder ----
   mark(S_FINDER);

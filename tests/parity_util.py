@@ -37,7 +37,8 @@ def run_oracle(row, pad, time, n_sectors, max_time_bin, sigma_y=0.08, sigma_z=0.
     g = oracle.default_geometry(n_sectors, max_time_bin)
     p = oracle.default_params(sigma_y, sigma_z)
     for k, v in param_overrides.items():
-        setattr(p, k, v)
+        if k != "follower":                   # a knob of the CUDA path only (which follower kernel runs)
+            setattr(p, k, v)
     return oracle.track(g, p, row, pad, time)
 
 

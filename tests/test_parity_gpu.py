@@ -55,6 +55,29 @@ def test_continuous_readout_short_frames(cid, seed):
     assert rep["n_tracks"] > 1000
 
 
+@pytest.mark.parametrize("cid,seed,frame_us", [(0, 1, None), (1, 2, None), (2, 1, 150.0), (4, 3, 150.0)])
+def test_row_synchronous_follower_matches_the_oracle(cid, seed, frame_us):
+    """params.follower = 1: the lock-step follower with bulk-copy-staged rows (csrc/follow_rows.cuh) -- not the default, kept
+    for A/B -- gives the same links, tracklets, tracks and fits, bit for bit; nearly every search runs on the staged rows."""
+    cfg, tf = _frame(cid, seed, frame_us)
+    g, o = _both(tf, cfg, follower=1)
+    rep = PU.compare(g, o)
+    assert rep["track_par_bit_identical"] and rep["tracklet_par_bit_identical"] and rep["track_cov_bit_identical"]
+    w = g["work"]
+    searches = w["follow_up"]["row_steps"] + w["follow_down"]["row_steps"]
+    assert searches > 1000 and w["rare_paths"]["searches_in_global_memory"] < 0.05 * searches
+
+
+def test_row_synchronous_follower_other_cuts_and_grids():
+    cfg, tf = _frame(0, 6)
+    for kw in (dict(seed_min_hits=5, miss_limit=4, min_hits=20, chi2_cut=4.0), dict(grid_time_bins=2, grid_pad_bins=3),
+               dict(grid_time_bins=16, grid_pad_bins=64), dict(miss_limit=30, win_slope=0.2)):
+        g = PU.run_gpu(tf.row, tf.pad, tf.time, 1, tf.max_time_bin, follower=1, **kw)
+        okw = {k: v for k, v in kw.items() if not k.startswith("grid_")}
+        o = PU.run_oracle(tf.row, tf.pad, tf.time, 1, tf.max_time_bin, **okw)
+        PU.compare(g, o)
+
+
 def test_rare_paths_of_the_constructor_are_taken_and_agree():
     """The refit's replay (a failed transport after a hole) and the refit that fails before its first update (the up
     pass's state is the result) are rare; this input takes both (device counters), and parity holds on it."""
@@ -285,3 +308,32 @@ def test_whole_frame_oracle_parity_at_full_size(cid):
     inner = np.ones(nh, bool); inner[off] = False
     assert np.all(r_in[inner] > r_in[np.nonzero(inner)[0] - 1]), "hit rows must ascend inside a track"
     assert np.array_equal(r_in[off], gpu["first_row"][:k]) and np.array_equal(r_in[off + n_hits - 1], gpu["last_row"][:k])
+
+
+def test_empty_and_sparse_frames_on_the_10ms_grid_are_cheap():
+    """2.8e8 grid bins and (almost) nothing in them: the runs of empty bins are filled by whole CTAs, not by one thread
+    (a single thread writing every bin took seconds); results still equal the oracle's."""
+    import time as _time
+    import torch
+    from paper_2102_08862_b200 import tracker as T
+    cfg, tf = _frame(0, 3)                                     # 1.3e4 clusters of one sector ...
+    row = tf.row + np.float32(17 * N_ROWS)                      # ... moved to sector 17 of the 36-sector, 10 ms geometry
+    time = (tf.time.astype(np.float64) + 30000.0).astype(np.float32)
+    tmax = 50485.0
+    g = T.default_geometry(36, tmax)
+    trk = T.Tracker(g, T.default_params(max_clusters=tf.n))
+    d = [torch.from_numpy(np.ascontiguousarray(a, np.float32)).to(trk.device) for a in (row, tf.pad, time)]
+    e = torch.zeros(0, dtype=torch.float32, device=trk.device)
+    for clusters, n in ((d, tf.n), ([e, e, e], 0)):
+        outs = trk.alloc_outputs(max(n, 1))
+        trk.tpc_track_timeframe(*clusters, n=n, outputs=outs)   # warm-up
+        torch.cuda.synchronize()
+        t0 = _time.perf_counter()
+        out = trk.tpc_track_timeframe(*clusters, n=n, outputs=outs)
+        torch.cuda.synchronize()
+        assert _time.perf_counter() - t0 < 0.05, "a sparse frame on the long-frame grid must not take longer than a full one"
+        assert int(out.status[0]) == 0
+    trk.close()
+    gres = PU.run_gpu(row, tf.pad, time, 36, tmax)
+    ores = PU.run_oracle(row, tf.pad, time, 36, tmax)
+    assert PU.compare(gres, ores)["n_tracks"] > 50
