@@ -72,6 +72,15 @@ def _load():
         lib.tfgen_copy.restype = C.c_int
         lib.tfgen_free.argtypes = [C.c_void_p]
         lib.tfgen_free.restype = None
+        lib.tfgen_digitize.argtypes = [C.c_int64] + [C.c_void_p] * 4 + [C.c_int32, C.c_int32, C.c_void_p, C.c_int32, C.c_double, C.c_double,
+                                       C.c_int32, C.c_int32, C.POINTER(C.c_void_p)]
+        lib.tfgen_digitize.restype = C.c_int
+        lib.tfgen_digits_n.argtypes = [C.c_void_p]
+        lib.tfgen_digits_n.restype = C.c_int64
+        lib.tfgen_digits_copy.argtypes = [C.c_void_p] * 5
+        lib.tfgen_digits_copy.restype = None
+        lib.tfgen_digits_free.argtypes = [C.c_void_p]
+        lib.tfgen_digits_free.restype = None
         _lib = lib
     return _lib
 
@@ -153,3 +162,42 @@ def generate(cfg: GenConfig, want_truth: bool = True) -> TimeFrame:
                          int(lib.tfgen_n_collisions(h)), float(lib.tfgen_max_time_bin(h)))
     finally:
         lib.tfgen_free(h)
+
+
+@dataclass
+class Digits:
+    """Zero-suppressed ADC samples (the cluster finder's input), sorted by (sector_row, time bin, pad)."""
+
+    row: np.ndarray    # int32[n]  sector*n_rows + pad row
+    pad: np.ndarray    # int32[n]
+    time: np.ndarray   # int32[n]  time bin
+    adc: np.ndarray    # float32[n] integer-valued ADC count
+
+    @property
+    def n(self) -> int:
+        return int(self.adc.shape[0])
+
+
+def digitize(row, pad, time, charge, n_sectors: int, max_time_bin: float, n_rows: int = 152, sigma_pad: float = 0.45,
+             sigma_time: float = 0.55, threshold: int = 3, n_threads: int = 0) -> Digits:
+    """Clusters -> zero-suppressed samples (see ``tfgen_digitize``): every cluster deposits its charge on the 3 x 3 cells
+    around it with Gaussian-integral weights, overlapping deposits add, ADC = floor, samples below ``threshold`` are dropped."""
+    lib = _load()
+    a = lambda v: np.ascontiguousarray(v, np.float32)
+    row, pad, time, charge = a(row), a(pad), a(time), a(charge)
+    x = 85.0 + 1.07 * np.arange(n_rows)
+    npads = np.floor(2.0 * x * np.tan(np.radians(10.0)) / 0.5).astype(np.int32)
+    h = C.c_void_p()
+    rc = lib.tfgen_digitize(int(row.shape[0]), row.ctypes.data, pad.ctypes.data, time.ctypes.data, charge.ctypes.data,
+                            int(n_sectors * n_rows), int(n_rows), npads.ctypes.data, int(max_time_bin), float(sigma_pad),
+                            float(sigma_time), int(threshold), int(n_threads), C.byref(h))
+    if rc != 0:
+        raise ValueError("tfgen_digitize rejected its arguments")
+    try:
+        n = lib.tfgen_digits_n(h)
+        r, p, t = (np.empty(n, np.int32) for _ in range(3))
+        q = np.empty(n, np.float32)
+        lib.tfgen_digits_copy(h, r.ctypes.data, p.ctypes.data, t.ctypes.data, q.ctypes.data)
+        return Digits(r, p, t, q)
+    finally:
+        lib.tfgen_digits_free(h)

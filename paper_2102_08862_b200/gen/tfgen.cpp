@@ -344,4 +344,93 @@ int tfgen_copy(const tfgen_frame* f, float* row, float* pad, float* time, float*
 
 void tfgen_free(tfgen_frame* f) { delete f; }
 
+
+// ---- digitisation: clusters -> zero-suppressed ADC samples (input of the cluster finder) ----
+// Stands in for "simulated Monte-Carlo time frames converted to raw data" one step earlier in the chain.
+// Every cluster (sector_row, pad, time, charge) deposits its charge on the 3 x 3 cells around (round(pad), round(time))
+// of its sector-row with separable weights = the integral of a Gaussian (sigma_pad, sigma_time, in cells) over each cell;
+// deposits that fall on the same cell add up; ADC = floor(sum); cells below `threshold` are suppressed (zero suppression in
+// the readout).  Output: samples sorted by (sector_row, time bin, pad), no duplicates -- the readout order the
+// cluster finder's input contract names.  Holds none of the cluster finder's arithmetic.
+struct tfgen_digits {
+  std::vector<int32_t> row, pad, time;
+  std::vector<float> adc;
+};
+
+int tfgen_digitize(int64_t n, const float* row, const float* pad, const float* time, const float* charge, int32_t n_sector_rows,
+                   int32_t n_rows, const int32_t* n_pads_of_row, int32_t max_time_bin, double sigma_pad, double sigma_time,
+                   int32_t threshold, int32_t n_threads, tfgen_digits** out) {
+  if (!out || n < 0 || n_sector_rows < 1 || n_rows < 1 || !n_pads_of_row || !(sigma_pad > 0) || !(sigma_time > 0)) return -1;
+  std::vector<int64_t> start((size_t)n_sector_rows + 1, 0);
+  for (int64_t i = 0; i < n; ++i) { const int sr = (int)row[i]; if (sr >= 0 && sr < n_sector_rows) ++start[(size_t)sr + 1]; }
+  for (int s = 0; s < n_sector_rows; ++s) start[(size_t)s + 1] += start[(size_t)s];
+  std::vector<int64_t> idx((size_t)start[(size_t)n_sector_rows]);
+  {
+    std::vector<int64_t> fill(start.begin(), start.end() - 1);
+    for (int64_t i = 0; i < n; ++i) { const int sr = (int)row[i]; if (sr >= 0 && sr < n_sector_rows) idx[(size_t)fill[(size_t)sr]++] = i; }
+  }
+  struct Part { std::vector<int32_t> pad, time; std::vector<float> adc; };
+  std::vector<Part> parts((size_t)n_sector_rows);
+  auto cdf = [](double x) { return 0.5 * std::erfc(-x / std::sqrt(2.0)); };
+  std::atomic<int> next(0);
+  auto work = [&]() {
+    std::vector<std::pair<uint64_t, double>> dep;
+    for (;;) {
+      const int sr = next.fetch_add(1);
+      if (sr >= n_sector_rows) break;
+      const int np = n_pads_of_row[sr % n_rows];
+      dep.clear();
+      for (int64_t q = start[(size_t)sr]; q < start[(size_t)sr + 1]; ++q) {
+        const int64_t i = idx[(size_t)q];
+        const int p0 = (int)std::floor((double)pad[i] + 0.5), t0 = (int)std::floor((double)time[i] + 0.5);
+        const double dp = (double)pad[i] - p0, dt = (double)time[i] - t0;
+        double wp[3], wt[3];
+        for (int k = -1; k <= 1; ++k) {
+          wp[k + 1] = cdf((k + 0.5 - dp) / sigma_pad) - cdf((k - 0.5 - dp) / sigma_pad);
+          wt[k + 1] = cdf((k + 0.5 - dt) / sigma_time) - cdf((k - 0.5 - dt) / sigma_time);
+        }
+        for (int a = -1; a <= 1; ++a)
+          for (int b = -1; b <= 1; ++b) {
+            const int pp = p0 + b, tt = t0 + a;
+            if (pp < 0 || pp >= np || tt < 0 || tt > max_time_bin) continue;
+            dep.emplace_back(((uint64_t)(uint32_t)tt << 16) | (uint64_t)(uint32_t)pp, (double)charge[i] * wt[a + 1] * wp[b + 1]);
+          }
+      }
+      std::sort(dep.begin(), dep.end(), [](const std::pair<uint64_t, double>& x, const std::pair<uint64_t, double>& y) { return x.first < y.first; });
+      Part& P = parts[(size_t)sr];
+      for (size_t a = 0; a < dep.size();) {
+        size_t b = a;
+        double sum = 0.0;
+        while (b < dep.size() && dep[b].first == dep[a].first) sum += dep[b++].second;
+        const double adc = std::floor(sum);
+        if (adc >= (double)threshold) { P.time.push_back((int32_t)(dep[a].first >> 16)); P.pad.push_back((int32_t)(dep[a].first & 0xFFFF)); P.adc.push_back((float)adc); }
+        a = b;
+      }
+    }
+  };
+  const int nt = std::max(1, n_threads > 0 ? n_threads : (int)std::thread::hardware_concurrency());
+  std::vector<std::thread> th;
+  for (int t = 0; t < nt; ++t) th.emplace_back(work);
+  for (auto& t : th) t.join();
+  tfgen_digits* D = new tfgen_digits();
+  size_t total = 0;
+  for (const Part& P : parts) total += P.adc.size();
+  D->row.reserve(total); D->pad.reserve(total); D->time.reserve(total); D->adc.reserve(total);
+  for (int sr = 0; sr < n_sector_rows; ++sr) {
+    const Part& P = parts[(size_t)sr];
+    D->row.insert(D->row.end(), P.adc.size(), sr);
+    D->pad.insert(D->pad.end(), P.pad.begin(), P.pad.end());
+    D->time.insert(D->time.end(), P.time.begin(), P.time.end());
+    D->adc.insert(D->adc.end(), P.adc.begin(), P.adc.end());
+  }
+  *out = D;
+  return 0;
+}
+int64_t tfgen_digits_n(const tfgen_digits* d) { return d ? (int64_t)d->adc.size() : -1; }
+void tfgen_digits_copy(const tfgen_digits* d, int32_t* row, int32_t* pad, int32_t* time, float* adc) {
+  const size_t n = d->adc.size();
+  std::memcpy(row, d->row.data(), n * 4); std::memcpy(pad, d->pad.data(), n * 4); std::memcpy(time, d->time.data(), n * 4); std::memcpy(adc, d->adc.data(), n * 4);
+}
+void tfgen_digits_free(tfgen_digits* d) { delete d; }
+
 }  // extern "C"
