@@ -221,6 +221,8 @@ def main():
     ap.add_argument("--grid-pad-bins", type=int, default=0, help="grid bins across a pad row (0 = library default)")
     ap.add_argument("--follower", type=int, default=0, help="0 = per-lane follower (default), 1 = row-synchronous follower (A/B)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cluster-finder", action="store_true")
+    ap.add_argument("--cf-frame-us", type=float, default=1000.0, help="frame length whose samples the cluster finder (C0) is timed on")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-inflight", type=int, default=2, help="time frames in flight in the end-to-end measurement")
     args = ap.parse_args()
@@ -331,6 +333,41 @@ def main():
                  "central_electrode": {"step": "central_electrode_merge (C10, tpc_merge_central_electrode)", "ms": round(ms_c, 4),
                                        "n_links": int(ce[3][0]), "gpu_launches": trk.last_merge_launches()}}
         del outs_c
+    # ---- widening step C0 (the cluster finder in front of the path, not part of `value`): timed on the samples of a 1 ms
+    # cut of the same generator (digitising the whole 10 ms frame would be 9e8 samples / 14 GB of host work per run)
+    cluster_finder = None
+    if not args.no_cluster_finder:
+        ccfg = gen.preset(cid, args.seed, min(args.cf_frame_us, cfg.frame_us) if cid >= 2 else None)
+        ccfg.n_threads = cfg.n_threads
+        ctf = gen.generate(ccfg, want_truth=False)
+        dg = gen.digitize(ctf.row, ctf.pad, ctf.time, ctf.charge, ccfg.n_sectors, ctf.max_time_bin)
+        dd = [torch.from_numpy(a).to(dev) for a in (dg.row, dg.pad, dg.time, dg.adc)]
+        cf_out = None
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n_rep = 5
+        for i in range(3 + n_rep):
+            if i == 3:
+                c0.record(stream)
+            with torch.cuda.stream(stream):
+                cf_out = trk.tpc_find_clusters(*dd, n=dg.n, out=cf_out, stream=stream)
+        c1.record(stream)
+        stream.synchronize()
+        ms_cf = c0.elapsed_time(c1) / n_rep
+        k_cf = int(cf_out[4][0])
+        cf_bytes = 16 * dg.n + 16 * k_cf
+        cluster_finder = {"step": "cluster_finder (C0, tpc_find_clusters)", "ms": round(ms_cf, 4), "n_samples": dg.n, "n_clusters": k_cf,
+                          "samples_per_s": dg.n / (ms_cf * 1e-3), "clusters_per_s": k_cf / (ms_cf * 1e-3),
+                          "sample": f"samples of the same generator cut to {ccfg.frame_us:g} us ({ctf.n} generated clusters)" if cid >= 2 else "the whole frame",
+                          "bound": "hbm", "achieved": round(cf_bytes / (ms_cf * 1e-3) / 1e9, 1), "unit": "GB/s",
+                          "algo_bytes": "16 per sample read + 16 per cluster written", "gpu_launches": trk.last_merge_launches(), "in_value": False}
+        if not args.no_cpu_baseline and rank == 0:          # the C0 oracle beside it, one core, on the first 3e6 samples
+            from oracle import clusterfinder as CFO
+            m = min(dg.n, 3_000_000)
+            t0 = time.perf_counter()
+            CFO.find_clusters(dg.row[:m], dg.pad[:m], dg.time[:m], dg.adc[:m])
+            dt = time.perf_counter() - t0
+            cluster_finder["cpu_baseline"] = {"value": m / dt, "unit": "samples/s", "cores": 1, "kind": "oracle", "sample": f"the first {m} samples", "seconds": dt}
+        del dd, cf_out
     trk.close()
     del trk, outs
 
@@ -391,6 +428,8 @@ def main():
 
     # ---- per-kernel rooflines; `roofline` = the dominant kernel's ----
     peak, peak_src = _peaks()
+    if cluster_finder:
+        cluster_finder.update({"peak": peak, "frac": round(cluster_finder["achieved"] / peak, 4)})
     clk = clocks.summary()
     mhz = clk["sm_mhz"] or clk["sm_max_mhz"] or 1965.0
     alu_derived = SM_COUNT * SMSP_PER_SM * LANES * mhz * 1e6 / 1e12          # T lane-instructions / s at the clock under load
@@ -470,6 +509,7 @@ def main():
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches,
             "step_ms": {k: round(v, 4) for k, v in step_acc.items()}, "kernels": kernels,
             "tracklet_constructor": constructor, "frame_vs_floors": frame, "rare_paths": work.get("rare_paths"), "merge": merge,
+            "cluster_finder": cluster_finder,
             "roofline": roof, "cpu_baseline": cpu}
     print(json.dumps(line))
     if world > 1:

@@ -199,6 +199,36 @@ int tpc_selftest_fast_math(void* cuda_stream, uint64_t* mismatches_out);
  * Returns TPC_OK or TPC_ECUDA.                                                                              */
 int tpc_selftest_alu_peak(void* cuda_stream, double* lane_inst_per_s_out);
 
+/* ---- C0: the TPC cluster finder, the step in front of the path (clusterization is part
+ * of the synchronous GPU load; DESIGN.md §3 "C0", readings D1..D6).  Zero-suppressed ADC samples in, clusters in the tracker's
+ * input format out: a sample is a peak iff adc >= peak_threshold and it beats its (up to) 8 neighbours in (pad, time) of the
+ * same sector-row (larger adc; ties to the earlier sample); a peak's cluster is the fp32 centre of gravity of its 3 x 3 window. */
+typedef struct {
+  const int32_t* row;    /* DEVICE [n_digits] sector * n_rows + pad row                                                  */
+  const int32_t* pad;    /* DEVICE [n_digits] pad                                                                        */
+  const int32_t* time;   /* DEVICE [n_digits] time bin.  Samples are sorted by (row, time, pad), no duplicates (reading D1:
+                            the readout order); an unsorted input gives unspecified clusters, never an out-of-bounds access */
+  const float* adc;      /* DEVICE [n_digits] ADC count                                                                  */
+} tpc_digits_t;
+
+typedef struct { float peak_threshold; /* 8 : smallest ADC of a cluster's peak sample (reading D4) */ } tpc_cluster_params_t;
+
+typedef struct {   /* caller-allocated DEVICE buffers: exactly the arrays tpc_clusters_t takes                              */
+  int64_t max_clusters;
+  float *row, *pad, *time, *charge;   /* [max_clusters], in the input order of the peak samples                          */
+  int64_t* n_clusters;   /* scalar: clusters found (may exceed max_clusters: the first max_clusters are written)         */
+  int32_t* status;       /* scalar: 1 = more clusters than max_clusters                                                  */
+} tpc_clusters_out_t;
+
+/* Arena bytes the call needs for n_digits samples (host arithmetic, 28 B per sample; 0 = invalid).                        */
+size_t tpc_cluster_finder_scratch_bytes(int64_t n_digits);
+
+/* Asynchronous on `cuda_stream`, never allocates: scratch = the handle's arena (the call precedes tpc_track_timeframe on the
+ * same stream, which then overwrites it).  Errors: TPC_EINVAL, TPC_ENOMEM (arena smaller than the scratch), TPC_ECUDA.
+ * tpc_merge_last_launches() reports its launches.                                                                       */
+int tpc_find_clusters(tpc_tracker_t* tracker, const tpc_cluster_params_t* params, const tpc_digits_t* digits, int64_t n_digits,
+                      void* cuda_stream, tpc_clusters_out_t* clusters_out);
+
 /* ---- C7: sector-boundary merging of the per-sector tracks (DESIGN.md §3 "C7", readings M1..M8; PAPER.md L23 / L25:
  * "full TPC tracking" -- the sector tracker is followed by a merger of the sector tracks; BASELINE.json L8: 36 sectors,
  * each in its rotated local frame).  A widening step after the hot path (linking only: the

@@ -10,6 +10,7 @@
 #include <new>
 
 #include "arena.h"
+#include "clusterizer.cuh"
 #include "common.cuh"
 #include "finder.cuh"
 #include "follow_rows.cuh"
@@ -467,6 +468,64 @@ int tpc_merge_tracks(tpc_tracker_t* t, const tpc_merge_params_t* mp, const tpc_t
     k_merge_match<<<(K + kMergeThreads - 1) / kMergeThreads, kMergeThreads, 0, st>>>(T, S, c); ++launches;
     k_merge_link<<<g256, 256, 0, st>>>(T, S, out->next, out->prev, out->n_links, c); ++launches;
     k_merge_root<<<g256, 256, 0, st>>>(T, out->prev, out->root, c); ++launches;
+  }
+  t->last_merge_launches = launches;
+  if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;
+  return TPC_OK;
+}
+
+
+// ---- C0: cluster finder in front of the path (clusterizer.cuh) ----
+namespace {
+struct CfLayout { size_t head, gnum, group_start, peak, sums, tiles_a, tiles_b, total; };
+CfLayout cf_layout(int64_t n) {
+  CfLayout L{};
+  const size_t N = (size_t)std::max<int64_t>(n, 1);
+  size_t off = 0;
+  auto take = [&](size_t bytes) { const size_t o = off; off += (bytes + 255) / 256 * 256; return o; };
+  L.head = take(4 * N); L.gnum = take(4 * N); L.group_start = take(4 * (N + 1)); L.peak = take(4 * N); L.sums = take(12 * N);
+  L.tiles_a = take(4 * (scan_tiles(N) + 2)); L.tiles_b = take(4 * (scan_tiles(N) + 2));
+  L.total = off;
+  return L;
+}
+}  // namespace
+
+size_t tpc_cluster_finder_scratch_bytes(int64_t n_digits) {
+  if (n_digits < 0 || n_digits >= ((int64_t)1 << 32) - 4096) return 0;
+  return cf_layout(n_digits).total;
+}
+
+int tpc_find_clusters(tpc_tracker_t* t, const tpc_cluster_params_t* cp, const tpc_digits_t* dg, int64_t n, void* cuda_stream, tpc_clusters_out_t* o) {
+  if (!t || !cp || !dg || !o || n < 0 || n >= ((int64_t)1 << 32) - 4096) return TPC_EINVAL;
+  if (!(cp->peak_threshold > 0) || !o->n_clusters || !o->status || o->max_clusters < 0) return TPC_EINVAL;
+  if (n > 0 && (!dg->row || !dg->pad || !dg->time || !dg->adc)) return TPC_EINVAL;
+  if (o->max_clusters > 0 && (!o->row || !o->pad || !o->time || !o->charge)) return TPC_EINVAL;
+  const CfLayout L = cf_layout(n);
+  if (!t->params.arena || L.total > t->params.arena_bytes) return TPC_ENOMEM;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* A = static_cast<char*>(t->params.arena);
+  uint32_t* head = reinterpret_cast<uint32_t*>(A + L.head);
+  uint32_t* gnum = reinterpret_cast<uint32_t*>(A + L.gnum);
+  uint32_t* group_start = reinterpret_cast<uint32_t*>(A + L.group_start);
+  uint32_t* peak = reinterpret_cast<uint32_t*>(A + L.peak);
+  CfSums* sums = reinterpret_cast<CfSums*>(A + L.sums);
+  uint32_t* tiles_a = reinterpret_cast<uint32_t*>(A + L.tiles_a);
+  uint32_t* tiles_b = reinterpret_cast<uint32_t*>(A + L.tiles_b);
+  int64_t launches = 0;
+  if (n == 0) {
+    cudaMemsetAsync(o->n_clusters, 0, 8, st);
+    cudaMemsetAsync(o->status, 0, 4, st);
+  } else {
+    const CfDigits d{dg->row, dg->pad, dg->time, dg->adc};
+    const CfOut out{o->max_clusters, o->row, o->pad, o->time, o->charge, o->n_clusters, o->status};
+    const int ctas = (int)((n + 255) / 256);
+    const size_t nt = scan_tiles((size_t)n);
+    k_cf_heads<<<ctas, 256, 0, st>>>(d, n, head); ++launches;
+    launches += exclusive_scan_u32(head, gnum, (size_t)n, tiles_a, st);                 // tiles_a[nt] = number of groups
+    k_cf_groups<<<ctas, 256, 0, st>>>(head, gnum, n, tiles_a + nt, group_start); ++launches;
+    k_cf_peaks<<<ctas, 256, 0, st>>>(d, n, head, gnum, group_start, tiles_a + nt, cp->peak_threshold, peak, sums); ++launches;
+    launches += exclusive_scan_u32(peak, peak, (size_t)n, tiles_b, st);                 // tiles_b[nt] = number of clusters
+    k_cf_emit<<<ctas, 256, 0, st>>>(d, n, peak, tiles_b + nt, sums, out); ++launches;
   }
   t->last_merge_launches = launches;
   if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;

@@ -18,6 +18,7 @@ STATUS_TRACKLET_OVERFLOW, STATUS_TRACK_OVERFLOW, STATUS_TRACK_HIT_OVERFLOW, STAT
 EXPORTS = ("tpc_tracker_arena_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
            "tpc_tracker_step_ms", "tpc_tracker_step_name", "tpc_tracker_last_launches", "tpc_tracker_work_counters",
            "tpc_tracker_arena_plan", "tpc_selftest_fast_math", "tpc_selftest_alu_peak",
+           "tpc_cluster_finder_scratch_bytes", "tpc_find_clusters",
            "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_merge_central_electrode", "tpc_refit_chains", "tpc_vertex_time", "tpc_merge_last_launches",
            "tpc_tracker_destroy", "tpc_strerror")
 
@@ -70,6 +71,22 @@ class MergeParams(C.Structure):
 class Merged(C.Structure):
     """``tpc_merged_t``"""
     _fields_ = [("next", C.c_void_p), ("prev", C.c_void_p), ("root", C.c_void_p), ("n_links", C.c_void_p)]
+
+
+class Digits(C.Structure):
+    """``tpc_digits_t``"""
+    _fields_ = [("row", C.c_void_p), ("pad", C.c_void_p), ("time", C.c_void_p), ("adc", C.c_void_p)]
+
+
+class ClusterParams(C.Structure):
+    """``tpc_cluster_params_t``"""
+    _fields_ = [("peak_threshold", C.c_float)]
+
+
+class ClustersOut(C.Structure):
+    """``tpc_clusters_out_t``"""
+    _fields_ = [("max_clusters", C.c_int64), ("row", C.c_void_p), ("pad", C.c_void_p), ("time", C.c_void_p), ("charge", C.c_void_p),
+                ("n_clusters", C.c_void_p), ("status", C.c_void_p)]
 
 
 class CeParams(C.Structure):
@@ -146,6 +163,10 @@ def load_library(build_if_missing: bool = True):
         L.tpc_merge_scratch_bytes.restype = C.c_size_t
         L.tpc_merge_tracks.argtypes = [vp, C.POINTER(MergeParams), C.POINTER(Tracks), vp, C.POINTER(Merged)]
         L.tpc_merge_tracks.restype = C.c_int
+        L.tpc_cluster_finder_scratch_bytes.argtypes = [C.c_int64]
+        L.tpc_cluster_finder_scratch_bytes.restype = C.c_size_t
+        L.tpc_find_clusters.argtypes = [vp, C.POINTER(ClusterParams), C.POINTER(Digits), C.c_int64, vp, C.POINTER(ClustersOut)]
+        L.tpc_find_clusters.restype = C.c_int
         L.tpc_merge_central_electrode.argtypes = [vp, C.POINTER(CeParams), C.POINTER(Tracks), vp, C.POINTER(CeMerged)]
         L.tpc_merge_central_electrode.restype = C.c_int
         L.tpc_refit_chains.argtypes = [vp, C.POINTER(Tracks), C.POINTER(Merged), vp, C.POINTER(Refit)]
@@ -339,6 +360,28 @@ class Tracker:
         rc = self.lib.tpc_track_timeframe_host(self.handle, C.byref(cl), n, C.c_void_p(s.cuda_stream), C.byref(st))
         if rc != TPC_OK:
             raise TpcError(rc, "tpc_track_timeframe_host")
+        return out
+
+    def tpc_find_clusters(self, row, pad, time, adc, n: int | None = None, max_clusters: int | None = None, peak_threshold: float = 8.0,
+                          out=None, stream=None):
+        """C0 on DEVICE int32 (row, pad, time) / float32 adc tensors sorted by (row, time, pad); returns
+        (row, pad, time, charge, n_clusters, status) device tensors -- the first three are ``tpc_track_timeframe``'s input."""
+        torch = self._torch
+        n = int(adc.shape[0]) if n is None else int(n)
+        for t_, dt in ((row, torch.int32), (pad, torch.int32), (time, torch.int32), (adc, torch.float32)):
+            if not (t_.is_cuda and t_.dtype == dt and t_.is_contiguous() and t_.shape[0] >= n):
+                raise ValueError("digits must be contiguous CUDA tensors: int32 row / pad / time, float32 adc, length >= n")
+        K = int(max_clusters) if max_clusters is not None else max(n, 1)
+        if out is None:
+            e = lambda dt, k=K: torch.empty(max(k, 1), dtype=dt, device=self.device)
+            out = (e(torch.float32), e(torch.float32), e(torch.float32), e(torch.float32), e(torch.int64, 1), e(torch.int32, 1))
+        dg = Digits(row.data_ptr(), pad.data_ptr(), time.data_ptr(), adc.data_ptr())
+        co = ClustersOut(K, out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr(), out[3].data_ptr(), out[4].data_ptr(), out[5].data_ptr())
+        cp = ClusterParams(float(peak_threshold))
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        rc = self.lib.tpc_find_clusters(self.handle, C.byref(cp), C.byref(dg), n, C.c_void_p(s.cuda_stream), C.byref(co))
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_find_clusters")
         return out
 
     def tpc_merge_tracks(self, outputs, merge_params: MergeParams | None = None, merged=None, stream=None):
