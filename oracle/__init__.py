@@ -81,6 +81,11 @@ def lib():
         L.orc_tables.argtypes = [C.POINTER(Geometry), C.POINTER(Params), vp, vp, vp, vp]
         L.orc_refit_chains.argtypes = [C.POINTER(Geometry), C.POINTER(Params), vp, vp, vp, C.c_int64] + [vp] * 12
         L.orc_refit_chains.restype = None
+        L.orc_compress_tracks.argtypes = [C.POINTER(Geometry), C.POINTER(Params), C.c_float, C.c_float, C.c_float, vp, vp, vp, C.c_int64,
+                                          C.c_int64] + [vp] * 9
+        L.orc_compress_tracks.restype = None
+        L.orc_decompress_tracks.argtypes = [C.POINTER(Geometry), C.POINTER(Params), C.c_float, C.c_float, C.c_int64] + [vp] * 10
+        L.orc_decompress_tracks.restype = None
         L.orc_rotate_with_cov.argtypes = [C.POINTER(Geometry), C.POINTER(Params), vp, vp, C.c_int32]
         L.orc_rotate_with_cov.restype = C.c_int
         for nm in ("orc_copy_links", "orc_copy_tracklets", "orc_copy_tracks", "orc_copy_stats", "orc_free",
@@ -217,3 +222,37 @@ def rotate_with_cov(geom: Geometry, params: Params, state6, cov9, q: int):
     cv = np.array(cov9, np.float32)
     rc = lib().orc_rotate_with_cov(C.byref(geom), C.byref(params), st.ctypes.data, cv.ctypes.data, int(q))
     return rc == 0, st, cv
+
+
+DEFAULT_REJECT_QPT, DEFAULT_STEP_Y, DEFAULT_STEP_Z = 1.0 / 0.15, 0.025, 0.025      # DESIGN.md §3 C11 readings R11-1, R11-3
+
+
+def compress_tracks(geom: Geometry, params: Params, row, pad, time, res: "Result", reject_qpt: float = DEFAULT_REJECT_QPT,
+                    step_y: float = DEFAULT_STEP_Y, step_z: float = DEFAULT_STEP_Z):
+    """C11: (reject uint8[n_clusters], ok int32[n_tracks], qy int16[n_track_hits], qz int16[n_track_hits])."""
+    a = lambda v, t: np.ascontiguousarray(v, t)
+    row, pad, time = a(row, np.float32), a(pad, np.float32), a(time, np.float32)
+    n, k, nh = int(row.shape[0]), int(len(res.tr_seed)), int(len(res.tr_hit_index))
+    reject, ok = np.zeros(n, np.uint8), np.zeros(k, np.int32)
+    qy, qz = np.zeros(nh, np.int16), np.zeros(nh, np.int16)
+    nhits, off, hi = a(res.tr_n_hits, np.int32), a(res.tr_hit_offset, np.int64), a(res.tr_hit_index, np.int32)
+    par, cov = a(res.tr_par, np.float32), a(res.tr_cov, np.float32)
+    lib().orc_compress_tracks(C.byref(geom), C.byref(params), float(reject_qpt), float(step_y), float(step_z), row.ctypes.data,
+                              pad.ctypes.data, time.ctypes.data, n, k, nhits.ctypes.data, off.ctypes.data, hi.ctypes.data,
+                              par.ctypes.data, cov.ctypes.data, reject.ctypes.data, ok.ctypes.data, qy.ctypes.data, qz.ctypes.data)
+    return reject, ok, qy, qz
+
+
+def decompress_tracks(geom: Geometry, params: Params, res: "Result", hit_row, ok, qy, qz, step_y: float = DEFAULT_STEP_Y,
+                      step_z: float = DEFAULT_STEP_Z):
+    """The C11 decoder (pins only): (y [cm], z relative to the track's time_ref [cm]) of every hit of the tracks with ok == 1."""
+    a = lambda v, t: np.ascontiguousarray(v, t)
+    k, nh = int(len(res.tr_seed)), int(len(res.tr_hit_index))
+    y, z = np.full(nh, np.nan, np.float32), np.full(nh, np.nan, np.float32)
+    nhits, off = a(res.tr_n_hits, np.int32), a(res.tr_hit_offset, np.int64)
+    par, cov, hr = a(res.tr_par, np.float32), a(res.tr_cov, np.float32), a(hit_row, np.uint8)
+    ok, qy, qz = a(ok, np.int32), a(qy, np.int16), a(qz, np.int16)
+    lib().orc_decompress_tracks(C.byref(geom), C.byref(params), float(step_y), float(step_z), k, nhits.ctypes.data, off.ctypes.data,
+                                hr.ctypes.data, par.ctypes.data, cov.ctypes.data, ok.ctypes.data, qy.ctypes.data, qz.ctypes.data,
+                                y.ctypes.data, z.ctypes.data)
+    return y, z

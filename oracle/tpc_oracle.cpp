@@ -584,6 +584,74 @@ void orc_refit_chains(const orc_geometry* gp, const orc_params* pp, const float*
   }
 }
 
+// ---- C11: track-based hit rejection and track-model residual coding ("the step after the path";
+// PAPER.md L23 (§1): the TPC data are compressed online by "removal of TPC hits of tracks not used for physics" and "reduction
+// of the hit property entropy" -- the reason the tracking runs synchronously at all).  The paper gives neither rule nor
+// format, so the definitions are readings of this build (R11-1..R11-6, DESIGN.md §3 "C11"); the entropy coder behind it (ANS)
+// is out of scope.
+//   Rejection: every hit a track OWNS (C6) is rejected iff |q/pT| of the track > reject_qpt (a low-momentum looper, "not used
+//   for physics"); hits no track owns are kept (R11-1).
+//   Residual coding of the hits of every KEPT track, a closed-loop predictive coder (R11-2..5): the state starts as the
+//   track's C6 parameters and covariance (they travel in the stream as the track header); for the owned hits in ascending row:
+//       transport(S, x_row)                          FAIL -> the track is flagged ok = 0 and its remaining symbols are 0
+//       ry = y(hit) - S.y;  rz = (time(hit) - time_ref) * Z - S.z
+//       qy = (int)rintf(ry / step_y), qz = (int)rintf(rz / step_z), each clamped to [-32767, 32767]
+//       yq = S.y + (float)qy * step_y;  zq = S.z + (float)qz * step_z        # what a decoder reconstructs
+//       update(S, yq, zq)                            # with the RECONSTRUCTED hit: the decoder's state is the same
+//   Output: (qy, qz) per track hit in hit_index order, ok per track, reject per cluster.
+// orc_decompress_tracks is the decoder (headers + symbols -> hit coordinates), used by the pins only.
+void orc_compress_tracks(const orc_geometry* gp, const orc_params* pp, float reject_qpt, float step_y, float step_z,
+                         const float* row, const float* pad, const float* time, int64_t n_clusters,
+                         int64_t n_tracks, const int32_t* n_hits, const int64_t* hit_offset, const int32_t* hit_index,
+                         const float* par, const float* cov, uint8_t* reject, int32_t* ok, int16_t* qy, int16_t* qz) {
+  const Derived D = derive(*gp, *pp);
+  const int nr = gp->n_rows;
+  for (int64_t i = 0; i < n_clusters; ++i) reject[i] = 0;
+  for (int64_t k = 0; k < n_tracks; ++k) {
+    const float* q = par + 7 * k;
+    const float* cv = cov + 9 * k;
+    const bool rej = std::fabs(q[5]) > reject_qpt;
+    ok[k] = rej ? -1 : 1;
+    State S{q[0], q[1], q[2], q[3], q[4], q[5], cv[0], cv[1], cv[2], cv[3], cv[4], cv[5], cv[6], cv[7], cv[8]};
+    bool good = !rej;
+    for (int64_t j = hit_offset[k]; j < hit_offset[k] + n_hits[k]; ++j) {
+      const int32_t h = hit_index[j];
+      if (rej) { reject[h] = 1; qy[j] = 0; qz[j] = 0; continue; }
+      if (good) good = transport(S, D.xr[(int)row[h] % nr], D.cB, pp->sin_phi_max);
+      if (!good) { ok[k] = 0; qy[j] = 0; qz[j] = 0; continue; }
+      const int r = (int)row[h] % nr;
+      const float ym = (pad[h] - D.cr[r]) * D.P;
+      const float zm = (time[h] - q[6]) * D.Z;
+      const float ry = ym - S.y, rz = zm - S.z;
+      int iy = (int)std::rint(ry / step_y), iz = (int)std::rint(rz / step_z);
+      iy = std::min(std::max(iy, -32767), 32767); iz = std::min(std::max(iz, -32767), 32767);
+      qy[j] = (int16_t)iy; qz[j] = (int16_t)iz;
+      const float yq = S.y + (float)iy * step_y, zq = S.z + (float)iz * step_z;
+      update(S, yq, zq, D.ry, D.rz);
+    }
+  }
+}
+
+// The decoder: from the track headers (par, cov, n_hits, rows of the hits) and the symbols back to (y, z relative to
+// time_ref) of every hit of the tracks with ok == 1.  Mirrors the encoder's state exactly.
+void orc_decompress_tracks(const orc_geometry* gp, const orc_params* pp, float step_y, float step_z, int64_t n_tracks,
+                           const int32_t* n_hits, const int64_t* hit_offset, const uint8_t* hit_row, const float* par, const float* cov,
+                           const int32_t* ok, const int16_t* qy, const int16_t* qz, float* y_out, float* z_out) {
+  const Derived D = derive(*gp, *pp);
+  for (int64_t k = 0; k < n_tracks; ++k) {
+    if (ok[k] != 1) continue;
+    const float* q = par + 7 * k;
+    const float* cv = cov + 9 * k;
+    State S{q[0], q[1], q[2], q[3], q[4], q[5], cv[0], cv[1], cv[2], cv[3], cv[4], cv[5], cv[6], cv[7], cv[8]};
+    for (int64_t j = hit_offset[k]; j < hit_offset[k] + n_hits[k]; ++j) {
+      transport(S, D.xr[hit_row[j]], D.cB, pp->sin_phi_max);
+      const float yq = S.y + (float)qy[j] * step_y, zq = S.z + (float)qz[j] * step_z;
+      y_out[j] = yq; z_out[j] = zq;
+      update(S, yq, zq, D.ry, D.rz);
+    }
+  }
+}
+
 // ---- hooks for the pins (K1..K3, G1): the same functions the tracker uses, callable one at a time ----
 // state6 = (x, y, z, s, t, k); cov9 = (c0..c5, d0..d2).  Returns 0, or 1 on transport FAIL.
 int orc_transport(const orc_params* p, float* st, float* cv, float xn) {
