@@ -306,9 +306,9 @@ def main():
     # ---- widening step C7 (sector-boundary merging of the tracks, not part of `value`): timed on its own ----
     merge = None
     if cfg.n_sectors >= 18:
-        m0, m1, m2, m3 = (torch.cuda.Event(enable_timing=True) for _ in range(4))
-        merged = refit = ce = None
-        ms_m = ms_r = ms_c = 0.0
+        m0, m1, m2, m3, m4 = (torch.cuda.Event(enable_timing=True) for _ in range(5))
+        merged = refit = ce = comp = None
+        ms_m = ms_r = ms_c = ms_q = 0.0
         outs_c = trk.alloc_outputs(n, hit_coords=True)      # C8 reads the hits' coordinates from two optional emit outputs
         for _ in range(3):
             with torch.cuda.stream(stream):
@@ -320,8 +320,10 @@ def main():
                 m2.record(stream)
                 ce = trk.tpc_merge_central_electrode(outs_c, merged=ce, stream=stream)
                 m3.record(stream)
+                comp = trk.tpc_compress_tracks(outs_c, n, out=comp, stream=stream)
+                m4.record(stream)
             stream.synchronize()
-            ms_m, ms_r, ms_c = m0.elapsed_time(m1), m1.elapsed_time(m2), m2.elapsed_time(m3)      # last of three
+            ms_m, ms_r, ms_c, ms_q = m0.elapsed_time(m1), m1.elapsed_time(m2), m2.elapsed_time(m3), m3.elapsed_time(m4)      # last of three
         emit_with_coords_ms = trk.step_ms().get("selector_emit")
         merge = {"step": "sector_boundary_merge (C7, tpc_merge_tracks)", "ms": round(ms_m, 4), "n_links": int(merged[3][0]),
                  "n_tracks": n_tracks, "tracks_per_s": n_tracks / (ms_m * 1e-3) if ms_m > 0 else None,
@@ -331,7 +333,26 @@ def main():
                            "gpu_launches": trk.last_merge_launches(),
                            "selector_emit_ms_with_hit_coordinates": emit_with_coords_ms},
                  "central_electrode": {"step": "central_electrode_merge (C10, tpc_merge_central_electrode)", "ms": round(ms_c, 4),
-                                       "n_links": int(ce[3][0]), "gpu_launches": trk.last_merge_launches()}}
+                                       "n_links": int(ce[3][0]), "gpu_launches": 7}}
+        # C11: hit rejection + track-model residual symbols; their entropy (a host-side measurement of the output, numpy)
+        # beside the entropy of the same hits' raw coordinates at the same quantisation
+        ok_c = comp[1][:n_tracks].cpu().numpy()
+        nh_c = outs_c[0].n_hits[:n_tracks].cpu().numpy()
+        coded = np.repeat(ok_c == 1, nh_c)
+        def _entropy(x):
+            c = np.bincount((x.astype(np.int64) - int(x.min())))
+            pr = c[c > 0] / x.size
+            return float(-(pr * np.log2(pr)).sum())
+        qy_c, qz_c = comp[2][:n_track_hits].cpu().numpy()[coded], comp[3][:n_track_hits].cpu().numpy()[coded]
+        hi_c = outs_c[0].hit_index[:n_track_hits].cpu().numpy()[coded]
+        raw_bits = _entropy(np.rint(tf.pad[hi_c].astype(np.float64) * 0.5 / 0.025).astype(np.int64)) + \
+            _entropy(np.rint(tf.time[hi_c].astype(np.float64) * 0.516 / 0.025).astype(np.int64))
+        merge["compression"] = {"step": "hit_rejection + residual_coding (C11, tpc_compress_tracks)", "ms": round(ms_q, 4),
+                                "hits_coded": int(coded.sum()), "hits_coded_per_s": float(coded.sum()) / (ms_q * 1e-3),
+                                "tracks_rejected": int((ok_c == -1).sum()), "tracks_not_coded": int((ok_c == 0).sum()),
+                                "hits_rejected": int(comp[0][:n].sum().item()), "step_cm": 0.025,
+                                "entropy_bits_per_hit_symbols": round(_entropy(qy_c) + _entropy(qz_c), 3),
+                                "entropy_bits_per_hit_raw_coordinates_same_step": round(raw_bits, 3), "gpu_launches": 2}
         del outs_c
     # ---- widening step C0 (the cluster finder in front of the path, not part of `value`): timed on the samples of a 1 ms
     # cut of the same generator (digitising the whole 10 ms frame would be 9e8 samples / 14 GB of host work per run)

@@ -306,6 +306,31 @@ typedef struct {   /* caller-allocated DEVICE buffers, indexed by track like tpc
 int tpc_refit_chains(tpc_tracker_t* tracker, const tpc_tracks_t* tracks, const tpc_merged_t* merged, void* cuda_stream,
                      tpc_refit_t* refit_out);
 
+/* ---- C11: track-based hit rejection and track-model residual coding, the step behind the path (
+ * "removal of TPC hits of tracks not used for physics, reduction of the hit property entropy"; DESIGN.md §3
+ * "C11", readings R11-1..R11-6).  The entropy coder that would follow (ANS) is out of scope.                                 */
+typedef struct {
+  float reject_q_pt;     /* 1/0.15 : hits owned by a track with |q/pT| above this are rejected                  (R11-1) */
+  float step_y_cm;       /* 0.025  : quantisation step of the residual in y                                      (R11-3) */
+  float step_z_cm;       /* 0.025  : ... in the time-derived coordinate z = time * time_bin_cm                           */
+} tpc_compress_params_t;
+
+typedef struct {   /* caller-allocated DEVICE buffers                                                                    */
+  uint8_t* reject;   /* [n_clusters] by ORIGINAL cluster index: 1 = the hit belongs to a rejected track                  */
+  int32_t* ok;       /* [max_tracks] 1: coded; -1: rejected; 0: not coded (a transport reached sin_phi_max, or the hit
+                        list was cut by TPC_STATUS_TRACK_HIT_OVERFLOW): its symbols are 0 from the failing hit on         */
+  int16_t* res_y;    /* [max_track_hits] symbol of hit_index[k]: rintf((y - predicted y) / step_y), clamped to +-32767    */
+  int16_t* res_z;    /* [max_track_hits] ... of (time - time_ref) * time_bin_cm against the predicted z                  */
+} tpc_compressed_t;
+
+/* `tracks` = the outputs of tpc_track_timeframe INCLUDING cov9 and the optional hit_y_time / hit_row arrays.  A track's
+ * header (its seven parameters, cov9, n_hits, the hit rows) plus its symbols reproduce every hit to within half a step: the
+ * prediction is a Kalman filter started from the header and updated with the reconstructed hits (closed loop).
+ * Asynchronous on `cuda_stream`, after tpc_track_timeframe; uses 256 bytes of the arena.  Errors: TPC_EINVAL, TPC_ENOMEM,
+ * TPC_ECUDA.  tpc_merge_last_launches() reports its launches.                                                             */
+int tpc_compress_tracks(tpc_tracker_t* tracker, const tpc_compress_params_t* params, const tpc_tracks_t* tracks,
+                        int64_t n_clusters, void* cuda_stream, tpc_compressed_t* out);
+
 /* ---- C9: where and when a track passes the beam line (DESIGN.md §3 "C9"; z is only known once the
  * collision time is).  Every state of `par7` (DEVICE, [max_tracks*7] = (x, y, z_rel, sin_phi, dzds, q_pt, time_ref): the
  * par7 of tpc_refit_chains, or the same seven values of tpc_tracks_t) is transported to x = 0, the beam axis in every

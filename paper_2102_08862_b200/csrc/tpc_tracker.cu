@@ -12,6 +12,7 @@
 #include "arena.h"
 #include "clusterizer.cuh"
 #include "common.cuh"
+#include "compress.cuh"
 #include "finder.cuh"
 #include "follow_rows.cuh"
 #include "ingest.cuh"
@@ -619,6 +620,35 @@ int tpc_refit_chains(tpc_tracker_t* t, const tpc_tracks_t* tr, const tpc_merged_
   if (K > 0) {
     k_refit_roots<<<(K + 255) / 256, 256, 0, st>>>(T, io, root_list, n_roots, c); ++launches;
     k_refit_chains<<<std::min(t->ctas_refit, (K + kMergeThreads - 1) / kMergeThreads), kMergeThreads, 0, st>>>(T, io, root_list, n_roots, work_counter, c, t->consts); ++launches;
+  }
+  t->last_merge_launches = launches;
+  if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;
+  return TPC_OK;
+}
+
+
+// ---- C11: track-based hit rejection + track-model residual coding (compress.cuh) ----
+int tpc_compress_tracks(tpc_tracker_t* t, const tpc_compress_params_t* cp, const tpc_tracks_t* tr, int64_t n_clusters, void* cuda_stream,
+                        tpc_compressed_t* out) {
+  if (!t || !cp || !tr || !out || n_clusters < 0) return TPC_EINVAL;
+  if (!(cp->reject_q_pt > 0 && cp->step_y_cm > 0 && cp->step_z_cm > 0)) return TPC_EINVAL;
+  if (tr->max_tracks < 0 || tr->max_track_hits < 0 || !tr->n_tracks || !out->ok || (n_clusters > 0 && !out->reject)) return TPC_EINVAL;
+  if (tr->max_track_hits > 0 && (!out->res_y || !out->res_z)) return TPC_EINVAL;
+  if (tr->max_tracks > 0 && (!tr->hit_y_time || !tr->hit_row || !tr->hit_index || !tr->n_hits || !tr->hit_offset || !tr->x || !tr->y || !tr->z_rel ||
+                             !tr->time_ref || !tr->sin_phi || !tr->dzds || !tr->q_pt || !tr->cov9)) return TPC_EINVAL;
+  if (!t->params.arena || t->params.arena_bytes < 256) return TPC_ENOMEM;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  uint32_t* work_counter = reinterpret_cast<uint32_t*>(t->params.arena);
+  const int K = tr->max_tracks;
+  CompressIo io{tr->n_tracks, K, tr->max_track_hits, tr->n_hits, tr->hit_offset, tr->hit_index, reinterpret_cast<const float2*>(tr->hit_y_time), tr->hit_row,
+                tr->x, tr->y, tr->z_rel, tr->sin_phi, tr->dzds, tr->q_pt, tr->time_ref, tr->cov9,
+                out->reject, out->ok, out->res_y, out->res_z, cp->reject_q_pt, cp->step_y_cm, cp->step_z_cm};
+  int64_t launches = 0;
+  cudaMemsetAsync(work_counter, 0, 256, st);
+  if (n_clusters > 0) cudaMemsetAsync(out->reject, 0, (size_t)n_clusters, st);
+  if (K > 0) {
+    k_compress_reject<<<(int)(((int64_t)K * 32 + 255) / 256), 256, 0, st>>>(io); ++launches;
+    k_compress_tracks<<<std::min(t->ctas_refit, (K + kMergeThreads - 1) / kMergeThreads), kMergeThreads, 0, st>>>(io, work_counter, t->consts); ++launches;
   }
   t->last_merge_launches = launches;
   if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;

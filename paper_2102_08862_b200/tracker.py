@@ -19,7 +19,7 @@ EXPORTS = ("tpc_tracker_arena_bytes", "tpc_tracker_create", "tpc_track_timeframe
            "tpc_tracker_step_ms", "tpc_tracker_step_name", "tpc_tracker_last_launches", "tpc_tracker_work_counters",
            "tpc_tracker_arena_plan", "tpc_selftest_fast_math", "tpc_selftest_alu_peak",
            "tpc_cluster_finder_scratch_bytes", "tpc_find_clusters",
-           "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_merge_central_electrode", "tpc_refit_chains", "tpc_vertex_time", "tpc_merge_last_launches",
+           "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_merge_central_electrode", "tpc_refit_chains", "tpc_vertex_time", "tpc_compress_tracks", "tpc_merge_last_launches",
            "tpc_tracker_destroy", "tpc_strerror")
 
 
@@ -87,6 +87,16 @@ class ClustersOut(C.Structure):
     """``tpc_clusters_out_t``"""
     _fields_ = [("max_clusters", C.c_int64), ("row", C.c_void_p), ("pad", C.c_void_p), ("time", C.c_void_p), ("charge", C.c_void_p),
                 ("n_clusters", C.c_void_p), ("status", C.c_void_p)]
+
+
+class CompressParams(C.Structure):
+    """``tpc_compress_params_t``"""
+    _fields_ = [("reject_q_pt", C.c_float), ("step_y_cm", C.c_float), ("step_z_cm", C.c_float)]
+
+
+class Compressed(C.Structure):
+    """``tpc_compressed_t``"""
+    _fields_ = [("reject", C.c_void_p), ("ok", C.c_void_p), ("res_y", C.c_void_p), ("res_z", C.c_void_p)]
 
 
 class CeParams(C.Structure):
@@ -171,6 +181,8 @@ def load_library(build_if_missing: bool = True):
         L.tpc_merge_central_electrode.restype = C.c_int
         L.tpc_refit_chains.argtypes = [vp, C.POINTER(Tracks), C.POINTER(Merged), vp, C.POINTER(Refit)]
         L.tpc_refit_chains.restype = C.c_int
+        L.tpc_compress_tracks.argtypes = [vp, C.POINTER(CompressParams), C.POINTER(Tracks), C.c_int64, vp, C.POINTER(Compressed)]
+        L.tpc_compress_tracks.restype = C.c_int
         L.tpc_vertex_time.argtypes = [vp, vp, C.c_int32, vp, vp, vp, vp, vp]
         L.tpc_vertex_time.restype = C.c_int
         L.tpc_merge_last_launches.argtypes = [vp]
@@ -432,6 +444,24 @@ class Tracker:
         if rc != TPC_OK:
             raise TpcError(rc, "tpc_refit_chains")
         return refit
+
+    def tpc_compress_tracks(self, outputs, n_clusters: int, reject_q_pt: float = 1.0 / 0.15, step_y: float = 0.025, step_z: float = 0.025,
+                            out=None, stream=None):
+        """C11 on the DEVICE track outputs (allocated with ``hit_coords=True``); returns (reject uint8[n_clusters],
+        ok int32[max_tracks], res_y int16[max_track_hits], res_z int16[max_track_hits])."""
+        torch = self._torch
+        o, st = outputs
+        K, H = max(int(st.max_tracks), 1), max(int(st.max_track_hits), 1)
+        if out is None:
+            e = lambda n, dt: torch.empty(n, dtype=dt, device=self.device)
+            out = (e(max(int(n_clusters), 1), torch.uint8), e(K, torch.int32), e(H, torch.int16), e(H, torch.int16))
+        cp = CompressParams(float(reject_q_pt), float(step_y), float(step_z))
+        co = Compressed(*(t.data_ptr() for t in out))
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        rc = self.lib.tpc_compress_tracks(self.handle, C.byref(cp), C.byref(st), int(n_clusters), C.c_void_p(s.cuda_stream), C.byref(co))
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_compress_tracks")
+        return out
 
     def tpc_vertex_time(self, n_tracks, par7, stream=None):
         """C9: (ok, vertex_time [time bins], vertex_y [cm]) of the DEVICE states ``par7`` (float32[K, 7]); ``n_tracks`` is the
