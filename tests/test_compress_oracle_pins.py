@@ -42,15 +42,17 @@ def _entropy(x):
     return float(-(pr * np.log2(pr)).sum())
 
 
-@pytest.mark.parametrize("step", [0.025, 0.01, 0.1])
-def test_QR_decoder_reproduces_every_hit_within_half_a_step(step):
+@pytest.mark.parametrize("step,step_z", [(0.025, 0.025), (0.01, 0.04), (0.1, 0.03)])
+def test_QR_decoder_reproduces_every_hit_within_half_a_step(step, step_z):
     tf, g, p, res = _tracked(1, 1)
-    rej, ok, qy, qz = oracle.compress_tracks(g, p, tf.row, tf.pad, tf.time, res, step_y=step, step_z=step)
+    rej, ok, qy, qz = oracle.compress_tracks(g, p, tf.row, tf.pad, tf.time, res, step_y=step, step_z=step_z)
     hr, y, z = _hit_truth(tf, res)
-    yd, zd = oracle.decompress_tracks(g, p, res, hr, ok, qy, qz, step_y=step, step_z=step)
+    yd, zd = oracle.decompress_tracks(g, p, res, hr, ok, qy, qz, step_y=step, step_z=step_z)
     keep = np.repeat(ok == 1, res.tr_n_hits)
     assert keep.sum() > 6e5 and (ok == 0).sum() < 0.005 * len(ok)
-    assert np.max(np.abs(yd - y)[keep]) <= 0.5 * step * 1.001 + 1e-5 and np.max(np.abs(zd - z)[keep]) <= 0.5 * step * 1.001 + 1e-5
+    assert np.max(np.abs(yd - y)[keep]) <= 0.5 * step * 1.001 + 1e-5 and np.max(np.abs(zd - z)[keep]) <= 0.5 * step_z * 1.001 + 1e-5
+    # the symbols scale with their OWN step: spread (in cm) of the coded residuals is the same whatever the steps
+    assert 0.05 < qy[keep].std() * step < 0.2 and 0.08 < qz[keep].std() * step_z < 0.3
     assert np.all(np.isnan(yd[~keep]))
     assert np.abs(qy).max() < 32767 and np.abs(qz).max() < 32767
 

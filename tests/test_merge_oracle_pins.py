@@ -345,3 +345,22 @@ def test_CEI_invariants_CEP_order_independence_and_purity_with_noise():
     s2 = np.where(r2.next >= 0, res.tr_seed[perm][np.maximum(r2.next, 0)], -1)
     np.testing.assert_array_equal(s1[perm], s2)
     np.testing.assert_array_equal(r.t_ce[perm], r2.t_ce)
+
+
+def test_MD_every_term_of_the_match_distance_decides():
+    """d2 = dy^2 wy + dz^2 wz + ds^2 ws + dk^2 wk: two candidates B1, B2 that differ from the extrapolated A in ONE quantity
+    only (B2 closer); whichever term it is, A must pick B2 -- and B1 when the roles are swapped."""
+    p = M.default_merge_params(36)
+    base = _pair_across_boundary(state_row_b=101, first_row_b=101)
+    par_a, par_b = base[4][0], base[4][1]
+    for col, d1, d2 in ((1, 0.9, 0.3), (2, 0.9, 0.3), (3, 0.03, 0.01), (5, 0.3, 0.1)):        # y, z, sin phi, q/pT
+        for swap in (False, True):
+            b1, b2 = par_b.copy(), par_b.copy()
+            b1[col] += d1
+            b2[col] += d2
+            if swap:
+                b1, b2 = b2, b1
+            par = np.array([par_a, b1, b2], np.float32)
+            r = M.merge(p, [11, 22, 33], [0, 1, 1], [40, 101, 101], [99, 140, 140], par)
+            assert r.next[0] == (1 if swap else 2), (col, swap, r.next)
+            assert r.n_links == 1 and r.prev[r.next[0]] == 0

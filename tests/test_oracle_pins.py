@@ -529,3 +529,88 @@ def test_P4_seed_state_is_direction_cosines_of_the_first_two_hits():
     assert abs(par[3] - 0.6) < 2e-4           # pads are fp32: the line is reproduced to ~1e-5 cm
     assert abs(par[4] - 0.8) < 2e-4           # dz/dx (= 1.0) here would be the mistake
     assert par[6] == time[1]
+
+
+def test_N1_tie_between_equal_lower_candidates_goes_to_the_lower_original_index():
+    """C2's second tie level: the same upper hit, two identical candidates in the LOWER row."""
+    rows = np.array([10, 10, 11, 12])
+    base = clusters_from_xyz(rows, [0.0, 0.0, 0.1, 0.2], [50.0, 50.0, 50.5, 51.0])
+    for perm in ([0, 1, 2, 3], [3, 2, 1, 0], [1, 3, 0, 2]):
+        row, pad, time = (a[perm] for a in base)
+        r = oracle.track(_geom(), oracle.default_params(), row, pad, time)
+        h = perm.index(2)
+        dup = sorted([perm.index(0), perm.index(1)])
+        assert r.up_raw[h] == perm.index(3) and r.down_raw[h] == dup[0]
+
+
+def test_P5_search_tie_goes_to_the_lower_original_index():
+    """C5 search: two identical hits in a followed row (not part of the seed chain): the tracklet takes the lower original
+    index, wherever the two sit in the input."""
+    lower, upper = np.arange(20, 46), np.arange(48, 61)
+    parts = [_line(lower), _line(upper), _line(np.array([50]))]               # row 50 twice
+    row, pad, time = concat(parts)
+    n = row.size
+    for perm in (np.arange(n), np.arange(n)[::-1], np.random.default_rng(4).permutation(n)):
+        r = oracle.track(_geom(), oracle.default_params(), row[perm], pad[perm], time[perm])
+        dup = np.nonzero(row[perm] == 50.0)[0]
+        assert dup.size == 2
+        seed_rows = row[perm][r.tl_seed].astype(int)
+        t = int(np.nonzero(seed_rows == 21)[0][0])                                 # the tracklet seeded in the lower part: it SEARCHES row 50
+        assert r.tl_row_hit[t, 50] == dup.min(), (r.tl_row_hit[t, 50], dup)
+        assert r.tl_row_hit[t, 46] == -1 and r.tl_row_hit[t, 48] >= 0
+
+
+def test_P6_holes_inside_the_collected_range_are_not_searched_again_on_the_way_down():
+    """Reading A13: the down pass refits through the collected hits and searches only BELOW the seed row.  A hit displaced
+    by 0.58 cm sits in a hole of the up pass (window 0.5535 cm one row after a hit); on the way down the last update is two
+    rows away (window 0.607 cm) -- a search there would attach it."""
+    rows = np.concatenate([np.arange(20, 25), np.arange(27, 61)])               # rows 25, 26 empty on the line
+    r, row = _track_one([_line(rows), _line(np.array([25]), dy=0.58)])
+    t = int(np.nonzero(row[r.tl_seed].astype(int) == 21)[0][0])      # the tracklet seeded BELOW the hole: rows 25, 26 are inside its collected range
+    assert r.tl_row_hit[t, 25] == -1 and r.tl_row_hit[t, 26] == -1 and r.tl_n_hits[t] == rows.size
+    # (the tracklet seeded above the hole, at row 28, searches rows 27 .. 0 on its way down and does attach it: window 0.607 cm)
+    t_up = int(np.nonzero(row[r.tl_seed].astype(int) == 28)[0][0])
+    assert r.tl_row_hit[t_up, 25] >= 0
+    # control: the same hit displaced by 0.50 cm IS attached (on the way up, window 0.5535)
+    r2, _ = _track_one([_line(rows), _line(np.array([25]), dy=0.50)])
+    row2 = concat([_line(rows), _line(np.array([25]), dy=0.50)])[0]
+    t2 = int(np.nonzero(row2[r2.tl_seed].astype(int) == 21)[0][0])
+    assert r2.tl_row_hit[t2, 25] >= 0
+
+
+def test_G3_validity_bounds_of_a_cluster_are_half_open_in_pad_and_closed_in_time():
+    """C1: pad in [-0.5, n_pads - 0.5) (pad p covers [p - 0.5, p + 0.5)), time in [0, max_time_bin].  A cluster exactly on a
+    bound is counted or ignored accordingly (the ignored ones are reported in stats)."""
+    tmax = 600.0
+    line = _line(np.arange(30, 70))
+    def n_invalid(pad_value, time_value, row_value=40.0):
+        row = np.concatenate([line[0], [row_value]]).astype(np.float32)
+        pad = np.concatenate([line[1], [pad_value]]).astype(np.float32)
+        time = np.concatenate([line[2], [time_value]]).astype(np.float32)
+        r = oracle.track(_geom(1, tmax), oracle.default_params(), row, pad, time)
+        assert len(r.tr_seed) == 1 and r.tr_n_hits[0] == 40             # the line itself is untouched
+        return int(r.stats["invalid_clusters"])
+    np40 = float(n_pads(40))
+    assert n_invalid(np40 - 0.5, 100.0) == 1                # the upper pad bound is excluded ...
+    assert n_invalid(np.float32(np40 - 0.5) - np.float32(1e-3), 100.0) == 0
+    assert n_invalid(-0.5, 100.0) == 0                      # ... the lower one included
+    assert n_invalid(np.float32(-0.5) - np.float32(1e-3), 100.0) == 1
+    assert n_invalid(10.0, tmax) == 0                       # time == max_time_bin is inside
+    assert n_invalid(10.0, np.nextafter(np.float32(tmax), np.float32(1e9))) == 1
+    assert n_invalid(10.0, 0.0) == 0 and n_invalid(10.0, -1e-3) == 1
+    assert n_invalid(10.0, 100.0, row_value=152.0) == 1     # beyond the single sector
+    assert n_invalid(10.0, 100.0, row_value=40.5) == 1      # not an integer row
+
+
+def test_N4_edge_rows_have_no_links_even_next_to_another_sector():
+    """Reading A5: rows 0 and n_rows - 1 are linkless; a link never crosses into the neighbouring sector (whose row 0 follows
+    row 151 in the sector-row numbering)."""
+    a = _line(np.arange(140, 152))                          # sector 0, up to its last row
+    b = _line(np.arange(0, 12), y_at=float(0.02 * 1.07 * 152), z_at=150.0 + 0.3 * 1.07 * 152)   # sector 1: the SAME line continued, as rows 0..11
+    b = (b[0] + np.float32(152.0), b[1], b[2])
+    row, pad, time = concat([a, b])
+    r = oracle.track(_geom(2, 800.0), oracle.default_params(), row, pad, time)
+    i151 = int(np.nonzero(row == 151.0)[0][0]); i152 = int(np.nonzero(row == 152.0)[0][0])
+    assert r.up_raw[i151] == -1 and r.down_raw[i151] == -1 and r.up_raw[i152] == -1 and r.down_raw[i152] == -1
+    i150 = int(np.nonzero(row == 150.0)[0][0])
+    assert r.up_raw[i150] == i151 and r.down_raw[i150] >= 0   # row 150 does link up to the edge row
