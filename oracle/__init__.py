@@ -88,6 +88,14 @@ def lib():
         L.orc_decompress_tracks.restype = None
         L.orc_rotate_with_cov.argtypes = [C.POINTER(Geometry), C.POINTER(Params), vp, vp, C.c_int32]
         L.orc_rotate_with_cov.restype = C.c_int
+        L.orc_refit_full.argtypes = [C.POINTER(Geometry), C.POINTER(Params), vp, vp, vp, vp, C.c_int64] + [vp] * 12
+        L.orc_refit_full.restype = None
+        L.orc_full_step.argtypes = [C.POINTER(Params), vp, vp, vp, C.c_float]
+        L.orc_full_step.restype = C.c_int
+        L.orc_full_update.argtypes = [vp, vp, C.c_float, C.c_float, C.c_float, C.c_float]
+        L.orc_full_update.restype = None
+        L.orc_full_rotate.argtypes = [C.POINTER(Geometry), C.POINTER(Params), vp, vp, C.c_int32]
+        L.orc_full_rotate.restype = C.c_int
         for nm in ("orc_copy_links", "orc_copy_tracklets", "orc_copy_tracks", "orc_copy_stats", "orc_free",
                    "orc_update", "orc_tables"):
             getattr(L, nm).restype = None
@@ -222,6 +230,50 @@ def rotate_with_cov(geom: Geometry, params: Params, state6, cov9, q: int):
     cv = np.array(cov9, np.float32)
     rc = lib().orc_rotate_with_cov(C.byref(geom), C.byref(params), st.ctypes.data, cv.ctypes.data, int(q))
     return rc == 0, st, cv
+
+
+# C12 material of the drift gas (DESIGN.md §3 C12 reading FF3): (1 / radiation length [1/cm], dE/dx of a minimum-ionising
+# particle [GeV/cm], particle mass [GeV], relative width of the energy loss)
+DEFAULT_FULL_PARAMS = (1.0 / 3.0e4, 1.7e-6, 0.13957, 0.1)
+
+
+def refit_full(geom: Geometry, params: Params, row, pad, time, res: "Result", nxt, prv, full_params=DEFAULT_FULL_PARAMS):
+    """C12: full-covariance refit with material of every chain root.  Returns (ok, chain_hits, chain_pieces, par[n,7], cov[n,15])."""
+    a = lambda v, t: np.ascontiguousarray(v, t)
+    row, pad, time = a(row, np.float32), a(pad, np.float32), a(time, np.float32)
+    nxt, prv = a(nxt, np.int32), a(prv, np.int32)
+    n = int(len(res.tr_seed))
+    ok, ch, cp = np.zeros(n, np.int32), np.zeros(n, np.int32), np.zeros(n, np.int32)
+    rp, rc = np.zeros((n, 7), np.float32), np.zeros((n, 15), np.float32)
+    sec, nh, off = a(res.tr_sector, np.int32), a(res.tr_n_hits, np.int32), a(res.tr_hit_offset, np.int64)
+    hi, par = a(res.tr_hit_index, np.int32), a(res.tr_par, np.float32)
+    f4 = np.array(full_params, np.float32)
+    lib().orc_refit_full(C.byref(geom), C.byref(params), f4.ctypes.data, row.ctypes.data, pad.ctypes.data, time.ctypes.data, n,
+                         sec.ctypes.data, nh.ctypes.data, off.ctypes.data, hi.ctypes.data, par.ctypes.data,
+                         nxt.ctypes.data, prv.ctypes.data, ok.ctypes.data, ch.ctypes.data, cp.ctypes.data,
+                         rp.ctypes.data, rc.ctypes.data)
+    return ok, ch, cp, rp, rc
+
+
+def full_step(params: Params, state6, cov15, xn: float, full_params=DEFAULT_FULL_PARAMS):
+    """One transport + material step of C12 (pins FF-*).  Returns (ok, state6, cov15)."""
+    st, cv, f4 = np.array(state6, np.float32), np.array(cov15, np.float32), np.array(full_params, np.float32)
+    rc = lib().orc_full_step(C.byref(params), f4.ctypes.data, st.ctypes.data, cv.ctypes.data, float(xn))
+    return rc == 0, st, cv
+
+
+def full_rotate(geom: Geometry, params: Params, state6, cov15, q: int):
+    """C12 rotation of state and covariance by q * 20 degrees (pin FF-R).  Returns (ok, state6, cov15)."""
+    st, cv = np.array(state6, np.float32), np.array(cov15, np.float32)
+    rc = lib().orc_full_rotate(C.byref(geom), C.byref(params), st.ctypes.data, cv.ctypes.data, int(q))
+    return rc == 0, st, cv
+
+
+def full_update(state6, cov15, ym: float, zm: float, ry: float, rz: float):
+    """The two scalar updates of C12 with one hit."""
+    st, cv = np.array(state6, np.float32), np.array(cov15, np.float32)
+    lib().orc_full_update(st.ctypes.data, cv.ctypes.data, float(ym), float(zm), float(ry), float(rz))
+    return st, cv
 
 
 DEFAULT_REJECT_QPT, DEFAULT_STEP_Y, DEFAULT_STEP_Z = 1.0 / 0.15, 0.025, 0.025      # DESIGN.md §3 C11 readings R11-1, R11-3

@@ -24,6 +24,8 @@
 // Also holds C8 (orc_refit_chains, further down: refit of the chains linked by the C7 oracle tpc_merge_oracle.cpp), pinned by
 // tests/test_refit_oracle_pins.py: F-J rotation Jacobian vs numerical derivative, F-H noise-free helices, F-N resolution and
 // pull width against generator truth, F-I bookkeeping.
+// Also holds C11 (orc_compress_tracks, pins Q-* in tests/test_compress_oracle_pins.py) and C12 (orc_refit_full: full 5x5
+// covariance, multiple scattering, energy loss; pins FF-* in tests/test_fullfit_oracle_pins.py).
 // Parity unpinned (no external truth exists): absolute fitted values on noisy data.
 #include <algorithm>
 #include <chrono>
@@ -650,6 +652,236 @@ void orc_decompress_tracks(const orc_geometry* gp, const orc_params* pp, float s
       update(S, yq, zq, D.ry, D.rz);
     }
   }
+}
+
+// ---- C12: refit with the full 5x5 covariance, multiple scattering and energy loss ("Full 5x5
+// covariance with multiple scattering / energy loss"; PAPER.md L37 (§2): "future improvement of the tracking efficiency, which
+// will require the fit of more tracks and more attached hits").  The paper gives no listing: the definitions are readings of
+// this build (FF1..FF7, DESIGN.md §3 "C12").  One inward Kalman pass over every ROOT of C7's chains -- single tracks too --
+// in C8's hit order and with C8's start (FF1); state (y, z, s, t, k) at x, covariance the full symmetric 5x5 matrix, stored as
+// its lower triangle in the order (yy | zy zz | sy sz ss | ty tz ts tt | ky kz ks kt kk).
+//   step(S, x_row):                                              # transport + material, FAIL as in C5
+//     state part and dx, T, rq, dS, fa, e, fb exactly as the C5 transport
+//     gm = t * (T / rq);  zs = gm * fa;  zk = gm * fb             # dz/ds, dz/dk to first order in the chord (FF2)
+//     F = rows  y: (1, 0, fa, 0, fb)   z: (0, 1, zs, dS, zk)   s: (0, 0, 1, 0, e)   t, k: unit
+//     A = F P:     A[y][j] = P[y][j] + fa*P[s][j] + fb*P[k][j];  A[z][j] = P[z][j] + zs*P[s][j] + dS*P[t][j] + zk*P[k][j];
+//                  A[s][j] = P[s][j] + e*P[k][j];  rows t, k unchanged
+//     P = A F^T:   P[i][y] = A[i][y] + fa*A[i][s] + fb*A[i][k];  P[i][z] = A[i][z] + zs*A[i][s] + dS*A[i][t] + zk*A[i][k];
+//                  P[i][s] = A[i][s] + e*A[i][k];  columns t, k = A's                      (lower triangle only)
+//     material of the step (FF3..FF6), with s the NEW sin phi and t, k unchanged by the transport:
+//       tt1 = 1 + t*t;  Lp = fabsf(dS) * sqrtf(tt1);  ip2 = (k*k) / tt1;  ib2 = 1 + m2*ip2;  ibp2 = ip2 * ib2
+//       th2 = (ms2 * ibp2) * (Lp * inv_x0)                         # Highland theta0^2 without the log term, ms2 = 0.0136^2
+//       P[ss] += th2 * ((1 - s*s) * tt1);  P[tt] += th2 * (tt1*tt1);  tk = t*k;  P[kt] += th2 * (tk * tt1);  P[kk] += th2 * (tk*tk)
+//       dl = ((dedx * ib2) * Lp) * sqrtf(ibp2)                     # dE / (beta p), dE/dx = dedx_mip / beta^2
+//       k = k * (1 - dl)                                           # inward = against the flight: the momentum comes back
+//       ek = (k * dl) * eloss_sigma;  P[kk] += ek * ek             # straggling (k already corrected)
+//   update1(S, i, meas, r):  scalar measurement of component i (0 = y, 1 = z)
+//       col[j] = P[j][i] (j = 0..4);  w = 1 / (col[i] + r);  res = meas - S[i];  K[j] = col[j] * w
+//       S[j] = S[j] + K[j]*res;  P[j][l] = P[j][l] - K[j]*col[l]   (l <= j)
+//   per hit:  step(S, x_row);  update1(S, 0, y(hit), r_y);  update1(S, 1, (time - time_ref_p)*Z, r_z)
+//   boundary: C8's rotation of (x, y, s); the row and column s of P are multiplied by J (ss by J twice) (FF7); z re-referenced.
+// Output per root: ok (1 fitted, -1 FAIL, 0 not a root), chain_hits, chain_pieces, par7, and the 15 covariance values.
+namespace {
+struct FullParams { float inv_x0, dedx_mip, mass, eloss_sigma; };
+struct FullState { float x, v[5]; float P[5][5]; };     // v = (y, z, s, t, k); P kept as a full symmetric matrix
+inline int tri(int i, int j) { return i >= j ? i * (i + 1) / 2 + j : j * (j + 1) / 2 + i; }
+
+// mass^2 and the squared Highland constant (13.6 MeV)^2 in GeV^2, derived in double and rounded once
+void full_consts(const FullParams& fp, float& m2, float& ms2) {
+  m2 = (float)((double)fp.mass * (double)fp.mass);
+  ms2 = (float)(0.0136 * 0.0136);
+}
+
+bool full_step(FullState& S, float xn, float cB, float sin_phi_max, const FullParams& fp, float m2, float ms2) {
+  const float s0 = S.v[2], t = S.v[3], k0 = S.v[4];
+  const float dx = xn - S.x;
+  const float kc = cB * k0;
+  const float sn = s0 + kc * dx;
+  if (!(std::fabs(s0) < sin_phi_max && std::fabs(sn) < sin_phi_max)) return false;
+  const float c = std::sqrt(1.0f - s0 * s0);
+  const float cn = std::sqrt(1.0f - sn * sn);
+  const float ss = s0 + sn;
+  const float cc = c + cn;
+  const float icc = 1.0f / cc;
+  const float T = ss * icc;
+  const float q = 1.0f + T * T;
+  const float rq = std::sqrt(q);
+  const float u = kc * dx;
+  const float a = (u * u) * q;
+  const float dS = (dx * rq) * (1.0f + a * (0.041666668f + a * (0.0046875f + a * 0.00069754466f)));
+  const float g0 = (1.0f + T * (s0 / c)) * icc;
+  const float g1 = (1.0f + T * (sn / cn)) * icc;
+  const float fa = dx * (g0 + g1);
+  const float e = cB * dx;
+  const float fb = (dx * g1) * e;
+  const float gm = t * (T / rq);
+  const float zs = gm * fa;
+  const float zk = gm * fb;
+  S.v[0] = S.v[0] + dx * T;
+  S.v[1] = S.v[1] + t * dS;
+  S.v[2] = sn;
+  S.x = xn;
+  float A[5][5];
+  for (int j = 0; j < 5; ++j) {
+    A[0][j] = S.P[0][j] + fa * S.P[2][j] + fb * S.P[4][j];
+    A[1][j] = S.P[1][j] + zs * S.P[2][j] + dS * S.P[3][j] + zk * S.P[4][j];
+    A[2][j] = S.P[2][j] + e * S.P[4][j];
+    A[3][j] = S.P[3][j];
+    A[4][j] = S.P[4][j];
+  }
+  float B[5][5];
+  for (int i = 0; i < 5; ++i) {
+    B[i][0] = A[i][0] + fa * A[i][2] + fb * A[i][4];
+    B[i][1] = A[i][1] + zs * A[i][2] + dS * A[i][3] + zk * A[i][4];
+    B[i][2] = A[i][2] + e * A[i][4];
+    B[i][3] = A[i][3];
+    B[i][4] = A[i][4];
+  }
+  for (int i = 0; i < 5; ++i) for (int j = 0; j <= i; ++j) { S.P[i][j] = B[i][j]; S.P[j][i] = B[i][j]; }   // the lower triangle is the result
+  // material
+  const float tt1 = 1.0f + t * t;
+  const float Lp = std::fabs(dS) * std::sqrt(tt1);
+  const float ip2 = (k0 * k0) / tt1;
+  const float ib2 = 1.0f + m2 * ip2;
+  const float ibp2 = ip2 * ib2;
+  const float th2 = (ms2 * ibp2) * (Lp * fp.inv_x0);
+  S.P[2][2] = S.P[2][2] + th2 * ((1.0f - sn * sn) * tt1);
+  S.P[3][3] = S.P[3][3] + th2 * (tt1 * tt1);
+  const float tk = t * k0;
+  S.P[4][3] = S.P[4][3] + th2 * (tk * tt1); S.P[3][4] = S.P[4][3];
+  S.P[4][4] = S.P[4][4] + th2 * (tk * tk);
+  const float dl = ((fp.dedx_mip * ib2) * Lp) * std::sqrt(ibp2);
+  S.v[4] = k0 * (1.0f - dl);
+  const float ek = (S.v[4] * dl) * fp.eloss_sigma;
+  S.P[4][4] = S.P[4][4] + ek * ek;
+  return true;
+}
+
+void full_update1(FullState& S, int i, float meas, float r) {
+  float col[5], K[5];
+  for (int j = 0; j < 5; ++j) col[j] = S.P[j][i];
+  const float w = 1.0f / (col[i] + r);
+  const float res = meas - S.v[i];
+  for (int j = 0; j < 5; ++j) K[j] = col[j] * w;
+  for (int j = 0; j < 5; ++j) S.v[j] = S.v[j] + K[j] * res;
+  for (int j = 0; j < 5; ++j) for (int l = 0; l <= j; ++l) { S.P[j][l] = S.P[j][l] - K[j] * col[l]; S.P[l][j] = S.P[j][l]; }
+}
+
+void full_reset(FullState& S, const orc_params& p) {
+  for (int i = 0; i < 5; ++i) for (int j = 0; j < 5; ++j) S.P[i][j] = 0.0f;
+  S.P[0][0] = p.c0_y2; S.P[1][1] = p.c0_z2; S.P[2][2] = p.c0_s2; S.P[3][3] = p.c0_t2; S.P[4][4] = p.c0_k2;
+}
+
+bool full_rotate(FullState& S, float qd, float Cd, float Sd, float sin_phi_max) {
+  const float s0 = S.v[2];
+  const float cs = std::sqrt(1.0f - s0 * s0);
+  const float J = Cd + qd * ((s0 / cs) * Sd);
+  const float x1 = S.x * Cd + qd * (S.v[0] * Sd);
+  const float y1 = S.v[0] * Cd - qd * (S.x * Sd);
+  const float s1 = s0 * Cd - qd * (cs * Sd);
+  if (!(std::fabs(s1) < sin_phi_max)) return false;
+  S.x = x1; S.v[0] = y1; S.v[2] = s1;
+  for (int j = 0; j < 5; ++j) if (j != 2) { S.P[2][j] = S.P[2][j] * J; S.P[j][2] = S.P[2][j]; }
+  S.P[2][2] = (S.P[2][2] * J) * J;
+  return true;
+}
+}  // namespace
+
+void orc_refit_full(const orc_geometry* gp, const orc_params* pp, const float* full4, const float* row, const float* pad,
+                    const float* time, int64_t n_tracks, const int32_t* sector, const int32_t* n_hits, const int64_t* hit_offset,
+                    const int32_t* hit_index, const float* par, const int32_t* next, const int32_t* prev,
+                    int32_t* ok, int32_t* chain_hits, int32_t* chain_pieces, float* rpar, float* rcov15) {
+  const Derived D = derive(*gp, *pp);
+  const FullParams fp{full4[0], full4[1], full4[2], full4[3]};
+  float m2, ms2;
+  full_consts(fp, m2, ms2);
+  const double T = (double)gp->tan_half_sector;
+  const float Cd = (float)((1.0 - T * T) / (1.0 + T * T)), Sd = (float)(2.0 * T / (1.0 + T * T));
+  const int nr = gp->n_rows;
+  for (int64_t i = 0; i < n_tracks; ++i) {
+    ok[i] = 0; chain_hits[i] = n_hits[i]; chain_pieces[i] = 1;
+    for (int k = 0; k < 7; ++k) rpar[7 * i + k] = par[7 * i + k];
+    for (int k = 0; k < 15; ++k) rcov15[15 * i + k] = 0.0f;
+    if (prev[i] >= 0) continue;
+    std::vector<int64_t> pieces;
+    for (int64_t p = i; p >= 0; p = next[p]) pieces.push_back(p);
+    int32_t total = 0;
+    for (int64_t p : pieces) total += n_hits[p];
+    chain_hits[i] = total; chain_pieces[i] = (int32_t)pieces.size();
+    const int64_t pm = pieces.back();
+    const float* q = par + 7 * pm;
+    FullState S;
+    S.x = q[0]; S.v[0] = q[1]; S.v[1] = q[2]; S.v[2] = q[3]; S.v[3] = q[4]; S.v[4] = q[5];
+    bool good = n_hits[pm] > 0;
+    if (good) {     // FF1: to the outermost hit with the plain C5 transport (no material), then the reset covariance
+      State S0{q[0], q[1], q[2], q[3], q[4], q[5], 0, 0, 0, 0, 0, 0, 0, 0, 0};
+      const int32_t h = hit_index[hit_offset[pm] + n_hits[pm] - 1];
+      good = transport(S0, D.xr[(int)row[h] % nr], D.cB, pp->sin_phi_max);
+      S.x = S0.x; S.v[0] = S0.y; S.v[1] = S0.z; S.v[2] = S0.s;
+    }
+    full_reset(S, *pp);
+    for (int ip = (int)pieces.size() - 1; ip >= 0 && good; --ip) {
+      const int64_t p = pieces[ip];
+      const float tref = par[7 * p + 6];
+      for (int64_t j = hit_offset[p] + n_hits[p] - 1; j >= hit_offset[p] && good; --j) {
+        const int32_t h = hit_index[j];
+        const int r = (int)row[h] % nr;
+        good = full_step(S, D.xr[r], D.cB, pp->sin_phi_max, fp, m2, ms2);
+        if (!good) break;
+        full_update1(S, 0, (pad[h] - D.cr[r]) * D.P, D.ry);
+        full_update1(S, 1, (time[h] - tref) * D.Z, D.rz);
+      }
+      if (good && ip > 0) {
+        const int64_t pin = pieces[ip - 1];
+        const float sg = ((sector[p] % 18) == ((sector[pin] % 18) + 1) % 18) ? 1.0f : -1.0f;
+        if (!full_rotate(S, -sg, Cd, Sd, pp->sin_phi_max)) { good = false; break; }
+        S.v[1] = S.v[1] + (tref - par[7 * pin + 6]) * D.Z;
+      }
+    }
+    if (good) {
+      ok[i] = 1;
+      float* o = rpar + 7 * i;
+      o[0] = S.x; o[1] = S.v[0]; o[2] = S.v[1]; o[3] = S.v[2]; o[4] = S.v[3]; o[5] = S.v[4];
+      for (int a = 0; a < 5; ++a) for (int b = 0; b <= a; ++b) rcov15[15 * i + tri(a, b)] = S.P[a][b];
+    } else {
+      ok[i] = -1;
+    }
+  }
+}
+
+// One step / one update of C12 on their own (pins FF-*): st6 = (x, y, z, s, t, k), cov15 = lower triangle.
+int orc_full_step(const orc_params* p, const float* full4, float* st, float* cov15, float xn) {
+  const FullParams fp{full4[0], full4[1], full4[2], full4[3]};
+  float m2, ms2;
+  full_consts(fp, m2, ms2);
+  FullState S;
+  S.x = st[0]; for (int j = 0; j < 5; ++j) S.v[j] = st[1 + j];
+  for (int a = 0; a < 5; ++a) for (int b = 0; b < 5; ++b) S.P[a][b] = cov15[tri(a, b)];
+  const bool ok = full_step(S, xn, p->inv_R_per_qpt, p->sin_phi_max, fp, m2, ms2);
+  st[0] = S.x; for (int j = 0; j < 5; ++j) st[1 + j] = S.v[j];
+  for (int a = 0; a < 5; ++a) for (int b = 0; b <= a; ++b) cov15[tri(a, b)] = S.P[a][b];
+  return ok ? 0 : 1;
+}
+// C12 rotation on its own (pin FF-R): q = +1 / -1.  Returns 0, or 1 when |s'| >= sin_phi_max (state unchanged).
+int orc_full_rotate(const orc_geometry* g, const orc_params* p, float* st, float* cov15, int32_t q) {
+  const double T = (double)g->tan_half_sector;
+  const float Cd = (float)((1.0 - T * T) / (1.0 + T * T)), Sd = (float)(2.0 * T / (1.0 + T * T));
+  FullState S;
+  S.x = st[0]; for (int j = 0; j < 5; ++j) S.v[j] = st[1 + j];
+  for (int a = 0; a < 5; ++a) for (int b = 0; b < 5; ++b) S.P[a][b] = cov15[tri(a, b)];
+  const bool ok = full_rotate(S, q >= 0 ? 1.0f : -1.0f, Cd, Sd, p->sin_phi_max);
+  st[0] = S.x; for (int j = 0; j < 5; ++j) st[1 + j] = S.v[j];
+  for (int a = 0; a < 5; ++a) for (int b = 0; b <= a; ++b) cov15[tri(a, b)] = S.P[a][b];
+  return ok ? 0 : 1;
+}
+void orc_full_update(float* st, float* cov15, float ym, float zm, float ry, float rz) {
+  FullState S;
+  S.x = st[0]; for (int j = 0; j < 5; ++j) S.v[j] = st[1 + j];
+  for (int a = 0; a < 5; ++a) for (int b = 0; b < 5; ++b) S.P[a][b] = cov15[tri(a, b)];
+  full_update1(S, 0, ym, ry);
+  full_update1(S, 1, zm, rz);
+  for (int j = 0; j < 5; ++j) st[1 + j] = S.v[j];
+  for (int a = 0; a < 5; ++a) for (int b = 0; b <= a; ++b) cov15[tri(a, b)] = S.P[a][b];
 }
 
 // ---- hooks for the pins (K1..K3, G1): the same functions the tracker uses, callable one at a time ----
