@@ -306,9 +306,9 @@ def main():
     # ---- widening step C7 (sector-boundary merging of the tracks, not part of `value`): timed on its own ----
     merge = None
     if cfg.n_sectors >= 18:
-        m0, m1, m2, m3, m4 = (torch.cuda.Event(enable_timing=True) for _ in range(5))
-        merged = refit = ce = comp = None
-        ms_m = ms_r = ms_c = ms_q = 0.0
+        m0, m1, m2, m3, m4, m5 = (torch.cuda.Event(enable_timing=True) for _ in range(6))
+        merged = refit = ce = comp = full = None
+        ms_m = ms_r = ms_c = ms_q = ms_f = 0.0
         outs_c = trk.alloc_outputs(n, hit_coords=True)      # C8 reads the hits' coordinates from two optional emit outputs
         for _ in range(3):
             with torch.cuda.stream(stream):
@@ -322,8 +322,10 @@ def main():
                 m3.record(stream)
                 comp = trk.tpc_compress_tracks(outs_c, n, out=comp, stream=stream)
                 m4.record(stream)
+                full = trk.tpc_refit_full(outs_c, merged, out=full, stream=stream)
+                m5.record(stream)
             stream.synchronize()
-            ms_m, ms_r, ms_c, ms_q = m0.elapsed_time(m1), m1.elapsed_time(m2), m2.elapsed_time(m3), m3.elapsed_time(m4)      # last of three
+            ms_m, ms_r, ms_c, ms_q, ms_f = m0.elapsed_time(m1), m1.elapsed_time(m2), m2.elapsed_time(m3), m3.elapsed_time(m4), m4.elapsed_time(m5)      # last of three
         emit_with_coords_ms = trk.step_ms().get("selector_emit")
         merge = {"step": "sector_boundary_merge (C7, tpc_merge_tracks)", "ms": round(ms_m, 4), "n_links": int(merged[3][0]),
                  "n_tracks": n_tracks, "tracks_per_s": n_tracks / (ms_m * 1e-3) if ms_m > 0 else None,
@@ -334,6 +336,16 @@ def main():
                            "selector_emit_ms_with_hit_coordinates": emit_with_coords_ms},
                  "central_electrode": {"step": "central_electrode_merge (C10, tpc_merge_central_electrode)", "ms": round(ms_c, 4),
                                        "n_links": int(ce[3][0]), "gpu_launches": 7}}
+        # C12: every chain root refitted with the full 5x5 covariance and the material of the gas.  ALU-bound like C5: 371 lane-
+        # instructions per hit with §6's convention (division, square root = 8): step 179 + 5 div + 5 sqrt = 259, two scalar
+        # updates 94 + 2 div = 110, measurement 2
+        hits_full = int(full[1][full[0] == 1].sum())
+        merge["full_refit"] = {"step": "full_covariance_refit (C12, tpc_refit_full)", "ms": round(ms_f, 4),
+                               "n_roots_refitted": int((full[0] == 1).sum()), "n_roots_failed": int((full[0] == -1).sum()),
+                               "hits_refitted": hits_full, "hits_per_s": hits_full / (ms_f * 1e-3) if ms_f > 0 else None,
+                               "bound": "alu", "lane_inst_per_hit": 371,
+                               "achieved_T_lane_inst_per_s": round(371 * hits_full / (ms_f * 1e-3) / 1e12, 3) if ms_f > 0 else None,
+                               "gpu_launches": 2}
         # C11: hit rejection + track-model residual symbols; their entropy (a host-side measurement of the output, numpy)
         # beside the entropy of the same hits' raw coordinates at the same quantisation
         ok_c = comp[1][:n_tracks].cpu().numpy()

@@ -10,7 +10,7 @@
  *   tpc_tracker_create(geometry, params), tpc_track_timeframe(clusters, n, stream, tracks_out),
  *   tpc_tracker_destroy.  The exact operations (steps C1..C6) are defined in DESIGN.md §3.
  * After the hot path, three widening steps are separate calls on the tracker's outputs:
- *   tpc_merge_tracks (C7), tpc_refit_chains (C8), tpc_vertex_time (C9); DESIGN.md §3 defines them too.
+ *   tpc_merge_tracks (C7), tpc_refit_chains (C8), tpc_vertex_time (C9), ... tpc_refit_full (C12); DESIGN.md §3 defines them too.
  *
  * Conventions
  *   - Plain C, no torch types.  Every pointer is marked DEVICE or HOST.
@@ -330,6 +330,35 @@ typedef struct {   /* caller-allocated DEVICE buffers                           
  * TPC_ECUDA.  tpc_merge_last_launches() reports its launches.                                                             */
 int tpc_compress_tracks(tpc_tracker_t* tracker, const tpc_compress_params_t* params, const tpc_tracks_t* tracks,
                         int64_t n_clusters, void* cuda_stream, tpc_compressed_t* out);
+
+/* ---- C12: refit with the full 5x5 covariance, multiple scattering and energy loss (§2:
+ * the planned "improvement of the tracking efficiency, which will require the fit of more tracks and more attached hits";
+ * DESIGN.md §3 "C12", readings FF1..FF7).  One inward Kalman pass over the hits of every ROOT of the chains of tpc_merge_tracks,
+ * single tracks included: state (y, z, sin_phi, dzds, q_pt) at x, the full symmetric covariance, process noise of multiple
+ * scattering (Highland's theta0 without the logarithm) and the mean energy loss dE/dx = dedx_mip / beta^2 of the drift gas.   */
+typedef struct {
+  float inv_x0_per_cm;        /* 1 / radiation length of the gas, e.g. 1 / 3e4; >= 0                                          */
+  float dedx_mip_gev_per_cm;  /* stopping power of a minimum-ionising particle, e.g. 1.7e-6; >= 0                             */
+  float mass_gev;             /* mass hypothesis, e.g. 0.13957 (pion); >= 0                                                   */
+  float eloss_sigma;          /* relative width of the energy loss (straggling), e.g. 0.1; >= 0                               */
+} tpc_fullfit_params_t;
+
+typedef struct {   /* caller-allocated DEVICE buffers, indexed by track like tpc_tracks_t                                     */
+  int32_t* ok;           /* [max_tracks] 1: root, refitted; 0: not a root (values passed through); -1: root whose refit failed
+                            (a transport / rotation reached sin_phi_max, or a hit list was cut by TPC_STATUS_TRACK_HIT_OVERFLOW) */
+  int32_t* chain_hits;   /* [max_tracks] hits of the whole chain (roots), else the track's own n_hits                         */
+  int32_t* chain_pieces; /* [max_tracks] pieces of the chain (roots), else 1                                                  */
+  float* par7;           /* [max_tracks*7] (x, y, z_rel, sin_phi, dzds, q_pt, time_ref) at the innermost hit of the root;
+                            the track's own parameters unless ok == 1                                                         */
+  float* cov15;          /* [max_tracks*15] lower triangle in the order (y, z, sin_phi, dzds, q_pt):
+                            yy | zy zz | sy sz ss | ty tz ts tt | ky kz ks kt kk; zeros unless ok == 1                        */
+} tpc_fullfit_t;
+
+/* Same calling rules as tpc_refit_chains (`tracks` with hit_y_time / hit_row, `merged` from tpc_merge_tracks, same stream,
+ * asynchronous, 512 + 4 bytes of arena per track).  Errors: TPC_EINVAL (null pointer, negative parameter, hit coordinates
+ * missing), TPC_ENOMEM, TPC_ECUDA.  tpc_merge_last_launches() then reports this call's launches.                             */
+int tpc_refit_full(tpc_tracker_t* tracker, const tpc_fullfit_params_t* params, const tpc_tracks_t* tracks,
+                   const tpc_merged_t* merged, void* cuda_stream, tpc_fullfit_t* out);
 
 /* ---- C9: where and when a track passes the beam line (DESIGN.md §3 "C9"; z is only known once the
  * collision time is).  Every state of `par7` (DEVICE, [max_tracks*7] = (x, y, z_rel, sin_phi, dzds, q_pt, time_ref): the

@@ -19,6 +19,7 @@
 #include "ingest.cuh"
 #include "links.cuh"
 #include "merge.cuh"
+#include "fullfit.cuh"
 #include "scan.cuh"
 #include "selector.cuh"
 #include "tracklet.cuh"
@@ -205,7 +206,7 @@ struct tpc_tracker {
   cudaEvent_t ev[N_STEPS + 1] = {};
   bool profile = false, have_times = false;
   int64_t last_launches = 0, last_merge_launches = 0;
-  int ctas_refit = 148 * 8;
+  int ctas_refit = 148 * 8, ctas_fullfit = 148 * 4;
   int ctas_fit_up = 148, ctas_follow_up = 148, ctas_fit_down = 148, ctas_follow_down = 148;   // persistent grids: SMs x resident CTAs per SM
   int ctas_rows_up = 148, ctas_rows_down = 148;
   bool follow_rows = false;        // row-synchronous follower (follow_rows.cuh) instead of the per-lane one
@@ -389,6 +390,7 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
     t->ctas_fit_down = resident(k_tracklet_fit<true>, TPC_FIT_CTAS_PER_SM);
     t->ctas_follow_down = resident(k_tracklet_follow<true>, TPC_FOLLOW_CTAS_PER_SM);
     t->ctas_refit = resident(k_refit_chains, 64);
+    t->ctas_fullfit = resident(k_refit_full, 64);
     t->follow_rows = p->follower == 1 && p->miss_limit <= 255;      // the packed per-tracklet counters are 8 bits wide
     if (cudaFuncSetAttribute(k_follow_rows<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FrSmem)) != cudaSuccess ||
         cudaFuncSetAttribute(k_follow_rows<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FrSmem)) != cudaSuccess) {
@@ -621,6 +623,48 @@ int tpc_refit_chains(tpc_tracker_t* t, const tpc_tracks_t* tr, const tpc_merged_
   if (K > 0) {
     k_refit_roots<<<(K + 255) / 256, 256, 0, st>>>(T, io, root_list, n_roots, c); ++launches;
     k_refit_chains<<<std::min(t->ctas_refit, (K + kMergeThreads - 1) / kMergeThreads), kMergeThreads, 0, st>>>(T, io, root_list, n_roots, work_counter, c, t->consts); ++launches;
+  }
+  t->last_merge_launches = launches;
+  if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;
+  return TPC_OK;
+}
+
+
+// ---- C12: refit of every chain root with the full covariance and the material of the gas (fullfit.cuh) ----
+int tpc_refit_full(tpc_tracker_t* t, const tpc_fullfit_params_t* fp, const tpc_tracks_t* tr, const tpc_merged_t* mg, void* cuda_stream,
+                   tpc_fullfit_t* out) {
+  if (!t || !fp || !tr || !mg || !out) return TPC_EINVAL;
+  if (!(fp->inv_x0_per_cm >= 0 && fp->dedx_mip_gev_per_cm >= 0 && fp->mass_gev >= 0 && fp->eloss_sigma >= 0)) return TPC_EINVAL;
+  if (tr->max_tracks < 0 || !tr->n_tracks || !out->ok || !out->chain_hits || !out->chain_pieces || !out->par7 || !out->cov15) return TPC_EINVAL;
+  if (tr->max_tracks > 0 && (!tr->hit_y_time || !tr->hit_row || !tr->sector || !tr->n_hits || !tr->hit_offset || !tr->x ||
+                             !tr->y || !tr->z_rel || !tr->time_ref || !tr->sin_phi || !tr->dzds || !tr->q_pt || !mg->next || !mg->prev)) return TPC_EINVAL;
+  const int K = tr->max_tracks;
+  const size_t need = 512 + 4 * (size_t)std::max(K, 1);
+  if (!t->params.arena || need > t->params.arena_bytes) return TPC_ENOMEM;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* A = static_cast<char*>(t->params.arena);
+  uint32_t* n_roots = reinterpret_cast<uint32_t*>(A);
+  uint32_t* work_counter = reinterpret_cast<uint32_t*>(A + 256);
+  uint32_t* root_list = reinterpret_cast<uint32_t*>(A + 512);
+  MergeConsts c{};
+  c.n_sectors = t->geom.n_sectors; c.n_rows = t->geom.n_rows; c.max_tracks = K;
+  {
+    const double T = (double)t->geom.tan_half_sector;
+    c.Cd = (float)((1.0 - T * T) / (1.0 + T * T));
+    c.Sd = (float)(2.0 * T / (1.0 + T * T));
+  }
+  FullFitConsts m{};                                   // constants derived in double, rounded once
+  m.inv_x0 = fp->inv_x0_per_cm; m.dedx_mip = fp->dedx_mip_gev_per_cm; m.eloss_sigma = fp->eloss_sigma;
+  m.m2 = (float)((double)fp->mass_gev * (double)fp->mass_gev);
+  m.ms2 = (float)(13.6e-3 * 13.6e-3);                  // Highland: 13.6 MeV, in GeV
+  MergeTracks T{tr->n_tracks, tr->seed_hit, tr->sector, tr->first_row, tr->last_row, tr->x, tr->y, tr->z_rel, tr->time_ref, tr->sin_phi, tr->dzds, tr->q_pt};
+  FullFitIo io{reinterpret_cast<const float2*>(tr->hit_y_time), tr->hit_row, tr->n_hits, tr->hit_offset, tr->max_track_hits, mg->next, mg->prev,
+               out->ok, out->chain_hits, out->chain_pieces, out->par7, out->cov15};
+  int64_t launches = 0;
+  cudaMemsetAsync(n_roots, 0, 512, st);
+  if (K > 0) {
+    k_fullfit_roots<<<(K + 255) / 256, 256, 0, st>>>(T, io, root_list, n_roots, c); ++launches;
+    k_refit_full<<<std::min(t->ctas_fullfit, (K + kMergeThreads - 1) / kMergeThreads), kMergeThreads, 0, st>>>(T, io, root_list, n_roots, work_counter, c, t->consts, m); ++launches;
   }
   t->last_merge_launches = launches;
   if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;

@@ -19,7 +19,7 @@ EXPORTS = ("tpc_tracker_arena_bytes", "tpc_tracker_create", "tpc_track_timeframe
            "tpc_tracker_step_ms", "tpc_tracker_step_name", "tpc_tracker_last_launches", "tpc_tracker_work_counters",
            "tpc_tracker_arena_plan", "tpc_selftest_fast_math", "tpc_selftest_alu_peak",
            "tpc_cluster_finder_scratch_bytes", "tpc_find_clusters",
-           "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_merge_central_electrode", "tpc_refit_chains", "tpc_vertex_time", "tpc_compress_tracks", "tpc_merge_last_launches",
+           "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_merge_central_electrode", "tpc_refit_chains", "tpc_refit_full", "tpc_vertex_time", "tpc_compress_tracks", "tpc_merge_last_launches",
            "tpc_tracker_destroy", "tpc_strerror")
 
 
@@ -120,6 +120,19 @@ class Refit(C.Structure):
     _fields_ = [("ok", C.c_void_p), ("chain_hits", C.c_void_p), ("chain_pieces", C.c_void_p), ("par7", C.c_void_p), ("cov9", C.c_void_p)]
 
 
+class FullFitParams(C.Structure):
+    """``tpc_fullfit_params_t``"""
+    _fields_ = [("inv_x0_per_cm", C.c_float), ("dedx_mip_gev_per_cm", C.c_float), ("mass_gev", C.c_float), ("eloss_sigma", C.c_float)]
+
+
+class FullFit(C.Structure):
+    """``tpc_fullfit_t``"""
+    _fields_ = [("ok", C.c_void_p), ("chain_hits", C.c_void_p), ("chain_pieces", C.c_void_p), ("par7", C.c_void_p), ("cov15", C.c_void_p)]
+
+
+DEFAULT_FULLFIT_PARAMS = (1.0 / 3.0e4, 1.7e-6, 0.13957, 0.1)      # DESIGN.md §3 C12 reading FF3: the drift gas, pions
+
+
 def default_merge_params() -> MergeParams:
     """DESIGN.md §3 C7 readings M4 / M5."""
     return MergeParams(2.0, 2.0, 0.05, 0.5, 12, 2)
@@ -181,6 +194,8 @@ def load_library(build_if_missing: bool = True):
         L.tpc_merge_central_electrode.restype = C.c_int
         L.tpc_refit_chains.argtypes = [vp, C.POINTER(Tracks), C.POINTER(Merged), vp, C.POINTER(Refit)]
         L.tpc_refit_chains.restype = C.c_int
+        L.tpc_refit_full.argtypes = [vp, C.POINTER(FullFitParams), C.POINTER(Tracks), C.POINTER(Merged), vp, C.POINTER(FullFit)]
+        L.tpc_refit_full.restype = C.c_int
         L.tpc_compress_tracks.argtypes = [vp, C.POINTER(CompressParams), C.POINTER(Tracks), C.c_int64, vp, C.POINTER(Compressed)]
         L.tpc_compress_tracks.restype = C.c_int
         L.tpc_vertex_time.argtypes = [vp, vp, C.c_int32, vp, vp, vp, vp, vp]
@@ -444,6 +459,24 @@ class Tracker:
         if rc != TPC_OK:
             raise TpcError(rc, "tpc_refit_chains")
         return refit
+
+    def tpc_refit_full(self, outputs, merged, full_params=DEFAULT_FULLFIT_PARAMS, out=None, stream=None):
+        """C12 on the DEVICE track outputs (allocated with ``hit_coords=True``) and C7 links (same stream); returns
+        (ok, chain_hits, chain_pieces, par7, cov15)."""
+        torch = self._torch
+        o, st = outputs
+        K = max(int(st.max_tracks), 1)
+        if out is None:
+            e = lambda shape, dt: torch.empty(shape, dtype=dt, device=self.device)
+            out = (e(K, torch.int32), e(K, torch.int32), e(K, torch.int32), e((K, 7), torch.float32), e((K, 15), torch.float32))
+        m = Merged(*(t.data_ptr() for t in merged))
+        r = FullFit(*(t.data_ptr() for t in out))
+        fp = FullFitParams(*(float(v) for v in full_params))
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        rc = self.lib.tpc_refit_full(self.handle, C.byref(fp), C.byref(st), C.byref(m), C.c_void_p(s.cuda_stream), C.byref(r))
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_refit_full")
+        return out
 
     def tpc_compress_tracks(self, outputs, n_clusters: int, reject_q_pt: float = 1.0 / 0.15, step_y: float = 0.025, step_z: float = 0.025,
                             out=None, stream=None):

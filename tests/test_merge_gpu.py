@@ -187,6 +187,7 @@ def test_full_10ms_frame_merge_invariants_and_sampled_oracle_parity():
     out = trk.tpc_track_timeframe(*d, n=n, outputs=outs)
     nxt, prv, root, n_links = merged = trk.tpc_merge_tracks(outs)
     rf_ok, rf_ch, rf_cp, rf_par, rf_cov = trk.tpc_refit_chains(outs, merged)
+    ff = trk.tpc_refit_full(outs, merged)                                        # C12 at full size: sampled parity below
     ce_next, ce_prev, ce_t, ce_n = trk.tpc_merge_central_electrode(outs)        # C10 at full size: invariants below
     torch.cuda.synchronize()
     k, nh = int(out.n_tracks[0]), int(out.n_track_hits[0])
@@ -195,6 +196,7 @@ def test_full_10ms_frame_merge_invariants_and_sampled_oracle_parity():
     dzds_all = out.dzds[:k].cpu().numpy()
     rf_ok, rf_ch, rf_cp, rf_par, rf_cov = (t[:k].cpu().numpy() for t in (rf_ok, rf_ch, rf_cp, rf_par, rf_cov))
     n_hits_all = out.n_hits[:k].cpu().numpy()
+    ff_ok, ff_ch, ff_cp, ff_par, ff_cov = (t[:k].cpu().numpy() for t in ff)
     seed, sec = out.seed_hit[:k].cpu().numpy(), out.sector[:k].cpu().numpy()
     first_row, last_row = out.first_row[:k].cpu().numpy(), out.last_row[:k].cpu().numpy()
     x = out.x[:k].cpu().numpy()
@@ -226,6 +228,8 @@ def test_full_10ms_frame_merge_invariants_and_sampled_oracle_parity():
     np.testing.assert_array_equal(rf_ch[is_root], np.bincount(root, weights=n_hits_all, minlength=k).astype(np.int64)[is_root])
     np.testing.assert_array_equal(rf_cp[is_root], np.bincount(root, minlength=k)[is_root])
     assert np.all(np.isfinite(rf_par)) and np.all(np.isfinite(rf_cov))
+    assert np.all(ff_ok[prv >= 0] == 0) and np.all(ff_ok[prv < 0] != 0) and (ff_ok[prv < 0] == -1).mean() < 0.03
+    assert np.all(np.isfinite(ff_par)) and np.all(np.isfinite(ff_cov)) and np.all(ff_cov[ff_ok == 1][:, [0, 2, 5, 9, 14]] > 0)
     # (b) sampled parity
     S, t_lo, width, margin = 7, 20000.0, 2000.0, 2200.0
     t_hi = t_lo + width
@@ -238,25 +242,31 @@ def test_full_10ms_frame_merge_invariants_and_sampled_oracle_parity():
     mr = M.merge(M.default_merge_params(36), o.tr_seed, o.tr_sector, o.tr_first_row, o.tr_last_row, o.tr_par)
     o_ok, o_ch, o_cp, o_rp, o_rc = oracle.refit_chains(oracle.default_geometry(36, tf.max_time_bin), oracle.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm),
                                                        tf.row[sel], tf.pad[sel], tf.time[sel], o, mr.next, mr.prev)
+    f_ok, f_ch, f_cp, f_rp, f_rc = oracle.refit_full(oracle.default_geometry(36, tf.max_time_bin), oracle.default_params(cfg.sigma_y_cm, cfg.sigma_z_cm),
+                                                      tf.row[sel], tf.pad[sel], tf.time[sel], o, mr.next, mr.prev)
     o_t = tf.time[sel][o.tr_hit_index]
     o_min = np.minimum.reduceat(o_t, o.tr_hit_offset); o_max = np.maximum.reduceat(o_t, o.tr_hit_offset)
     core = np.nonzero((o.tr_sector == S) & (o_min >= t_lo) & (o_max <= t_hi))[0]
     assert core.size > 300
     o_seed_global = sel[o.tr_seed]
     lookup = {int(s): i for i, s in enumerate(seed)}
-    n_with_link = n_refitted = 0
+    n_with_link = n_refitted = n_full = 0
     for i in core:
         gi = lookup[int(o_seed_global[i])]                      # the same track exists on the GPU (sampled tracking parity)
         # C8: a chain whose root lies in the core is refitted from the same hits on both sides -> bit-identical
         assert rf_ok[gi] == o_ok[i] and rf_ch[gi] == o_ch[i] and rf_cp[gi] == o_cp[i]
         assert np.array_equal(rf_par[gi], o_rp[i]) and np.array_equal(rf_cov[gi], o_rc[i])
         n_refitted += int(o_ok[i] == 1)
+        # C12: every root in the core (single tracks too), full covariance -> bit-identical
+        assert ff_ok[gi] == f_ok[i] and ff_ch[gi] == f_ch[i] and ff_cp[gi] == f_cp[i]
+        assert np.array_equal(ff_par[gi], f_rp[i]) and np.array_equal(ff_cov[gi], f_rc[i])
+        n_full += int(f_ok[i] == 1)
         for o_idx, g_idx in ((mr.next[i], nxt[gi]), (mr.prev[i], prv[gi])):
             o_link = int(o_seed_global[o_idx]) if o_idx >= 0 else -1
             g_link = int(seed[g_idx]) if g_idx >= 0 else -1
             assert o_link == g_link, (int(o_seed_global[i]), o_link, g_link)
             n_with_link += o_link >= 0
-    assert n_with_link > 50 and n_refitted > 20
+    assert n_with_link > 50 and n_refitted > 20 and n_full > 250
 
 
 def test_refit_with_truncated_hit_lists_flags_the_chains_instead_of_reading_past_the_buffers():
