@@ -220,7 +220,7 @@ typedef struct {   /* caller-allocated DEVICE buffers: exactly the arrays tpc_cl
   int32_t* status;       /* scalar: 1 = more clusters than max_clusters                                                  */
 } tpc_clusters_out_t;
 
-/* Arena bytes the call needs for n_digits samples (host arithmetic, 28 B per sample; 0 = invalid).                        */
+/* Arena bytes the call needs for n_digits samples (host arithmetic, 16 B per sample: the staged clusters; 0 = invalid).   */
 size_t tpc_cluster_finder_scratch_bytes(int64_t n_digits);
 
 /* Asynchronous on `cuda_stream`, never allocates: scratch = the handle's arena (the call precedes tpc_track_timeframe on the

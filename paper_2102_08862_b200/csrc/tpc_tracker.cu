@@ -392,6 +392,9 @@ int tpc_tracker_create(const tpc_geometry_t* g, const tpc_params_t* p, tpc_track
     t->ctas_refit = resident(k_refit_chains, 64);
     t->ctas_fullfit = resident(k_refit_full, 64);
     t->follow_rows = p->follower == 1 && p->miss_limit <= 255;      // the packed per-tracklet counters are 8 bits wide
+    if (cudaFuncSetAttribute(k_cf_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(CfSmem)) != cudaSuccess) {
+      cudaGetLastError(); tpc_tracker_destroy(t); return TPC_ECUDA;
+    }
     if (cudaFuncSetAttribute(k_follow_rows<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FrSmem)) != cudaSuccess ||
         cudaFuncSetAttribute(k_follow_rows<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FrSmem)) != cudaSuccess) {
       cudaGetLastError(); tpc_tracker_destroy(t); return TPC_ECUDA;
@@ -481,14 +484,15 @@ int tpc_merge_tracks(tpc_tracker_t* t, const tpc_merge_params_t* mp, const tpc_t
 
 // ---- C0: cluster finder in front of the path (clusterizer.cuh) ----
 namespace {
-struct CfLayout { size_t head, gnum, group_start, peak, sums, tiles_a, tiles_b, total; };
+struct CfLayout { size_t st_row, st_pad, st_time, st_charge, tile_count, tile_off, scan_tiles, total; size_t n_tiles; };
 CfLayout cf_layout(int64_t n) {
   CfLayout L{};
   const size_t N = (size_t)std::max<int64_t>(n, 1);
+  L.n_tiles = (N + kCfTile - 1) / kCfTile;
   size_t off = 0;
   auto take = [&](size_t bytes) { const size_t o = off; off += (bytes + 255) / 256 * 256; return o; };
-  L.head = take(4 * N); L.gnum = take(4 * N); L.group_start = take(4 * (N + 1)); L.peak = take(4 * N); L.sums = take(12 * N);
-  L.tiles_a = take(4 * (scan_tiles(N) + 2)); L.tiles_b = take(4 * (scan_tiles(N) + 2));
+  L.st_row = take(4 * N); L.st_pad = take(4 * N); L.st_time = take(4 * N); L.st_charge = take(4 * N);
+  L.tile_count = take(4 * L.n_tiles); L.tile_off = take(4 * L.n_tiles); L.scan_tiles = take(4 * (scan_tiles(L.n_tiles) + 2));
   L.total = off;
   return L;
 }
@@ -508,13 +512,11 @@ int tpc_find_clusters(tpc_tracker_t* t, const tpc_cluster_params_t* cp, const tp
   if (!t->params.arena || L.total > t->params.arena_bytes) return TPC_ENOMEM;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   char* A = static_cast<char*>(t->params.arena);
-  uint32_t* head = reinterpret_cast<uint32_t*>(A + L.head);
-  uint32_t* gnum = reinterpret_cast<uint32_t*>(A + L.gnum);
-  uint32_t* group_start = reinterpret_cast<uint32_t*>(A + L.group_start);
-  uint32_t* peak = reinterpret_cast<uint32_t*>(A + L.peak);
-  CfSums* sums = reinterpret_cast<CfSums*>(A + L.sums);
-  uint32_t* tiles_a = reinterpret_cast<uint32_t*>(A + L.tiles_a);
-  uint32_t* tiles_b = reinterpret_cast<uint32_t*>(A + L.tiles_b);
+  const CfStage stage{reinterpret_cast<float*>(A + L.st_pad), reinterpret_cast<float*>(A + L.st_time), reinterpret_cast<float*>(A + L.st_charge),
+                      reinterpret_cast<int32_t*>(A + L.st_row)};
+  uint32_t* tile_count = reinterpret_cast<uint32_t*>(A + L.tile_count);
+  uint32_t* tile_off = reinterpret_cast<uint32_t*>(A + L.tile_off);
+  uint32_t* scan_scratch = reinterpret_cast<uint32_t*>(A + L.scan_tiles);
   int64_t launches = 0;
   if (n == 0) {
     cudaMemsetAsync(o->n_clusters, 0, 8, st);
@@ -522,14 +524,10 @@ int tpc_find_clusters(tpc_tracker_t* t, const tpc_cluster_params_t* cp, const tp
   } else {
     const CfDigits d{dg->row, dg->pad, dg->time, dg->adc};
     const CfOut out{o->max_clusters, o->row, o->pad, o->time, o->charge, o->n_clusters, o->status};
-    const int ctas = (int)((n + 255) / 256);
-    const size_t nt = scan_tiles((size_t)n);
-    k_cf_heads<<<ctas, 256, 0, st>>>(d, n, head); ++launches;
-    launches += exclusive_scan_u32(head, gnum, (size_t)n, tiles_a, st);                 // tiles_a[nt] = number of groups
-    k_cf_groups<<<ctas, 256, 0, st>>>(head, gnum, n, tiles_a + nt, group_start); ++launches;
-    k_cf_peaks<<<ctas, 256, 0, st>>>(d, n, head, gnum, group_start, tiles_a + nt, cp->peak_threshold, peak, sums); ++launches;
-    launches += exclusive_scan_u32(peak, peak, (size_t)n, tiles_b, st);                 // tiles_b[nt] = number of clusters
-    k_cf_emit<<<ctas, 256, 0, st>>>(d, n, peak, tiles_b + nt, sums, out); ++launches;
+    const int n_tiles = (int)L.n_tiles;
+    k_cf_tile<<<n_tiles, kCfThreads, sizeof(CfSmem), st>>>(d, n, cp->peak_threshold, stage, tile_count); ++launches;
+    launches += exclusive_scan_u32(tile_count, tile_off, (size_t)n_tiles, scan_scratch, st);       // scan_scratch[tiles] = number of clusters
+    k_cf_compact<<<n_tiles, kCfThreads, 0, st>>>(stage, tile_count, tile_off, scan_scratch + scan_tiles((size_t)n_tiles), out); ++launches;
   }
   t->last_merge_launches = launches;
   if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;
