@@ -16,9 +16,27 @@ namespace tpc {
 #endif
 constexpr int kSelectorThreads = TPC_SELECTOR_THREADS;   // 8 tracklets per CTA at 256
 
-// One warp per tracklet; the five row words are loaded back to back, then the atomics are fired (no return value).
+// Claim, step 1: every tracklet claims its TOP hit (one thread per tracklet).  The ~7 tracklets that follow one track from its
+// different seed chains nearly always end on the same hit, so afterwards claim[top hit] names the best of them (or an even
+// better tracklet through that hit): the LEADER step 2 compares against.
+__global__ void __launch_bounds__(256) k_selector_claim_top(TrackletStore tl, const int32_t* __restrict__ counters,
+                                                            unsigned long long* __restrict__ claim, const __grid_constant__ Consts c) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= counters[0]) return;
+  const int4 meta = tl.meta[j];                      // n_hits, first_row, last_row, seed_orig
+  if (meta.x < c.min_hits) return;
+  const int top = tl.row_hit[(size_t)j * kRowStride + meta.z];
+  if (top >= 0) atomicMax(claim + top, tracklet_key(meta.x, (uint32_t)meta.w, (uint32_t)j));
+}
+
+// Claim, step 2: one warp per tracklet, lanes over rows.  L = the tracklet named by claim[top hit]: its key is >= this one's
+// and it holds the top hit.  If L is another tracklet, every hit this tracklet shares with L ON THE SAME ROW needs no atomic:
+// L's key is larger, and L either claims that hit itself or skips it for the same reason against a still larger key -- the
+// chain of leaders is strictly increasing in the key, so it ends at a tracklet that does claim the hit.  claim[] therefore
+// ends as the same maximum over all tracklets (whatever value the racing read of claim[top] returns: any tracklet it can name
+// qualifies), with ~ 6 of 7 atomics replaced by a coalesced read of the leader's row table.
 // (Claiming from inside the constructor when a tracklet retires was measured: it stalls the whole warp on the row
-// reads and costs 10 ms against 6 ms for this kernel.)
+// reads and costs 10 ms against 6 ms for a claim kernel.)
 __global__ void __launch_bounds__(kSelectorThreads) k_selector_claim(TrackletStore tl, const int32_t* __restrict__ counters,
                                                                      unsigned long long* __restrict__ claim,
                                                                      const __grid_constant__ Consts c) {
@@ -36,6 +54,19 @@ __global__ void __launch_bounds__(kSelectorThreads) k_selector_claim(TrackletSto
   for (int i = 0; i < kWords; ++i) {
     const int r = i * 32 + (int)lane_id();
     m[i] = (r >= first && r <= last) ? rows[r] : -1;
+  }
+  const int top = rows[last];
+  int L = j;
+  if (top >= 0) L = (int)(claim[top] & ((1ull << kKeySlotBits) - 1ull));
+  if (L != j) {
+    const int4 ml = tl.meta[L];
+    const int* rows_l = tl.row_hit + (size_t)L * kRowStride;
+#pragma unroll
+    for (int i = 0; i < kWords; ++i) {
+      const int r = i * 32 + (int)lane_id();
+      const int h = (r >= ml.y && r <= ml.z) ? rows_l[r] : -1;
+      if (h == m[i]) m[i] = -1;                       // shared with the leader on this row: the leader's claim covers it
+    }
   }
 #pragma unroll
   for (int i = 0; i < kWords; ++i)

@@ -909,6 +909,7 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* cl, int64_t n, v
   // ---- C6 tracklet selector ----
   mark(S_CLAIM);
   if (n > 0) cudaMemsetAsync(claim, 0, 8 * (size_t)n, st);
+  k_selector_claim_top<<<(int)((tl_bound + 255) / 256), 256, 0, st>>>(tl, counters, claim, c); ++launches;
   k_selector_claim<<<warp_ctas, kSelectorThreads, 0, st>>>(tl, counters, claim, c); ++launches;
   mark(S_COUNT);
   cudaMemsetAsync(owned, 0, 4 * (size_t)T, st);
