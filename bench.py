@@ -409,15 +409,16 @@ def main():
 
     # ---- end to end through the C-ABI host entry point (pinned host buffers) ----
     # Every step copies the frame host->device, tracks it and copies the tracks back, all inside tpc_track_timeframe_host.
-    # `--e2e-inflight 2` (default) keeps two frames in flight on two handles / streams / host threads, the way a
-    # processing node double-buffers time frames: the PCIe copies of one frame overlap the kernels of the other.
+    # `--e2e-inflight 3` (default) keeps three frames in flight on three handles / streams / host threads, the way a
+    # processing node buffers time frames: the PCIe copies of one frame overlap the kernels of another.
     e2e = None
     if not args.no_e2e:
         def measure_e2e(n_fl):
             trks = [T.Tracker(g, _tracker_params(T, cfg, n, True, False, gp, args.follower), device=str(dev)) for _ in range(n_fl)]
             houts = [t.alloc_outputs(n, host=True) for t in trks]
             streams = [torch.cuda.Stream(device=dev) for _ in range(n_fl)]
-            k_each = max(2, (max(3, args.steps // 2) + n_fl - 1) // n_fl)
+            k_each = max(2, (max(3, args.steps) + n_fl - 1) // n_fl)     # at least `steps` frames in all: the timed region includes the
+                                                                          # pipeline's fill (first H2D) and drain (last D2H), amortised over them
 
             def run_frames(i, k):
                 torch.cuda.set_device(local_rank)

@@ -96,6 +96,22 @@ def test_K1_transport_fails_beyond_sin_phi_max_and_keeps_state():
     np.testing.assert_array_equal(cv1, np.array(cv, np.float32))
 
 
+def test_K1_sin_phi_exactly_on_the_limit_fails_at_either_end():
+    """A12: the step needs |sin phi| < sin_phi_max at BOTH ends, strictly (all values below are exact in fp32)."""
+    p = oracle.default_params()
+    p.sin_phi_max = 0.75
+    p.inv_R_per_qpt = 0.5
+    cv = [1, 0, 1, 0, 0, 1, 1, 0, 1]
+    ok, st, _ = oracle.transport(p, [100.0, 0.0, 0.0, 0.75, 0.0, 0.0], cv, 101.0)             # starts on the limit
+    assert not ok and st[0] == 100.0
+    ok, st, _ = oracle.transport(p, [100.0, 0.0, 0.0, 0.5, 0.0, 0.5], cv, 101.0)              # ends on it: 0.5 + 0.5 * 0.5 * 1
+    assert not ok and st[0] == 100.0
+    ok, st, _ = oracle.transport(p, [100.0, 0.0, 0.0, 0.5, 0.0, 0.5], cv, 100.96875)          # ends just inside
+    assert ok and st[3] == np.float32(0.5 + 0.25 * 0.96875)
+    ok, st, _ = oracle.transport(p, [100.0, 0.0, 0.0, -0.75, 0.0, 0.0], cv, 101.0)
+    assert not ok
+
+
 def test_K1_transport_never_leaves_the_domain_of_the_circle():
     """Reading A12 on both ends: whatever an update did to sin phi (even |s| >= 1, where sqrt(1 - s^2) does not exist),
     a transport either FAILs and keeps the state or returns finite numbers."""
