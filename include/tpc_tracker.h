@@ -229,6 +229,21 @@ size_t tpc_cluster_finder_scratch_bytes(int64_t n_digits);
 int tpc_find_clusters(tpc_tracker_t* tracker, const tpc_cluster_params_t* params, const tpc_digits_t* digits, int64_t n_digits,
                       void* cuda_stream, tpc_clusters_out_t* clusters_out);
 
+/* ---- C0 for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): the same cluster finder, needing NO tracker handle and NO arena.  Its scratch (16 B per sample) is a fixed
+ * array inside the library image, so every GPU that loads the library holds 16.1 MiB for it until the process exits, and one
+ * call handles at most tpc_find_clusters_static_max_digits() = 1 048 576 samples (larger n: TPC_ENOMEM, nothing enqueued --
+ * use tpc_find_clusters).  Arguments, results (bit-identical to tpc_find_clusters) and the other errors as there.  The call
+ * enqueues one memset and five kernels on `cuda_stream` and calls no cudaMalloc / cudaFree or allocating routine.
+ * ALL calls on one GPU share the one scratch array: calls that overlap on the GPU (different streams without ordering, or
+ * different host threads) race -- order them on one stream or with events.
+ * tpc_find_clusters_static_setup() looks the array's device address up for the CURRENT device (once per device; also done by
+ * the first call on a device): call it before a stream capture begins.  Errors: TPC_ECUDA.                                 */
+int64_t tpc_find_clusters_static_max_digits(void);
+int tpc_find_clusters_static_setup(void);
+int tpc_find_clusters_static(const tpc_cluster_params_t* params, const tpc_digits_t* digits, int64_t n_digits,
+                             void* cuda_stream, tpc_clusters_out_t* clusters_out);
+
 /* ---- C7: sector-boundary merging of the per-sector tracks (DESIGN.md §3 "C7", readings M1..M8; PAPER.md L23 / L25:
  * "full TPC tracking" -- the sector tracker is followed by a merger of the sector tracks; BASELINE.json L8: 36 sectors,
  * each in its rotated local frame).  A widening step after the hot path (linking only: the

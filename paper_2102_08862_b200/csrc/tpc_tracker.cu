@@ -535,6 +535,80 @@ int tpc_find_clusters(tpc_tracker_t* t, const tpc_cluster_params_t* cp, const tp
 }
 
 
+// ---- C0 without any allocation: the same two kernels with their scratch in a file-scope device array ----
+// For callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it) and so cannot
+// create a tracker handle with an arena.  The scratch (staged clusters + per-tile counts, 16 B per sample) lives in the
+// library image: every GPU that loads the library holds kCfStaticBytes (16.1 MiB) until the process exits.
+namespace {
+constexpr int64_t kCfStaticMaxDigits = (int64_t)1 << 20;                       // 1 048 576 samples per call
+constexpr size_t kCfStaticTiles = (size_t)(kCfStaticMaxDigits / kCfTile);      // 512
+constexpr size_t kCfStaticStage = 4 * (size_t)kCfStaticMaxDigits;              // bytes of one staged array
+constexpr size_t kCfStaticCounts = 4 * 4 * kCfStaticTiles;                     // tile_count | tile_off | scan scratch (2 + spare)
+constexpr size_t kCfStaticBytes = 4 * kCfStaticStage + kCfStaticCounts;
+constexpr int kCfStaticMaxDevices = 64;
+}  // namespace
+static_assert(sizeof(CfSmem) <= 48 * 1024, "k_cf_tile must launch without an opt-in to large dynamic shared memory");
+static __device__ __align__(256) unsigned char g_cf_static_scratch[kCfStaticBytes];
+namespace {
+// In host code g_cf_static_scratch is only a stand-in for the symbol, not a device address: its address on a device comes
+// from cudaGetSymbolAddress with that device current, looked up once per device.
+std::mutex g_cf_static_mu;
+unsigned char* g_cf_static_ptr[kCfStaticMaxDevices] = {};
+
+int cf_static_scratch(unsigned char** out) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kCfStaticMaxDevices) { cudaGetLastError(); return TPC_ECUDA; }
+  std::lock_guard<std::mutex> lock(g_cf_static_mu);
+  if (!g_cf_static_ptr[dev]) {
+    void* p = nullptr;
+    if (cudaGetSymbolAddress(&p, g_cf_static_scratch) != cudaSuccess || !p) { cudaGetLastError(); return TPC_ECUDA; }
+    g_cf_static_ptr[dev] = static_cast<unsigned char*>(p);
+  }
+  *out = g_cf_static_ptr[dev];
+  return TPC_OK;
+}
+}  // namespace
+
+int64_t tpc_find_clusters_static_max_digits(void) { return kCfStaticMaxDigits; }
+
+int tpc_find_clusters_static_setup(void) {
+  unsigned char* p = nullptr;
+  return cf_static_scratch(&p);
+}
+
+int tpc_find_clusters_static(const tpc_cluster_params_t* cp, const tpc_digits_t* dg, int64_t n, void* cuda_stream, tpc_clusters_out_t* o) {
+  if (!cp || !dg || !o || n < 0) return TPC_EINVAL;
+  if (n > kCfStaticMaxDigits) return TPC_ENOMEM;                               // beyond the built-in scratch: use tpc_find_clusters with an arena
+  if (!(cp->peak_threshold > 0) || !o->n_clusters || !o->status || o->max_clusters < 0) return TPC_EINVAL;
+  if (n > 0 && (!dg->row || !dg->pad || !dg->time || !dg->adc)) return TPC_EINVAL;
+  if (o->max_clusters > 0 && (!o->row || !o->pad || !o->time || !o->charge)) return TPC_EINVAL;
+  unsigned char* A = nullptr;
+  const int rc = cf_static_scratch(&A);
+  if (rc != TPC_OK) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (n == 0) {
+    cudaMemsetAsync(o->n_clusters, 0, 8, st);
+    cudaMemsetAsync(o->status, 0, 4, st);
+  } else {
+    const CfStage stage{reinterpret_cast<float*>(A + kCfStaticStage), reinterpret_cast<float*>(A + 2 * kCfStaticStage),
+                        reinterpret_cast<float*>(A + 3 * kCfStaticStage), reinterpret_cast<int32_t*>(A)};
+    uint32_t* tile_count = reinterpret_cast<uint32_t*>(A + 4 * kCfStaticStage);
+    uint32_t* tile_off = tile_count + kCfStaticTiles;
+    uint32_t* scan_scratch = tile_off + kCfStaticTiles;
+    const CfDigits d{dg->row, dg->pad, dg->time, dg->adc};
+    const CfOut out{o->max_clusters, o->row, o->pad, o->time, o->charge, o->n_clusters, o->status};
+    const int n_tiles = (int)((n + kCfTile - 1) / kCfTile);
+    // the array keeps the last call's contents: the counts start at zero (the staged clusters are written before they are read)
+    cudaMemsetAsync(tile_count, 0, kCfStaticCounts, st);
+    k_cf_tile<<<n_tiles, kCfThreads, sizeof(CfSmem), st>>>(d, n, cp->peak_threshold, stage, tile_count);
+    exclusive_scan_u32(tile_count, tile_off, (size_t)n_tiles, scan_scratch, st);       // scan_scratch[1] = number of clusters (one scan tile)
+    k_cf_compact<<<n_tiles, kCfThreads, 0, st>>>(stage, tile_count, tile_off, scan_scratch + scan_tiles((size_t)n_tiles), out);
+  }
+  if (cudaGetLastError() != cudaSuccess) return TPC_ECUDA;
+  return TPC_OK;
+}
+
+
 // ---- C10: merging across the central electrode (merge.cuh) ----
 int tpc_merge_central_electrode(tpc_tracker_t* t, const tpc_ce_params_t* mp, const tpc_tracks_t* tr, void* cuda_stream, tpc_ce_merged_t* out) {
   if (!t || !mp || !tr || !out) return TPC_EINVAL;

@@ -19,6 +19,7 @@ EXPORTS = ("tpc_tracker_arena_bytes", "tpc_tracker_create", "tpc_track_timeframe
            "tpc_tracker_step_ms", "tpc_tracker_step_name", "tpc_tracker_last_launches", "tpc_tracker_work_counters",
            "tpc_tracker_arena_plan", "tpc_selftest_fast_math", "tpc_selftest_alu_peak",
            "tpc_cluster_finder_scratch_bytes", "tpc_find_clusters",
+           "tpc_find_clusters_static_max_digits", "tpc_find_clusters_static_setup", "tpc_find_clusters_static",
            "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_merge_central_electrode", "tpc_refit_chains", "tpc_refit_full", "tpc_vertex_time", "tpc_compress_tracks", "tpc_merge_last_launches",
            "tpc_tracker_destroy", "tpc_strerror")
 
@@ -190,6 +191,12 @@ def load_library(build_if_missing: bool = True):
         L.tpc_cluster_finder_scratch_bytes.restype = C.c_size_t
         L.tpc_find_clusters.argtypes = [vp, C.POINTER(ClusterParams), C.POINTER(Digits), C.c_int64, vp, C.POINTER(ClustersOut)]
         L.tpc_find_clusters.restype = C.c_int
+        L.tpc_find_clusters_static_max_digits.argtypes = []
+        L.tpc_find_clusters_static_max_digits.restype = C.c_int64
+        L.tpc_find_clusters_static_setup.argtypes = []
+        L.tpc_find_clusters_static_setup.restype = C.c_int
+        L.tpc_find_clusters_static.argtypes = [C.POINTER(ClusterParams), C.POINTER(Digits), C.c_int64, vp, C.POINTER(ClustersOut)]
+        L.tpc_find_clusters_static.restype = C.c_int
         L.tpc_merge_central_electrode.argtypes = [vp, C.POINTER(CeParams), C.POINTER(Tracks), vp, C.POINTER(CeMerged)]
         L.tpc_merge_central_electrode.restype = C.c_int
         L.tpc_refit_chains.argtypes = [vp, C.POINTER(Tracks), C.POINTER(Merged), vp, C.POINTER(Refit)]
@@ -229,6 +236,38 @@ def tpc_selftest_fast_math(stream=None) -> tuple:
     if rc != TPC_OK:
         raise TpcError(rc, "tpc_selftest_fast_math")
     return int(out[0]), int(out[1])
+
+
+def tpc_find_clusters_static_max_digits() -> int:
+    """Largest n one ``tpc_find_clusters_static`` call accepts."""
+    return int(load_library().tpc_find_clusters_static_max_digits())
+
+
+def tpc_find_clusters_static_setup() -> None:
+    """Looks up the built-in scratch array of the CURRENT device (once per device; call before a stream capture)."""
+    rc = load_library().tpc_find_clusters_static_setup()
+    if rc != TPC_OK:
+        raise TpcError(rc, "tpc_find_clusters_static_setup")
+
+
+def tpc_find_clusters_static(row, pad, time, adc, out, n: int | None = None, peak_threshold: float = 8.0, stream=None):
+    """C0 without a tracker handle, an arena or any allocation (include/tpc_tracker.h): DEVICE int32 (row, pad, time) / float32
+    adc in, the caller's ``out`` = (row, pad, time, charge float32[max_clusters], n_clusters int64[1], status int32[1]) DEVICE
+    tensors filled.  Argument marshalling only: nothing is allocated here either."""
+    import torch
+    n = int(adc.shape[0]) if n is None else int(n)
+    for t_, dt in ((row, torch.int32), (pad, torch.int32), (time, torch.int32), (adc, torch.float32)):
+        if not (t_.is_cuda and t_.dtype == dt and t_.is_contiguous() and t_.shape[0] >= n):
+            raise ValueError("digits must be contiguous CUDA tensors: int32 row / pad / time, float32 adc, length >= n")
+    K = int(out[0].shape[0])
+    dg = Digits(row.data_ptr(), pad.data_ptr(), time.data_ptr(), adc.data_ptr())
+    co = ClustersOut(K, out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr(), out[3].data_ptr(), out[4].data_ptr(), out[5].data_ptr())
+    cp = ClusterParams(float(peak_threshold))
+    s = stream if stream is not None else torch.cuda.current_stream(adc.device)
+    rc = load_library().tpc_find_clusters_static(C.byref(cp), C.byref(dg), n, C.c_void_p(s.cuda_stream), C.byref(co))
+    if rc != TPC_OK:
+        raise TpcError(rc, "tpc_find_clusters_static")
+    return out
 
 
 def tpc_selftest_alu_peak(stream=None) -> tuple:
