@@ -630,3 +630,116 @@ def test_N4_edge_rows_have_no_links_even_next_to_another_sector():
     assert r.up_raw[i151] == -1 and r.down_raw[i151] == -1 and r.up_raw[i152] == -1 and r.down_raw[i152] == -1
     i150 = int(np.nonzero(row == 150.0)[0][0])
     assert r.up_raw[i150] == i151 and r.down_raw[i150] >= 0   # row 150 does link up to the edge row
+
+
+# ---- pins from the line-by-line mutation sweep of orc_track ------------------------------------------------
+
+def test_P7_search_distance_adds_the_z_term():
+    """C5 search: nearest in dy^2 + dz^2.  Row 50 holds A (dy 0.30, dz 0) and B (dy 0.10, dz 0.35): dd = 0.090 against 0.1325, A
+    is attached; with the z term dropped or subtracted B would be.  (Neither links in the finder: |ez| or |ey| beyond W1 on one
+    side, so row 50 is reached by the follower's search -- from below and, by the tracklet seeded above, from above.)"""
+    rows = np.concatenate([np.arange(20, 50), np.arange(51, 61)])
+    row, pad, time = concat([_line(rows), _line(np.array([50]), dy=0.30), _line(np.array([50]), dy=0.10, dz=0.35)])
+    ia, ib = rows.size, rows.size + 1
+    r = oracle.track(_geom(), oracle.default_params(), row, pad, time)
+    assert r.link_up[int(np.nonzero(row == 49.0)[0][0])] == -1                  # no cleaned link into row 50
+    seed_rows = row[r.tl_seed].astype(int)
+    for seed_row in (21, 51):
+        t = int(np.nonzero(seed_rows == seed_row)[0][0])
+        assert r.tl_row_hit[t, 50] == ia, (seed_row, r.tl_row_hit[t, 50], ia, ib)
+    # control: B moved to dz = 0.25 is the nearer one (0.0725)
+    row, pad, time = concat([_line(rows), _line(np.array([50]), dy=0.30), _line(np.array([50]), dy=0.10, dz=0.25)])
+    r = oracle.track(_geom(), oracle.default_params(), row, pad, time)
+    t = int(np.nonzero(row[r.tl_seed].astype(int) == 21)[0][0])
+    assert r.tl_row_hit[t, 50] == ib
+
+
+def test_P8_finder_chi2_adds_the_z_term():
+    """C2: chi2 = ey^2 w_y + ez^2 w_z.  Above the hit of row 30 sit u1 (ey 0.20, ez 0) and u2 (ey 0.05, ez 0.35):
+    chi2 = 1.04 against 0.065 + 1.42 = 1.48, the link goes to u1; with the z term subtracted it would go to u2."""
+    row, pad, time = concat([_line(np.arange(20, 31)), _line(np.array([31]), dy=0.20), _line(np.array([31]), dy=0.05, dz=0.35)])
+    r = oracle.track(_geom(), oracle.default_params(), row, pad, time)
+    h30 = int(np.nonzero(row == 30.0)[0][0])
+    assert r.up_raw[h30] == 11                                                  # u1 (index 11), not u2 (12)
+    row, pad, time = concat([_line(np.arange(20, 31)), _line(np.array([31]), dy=0.20), _line(np.array([31]), dy=0.05, dz=0.10)])
+    r = oracle.track(_geom(), oracle.default_params(), row, pad, time)
+    assert r.up_raw[h30] == 12                                                  # control: u2 at ez 0.10 (chi2 0.18) wins
+
+
+def test_P9_chi2_cut_is_strict():
+    """Three hits on the pad centres of rows 29, 30, 31 (y = 0 exactly) at times 100, 101, 103: ey = 0 and ez = 2Z - Z = Z exactly,
+    so chi2 = fl(fl(Z Z) w_z) -- one value, computed here from the oracle's own rounded w_z.  The link needs chi2 < chi2_cut."""
+    g = _geom()
+    rows = np.array([29, 30, 31])
+    rowv = rows.astype(np.float32)
+    padv = (0.5 * (n_pads(rows) - 1)).astype(np.float32)                       # c_r: exact in fp32
+    timev = np.array([100.0, 101.0, 103.0], np.float32)
+    _, _, _, consts = oracle.tables(g, oracle.default_params())
+    Z = np.float32(ZBIN)
+    chi2 = np.float32(np.float32(Z * Z) * np.float32(consts["wz"]))
+    assert 1.0 < chi2 < 9.0
+    p = oracle.default_params()
+    p.chi2_cut = float(chi2)
+    assert oracle.track(g, p, rowv, padv, timev).up_raw[1] == -1
+    p.chi2_cut = float(np.nextafter(chi2, np.float32(100.0)))
+    assert oracle.track(g, p, rowv, padv, timev).up_raw[1] == 2
+
+
+def test_P10_transport_count_of_one_straight_track():
+    """Row steps of a lone noise-free line on rows 20 .. 60 (statistics block of the oracle = the units of the constructor's
+    roofline).  Rows 20 and 60 carry no link (a link needs both neighbours), so the start hit is row 21 and the cleaned chain
+    ends on row 59:  chain 22 .. 59 = 38;  following up: row 60 (found) + 61 .. 70 (ten misses) = 11;  down pass: 60 .. 21 through
+    the collected hits = 40, row 20 (found by the search) + 19 .. 10 (ten misses) = 11.  100 in all, 41 hits."""
+    r, row = _track_one([_line(np.arange(20, 61))])
+    assert len(r.tl_seed) == 1 and int(row[r.tl_seed[0]]) == 21 and r.tl_n_hits[0] == 41
+    assert r.stats["transports"] == 100.0
+    assert r.stats["updates"] == 38 + 1 + 40 + 1                                # every transport that met a hit
+
+
+@pytest.mark.parametrize("n_hits,is_track", [(30, True), (29, False)])
+def test_P11_a_tracklet_with_exactly_min_hits_is_a_track(n_hits, is_track):
+    """B:L7 '>= 30 unshared hits': 30 hits make a track, 29 do not."""
+    r, row = _track_one([_line(np.arange(20, 20 + n_hits))])
+    assert len(r.tl_seed) == 1 and r.tl_n_hits[0] == n_hits
+    assert len(r.tr_seed) == (1 if is_track else 0)
+    if is_track:
+        assert r.tr_n_hits[0] == 30
+
+
+def test_P12_result_does_not_depend_on_the_input_order_with_cluster_0_in_every_role():
+    """C1: 'the result is order-free (all ties break on the original cluster index)'.  The same small frame with one chosen
+    cluster swapped to index 0 -- a start hit, the top hit of a tracklet, a hit in the middle of one, a hit no tracklet holds --
+    must give the same links, tracklets, fits (bit for bit) and tracks once indices are mapped back."""
+    tf = _small_frame(6, n_tracks=12)
+    g, p = _geom(1, tf.max_time_bin), oracle.default_params(0.08, 0.12)
+    base = oracle.track(g, p, tf.row, tf.pad, tf.time)
+    assert len(base.tl_seed) > 20 and len(base.tr_seed) >= 8
+    t_long = int(np.argmax(base.tl_n_hits))
+    rows_t = np.nonzero(base.tl_row_hit[t_long] >= 0)[0]
+    held = np.zeros(tf.n, bool)
+    held[base.tl_row_hit[base.tl_row_hit >= 0]] = True
+    roles = {"start hit": int(base.tl_seed[t_long]), "top hit": int(base.tl_row_hit[t_long, rows_t[-1]]),
+             "middle hit": int(base.tl_row_hit[t_long, rows_t[len(rows_t) // 2]]), "bottom hit": int(base.tl_row_hit[t_long, rows_t[0]]),
+             "free hit": int(np.nonzero(~held)[0][0])}
+
+    def canon(r, new_of_old):
+        old_of_new = np.argsort(new_of_old)
+        m = lambda a: np.where(a >= 0, old_of_new[np.maximum(a, 0)], -1)
+        order = np.argsort(m(r.tl_seed))
+        ko = np.argsort(m(r.tr_seed))
+        hits = [tuple(sorted(m(r.tr_hit_index[r.tr_hit_offset[k]:r.tr_hit_offset[k] + r.tr_n_hits[k]]))) for k in ko]
+        return (m(r.link_up)[new_of_old], m(r.link_down)[new_of_old], m(r.tl_seed)[order], m(r.tl_row_hit)[order], r.tl_par[order],
+                m(r.tr_seed)[ko], r.tr_par[ko], hits)
+
+    ref = canon(base, np.arange(tf.n))
+    for role, c in roles.items():
+        if c == 0:
+            continue
+        new_of_old = np.arange(tf.n)
+        new_of_old[[0, c]] = [c, 0]                                             # old cluster c sits at index 0, old cluster 0 at c
+        perm = np.argsort(new_of_old)                                           # perm[new] = old
+        r = oracle.track(g, p, tf.row[perm], tf.pad[perm], tf.time[perm])
+        got = canon(r, new_of_old)
+        for i, (a, b) in enumerate(zip(ref[:7], got[:7])):
+            assert np.array_equal(a, b), (role, i)
+        assert ref[7] == got[7], role
