@@ -50,7 +50,8 @@ TRACKLET_PHASES = {"tracklet_fit_up": "fit_up", "tracklet_follow_up": "follow_up
 NCU_TRAFFIC_CSV = "r02_ncu_traffic_config3.csv"
 STEP_KERNEL = {"tracklet_follow_up": "k_tracklet_follow<0>", "tracklet_follow_down": "k_tracklet_follow<1>",
                "tracklet_fit_up": "k_tracklet_fit<0>", "tracklet_fit_down": "k_tracklet_fit<1>", "neighbours_finder": "k_neighbours_finder",
-               "selector_claim": "k_selector_claim", "selector_count": "k_selector_count", "tracklet_init": "k_tracklet_init"}
+               "selector_claim": ("k_selector_claim_top", "k_selector_claim"), "selector_count": "k_selector_count_hits",
+               "tracklet_init": "k_tracklet_init"}       # a step of several kernels: their traffic is summed
 
 
 def _ncu_traffic():
@@ -65,6 +66,14 @@ def _ncu_traffic():
     except OSError:
         pass
     return out
+def _step_traffic(traffic, step):
+    """(bytes per launch summed over the step's kernels, commit) or None."""
+    ks = STEP_KERNEL.get(step, ())
+    ks = (ks,) if isinstance(ks, str) else ks
+    got = [traffic[k] for k in ks if k in traffic]
+    return (sum(g[0] for g in got), got[0][1]) if got and len(got) == len(ks) else None
+
+
 SM_COUNT, SMSP_PER_SM, LANES = 148, 4, 32      # B300_MICROARCH.md: 4 schedulers per SM, <= 1 warp instruction per cycle each
 
 
@@ -487,12 +496,12 @@ def main():
             a = inst / (ms * 1e-3) / 1e12
             row.update({"bound": "alu", "achieved": round(a, 3), "peak": round(alu_peak, 3), "unit": "T lane-inst/s",
                         "frac": round(a / alu_peak, 4), "units": w})
-        t = traffic.get(STEP_KERNEL.get(k, ""))
+        t = _step_traffic(traffic, k)
         if t:
             row["traffic"] = t[0]
         kernels[k] = row
     dom = max(step_acc, key=step_acc.get)
-    t = traffic.get(STEP_KERNEL.get(dom, ""))
+    t = _step_traffic(traffic, dom)
     roof = {"kernel": dom, "ms": step_acc[dom], "share_of_step": step_acc[dom] / total_step_ms,
             "traffic": t[0] if t else None,
             "traffic_source": (f"profiles/{NCU_TRAFFIC_CSV} (dram read + write bytes per launch, ncu --set full at commit {t[1]})" if t else None)}
