@@ -10,7 +10,8 @@ entry point with pinned HOST buffers (H2D of the clusters and D2H of the tracks 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--frame-us F] [--impl reference]
 
 N > 1 (torchrun, one rank per GPU): every rank tracks its own time frame (the paper's farm runs independent time
-frames per GPU) -> weak scaling, no data-path collective.
+frames per GPU) -> weak scaling, no data-path collective.  `--shard sectors` instead cuts ONE frame by sector
+across the ranks (strong scaling, still no collective inside the tracking; paper_2102_08862_b200/shard.py).
 """
 from __future__ import annotations
 
@@ -228,6 +229,11 @@ def main():
     ap.add_argument("--grid-time-bins", type=int, default=0, help="grid bin width in time bins (0 = library default)")
     ap.add_argument("--slice-time-bins", type=int, default=0, help="processing-order time slice (0 = library default)")
     ap.add_argument("--grid-pad-bins", type=int, default=0, help="grid bins across a pad row (0 = library default)")
+    ap.add_argument("--shard", default="frames", choices=["frames", "sectors"],
+                    help="N > 1: frames = every rank tracks its own frame (replicas, weak scaling; the default); sectors = ONE frame cut by "
+                         "sector across the ranks (strong scaling; paper_2102_08862_b200/shard.py)")
+    ap.add_argument("--shard-of", default="", help="W:R with --shard sectors in a single process: track the sectors rank R of W ranks would get "
+                                                  "(the per-rank work of a W-GPU job measured on one GPU; value then covers that shard only)")
     ap.add_argument("--follower", type=int, default=0, help="0 = per-lane follower (default), 1 = row-synchronous follower (A/B)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cluster-finder", action="store_true")
@@ -255,11 +261,23 @@ def main():
 
     # ---- synthetic time frame (one per rank; seeded) ----
     cid = args.config
-    cfg = gen.preset(cid, replicas.frame_seed(args.seed, rank), args.frame_us if cid >= 2 else None)
+    by_sector = args.shard == "sectors"
+    cfg = gen.preset(cid, args.seed if by_sector else replicas.frame_seed(args.seed, rank), args.frame_us if cid >= 2 else None)
     cfg.n_threads = max(1, (os.cpu_count() or 8) // max(world, 1))
     t_gen = time.perf_counter()
     tf = gen.generate(cfg, want_truth=False)
     t_gen = time.perf_counter() - t_gen
+    sector_range = None
+    if by_sector:                                    # every rank holds the same frame and keeps the clusters of its sectors, in order
+        import dataclasses
+        from paper_2102_08862_b200 import shard
+        n_rows = 152
+        w_eff, r_eff = (int(v) for v in args.shard_of.split(":")) if (args.shard_of and world == 1) else (world, rank)
+        sector_range = shard.sector_ranges(cfg.n_sectors, w_eff, shard.sector_histogram(tf.row, cfg.n_sectors, n_rows))[r_eff]
+        sel = shard.shard_indices(tf.row, n_rows, *sector_range)
+        tf = dataclasses.replace(tf, row=np.ascontiguousarray(tf.row[sel]), pad=np.ascontiguousarray(tf.pad[sel]),
+                                 time=np.ascontiguousarray(tf.time[sel]), charge=np.ascontiguousarray(tf.charge[sel]),
+                                 truth_track=tf.truth_track[:0], truth_arc=tf.truth_arc[:0])
     n = tf.n
     host = [torch.from_numpy(a).pin_memory() for a in (tf.row, tf.pad, tf.time)]
     devc = [h.to(dev, non_blocking=True) for h in host]
@@ -542,11 +560,12 @@ def main():
 
     line = {"metric": "tpc_clusters_tracked_per_s", "value": value, "unit": "clusters/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "scaling": "strong" if by_sector else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": CONFIG_NAMES[cid] + (f" (frame cut to {args.frame_us:g} us)" if args.frame_us else ""),
                        "n_clusters_rank0": n, "n_clusters_all_ranks": int(n_all), "n_collisions": tf.n_collisions,
                        "n_tracks": n_tracks, "n_track_hits": n_track_hits, "status": status, "seed": args.seed,
-                       "parallelism": f"{world} independent time frame(s), one per GPU", "arena_gb": round(arena_gb, 2),
+                       "parallelism": (f"one time frame cut by sector across {args.shard_of or world} GPU(s) (sectors {sector_range[0]}..{sector_range[1] - 1} on rank 0), "
+                                       "no collective inside the tracking" if by_sector else f"{world} independent time frame(s), one per GPU"), "arena_gb": round(arena_gb, 2),
                        "l2": "inputs and scratch are larger than L2 (no flush needed)" if n * 12 > 2.5e8 else
                              "working set may fit L2 (small config)", "gen_seconds": round(t_gen, 1)},
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches,
