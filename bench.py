@@ -312,6 +312,28 @@ def main():
         barrier()
     total_ms = e0.elapsed_time(e1)
     launches = trk.last_launches() * args.steps
+    # the same call captured once in a CUDA graph and replayed (the call only enqueues work, so it can be captured): what a
+    # caller gains on frames whose launches cost more than their kernels (configs[0], [1]); not part of `value`
+    graph_replay = None
+    try:
+        gr = torch.cuda.CUDAGraph()
+        torch.cuda.synchronize()
+        with torch.cuda.graph(gr, stream=stream):
+            trk.tpc_track_timeframe(*devc, n=n, outputs=outs, stream=torch.cuda.current_stream(dev))
+        with torch.cuda.stream(stream):
+            for _ in range(args.warmup):
+                gr.replay()
+            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            g0.record(stream)
+            for _ in range(args.steps):
+                gr.replay()
+            g1.record(stream)
+        stream.synchronize()
+        graph_replay = {"ms_per_step": g0.elapsed_time(g1) / args.steps, "eager_ms_per_step_this_rank": total_ms / args.steps,
+                        "kernels_per_graph": trk.last_launches()}
+        del gr
+    except Exception as e:                            # reported, never fatal: the eager numbers above stand
+        graph_replay = {"error": repr(e)[:200]}
     trk.close()
     del trk
     # per-kernel durations: CUDA events recorded by the library on the same stream (a second handle with
@@ -571,7 +593,7 @@ def main():
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches,
             "step_ms": {k: round(v, 4) for k, v in step_acc.items()}, "kernels": kernels,
             "tracklet_constructor": constructor, "frame_vs_floors": frame, "rare_paths": work.get("rare_paths"), "merge": merge,
-            "cluster_finder": cluster_finder,
+            "cluster_finder": cluster_finder, "graph_replay": graph_replay,
             "roofline": roof, "cpu_baseline": cpu}
     print(json.dumps(line))
     if world > 1:
