@@ -67,6 +67,17 @@ def _ncu_traffic():
     except OSError:
         pass
     return out
+def _cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return None
+
+
 def _step_traffic(traffic, step):
     """(bytes per launch summed over the step's kernels, commit) or None."""
     ks = STEP_KERNEL.get(step, ())
@@ -207,7 +218,7 @@ def run_reference(args):
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_t / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": CONFIG_NAMES[cid], "sample": sample, "clusters_per_step": total_n // args.steps},
-            "cpu_baseline": {"value": value, "unit": "clusters/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": "clusters/s", "cores": cores, "kind": "oracle", "sample": sample, "cpu_model": _cpu_model()},
             "e2e": {"value": value, "unit": "clusters/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -575,7 +586,7 @@ def main():
             # WHOLE frame the GPU arm timed -- the same configuration, about 20 s for a 10 ms frame on 16 cores
             whole = bool(args.cpu_whole_frame) and not args.frame_us
             an, adt, athreads, atracks = _cpu_oracle_run_all_cores(cid, args.seed, args.cpu_sample_us, tf=tf if whole else None)
-            cpu = {"value": an / adt, "unit": "clusters/s", "cores": athreads, "host_cpus": os.cpu_count(),
+            cpu = {"value": an / adt, "unit": "clusters/s", "cores": athreads, "host_cpus": os.cpu_count(), "cpu_model": _cpu_model(),
                    "kind": "oracle", "how": "the unchanged oracle, one call per sector from a thread pool",
                    "sample": (f"the whole frame the GPU arm timed ({an} clusters, same configuration)" if whole else sample),
                    "same_config": whole, "seconds": adt, "n_tracks": atracks, "one_core": one_core}
