@@ -74,7 +74,8 @@ typedef struct {
   float sin_phi_max;              /* 0.95                                                     (reading A12) */
   float inv_R_per_qpt;            /* (float)(1/666.7) : curvature [1/cm] per q/pT [1/GeV]     (BASELINE L7) */
   float c0_y2, c0_s2, c0_k2, c0_z2, c0_t2; /* initial / reset covariance diagonal             (reading A8)  */
-  int32_t grid_time_bins;         /* width of one grid bin in time bins; 0 = default (8)                    */
+  int32_t grid_time_bins;         /* width of one grid bin in time bins; 0 = default: 8, or 9 / 10 when that makes
+                                     the grid bin index -- the radix sort key -- one digit size shorter          */
   int32_t grid_pad_bins;          /* grid bins across a pad row; 0 = default (8); lowered automatically so that
                                      no lookup window spans more than two of them.  The grid only accelerates:
                                      results do not depend on either value.                                  */

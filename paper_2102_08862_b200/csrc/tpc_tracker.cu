@@ -87,7 +87,6 @@ bool capacities(const tpc_geometry_t* g, const tpc_params_t* p, int64_t max_clus
   c.max_tracklets = p->max_tracklets > 0 ? p->max_tracklets : std::min<int64_t>(c.max_clusters / 10 + 4096, (int64_t)1 << kKeySlotBits);   // a claim word carries the slot in 24 bits
   c.max_tracks = p->max_tracks > 0 ? p->max_tracks : c.max_clusters / 64 + 4096;
   c.max_track_hits = p->max_track_hits > 0 ? p->max_track_hits : c.max_clusters;
-  c.grid_w = p->grid_time_bins > 0 ? p->grid_time_bins : kDefaultGridTimeBins;
   // Pad bins per row: as requested, but a lookup window must never span more than two of them.  Widest windows:
   // the finder's search area A_y and the follower's window after miss_limit missed rows, each with its margin.
   {
@@ -100,6 +99,20 @@ bool capacities(const tpc_geometry_t* g, const tpc_params_t* p, int64_t max_clus
     while (npb > 1 && 2.0 * std::max(ay, wf) * 1.01 > narrowest / (double)npb) --npb;
     c.n_pb = npb;
   }
+  // Time bins per grid bin: as requested; by default kDefaultGridTimeBins, widened by up to a quarter if that makes the sort key
+  // (the grid bin index) one radix digit size cheaper -- configs[3] at 8 time bins has 2.76e8 bins = 29 bits = four 8-bit passes,
+  // at 9 it has 2.45e8 = 28 bits = four 7-bit passes (ingest 8.7 -> 7.4 ms; the searches see 5 % more candidates, +0.1 ms each).
+  auto key_bits = [&](int w) {
+    const double nbw = (std::floor((double)g->max_time_bin / (double)w) + 1.0) * (double)c.n_pb * (double)g->n_sectors * (double)g->n_rows;
+    int b = 1;
+    while (std::ldexp(1.0, b) <= nbw) ++b;                            // the sentinel key n_bins must be representable
+    return b;
+  };
+  auto sort_cost = [&](int w) { const int b = key_bits(w), passes = (b + kRadixMaxBits - 1) / kRadixMaxBits; return passes * 16 + (b + passes - 1) / passes; };
+  c.grid_w = p->grid_time_bins > 0 ? p->grid_time_bins : kDefaultGridTimeBins;
+  if (p->grid_time_bins <= 0)
+    for (int w = kDefaultGridTimeBins + 1; w <= kDefaultGridTimeBins + kDefaultGridTimeBins / 4; ++w)
+      if (sort_cost(w) < sort_cost(c.grid_w)) c.grid_w = w;
   const double ntb = std::floor((double)g->max_time_bin / (double)c.grid_w) + 1.0;
   const double nb = ntb * (double)c.n_pb * (double)g->n_sectors * (double)g->n_rows;
   if (nb >= 2147483000.0) return false;
