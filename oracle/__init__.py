@@ -90,6 +90,10 @@ def lib():
         L.orc_rotate_with_cov.restype = C.c_int
         L.orc_refit_full.argtypes = [C.POINTER(Geometry), C.POINTER(Params), vp, vp, vp, vp, C.c_int64] + [vp] * 12
         L.orc_refit_full.restype = None
+        L.orc_refit_full_ce.argtypes = [C.POINTER(Geometry), C.POINTER(Params), vp, vp, vp, vp, C.c_int64] + [vp] * 15
+        L.orc_refit_full_ce.restype = None
+        L.orc_full_reflect.argtypes = [vp, vp, C.c_float, C.c_float, C.c_float, C.c_float]
+        L.orc_full_reflect.restype = None
         L.orc_full_step.argtypes = [C.POINTER(Params), vp, vp, vp, C.c_float]
         L.orc_full_step.restype = C.c_int
         L.orc_full_update.argtypes = [vp, vp, C.c_float, C.c_float, C.c_float, C.c_float]
@@ -255,6 +259,25 @@ def refit_full(geom: Geometry, params: Params, row, pad, time, res: "Result", nx
     return ok, ch, cp, rp, rc
 
 
+def refit_full_ce(geom: Geometry, params: Params, row, pad, time, res: "Result", nxt, prv, ce_next, ce_prev, t_ce,
+                  full_params=DEFAULT_FULL_PARAMS):
+    """C12 over chains that may continue behind the central electrode (C10's links; reading FF8).  Returns like refit_full."""
+    a = lambda v, t: np.ascontiguousarray(v, t)
+    row, pad, time = a(row, np.float32), a(pad, np.float32), a(time, np.float32)
+    nxt, prv, cn, cp_, tc = a(nxt, np.int32), a(prv, np.int32), a(ce_next, np.int32), a(ce_prev, np.int32), a(t_ce, np.float32)
+    n = int(len(res.tr_seed))
+    ok, ch, cp = np.zeros(n, np.int32), np.zeros(n, np.int32), np.zeros(n, np.int32)
+    rp, rc = np.zeros((n, 7), np.float32), np.zeros((n, 15), np.float32)
+    sec, nh, off = a(res.tr_sector, np.int32), a(res.tr_n_hits, np.int32), a(res.tr_hit_offset, np.int64)
+    hi, par = a(res.tr_hit_index, np.int32), a(res.tr_par, np.float32)
+    f4 = np.array(full_params, np.float32)
+    lib().orc_refit_full_ce(C.byref(geom), C.byref(params), f4.ctypes.data, row.ctypes.data, pad.ctypes.data, time.ctypes.data, n,
+                            sec.ctypes.data, nh.ctypes.data, off.ctypes.data, hi.ctypes.data, par.ctypes.data,
+                            nxt.ctypes.data, prv.ctypes.data, cn.ctypes.data, cp_.ctypes.data, tc.ctypes.data,
+                            ok.ctypes.data, ch.ctypes.data, cp.ctypes.data, rp.ctypes.data, rc.ctypes.data)
+    return ok, ch, cp, rp, rc
+
+
 def full_step(params: Params, state6, cov15, xn: float, full_params=DEFAULT_FULL_PARAMS):
     """One transport + material step of C12 (pins FF-*).  Returns (ok, state6, cov15)."""
     st, cv, f4 = np.array(state6, np.float32), np.array(cov15, np.float32), np.array(full_params, np.float32)
@@ -267,6 +290,13 @@ def full_rotate(geom: Geometry, params: Params, state6, cov15, q: int):
     st, cv = np.array(state6, np.float32), np.array(cov15, np.float32)
     rc = lib().orc_full_rotate(C.byref(geom), C.byref(params), st.ctypes.data, cv.ctypes.data, int(q))
     return rc == 0, st, cv
+
+
+def full_reflect(state6, cov15, tc: float, tref_b: float, tref_e: float, Z: float = 0.516):
+    """C12's reflection at the central electrode (pin FF-CE-R).  Returns (state6, cov15)."""
+    st, cv = np.array(state6, np.float32), np.array(cov15, np.float32)
+    lib().orc_full_reflect(st.ctypes.data, cv.ctypes.data, float(tc), float(tref_b), float(tref_e), float(Z))
+    return st, cv
 
 
 def full_update(state6, cov15, ym: float, zm: float, ry: float, rz: float):

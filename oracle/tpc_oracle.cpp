@@ -772,6 +772,15 @@ void full_reset(FullState& S, const orc_params& p) {
   S.P[0][0] = p.c0_y2; S.P[1][1] = p.c0_z2; S.P[2][2] = p.c0_s2; S.P[3][3] = p.c0_t2; S.P[4][4] = p.c0_k2;
 }
 
+// C12 at the central electrode (FF8): the time coordinate reflected about the crossing time tc; z was relative to tref_b (the
+// piece behind the electrode) and becomes relative to tref_e (the piece in front of it).
+void full_reflect(FullState& S, float tc, float tref_b, float tref_e, float Z) {
+  S.v[1] = (((tc + tc) - tref_b) - tref_e) * Z - S.v[1];
+  S.v[3] = -S.v[3];
+  for (int a = 0; a < 5; ++a) for (int b = 0; b < 5; ++b)
+    if (((a == 1 || a == 3) ? 1 : 0) != ((b == 1 || b == 3) ? 1 : 0)) S.P[a][b] = -S.P[a][b];
+}
+
 bool full_rotate(FullState& S, float qd, float Cd, float Sd, float sin_phi_max) {
   const float s0 = S.v[2];
   const float cs = std::sqrt(1.0f - s0 * s0);
@@ -787,10 +796,18 @@ bool full_rotate(FullState& S, float qd, float Cd, float Sd, float sin_phi_max) 
 }
 }  // namespace
 
-void orc_refit_full(const orc_geometry* gp, const orc_params* pp, const float* full4, const float* row, const float* pad,
-                    const float* time, int64_t n_tracks, const int32_t* sector, const int32_t* n_hits, const int64_t* hit_offset,
-                    const int32_t* hit_index, const float* par, const int32_t* next, const int32_t* prev,
-                    int32_t* ok, int32_t* chain_hits, int32_t* chain_pieces, float* rpar, float* rcov15) {
+// C12 with the links of C10 (reading FF8): a chain may continue behind the central electrode.  Pieces of a root: follow C7's
+// `next`; where that ends at piece e, a C10 link ce_next[e] = b is taken iff prev[b] < 0 (b starts a C7 chain on the other
+// side) and the chain has not crossed yet; then b's `next` links.  A track is a root iff prev < 0 and it is not such a b.
+// The pass runs inward as before.  At the electrode, between b (just fitted down to its innermost hit) and e:
+//     z = (((t_ce[e] + t_ce[e]) - time_ref_b) - time_ref_e) * Z - z          # the time coordinate reflected about t_ce, now relative to e
+//     t = -t;   P[i][j] = -P[i][j] for exactly one of i, j in {z, t}              # D P D with D = diag(1, -1, 1, -1, 1)
+// x, y, sin phi, q/pT are continuous: the mirror sector shares the local frame (no rotation).  ce_next == nullptr: plain C12.
+void orc_refit_full_ce(const orc_geometry* gp, const orc_params* pp, const float* full4, const float* row, const float* pad,
+                       const float* time, int64_t n_tracks, const int32_t* sector, const int32_t* n_hits, const int64_t* hit_offset,
+                       const int32_t* hit_index, const float* par, const int32_t* next, const int32_t* prev,
+                       const int32_t* ce_next, const int32_t* ce_prev, const float* t_ce,
+                       int32_t* ok, int32_t* chain_hits, int32_t* chain_pieces, float* rpar, float* rcov15) {
   const Derived D = derive(*gp, *pp);
   const FullParams fp{full4[0], full4[1], full4[2], full4[3]};
   float m2, ms2;
@@ -798,13 +815,27 @@ void orc_refit_full(const orc_geometry* gp, const orc_params* pp, const float* f
   const double T = (double)gp->tan_half_sector;
   const float Cd = (float)((1.0 - T * T) / (1.0 + T * T)), Sd = (float)(2.0 * T / (1.0 + T * T));
   const int nr = gp->n_rows;
+  auto crosses_into = [&](int64_t e) -> int64_t {      // the piece behind the electrode that continues e, or -1
+    if (!ce_next || next[e] >= 0) return -1;
+    const int64_t b = ce_next[e];
+    return (b >= 0 && prev[b] < 0) ? b : -1;
+  };
   for (int64_t i = 0; i < n_tracks; ++i) {
     ok[i] = 0; chain_hits[i] = n_hits[i]; chain_pieces[i] = 1;
     for (int k = 0; k < 7; ++k) rpar[7 * i + k] = par[7 * i + k];
     for (int k = 0; k < 15; ++k) rcov15[15 * i + k] = 0.0f;
     if (prev[i] >= 0) continue;
+    if (ce_next && ce_prev[i] >= 0 && crosses_into(ce_prev[i]) == i) continue;      // continuation of a chain from the other side
     std::vector<int64_t> pieces;
-    for (int64_t p = i; p >= 0; p = next[p]) pieces.push_back(p);
+    int64_t ce_at = -1;                                // index in `pieces` of the first piece behind the electrode
+    for (int64_t p = i; p >= 0;) {
+      pieces.push_back(p);
+      if ((int64_t)pieces.size() > 4 * (int64_t)nr) break;          // cannot happen (M7): never walk a corrupted link list for ever
+      if (next[p] >= 0) { p = next[p]; continue; }
+      const int64_t b = ce_at < 0 ? crosses_into(p) : -1;
+      if (b >= 0) ce_at = (int64_t)pieces.size();
+      p = b;
+    }
     int32_t total = 0;
     for (int64_t p : pieces) total += n_hits[p];
     chain_hits[i] = total; chain_pieces[i] = (int32_t)pieces.size();
@@ -833,9 +864,13 @@ void orc_refit_full(const orc_geometry* gp, const orc_params* pp, const float* f
       }
       if (good && ip > 0) {
         const int64_t pin = pieces[ip - 1];
-        const float sg = ((sector[p] % 18) == ((sector[pin] % 18) + 1) % 18) ? 1.0f : -1.0f;
-        if (!full_rotate(S, -sg, Cd, Sd, pp->sin_phi_max)) { good = false; break; }
-        S.v[1] = S.v[1] + (tref - par[7 * pin + 6]) * D.Z;
+        if (ip == ce_at) {                             // the central electrode: reflect the time coordinate
+          full_reflect(S, t_ce[pin], tref, par[7 * pin + 6], D.Z);
+        } else {
+          const float sg = ((sector[p] % 18) == ((sector[pin] % 18) + 1) % 18) ? 1.0f : -1.0f;
+          if (!full_rotate(S, -sg, Cd, Sd, pp->sin_phi_max)) { good = false; break; }
+          S.v[1] = S.v[1] + (tref - par[7 * pin + 6]) * D.Z;
+        }
       }
     }
     if (good) {
@@ -847,6 +882,14 @@ void orc_refit_full(const orc_geometry* gp, const orc_params* pp, const float* f
       ok[i] = -1;
     }
   }
+}
+
+void orc_refit_full(const orc_geometry* gp, const orc_params* pp, const float* full4, const float* row, const float* pad,
+                    const float* time, int64_t n_tracks, const int32_t* sector, const int32_t* n_hits, const int64_t* hit_offset,
+                    const int32_t* hit_index, const float* par, const int32_t* next, const int32_t* prev,
+                    int32_t* ok, int32_t* chain_hits, int32_t* chain_pieces, float* rpar, float* rcov15) {
+  orc_refit_full_ce(gp, pp, full4, row, pad, time, n_tracks, sector, n_hits, hit_offset, hit_index, par, next, prev, nullptr, nullptr, nullptr,
+                    ok, chain_hits, chain_pieces, rpar, rcov15);
 }
 
 // One step / one update of C12 on their own (pins FF-*): st6 = (x, y, z, s, t, k), cov15 = lower triangle.
@@ -873,6 +916,14 @@ int orc_full_rotate(const orc_geometry* g, const orc_params* p, float* st, float
   st[0] = S.x; for (int j = 0; j < 5; ++j) st[1 + j] = S.v[j];
   for (int a = 0; a < 5; ++a) for (int b = 0; b <= a; ++b) cov15[tri(a, b)] = S.P[a][b];
   return ok ? 0 : 1;
+}
+void orc_full_reflect(float* st, float* cov15, float tc, float tref_b, float tref_e, float Z) {
+  FullState S;
+  S.x = st[0]; for (int j = 0; j < 5; ++j) S.v[j] = st[1 + j];
+  for (int a = 0; a < 5; ++a) for (int b = 0; b < 5; ++b) S.P[a][b] = cov15[tri(a, b)];
+  full_reflect(S, tc, tref_b, tref_e, Z);
+  for (int j = 0; j < 5; ++j) st[1 + j] = S.v[j];
+  for (int a = 0; a < 5; ++a) for (int b = 0; b <= a; ++b) cov15[tri(a, b)] = S.P[a][b];
 }
 void orc_full_update(float* st, float* cov15, float ym, float zm, float ry, float rz) {
   FullState S;

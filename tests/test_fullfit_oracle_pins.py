@@ -476,3 +476,145 @@ def test_FFI_bookkeeping_every_root_is_fitted_single_tracks_too():
     r0 = (tf.row[res.tr_hit_index[res.tr_hit_offset[good]]].astype(np.int64)) % 152
     np.testing.assert_allclose(rp[good, 0], 85.0 + 1.07 * r0, atol=1e-4)
     assert np.all(rp[good, 6] == res.tr_par[good, 6])
+
+
+# ---- FF-CE: chains that continue behind the central electrode (reading FF8) -------------------------------------------------
+
+def test_FFCE_R_reflection_is_D_P_D_and_an_involution():
+    rng = np.random.default_rng(2)
+    L = rng.normal(size=(5, 5)) * np.array([0.2, 0.3, 0.02, 0.03, 0.4])[:, None]
+    P0 = (L @ L.T).astype(np.float32).astype(np.float64)
+    st0 = [120.0, 3.0, 7.25, 0.2, 0.375, -1.5]
+    tc, tb, te = 5000.5, 4990.0, 4980.25                                        # all exact in fp32
+    st, cv = oracle.full_reflect(st0, pack(P0), tc, tb, te)
+    D = np.diag([1.0, -1.0, 1.0, -1.0, 1.0])
+    assert np.array_equal(full(cv), (D @ P0 @ D).astype(np.float32).astype(np.float64))
+    assert st[2] == np.float32(np.float32((2 * tc - tb - te)) * np.float32(0.516) - np.float32(7.25)) and st[4] == np.float32(-0.375)
+    assert st[0] == 120.0 and st[1] == 3.0 and st[3] == np.float32(0.2) and st[5] == -1.5
+    # the time of the point itself is mirrored about tc:  time' = 2 tc - time
+    time_before = tb + 7.25 / 0.516
+    assert abs((te + float(st[2]) / 0.516) - (2 * tc - time_before)) < 1e-3
+    st2, cv2 = oracle.full_reflect(st, cv, tc, te, tb)                          # back again: the other side's reference first
+    np.testing.assert_allclose(st2, np.array(st0, np.float32), atol=2e-3)
+    assert np.array_equal(cv2, np.array(pack(P0), np.float32))
+
+
+def _mirrored_line(slope=0.4, x_c=None, sec_a=3):
+    """A straight line at y = 0 in sector sec_a (rows 60 .. 110, time rising outward with dz/dx = slope) that passes the electrode at
+    x_c and goes on in the mirror sector (rows 112 .. 151, time falling with the same slope)."""
+    from helpers import clusters_from_xyz, concat, row_x
+    ra, rb = np.arange(60, 111), np.arange(112, 152)
+    x_c = float(row_x(111)) if x_c is None else x_c
+    z_c = 3000.0
+    za = z_c - slope * (x_c - row_x(ra))
+    zb = z_c - slope * (row_x(rb) - x_c)
+    a = clusters_from_xyz(ra, np.zeros(ra.size), za, sector=sec_a)
+    b = clusters_from_xyz(rb, np.zeros(rb.size), zb, sector=(sec_a + 18) % 36)
+    return concat([a, b]), z_c / 0.516, ra, rb
+
+
+def test_FFCE_L_mirrored_straight_line_is_fitted_as_one_line():
+    """B = 0, y = 0: the two halves are ONE straight line in (x, reflected z).  After the refit across the electrode the state
+    on the innermost hit has the true slope and z, and var(dz/ds) is that of a line fit through all 91 hits, not 51."""
+    (row, pad, time), t_cross, ra, rb = _mirrored_line()
+    g = oracle.default_geometry(36, 8000.0)
+    p = oracle.default_params(0.08, 0.12)
+    p.inv_R_per_qpt = 0.0
+    res = oracle.track(g, p, row, pad, time)
+    assert len(res.tr_seed) == 2 and sorted(res.tr_sector.tolist()) == [3, 21]
+    mr = M.merge(M.default_merge_params(36), res.tr_seed, res.tr_sector, res.tr_first_row, res.tr_last_row, res.tr_par)
+    ce = M.merge_ce(M.default_ce_params(36), res.tr_seed, res.tr_sector, res.tr_first_row, res.tr_last_row, res.tr_par)
+    ia, ib = int(np.nonzero(res.tr_sector == 3)[0][0]), int(np.nonzero(res.tr_sector == 21)[0][0])
+    assert mr.n_links == 0 and ce.n_links == 1 and ce.next[ia] == ib and abs(float(ce.t_ce[ia]) - t_cross) < 5e-3
+    ok, ch, cp, rp, rc = oracle.refit_full_ce(g, p, row, pad, time, res, mr.next, mr.prev, ce.next, ce.prev, ce.t_ce, NO_MATERIAL)
+    assert ok[ia] == 1 and ok[ib] == 0 and ch[ia] == ra.size + rb.size and cp[ia] == 2 and ch[ib] == rb.size
+    np.testing.assert_array_equal(rp[ib], res.tr_par[ib])
+    x60 = 85.0 + 1.07 * 60
+    assert abs(rp[ia, 0] - x60) < 1e-4 and abs(rp[ia, 1]) < 1e-4 and abs(rp[ia, 3]) < 1e-5
+    assert abs(rp[ia, 4] - 0.4) < 2e-4                                          # dz/ds of the A side, B's mirrored slope included
+    z60 = (time[np.nonzero(row == 3 * 152 + 60)[0][0]] - rp[ia, 6]) * 0.516
+    assert abs(rp[ia, 2] - z60) < 5e-3
+    # var(t) of a straight-line fit: r_z / sum (x - mean x)^2 over ALL hits (the prior 1 / c0_t2 is negligible)
+    xs = 85.0 + 1.07 * np.concatenate([ra, rb]).astype(np.float64)
+    var_all = 0.12 ** 2 / np.sum((xs - xs.mean()) ** 2)
+    var_a = 0.12 ** 2 / np.sum((xs[:ra.size] - xs[:ra.size].mean()) ** 2)
+    assert abs(rc[ia, 9] / var_all - 1) < 0.02 and var_a > 4 * var_all, (rc[ia, 9], var_all, var_a)
+    # without the C10 links the root is fitted from its own 51 hits
+    ok0, ch0, _, rp0, rc0 = oracle.refit_full(g, p, row, pad, time, res, mr.next, mr.prev, NO_MATERIAL)
+    assert ok0[ia] == 1 and ok0[ib] == 1 and ch0[ia] == ra.size and abs(rc0[ia, 9] / var_a - 1) < 0.02
+
+
+def test_FFCE_H_noise_free_helices_and_FFCE_N_resolution_with_noise():
+    import merge_eval as ME
+    for noise_free in (True, False):
+        c = gen.preset(1, 3)
+        c.fixed_tracks, c.zv_sigma_cm, c.eta_max, c.pt_min = 3000, 30.0, 0.3, 0.3                 # many tracks through the electrode INSIDE the TPC
+        if noise_free:
+            c.sigma_y_cm = c.sigma_z_cm = c.dropout = c.noise_frac = 0.0
+        tf = gen.generate(c)
+        g, p = oracle.default_geometry(36, tf.max_time_bin), oracle.default_params()
+        res = oracle.track(g, p, tf.row, tf.pad, tf.time)
+        mr = M.merge(M.default_merge_params(36), res.tr_seed, res.tr_sector, res.tr_first_row, res.tr_last_row, res.tr_par)
+        ce = M.merge_ce(M.default_ce_params(36), res.tr_seed, res.tr_sector, res.tr_first_row, res.tr_last_row, res.tr_par)
+        ok0, ch0, cp0, rp0, rc0 = oracle.refit_full(g, p, tf.row, tf.pad, tf.time, res, mr.next, mr.prev, NO_MATERIAL)
+        ok, ch, cp, rp, rc = oracle.refit_full_ce(g, p, tf.row, tf.pad, tf.time, res, mr.next, mr.prev, ce.next, ce.prev, ce.t_ce, NO_MATERIAL)
+        used = np.array([a for a in np.nonzero(ce.next >= 0)[0] if mr.next[a] < 0 and mr.prev[ce.next[a]] < 0])
+        assert used.size >= 250
+        cont, roots = ce.next[used], mr.root[used]
+        # bookkeeping: the continuation is no root any more, the root's chain holds both sides, everything else is plain C12
+        assert np.all(ok[cont] == 0) and np.all(ok0[cont] == 1) and np.all(ok[roots] == 1)
+        np.testing.assert_array_equal(rp[cont], res.tr_par[cont])
+        pieces0 = np.bincount(mr.root, minlength=len(ok))
+        hits0 = np.bincount(mr.root, weights=res.tr_n_hits, minlength=len(ok)).astype(np.int64)
+        np.testing.assert_array_equal(cp[roots], pieces0[roots] + pieces0[cont])
+        np.testing.assert_array_equal(ch[roots], hits0[roots] + hits0[cont])
+        other = np.ones(len(ok), bool); other[roots] = False; other[cont] = False
+        assert np.array_equal(ok[other], ok0[other]) and np.array_equal(rp[other], rp0[other]) and np.array_equal(rc[other], rc0[other])
+        keys = ME.track_truth_keys(tf, res.tr_hit_offset, res.tr_n_hits, res.tr_hit_index)
+        part = np.where(keys >= 0, keys // (64 * 16), 0)
+        k_true = tf.tracks["charge_sense"][part] / tf.tracks["pt"][part]
+        sel = roots[(keys[roots] >= 0) & ((keys[roots] % 16) % 2 == 0) & (ok0[roots] == 1)]
+        assert sel.size >= 200
+        h = res.tr_hit_index[res.tr_hit_offset[sel]]
+        dz = np.abs(rp[sel, 2] - (tf.time[h] - rp[sel, 6]) * 0.516)
+        dk, dk0 = np.abs(rp[sel, 5] - k_true[sel]), np.abs(rp0[sel, 5] - k_true[sel])
+        assert np.mean(rc[sel, 14] < 0.5 * rc0[sel, 14]) > 0.9 and np.median(rc[sel, 14] / rc0[sel, 14]) < 0.05   # a much longer lever arm
+        if noise_free:
+            assert np.median(dz) < 1e-4 and np.quantile(dz, 0.95) < 0.05 and dz.max() < 0.6       # (a clamped crossing time shifts z by up to 2 * 0.5 bins)
+            assert np.quantile(dk / np.abs(k_true[sel]), 0.95) < 1e-3
+        else:
+            assert np.median(dk) < 0.25 * np.median(dk0), (np.median(dk), np.median(dk0))
+            pull = (rp[sel, 5] - k_true[sel]) / np.sqrt(rc[sel, 14])
+            assert 0.8 < np.std(pull[np.abs(pull) < 8]) < 1.25
+            assert np.median(dz) < 0.15
+
+
+def test_FFCE_C_a_sector_boundary_link_takes_precedence_over_a_link_through_the_electrode():
+    """FF8: the C10 link e -> b is used only if e has no C7 continuation and b is no C7 continuation of something else."""
+    from helpers import clusters_from_xyz, concat, row_x
+    (row, pad, time), t_cross, ra, rb = _mirrored_line()
+    rc_ = np.arange(70, 115)
+    c3 = clusters_from_xyz(rc_, np.full(rc_.size, 5.0), 900.0 + 0.2 * (row_x(rc_) - 85.0), sector=4)     # a third, unrelated track
+    row, pad, time = concat([(row, pad, time), c3])
+    g = oracle.default_geometry(36, 8000.0)
+    p = oracle.default_params(0.08, 0.12)
+    p.inv_R_per_qpt = 0.0
+    res = oracle.track(g, p, row, pad, time)
+    assert len(res.tr_seed) == 3
+    ia, ib, ic = (int(np.nonzero(res.tr_sector == s)[0][0]) for s in (3, 21, 4))
+    none = np.full(3, -1, np.int32)
+    ce_next, ce_prev, t_ce = none.copy(), none.copy(), np.zeros(3, np.float32)
+    ce_next[ia], ce_prev[ib], t_ce[ia] = ib, ia, t_cross
+    call = lambda nxt, prv: oracle.refit_full_ce(g, p, row, pad, time, res, nxt, prv, ce_next, ce_prev, t_ce, NO_MATERIAL)
+    ok, ch, cp, _, _ = call(none, none)                                         # no conflict: A + B
+    assert ok[ia] == 1 and ok[ib] == 0 and ok[ic] == 1 and ch[ia] == ra.size + rb.size and cp[ia] == 2 and ch[ic] == rc_.size
+    nxt, prv = none.copy(), none.copy()
+    nxt[ic], prv[ib] = ib, ic                                                   # B already continues C across a sector boundary
+    ok, ch, cp, _, _ = call(nxt, prv)
+    assert ok[ia] == 1 and ch[ia] == ra.size and cp[ia] == 1                    # A is fitted alone
+    assert ok[ib] == 0 and ok[ic] != 0 and ch[ic] == rc_.size + rb.size and cp[ic] == 2
+    nxt, prv = none.copy(), none.copy()
+    nxt[ia], prv[ic] = ic, ia                                                   # A already continues into C across a sector boundary
+    ok, ch, cp, _, _ = call(nxt, prv)
+    assert ok[ia] != 0 and ch[ia] == ra.size + rc_.size and cp[ia] == 2 and ok[ic] == 0
+    assert ok[ib] == 1 and ch[ib] == rb.size and cp[ib] == 1                    # B is a root of its own
