@@ -366,9 +366,9 @@ def main():
     # ---- widening step C7 (sector-boundary merging of the tracks, not part of `value`): timed on its own ----
     merge = None
     if cfg.n_sectors >= 18:
-        m0, m1, m2, m3, m4, m5 = (torch.cuda.Event(enable_timing=True) for _ in range(6))
-        merged = refit = ce = comp = full = None
-        ms_m = ms_r = ms_c = ms_q = ms_f = 0.0
+        m0, m1, m2, m3, m4, m5, m6 = (torch.cuda.Event(enable_timing=True) for _ in range(7))
+        merged = refit = ce = comp = full = full_ce = None
+        ms_m = ms_r = ms_c = ms_q = ms_f = ms_fc = 0.0
         outs_c = trk.alloc_outputs(n, hit_coords=True)      # C8 reads the hits' coordinates from two optional emit outputs
         for _ in range(3):
             with torch.cuda.stream(stream):
@@ -384,8 +384,11 @@ def main():
                 m4.record(stream)
                 full = trk.tpc_refit_full(outs_c, merged, out=full, stream=stream)
                 m5.record(stream)
+                full_ce = trk.tpc_refit_full(outs_c, merged, out=full_ce, stream=stream, ce_merged=ce)
+                m6.record(stream)
             stream.synchronize()
-            ms_m, ms_r, ms_c, ms_q, ms_f = m0.elapsed_time(m1), m1.elapsed_time(m2), m2.elapsed_time(m3), m3.elapsed_time(m4), m4.elapsed_time(m5)      # last of three
+            ms_m, ms_r, ms_c, ms_q, ms_f, ms_fc = (m0.elapsed_time(m1), m1.elapsed_time(m2), m2.elapsed_time(m3), m3.elapsed_time(m4),
+                                                   m4.elapsed_time(m5), m5.elapsed_time(m6))      # last of three
         emit_with_coords_ms = trk.step_ms().get("selector_emit")
         merge = {"step": "sector_boundary_merge (C7, tpc_merge_tracks)", "ms": round(ms_m, 4), "n_links": int(merged[3][0]),
                  "n_tracks": n_tracks, "tracks_per_s": n_tracks / (ms_m * 1e-3) if ms_m > 0 else None,
@@ -405,7 +408,10 @@ def main():
                                "hits_refitted": hits_full, "hits_per_s": hits_full / (ms_f * 1e-3) if ms_f > 0 else None,
                                "bound": "alu", "lane_inst_per_hit": 371,
                                "achieved_T_lane_inst_per_s": round(371 * hits_full / (ms_f * 1e-3) / 1e12, 3) if ms_f > 0 else None,
-                               "gpu_launches": 2}
+                               "gpu_launches": 2,
+                               "across_the_central_electrode": {"step": "tpc_refit_full_ce (C12 over C7 + C10 links)", "ms": round(ms_fc, 4),
+                                                                "n_roots_refitted": int((full_ce[0] == 1).sum()),
+                                                                "n_chains_through_the_electrode": int(((full_ce[1] > full[1]) & (full_ce[0] == 1)).sum())}}
         # C11: hit rejection + track-model residual symbols; their entropy (a host-side measurement of the output, numpy)
         # beside the entropy of the same hits' raw coordinates at the same quantisation
         ok_c = comp[1][:n_tracks].cpu().numpy()

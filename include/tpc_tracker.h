@@ -376,6 +376,15 @@ typedef struct {   /* caller-allocated DEVICE buffers, indexed by track like tpc
 int tpc_refit_full(tpc_tracker_t* tracker, const tpc_fullfit_params_t* params, const tpc_tracks_t* tracks,
                    const tpc_merged_t* merged, void* cuda_stream, tpc_fullfit_t* out);
 
+/* The same refit over chains that may CONTINUE BEHIND THE CENTRAL ELECTRODE (DESIGN.md §3 reading FF8): `ce_merged` = the output
+ * of tpc_merge_central_electrode for the same tracks (NULL = tpc_refit_full).  The link e -> b of C10 is used where e has no
+ * sector-boundary continuation and b continues nothing across a sector boundary; b is then no root (ok = 0, values passed
+ * through) and the root of e's chain is fitted over the hits of both sides: at the electrode the time coordinate is reflected
+ * about t_ce[e] (z = (2 t_ce - time_ref_b - time_ref_e) time_bin_cm - z, dzds = -dzds, covariance D P D), x, y, sin_phi, q_pt
+ * are continuous.  Same calling rules and errors as tpc_refit_full; the links must be C10's (reciprocal).                     */
+int tpc_refit_full_ce(tpc_tracker_t* tracker, const tpc_fullfit_params_t* params, const tpc_tracks_t* tracks,
+                      const tpc_merged_t* merged, const tpc_ce_merged_t* ce_merged, void* cuda_stream, tpc_fullfit_t* out);
+
 /* ---- C9: where and when a track passes the beam line (DESIGN.md §3 "C9"; z is only known once the
  * collision time is).  Every state of `par7` (DEVICE, [max_tracks*7] = (x, y, z_rel, sin_phi, dzds, q_pt, time_ref): the
  * par7 of tpc_refit_chains, or the same seven values of tpc_tracks_t) is transported to x = 0, the beam axis in every

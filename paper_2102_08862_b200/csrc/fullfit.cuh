@@ -27,9 +27,18 @@ struct FullFitIo {
   const float2* hit_yt; const uint8_t* hit_row;
   const int32_t* n_hits; const int64_t* hit_offset; int64_t max_track_hits;
   const int32_t *next, *prev;
+  const int32_t *ce_next, *ce_prev; const float* t_ce;   // C10's links (reading FF8); all three nullptr = plain C12
   int32_t *ok, *chain_hits, *chain_pieces;   // [max_tracks]
   float *par7, *cov15;                       // [max_tracks * 7], [max_tracks * 15]
 };
+
+// FF8: the piece behind the central electrode that continues piece e, or -1: C10's link counts only where no sector-boundary
+// link competes at either end.
+__device__ __forceinline__ int fullfit_crosses_into(const FullFitIo& io, int e) {
+  if (!io.ce_next || io.next[e] >= 0) return -1;
+  const int b = io.ce_next[e];
+  return (b >= 0 && io.prev[b] < 0) ? b : -1;
+}
 
 // Pass-through values for every track + the list of roots (prev < 0), in any order: results are indexed by track.
 __global__ void __launch_bounds__(256) k_fullfit_roots(MergeTracks T, FullFitIo io, uint32_t* __restrict__ root_list,
@@ -38,6 +47,7 @@ __global__ void __launch_bounds__(256) k_fullfit_roots(MergeTracks T, FullFitIo 
   bool is_root = false;
   if (i < merge_n(T, c)) {
     is_root = io.prev[i] < 0;
+    if (is_root && io.ce_next) { const int a = io.ce_prev[i]; if (a >= 0 && fullfit_crosses_into(io, a) == i) is_root = false; }   // continuation of a chain from the other side
     io.ok[i] = 0; io.chain_hits[i] = io.n_hits[i]; io.chain_pieces[i] = 1;
     float* rp = io.par7 + 7 * (size_t)i;
     rp[0] = T.x[i]; rp[1] = T.y[i]; rp[2] = T.z[i]; rp[3] = T.s[i]; rp[4] = T.t[i]; rp[5] = T.k[i]; rp[6] = T.time_ref[i];
@@ -197,8 +207,12 @@ __global__ void __launch_bounds__(kMergeThreads) k_refit_full(MergeTracks T, Ful
           root = (int)root_list[e];
           int pm = root, pieces = 1, total = io.n_hits[root];
           bool complete = io.n_hits[root] > 0 && io.hit_offset[root] + io.n_hits[root] <= io.max_track_hits;   // list not cut by TPC_STATUS_TRACK_HIT_OVERFLOW
-          for (int q = io.next[pm]; q >= 0; q = io.next[pm]) {
-            if (pieces >= c.n_rows) { complete = false; break; }          // cannot happen (M7); never walk a corrupted link list for ever
+          bool crossed = false;
+          for (;;) {
+            int q = io.next[pm];
+            if (q < 0 && !crossed) { q = fullfit_crosses_into(io, pm); crossed = q >= 0; }       // FF8: once, behind the electrode
+            if (q < 0) break;
+            if (pieces >= 4 * c.n_rows) { complete = false; break; }      // cannot happen (M7); never walk a corrupted link list for ever
             pm = q; ++pieces; total += io.n_hits[q];
             complete = complete && io.n_hits[q] > 0 && io.hit_offset[q] + io.n_hits[q] <= io.max_track_hits;
           }
@@ -238,6 +252,14 @@ __global__ void __launch_bounds__(kMergeThreads) k_refit_full(MergeTracks T, Ful
           rc[0] = S.P00; rc[1] = S.P10; rc[2] = S.P11; rc[3] = S.P20; rc[4] = S.P21; rc[5] = S.P22; rc[6] = S.P30; rc[7] = S.P31;
           rc[8] = S.P32; rc[9] = S.P33; rc[10] = S.P40; rc[11] = S.P41; rc[12] = S.P42; rc[13] = S.P43; rc[14] = S.P44;
           active = false;
+        } else if (io.prev[p] < 0) {                   // the central electrode (FF8): reflect the time coordinate about t_ce, no rotation
+          const int pin = io.ce_prev[p];
+          const float tce = io.t_ce[pin], tref_in = T.time_ref[pin];
+          S.z = (((tce + tce) - tref) - tref_in) * tc.Z - S.z;
+          S.t = -S.t;
+          S.P10 = -S.P10; S.P21 = -S.P21; S.P30 = -S.P30; S.P32 = -S.P32; S.P41 = -S.P41; S.P43 = -S.P43;
+          p = pin; tref = tref_in; off = io.hit_offset[pin]; j = off + io.n_hits[pin] - 1;
+          hy = io.hit_yt[j]; hr = io.hit_row[j];
         } else {                                       // piece boundary: rotate into the frame of the next inner piece
           const int pin = io.prev[p];
           const float sg = ((T.sector[p] % 18) == ((T.sector[pin] % 18) + 1) % 18) ? 1.0f : -1.0f;

@@ -718,6 +718,11 @@ int tpc_refit_chains(tpc_tracker_t* t, const tpc_tracks_t* tr, const tpc_merged_
 // ---- C12: refit of every chain root with the full covariance and the material of the gas (fullfit.cuh) ----
 int tpc_refit_full(tpc_tracker_t* t, const tpc_fullfit_params_t* fp, const tpc_tracks_t* tr, const tpc_merged_t* mg, void* cuda_stream,
                    tpc_fullfit_t* out) {
+  return tpc_refit_full_ce(t, fp, tr, mg, nullptr, cuda_stream, out);
+}
+
+int tpc_refit_full_ce(tpc_tracker_t* t, const tpc_fullfit_params_t* fp, const tpc_tracks_t* tr, const tpc_merged_t* mg, const tpc_ce_merged_t* ce,
+                      void* cuda_stream, tpc_fullfit_t* out) {
   if (!t || !fp || !tr || !mg || !out) return TPC_EINVAL;
   if (!(fp->inv_x0_per_cm >= 0 && fp->dedx_mip_gev_per_cm >= 0 && fp->mass_gev >= 0 && fp->eloss_sigma >= 0)) return TPC_EINVAL;
   if (tr->max_tracks < 0 || !tr->n_tracks || !out->ok || !out->chain_hits || !out->chain_pieces || !out->par7 || !out->cov15) return TPC_EINVAL;
@@ -743,7 +748,9 @@ int tpc_refit_full(tpc_tracker_t* t, const tpc_fullfit_params_t* fp, const tpc_t
   m.m2 = (float)((double)fp->mass_gev * (double)fp->mass_gev);
   m.ms2 = (float)(13.6e-3 * 13.6e-3);                  // Highland: 13.6 MeV, in GeV
   MergeTracks T{tr->n_tracks, tr->seed_hit, tr->sector, tr->first_row, tr->last_row, tr->x, tr->y, tr->z_rel, tr->time_ref, tr->sin_phi, tr->dzds, tr->q_pt};
+  if (ce && tr->max_tracks > 0 && (!ce->next || !ce->prev || !ce->t_ce)) return TPC_EINVAL;
   FullFitIo io{reinterpret_cast<const float2*>(tr->hit_y_time), tr->hit_row, tr->n_hits, tr->hit_offset, tr->max_track_hits, mg->next, mg->prev,
+               ce ? ce->next : nullptr, ce ? ce->prev : nullptr, ce ? ce->t_ce : nullptr,
                out->ok, out->chain_hits, out->chain_pieces, out->par7, out->cov15};
   int64_t launches = 0;
   cudaMemsetAsync(n_roots, 0, 512, st);

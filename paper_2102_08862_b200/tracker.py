@@ -20,7 +20,7 @@ EXPORTS = ("tpc_tracker_arena_bytes", "tpc_tracker_create", "tpc_track_timeframe
            "tpc_tracker_arena_plan", "tpc_selftest_fast_math", "tpc_selftest_alu_peak",
            "tpc_cluster_finder_scratch_bytes", "tpc_find_clusters",
            "tpc_find_clusters_static_max_digits", "tpc_find_clusters_static_setup", "tpc_find_clusters_static",
-           "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_merge_central_electrode", "tpc_refit_chains", "tpc_refit_full", "tpc_vertex_time", "tpc_compress_tracks", "tpc_merge_last_launches",
+           "tpc_merge_scratch_bytes", "tpc_merge_tracks", "tpc_merge_central_electrode", "tpc_refit_chains", "tpc_refit_full", "tpc_refit_full_ce", "tpc_vertex_time", "tpc_compress_tracks", "tpc_merge_last_launches",
            "tpc_tracker_destroy", "tpc_strerror")
 
 
@@ -203,6 +203,8 @@ def load_library(build_if_missing: bool = True):
         L.tpc_refit_chains.restype = C.c_int
         L.tpc_refit_full.argtypes = [vp, C.POINTER(FullFitParams), C.POINTER(Tracks), C.POINTER(Merged), vp, C.POINTER(FullFit)]
         L.tpc_refit_full.restype = C.c_int
+        L.tpc_refit_full_ce.argtypes = [vp, C.POINTER(FullFitParams), C.POINTER(Tracks), C.POINTER(Merged), C.POINTER(CeMerged), vp, C.POINTER(FullFit)]
+        L.tpc_refit_full_ce.restype = C.c_int
         L.tpc_compress_tracks.argtypes = [vp, C.POINTER(CompressParams), C.POINTER(Tracks), C.c_int64, vp, C.POINTER(Compressed)]
         L.tpc_compress_tracks.restype = C.c_int
         L.tpc_vertex_time.argtypes = [vp, vp, C.c_int32, vp, vp, vp, vp, vp]
@@ -499,9 +501,10 @@ class Tracker:
             raise TpcError(rc, "tpc_refit_chains")
         return refit
 
-    def tpc_refit_full(self, outputs, merged, full_params=DEFAULT_FULLFIT_PARAMS, out=None, stream=None):
-        """C12 on the DEVICE track outputs (allocated with ``hit_coords=True``) and C7 links (same stream); returns
-        (ok, chain_hits, chain_pieces, par7, cov15)."""
+    def tpc_refit_full(self, outputs, merged, full_params=DEFAULT_FULLFIT_PARAMS, out=None, stream=None, ce_merged=None):
+        """C12 on the DEVICE track outputs (allocated with ``hit_coords=True``) and C7 links (same stream); with ``ce_merged``
+        (the tensors of ``tpc_merge_central_electrode``) over chains that continue behind the central electrode
+        (``tpc_refit_full_ce``).  Returns (ok, chain_hits, chain_pieces, par7, cov15)."""
         torch = self._torch
         o, st = outputs
         K = max(int(st.max_tracks), 1)
@@ -512,7 +515,11 @@ class Tracker:
         r = FullFit(*(t.data_ptr() for t in out))
         fp = FullFitParams(*(float(v) for v in full_params))
         s = stream if stream is not None else torch.cuda.current_stream(self.device)
-        rc = self.lib.tpc_refit_full(self.handle, C.byref(fp), C.byref(st), C.byref(m), C.c_void_p(s.cuda_stream), C.byref(r))
+        if ce_merged is None:
+            rc = self.lib.tpc_refit_full(self.handle, C.byref(fp), C.byref(st), C.byref(m), C.c_void_p(s.cuda_stream), C.byref(r))
+        else:
+            cm = CeMerged(*(t.data_ptr() for t in ce_merged))
+            rc = self.lib.tpc_refit_full_ce(self.handle, C.byref(fp), C.byref(st), C.byref(m), C.byref(cm), C.c_void_p(s.cuda_stream), C.byref(r))
         if rc != TPC_OK:
             raise TpcError(rc, "tpc_refit_full")
         return out

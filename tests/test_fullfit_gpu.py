@@ -134,3 +134,46 @@ def test_fullfit_rejects_bad_arguments():
         trk.tpc_refit_full(no_coords, trk.tpc_merge_tracks(no_coords))
     torch.cuda.synchronize()
     trk.close()
+
+
+def _gpu_ce(tf, cfg, material):
+    import torch
+    from paper_2102_08862_b200 import tracker as T
+    n = tf.n
+    trk = T.Tracker(T.default_geometry(36, tf.max_time_bin), T.default_params(max(cfg.sigma_y_cm, 0.08), max(cfg.sigma_z_cm, 0.12), max_clusters=max(n, 1)))
+    d = [torch.from_numpy(np.ascontiguousarray(a, np.float32)).to(trk.device) for a in (tf.row, tf.pad, tf.time)]
+    outs = trk.alloc_outputs(n, hit_coords=True)
+    out = trk.tpc_track_timeframe(*d, n=n, outputs=outs)
+    merged = trk.tpc_merge_tracks(outs)
+    ce = trk.tpc_merge_central_electrode(outs)
+    fit = trk.tpc_refit_full(outs, merged, material, ce_merged=ce)
+    plain = trk.tpc_refit_full(outs, merged, material)
+    torch.cuda.synchronize()
+    k = int(out.n_tracks[0])
+    g = dict(k=k, status=int(out.status[0]), seed=out.seed_hit[:k].cpu().numpy(), fits=[tuple(t[:k].cpu().numpy() for t in f) for f in (fit, plain)],
+             ce_links=int(ce[3][0]))
+    trk.close()
+    return g
+
+
+@pytest.mark.parametrize("seed,noise_free", [(3, True), (4, False), (5, False)])
+def test_fullfit_across_the_central_electrode(seed, noise_free):
+    import oracle
+    from oracle import merge as M
+    cfg = gen.preset(1, seed)
+    cfg.fixed_tracks, cfg.zv_sigma_cm, cfg.eta_max, cfg.pt_min = 3000, 30.0, 0.3, 0.3        # many tracks through the electrode INSIDE the TPC
+    if noise_free:
+        cfg.sigma_y_cm = cfg.sigma_z_cm = cfg.dropout = cfg.noise_frac = 0.0
+    tf = gen.generate(cfg, want_truth=False)
+    g = _gpu_ce(tf, cfg, GAS)
+    geo, par = oracle.default_geometry(36, tf.max_time_bin), oracle.default_params(max(cfg.sigma_y_cm, 0.08), max(cfg.sigma_z_cm, 0.12))
+    res = oracle.track(geo, par, tf.row, tf.pad, tf.time)
+    mr = M.merge(M.default_merge_params(36), res.tr_seed, res.tr_sector, res.tr_first_row, res.tr_last_row, res.tr_par)
+    ce = M.merge_ce(M.default_ce_params(36), res.tr_seed, res.tr_sector, res.tr_first_row, res.tr_last_row, res.tr_par)
+    o_fit = oracle.refit_full_ce(geo, par, tf.row, tf.pad, tf.time, res, mr.next, mr.prev, ce.next, ce.prev, ce.t_ce, GAS)
+    o_plain = oracle.refit_full(geo, par, tf.row, tf.pad, tf.time, res, mr.next, mr.prev, GAS)
+    assert g["ce_links"] == ce.n_links >= 150
+    _compare(g, res, mr, [o_fit, o_plain])
+    # the electrode really is crossed by fitted chains: roots whose chain is longer than without C10's links
+    longer = (o_fit[1] > o_plain[1]) & (o_fit[0] == 1)
+    assert longer.sum() >= 0.9 * ce.n_links and (o_fit[0] == 0).sum() > (o_plain[0] == 0).sum()
