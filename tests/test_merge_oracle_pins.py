@@ -364,3 +364,105 @@ def test_MD_every_term_of_the_match_distance_decides():
             r = M.merge(p, [11, 22, 33], [0, 1, 1], [40, 101, 101], [99, 140, 140], par)
             assert r.next[0] == (1 if swap else 2), (col, swap, r.next)
             assert r.n_links == 1 and r.prev[r.next[0]] == 0
+
+
+# ---- pins from the line-by-line mutation sweep of the merge oracle -------------------------------------------
+
+def test_MW_the_weights_are_one_over_the_squared_cuts():
+    """Two candidates that miss in DIFFERENT quantities: which one wins is decided by w = 1 / cut^2 (cuts chosen so that
+    cut^2 differs from 2 cut for every one of them)."""
+    p = M.default_merge_params(36)
+    p.cut_y_cm, p.cut_z_cm, p.cut_sin_phi, p.cut_q_pt = 1.0, 3.0, 0.05, 0.5
+    base = _pair_across_boundary(state_row_b=101, first_row_b=101)
+    par_a, par_b = base[4][0], base[4][1]
+    # (column, offset) of candidate 1 and of candidate 2; in units of its cut:  0.60 vs 0.50, so candidate 2 wins every time
+    y, z, s, k = (1, 1.0), (2, 3.0), (3, 0.05), (5, 0.5)
+    for (c1, cut1), (c2, cut2) in ((y, z), (z, y), (y, s), (s, y), (z, k), (k, z), (s, k), (k, s)):
+        b1, b2 = par_b.copy(), par_b.copy()
+        b1[c1] += 0.60 * cut1
+        b2[c2] += 0.50 * cut2
+        r = M.merge(p, [11, 22, 33], [0, 1, 1], [40, 101, 101], [99, 140, 140], np.array([par_a, b1, b2], np.float32))
+        assert r.next[0] == 2 and r.n_links == 1, (c1, c2, r.next)
+        r = M.merge(p, [11, 33, 22], [0, 1, 1], [40, 101, 101], [99, 140, 140], np.array([par_a, b2, b1], np.float32))
+        assert r.next[0] == 1, (c1, c2, r.next)
+
+
+def test_M0_track_index_zero_is_a_track_like_any_other():
+    """Index 0 as the better of two candidates, as the link target, and as the better of two predecessors (C7 and C10)."""
+    p = M.default_merge_params(36)
+    base = _pair_across_boundary(state_row_b=101, first_row_b=101)
+    par_a, par_b = base[4][0], base[4][1]
+    worse = par_b.copy(); worse[1] += 0.9
+    # B (good) at index 0, a worse B' at 1, A at 2: A -> 0
+    r = M.merge(p, [22, 33, 11], [1, 1, 0], [101, 101, 40], [140, 140, 99], np.array([par_b, worse, par_a], np.float32))
+    assert r.next[2] == 0 and r.prev[0] == 2 and r.n_links == 1 and r.root[0] == 2
+    # two predecessors compete for one B: the better A at index 0, a worse A' (shifted in y) at 1
+    a_worse = par_a.copy(); a_worse[1] += 0.9
+    r = M.merge(p, [11, 12, 22], [0, 0, 1], [40, 40, 101], [99, 99, 140], np.array([par_a, a_worse, par_b], np.float32))
+    assert r.next[0] == 2 and r.prev[2] == 0 and r.next[1] == -1
+    # C10: the continuation at index 0
+    pc = M.default_ce_params(36)
+    args, t_cross = _ce_pair()
+    seed, sec, fr, lr, par = args
+    r = M.merge_ce(pc, seed[::-1], sec[::-1], fr[::-1], lr[::-1], par[::-1].copy())
+    assert r.n_links == 1 and r.next[1] == 0 and r.prev[0] == 1 and abs(float(r.t_ce[1]) - t_cross) < 2e-3
+    # C10: the better of two continuations at index 0 (the worse one 1 cm off in y)
+    b_worse = par[1].copy(); b_worse[1] += 1.0
+    r = M.merge_ce(pc, [22, 33, 11], [sec[1], sec[1], sec[0]], [fr[1], fr[1], fr[0]], [lr[1], lr[1], lr[0]], np.array([par[1], b_worse, par[0]], np.float32))
+    assert r.next[2] == 0 and r.n_links == 1
+
+
+def test_CEW_every_term_of_the_electrode_match_distance_adds():
+    """C10's d2 = dy^2 wy + ez^2 wz + ds^2 ws + dk^2 wk + dt^2 wt with w = 1 / cut^2: candidates that miss in different
+    quantities, 0.6 against 0.5 of the cut."""
+    pc = M.default_ce_params(36)
+    args, _ = _ce_pair()
+    seed, sec, fr, lr, par = args
+    cuts = {1: float(pc.cut_y_cm), 3: float(pc.cut_sin_phi), 5: float(pc.cut_q_pt), 4: float(pc.cut_dzds)}
+    cols = list(cuts)
+    for c1 in cols:
+        for c2 in cols:
+            if c1 == c2:
+                continue
+            b1, b2 = par[1].copy(), par[1].copy()
+            b1[c1] += 0.60 * cuts[c1]
+            b2[c2] += 0.50 * cuts[c2]
+            r = M.merge_ce(pc, [11, 22, 33], [sec[0], sec[1], sec[1]], [fr[0], fr[1], fr[1]], [lr[0], lr[1], lr[1]], np.array([par[0], b1, b2], np.float32))
+            assert r.next[0] == 2 and r.n_links == 1, (c1, c2, r.next)
+    # the time term: B shifted along z until dzm (1.93 cm unshifted, allowed interval [0, 4.28]) is -1.2 cm: ez = -1.2 = 0.6 cut_z;
+    # a candidate 0.5 cut_y off wins against it, one 0.7 cut_y off loses
+    (s1, s_, f_, l_, par1), _ = _ce_pair(shift_b=1.93 + 0.6 * float(pc.cut_z_cm))
+    for off, winner in ((0.5, 2), (0.7, 1)):
+        b2 = par[1].copy(); b2[1] += off * float(pc.cut_y_cm)
+        r = M.merge_ce(pc, [11, 22, 33], [sec[0], sec[1], sec[1]], [fr[0], fr[1], fr[1]], [lr[0], lr[1], lr[1]], np.array([par[0], par1[1], b2], np.float32))
+        assert r.next[0] == winner, (off, r.next)
+
+
+def test_CERW_row_window_of_the_electrode_merger():
+    """l_A + 1 - overlap <= r_B <= l_A + 1 + gap with r_B = floor((x_B - x0) / pitch + 0.5): the edges, with A ending on row 58."""
+    pc = M.default_ce_params(36)
+    gap, over = int(pc.max_row_gap), int(pc.max_row_overlap)
+    link = lambda row_b: M.merge_ce(pc, *_ce_pair(row_b=row_b, x_c=85.0 + 1.07 * 58.5)[0]).n_links
+    assert link(58 + 1 + gap) == 1 and link(58 + 2 + gap) == 0
+    assert link(58 + 1 - over) == 1 and link(58 - over) == 0
+    # half a TPC (18 sectors) has no mirror sectors but does merge across sector boundaries
+    p18 = M.default_merge_params(18)
+    base = _pair_across_boundary(state_row_b=101, first_row_b=101)
+    assert M.merge(p18, *base).n_links == 1
+
+
+def test_M7A_the_continuation_must_lie_above_the_state_row_of_A_and_index_zero_as_a_predecessor_in_C10():
+    """M7: r_B > max(f_A, r_A) with r_A the row A's state sits on -- which is above f_A when the down refit failed early."""
+    p = M.default_merge_params(36)
+    link = lambda rb: M.merge(p, *_pair_across_boundary(state_row_b=rb, first_row_b=rb, state_row_a=60, first_row_a=40, last_row_a=61)).n_links
+    assert link(60) == 0 and link(61) == 1              # row 60 is inside the row window [60, 74] but not above A's state row
+    pc = M.default_ce_params(36)
+    (seed, sec, fr, lr, par), _ = _ce_pair(rows_a=(40, 58), row_b=58)
+    par[0][0] = np.float32(85.0 + 1.07 * 58)            # C10 likewise: A's state moved up to row 58 = r_B
+    par[0][1] = np.float32(0.05 * float(par[0][0]))
+    assert M.merge_ce(pc, seed, sec, fr, lr, par).n_links == 0
+    # two tracks compete to continue into one B behind the electrode: the better one has index 0
+    (seed, sec, fr, lr, par), _ = _ce_pair()
+    a_worse = par[0].copy(); a_worse[1] += 1.0
+    r = M.merge_ce(pc, [11, 12, 22], [sec[0], sec[0], sec[1]], [fr[0], fr[0], fr[1]], [lr[0], lr[0], lr[1]], np.array([par[0], a_worse, par[1]], np.float32))
+    assert r.next[0] == 2 and r.prev[2] == 0 and r.next[1] == -1 and r.n_links == 1
