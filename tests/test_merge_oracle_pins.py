@@ -457,10 +457,9 @@ def test_M7A_the_continuation_must_lie_above_the_state_row_of_A_and_index_zero_a
     link = lambda rb: M.merge(p, *_pair_across_boundary(state_row_b=rb, first_row_b=rb, state_row_a=60, first_row_a=40, last_row_a=61)).n_links
     assert link(60) == 0 and link(61) == 1              # row 60 is inside the row window [60, 74] but not above A's state row
     pc = M.default_ce_params(36)
-    (seed, sec, fr, lr, par), _ = _ce_pair(rows_a=(40, 58), row_b=58)
-    par[0][0] = np.float32(85.0 + 1.07 * 58)            # C10 likewise: A's state moved up to row 58 = r_B
-    par[0][1] = np.float32(0.05 * float(par[0][0]))
-    assert M.merge_ce(pc, seed, sec, fr, lr, par).n_links == 0
+    for state_row, linked in ((58, 1), (59, 0)):        # C10 likewise: A (rows 40 .. 58) with its state on row 58 / on r_B = 59
+        (seed, sec, fr, lr, par), _ = _ce_pair(rows_a=(state_row, 58), row_b=59)
+        assert M.merge_ce(pc, seed, sec, [40, fr[1]], lr, par).n_links == linked, state_row
     # two tracks compete to continue into one B behind the electrode: the better one has index 0
     (seed, sec, fr, lr, par), _ = _ce_pair()
     a_worse = par[0].copy(); a_worse[1] += 1.0
