@@ -101,6 +101,12 @@ def test_QJ_rejection_rule():
     assert not rej[~owned].any()                                   # hits no track owns are kept
     none = oracle.compress_tracks(g, p, tf.row, tf.pad, tf.time, res, reject_qpt=1e9)
     assert none[0].sum() == 0 and (none[1] == -1).sum() == 0
+    # the bound is strict: a track with |q/pT| exactly on the cut is kept, one float below the cut it is rejected
+    k_abs = np.abs(res.tr_par[:, 5])
+    i = int(np.argsort(k_abs)[len(k_abs) // 2])
+    on = oracle.compress_tracks(g, p, tf.row, tf.pad, tf.time, res, reject_qpt=float(k_abs[i]))
+    below = oracle.compress_tracks(g, p, tf.row, tf.pad, tf.time, res, reject_qpt=float(np.nextafter(k_abs[i], np.float32(0))))
+    assert on[1][i] != -1 and below[1][i] == -1
 
 
 def test_QH_noise_free_helices_code_to_almost_nothing():
