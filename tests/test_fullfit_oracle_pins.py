@@ -590,7 +590,9 @@ def test_FFCE_H_noise_free_helices_and_FFCE_N_resolution_with_noise():
 
 
 def test_FFCE_C_a_sector_boundary_link_takes_precedence_over_a_link_through_the_electrode():
-    """FF8: the C10 link e -> b is used only if e has no C7 continuation and b is no C7 continuation of something else."""
+    """FF8: the C10 link e -> b is used only if e has no C7 continuation and b is no C7 continuation of something else.
+    Run with the three tracks in every order, so that track index 0 takes every role."""
+    import itertools
     from helpers import clusters_from_xyz, concat, row_x
     (row, pad, time), t_cross, ra, rb = _mirrored_line()
     rc_ = np.arange(70, 115)
@@ -599,22 +601,26 @@ def test_FFCE_C_a_sector_boundary_link_takes_precedence_over_a_link_through_the_
     g = oracle.default_geometry(36, 8000.0)
     p = oracle.default_params(0.08, 0.12)
     p.inv_R_per_qpt = 0.0
-    res = oracle.track(g, p, row, pad, time)
-    assert len(res.tr_seed) == 3
-    ia, ib, ic = (int(np.nonzero(res.tr_sector == s)[0][0]) for s in (3, 21, 4))
-    none = np.full(3, -1, np.int32)
-    ce_next, ce_prev, t_ce = none.copy(), none.copy(), np.zeros(3, np.float32)
-    ce_next[ia], ce_prev[ib], t_ce[ia] = ib, ia, t_cross
-    call = lambda nxt, prv: oracle.refit_full_ce(g, p, row, pad, time, res, nxt, prv, ce_next, ce_prev, t_ce, NO_MATERIAL)
-    ok, ch, cp, _, _ = call(none, none)                                         # no conflict: A + B
-    assert ok[ia] == 1 and ok[ib] == 0 and ok[ic] == 1 and ch[ia] == ra.size + rb.size and cp[ia] == 2 and ch[ic] == rc_.size
-    nxt, prv = none.copy(), none.copy()
-    nxt[ic], prv[ib] = ib, ic                                                   # B already continues C across a sector boundary
-    ok, ch, cp, _, _ = call(nxt, prv)
-    assert ok[ia] == 1 and ch[ia] == ra.size and cp[ia] == 1                    # A is fitted alone
-    assert ok[ib] == 0 and ok[ic] != 0 and ch[ic] == rc_.size + rb.size and cp[ic] == 2
-    nxt, prv = none.copy(), none.copy()
-    nxt[ia], prv[ic] = ic, ia                                                   # A already continues into C across a sector boundary
-    ok, ch, cp, _, _ = call(nxt, prv)
-    assert ok[ia] != 0 and ch[ia] == ra.size + rc_.size and cp[ia] == 2 and ok[ic] == 0
-    assert ok[ib] == 1 and ch[ib] == rb.size and cp[ib] == 1                    # B is a root of its own
+    res0 = oracle.track(g, p, row, pad, time)
+    assert len(res0.tr_seed) == 3
+    for order in itertools.permutations(range(3)):
+        o = np.array(order)
+        res = SimpleNamespace(tr_seed=res0.tr_seed[o], tr_sector=res0.tr_sector[o], tr_n_hits=res0.tr_n_hits[o], tr_hit_offset=res0.tr_hit_offset[o],
+                              tr_hit_index=res0.tr_hit_index, tr_par=res0.tr_par[o])
+        ia, ib, ic = (int(np.nonzero(res.tr_sector == s)[0][0]) for s in (3, 21, 4))
+        none = np.full(3, -1, np.int32)
+        ce_next, ce_prev, t_ce = none.copy(), none.copy(), np.zeros(3, np.float32)
+        ce_next[ia], ce_prev[ib], t_ce[ia] = ib, ia, t_cross
+        call = lambda nxt, prv: oracle.refit_full_ce(g, p, row, pad, time, res, nxt, prv, ce_next, ce_prev, t_ce, NO_MATERIAL)
+        ok, ch, cp, _, _ = call(none, none)                                     # no conflict: A + B
+        assert ok[ia] == 1 and ok[ib] == 0 and ok[ic] == 1 and ch[ia] == ra.size + rb.size and cp[ia] == 2 and ch[ic] == rc_.size, order
+        nxt, prv = none.copy(), none.copy()
+        nxt[ic], prv[ib] = ib, ic                                               # B already continues C across a sector boundary
+        ok, ch, cp, _, _ = call(nxt, prv)
+        assert ok[ia] == 1 and ch[ia] == ra.size and cp[ia] == 1, order         # A is fitted alone
+        assert ok[ib] == 0 and ok[ic] != 0 and ch[ic] == rc_.size + rb.size and cp[ic] == 2, order
+        nxt, prv = none.copy(), none.copy()
+        nxt[ia], prv[ic] = ic, ia                                               # A already continues into C across a sector boundary
+        ok, ch, cp, _, _ = call(nxt, prv)
+        assert ok[ia] != 0 and ch[ia] == ra.size + rc_.size and cp[ia] == 2 and ok[ic] == 0, order
+        assert ok[ib] == 1 and ch[ib] == rb.size and cp[ib] == 1, order         # B is a root of its own
